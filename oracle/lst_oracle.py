@@ -1,0 +1,191 @@
+"""ctypes loader for the CPU oracle (oracle/lst_oracle.cpp) -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from the CUDA package.
+"""
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lst_oracle.cpp")
+_LIB = os.path.join(_HERE, "liblst_oracle.so")
+CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+
+CUTS = ["M2", "M3", "L1", "L2", "L3", "T1", "T2", "T3", "Q1", "Q2", "P5", "P3"]
+STAGE = {"sort": 0, "md": 1, "ls": 2, "t3": 3, "t5": 4, "tc": 5}
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", *CXXFLAGS, "-o", _LIB, _SRC])
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.lst_oracle_run.restype = C.c_void_p
+        L.lst_oracle_run.argtypes = [C.c_int32] + [C.c_void_p] * 5 + [C.c_int32] + [C.c_void_p] * 4 + \
+            [C.c_int32] + [C.c_void_p] * 5 + [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32]
+        L.lst_oracle_count.restype = C.c_int64
+        L.lst_oracle_count.argtypes = [C.c_void_p, C.c_int32]
+        L.lst_oracle_copy_int.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+        L.lst_oracle_copy_real.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+        L.lst_oracle_free.argtypes = [C.c_void_p]
+        L.lst_oracle_md_eval.restype = C.c_int32
+        L.lst_oracle_md_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+        L.lst_oracle_ls_eval.restype = C.c_int32
+        L.lst_oracle_ls_eval.argtypes = [C.c_void_p] * 3
+        L.lst_oracle_t3_eval.restype = C.c_int32
+        L.lst_oracle_t3_eval.argtypes = [C.c_void_p] * 3 + [C.c_float, C.c_float, C.c_void_p]
+        L.lst_oracle_bridge_eval.restype = C.c_int32
+        L.lst_oracle_bridge_eval.argtypes = [C.c_void_p] * 4
+        L.lst_oracle_pls_match.restype = C.c_int32
+        L.lst_oracle_pls_match.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
+        L.lst_oracle_pls_residual.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+        L.lst_oracle_arcfac.restype = C.c_float
+        L.lst_oracle_arcfac.argtypes = [C.c_float]
+        L.lst_oracle_arcfac_f64.restype = C.c_double
+        L.lst_oracle_arcfac_f64.argtypes = [C.c_double]
+        L.lst_oracle_features.argtypes = [C.c_void_p] * 4 + [C.c_float] * 3 + [C.c_void_p]
+        L.lst_oracle_mlp.restype = C.c_float
+        L.lst_oracle_mlp.argtypes = [C.c_void_p, C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class OracleResult:
+    """Outputs of one oracle run.  Index tables are in the oracle's build order (SPEC.md 5):
+    md_hits[n,2] original hit indices (lower, upper); ls[n,2] MD indices; t3[n,5] = MD a,b,c + LS i,j;
+    t5c[n,8] = MD[5], T3 in, T3 out, pass; t5[n] candidate indices; tc[n,3] = type, pLS, object."""
+
+    def __init__(self, h, L):
+        cnt = lambda w: int(L.lst_oracle_count(h, w))
+
+        def ints(w, k):
+            n = cnt(w if w < 7 else 5)
+            o = np.zeros((n, k), dtype=np.int32)
+            if n:
+                L.lst_oracle_copy_int(h, w, _p(o))
+            return o
+
+        def reals(w, k, nw=None):
+            n = cnt(w if nw is None else nw)
+            o = np.zeros((n, k), dtype=np.float64)
+            if n:
+                L.lst_oracle_copy_real(h, w, _p(o))
+            return o
+
+        self.flags = cnt(20)
+        self.hit_orig = ints(0, 1)[:, 0]
+        ss = np.zeros(cnt(21), dtype=np.int32)
+        L.lst_oracle_copy_int(h, 21, _p(ss))
+        self.sensor_start = ss
+        md = ints(1, 3)
+        self.md_hits, self.md_mod = md[:, :2].copy(), md[:, 2].copy()
+        self.md_real = reals(1, 6)          # c, w, x, y, z, r
+        self.ls = ints(2, 2)
+        self.ls_c = reals(2, 1)[:, 0]
+        self.t3 = ints(3, 5)
+        self.t3_k = reals(3, 1)[:, 0]
+        self.t5c = ints(4, 8)
+        r5 = reals(4, 27)
+        self.t5c_curv, self.t5c_score, self.t5c_feat = r5[:, :3].copy(), r5[:, 3].copy(), r5[:, 4:].copy()
+        self.t5 = ints(5, 1)[:, 0]
+        self.tc = ints(6, 3)
+        self.best5_pls = ints(7, 1)[:, 0]
+        self.chi5 = reals(7, 1, nw=5)[:, 0]
+        self.counts = dict(hits=cnt(0), md=cnt(1), ls=cnt(2), t3=cnt(3), t5c=cnt(4), t5=cnt(5), tc=cnt(6),
+                           md_pairs=cnt(10), ls_pairs=cnt(11), t3_pairs=cnt(12), t5_pairs=cnt(13),
+                           match5=cnt(14), match3=cnt(15))
+
+
+def run(geo, weights, ev, *, t5_override=None, loosen=None, use_double=False, last_stage="tc",
+        counts_only=False):
+    """Run the whole chain on one event.  `geo` needs n_modules, subdet, mtype, conn_rowptr, conn_col."""
+    L = lib()
+    w = np.ascontiguousarray(weights, dtype=np.float32)
+    ov = None if t5_override is None else np.ascontiguousarray(t5_override, dtype=np.int8)
+    lo = None
+    if loosen is not None:
+        lo = np.ones(len(CUTS), dtype=np.float32)
+        for k, v in loosen.items():
+            lo[CUTS.index(k)] = v
+    h = L.lst_oracle_run(int(geo.n_modules), _p(geo.subdet), _p(geo.mtype), _p(geo.conn_rowptr), _p(geo.conn_col),
+                         _p(w), ev.n_hits, _p(ev.x), _p(ev.y), _p(ev.z), _p(ev.key), ev.n_pls, _p(ev.pls_px),
+                         _p(ev.pls_py), _p(ev.pls_pz), _p(ev.pls_z0), _p(ev.pls_q), _p(ov),
+                         0 if ov is None else int(ov.size), _p(lo), int(bool(use_double)), STAGE[last_stage])
+    try:
+        if counts_only:
+            names = dict(hits=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, md_pairs=10, ls_pairs=11, t3_pairs=12,
+                         t5_pairs=13, match5=14, match3=15)
+            return {k: int(L.lst_oracle_count(h, v)) for k, v in names.items()}
+        return OracleResult(h, L)
+    finally:
+        L.lst_oracle_free(h)
+
+
+# ---- single predicates (for the brute-force / closed-form pins) ----
+def md_eval(h1, h2, subdet, mtype):
+    a = np.ascontiguousarray(h1, dtype=np.float32); b = np.ascontiguousarray(h2, dtype=np.float32)
+    out = np.zeros(6, dtype=np.float32)
+    ok = lib().lst_oracle_md_eval(_p(a), _p(b), int(subdet), int(mtype), _p(out))
+    return bool(ok), out
+
+
+def ls_eval(a9, b9):
+    a = np.ascontiguousarray(a9, dtype=np.float32); b = np.ascontiguousarray(b9, dtype=np.float32)
+    c = np.zeros(1, dtype=np.float32)
+    return bool(lib().lst_oracle_ls_eval(_p(a), _p(b), _p(c))), float(c[0])
+
+
+def t3_eval(a9, b9, c9, c_ab, c_bc):
+    a, b, c = (np.ascontiguousarray(v, dtype=np.float32) for v in (a9, b9, c9))
+    k = np.zeros(1, dtype=np.float32)
+    return bool(lib().lst_oracle_t3_eval(_p(a), _p(b), _p(c), float(c_ab), float(c_bc), _p(k))), float(k[0])
+
+
+def bridge_eval(a9, b9, c9):
+    a, b, c = (np.ascontiguousarray(v, dtype=np.float32) for v in (a9, b9, c9))
+    k = np.zeros(1, dtype=np.float32)
+    return bool(lib().lst_oracle_bridge_eval(_p(a), _p(b), _p(c), _p(k))), float(k[0])
+
+
+def pls_match(pls5, q, anchors9):
+    p = np.ascontiguousarray(pls5, dtype=np.float32)
+    a = np.ascontiguousarray(anchors9, dtype=np.float32).reshape(-1, 9)
+    chi = np.zeros(1, dtype=np.float32)
+    return bool(lib().lst_oracle_pls_match(_p(p), int(q), _p(a), int(a.shape[0]), _p(chi))), float(chi[0])
+
+
+def pls_residual(pls5, q, xyz):
+    p = np.ascontiguousarray(pls5, dtype=np.float64); a = np.ascontiguousarray(xyz, dtype=np.float64)
+    out = np.zeros(3, dtype=np.float64)
+    lib().lst_oracle_pls_residual(_p(p), int(q), _p(a), _p(out))
+    return out
+
+
+def arcfac(u, f64=False):
+    return lib().lst_oracle_arcfac_f64(float(u)) if f64 else lib().lst_oracle_arcfac(float(u))
+
+
+def features(ax, ay, az, ar, cin, cbr, cout):
+    a = [np.ascontiguousarray(v, dtype=np.float32) for v in (ax, ay, az, ar)]
+    out = np.zeros(23, dtype=np.float32)
+    lib().lst_oracle_features(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), float(cin), float(cbr), float(cout), _p(out))
+    return out
+
+
+def mlp(weights, x23):
+    w = np.ascontiguousarray(weights, dtype=np.float32); x = np.ascontiguousarray(x23, dtype=np.float32)
+    return float(lib().lst_oracle_mlp(_p(w), _p(x)))

@@ -1,0 +1,29 @@
+import os
+import sys
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+
+
+@pytest.fixture(scope="session")
+def geo_full():
+    from lstgen import build_geometry
+    return build_geometry(True)
+
+
+@pytest.fixture(scope="session")
+def geo_barrel():
+    from lstgen import build_geometry
+    return build_geometry(False)
+
+
+@pytest.fixture(scope="session")
+def geo_sym4():
+    from lstgen import build_geometry
+    return build_geometry(True, nphi_multiple=4)
