@@ -1,0 +1,149 @@
+/* include/lst.h -- C ABI of the B200-native line-segment-tracking (LST) hot path.
+ *
+ * What the library computes: the segment-building chain of arXiv:2403.13166 for one event's
+ * outer-tracker hits -- mini-doublets, line segments, triplets, quintuplets, the T5-DNN score of
+ * every quintuplet and the four mutually exclusive track-candidate types (Table 1,
+ * PAPER.md:45-60; T5-DNN PAPER.md:62-68, :90).  The cuts the paper leaves out are frozen in
+ * SPEC.md; section numbers below refer to it.  Entry-point names follow BASELINE.json north_star (1):
+ * lst_create / lst_load_event / lst_run / lst_get.
+ *
+ * Conventions
+ *  - Every function returns LST_OK (0) or a negative error; none throws, aborts or prints.
+ *  - "HOST" / "DEVICE" on a pointer says where the memory lives.  The caller owns ALL memory:
+ *    the library allocates nothing on the device; it carves the caller's workspace.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (torch.cuda.Stream().cuda_stream); 0 = default
+ *    stream.  lst_load_event*, lst_run* and lst_read_* only ENQUEUE work; lst_status synchronises.
+ *  - A context holds `n_slots` independent event slots that share one uploaded geometry
+ *    (BASELINE.json configs[3]: "geometry and connectivity uploaded once").
+ *  - Overflow of a stage capacity is NOT an error return: the stage keeps the first `cap` objects in
+ *    build order and sets its bit in the slot's status word (SPEC.md 6) -- flagged, never silent.
+ */
+#ifndef LST_H_
+#define LST_H_
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LST_OK 0
+#define LST_EINVAL (-1)  /* null pointer, size above capacity, malformed CSR, bad slot / objtype   */
+#define LST_ECUDA (-2)   /* a CUDA runtime call failed (sticky)                                   */
+#define LST_ENOMEM (-3)  /* workspace smaller than lst_workspace_bytes()                          */
+
+/* status bits (lst_status) */
+#define LST_ST_BAD_KEY (1u << 0)   /* a hit key >= 2*n_modules was dropped (SPEC.md 4.0)          */
+#define LST_ST_OVF_MD (1u << 1)
+#define LST_ST_OVF_LS (1u << 2)
+#define LST_ST_OVF_T3 (1u << 3)
+#define LST_ST_OVF_T5C (1u << 4)
+#define LST_ST_OVF_T5 (1u << 5)
+#define LST_ST_OVF_TC (1u << 6)
+
+/* object types for lst_get */
+enum { LST_OBJ_HIT = 0, LST_OBJ_MD = 1, LST_OBJ_LS = 2, LST_OBJ_T3 = 3, LST_OBJ_T5C = 4, LST_OBJ_T5 = 5,
+       LST_OBJ_TC = 6, LST_OBJ_MATCH5 = 7, LST_N_OBJ = 8 };
+
+/* indices into counts[] of lst_status: number of objects per type after clamping to capacity,
+ * then the UNCLAMPED totals (what the stage would have produced), then pair-test counts. */
+enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT_T5, LST_CNT_TC,
+       LST_CNT_RAW_MD, LST_CNT_RAW_LS, LST_CNT_RAW_T3, LST_CNT_RAW_T5C, LST_CNT_RAW_T5, LST_CNT_RAW_TC,
+       LST_CNT_PT5, LST_CNT_T5TC, LST_CNT_PT3, LST_CNT_PLSTC, LST_N_CNT = 32 };
+
+typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
+
+/* Static detector description (SPEC.md 2).  All pointers HOST; copied to the device by lst_create. */
+typedef struct {
+  int32_t n_modules;
+  const uint8_t* subdet;      /* [n_modules] 0 barrel, 1 endcap                                   */
+  const uint8_t* mtype;       /* [n_modules] 0 PS, 1 2S                                           */
+  const int32_t* conn_rowptr; /* [n_modules+1] CSR of module -> connected modules, rowptr[0] = 0  */
+  const int32_t* conn_col;    /* [rowptr[n_modules]] ascending and unique within a row, no self   */
+  const float* dnn_weights;   /* [1857] W1[32][23], b1[32], W2[32][32], b2[32], w3[32], b3        */
+} lst_geometry;
+
+/* Per-slot capacities (objects).  max_tc is forced to >= max_pls + max_t5 internally. */
+typedef struct {
+  int32_t n_slots, max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls;
+} lst_caps;
+
+/* Device view of one object list of one slot (lst_get).  Pointers are DEVICE pointers into the
+ * caller's workspace, valid until lst_destroy; contents are valid after the lst_run that produced
+ * them completes and until the next lst_run on that slot.  `count` is a DEVICE pointer to the
+ * clamped object count.  Unused entries are NULL.  Layouts (row-major, `capacity` rows):
+ *  HIT   : i0 = orig[n] int32 (sorted position -> original hit index), i1 = sensor_start[2M+1],
+ *          f0 = xyz as float4 (x, y, z, key as int bits)
+ *  MD    : i0 = hits[n][2] int32 (ORIGINAL lower, upper hit index), i1 = modt[n] int32 (module<<2 |
+ *          subdet<<1 | mtype), f0 = anchor[n] float4 (x, y, z, r), f1 = cw[n] float2 (c, w),
+ *          i2 = md_start[M+1]
+ *  LS    : i0 = ab[n][2] int32 MD indices, f0 = c[n], i1 = ls_start[n_md+1]
+ *  T3    : i0 = abc[n][4] int32 (MD a, b, c, first LS), i1 = second LS [n], f0 = k[n],
+ *          i2 = t3_start[n_md+1]
+ *  T5C   : i0 = md[n][5] int32, i1 = t3[n][2] int32, f0 = curv[n][3] (c_in, c_br, c_out),
+ *          f1 = feat[n][23], f2 = score[n], i2 = pass[n] int32 (0/1)
+ *  T5    : i0 = cand[n] int32 (index into T5C)
+ *  TC    : i0 = tc[n][3] int32 (type 0 pT5 / 1 T5 / 2 pT3 / 3 pLS, pLS index or -1, T5-list or T3
+ *          index or -1)
+ *  MATCH5: i0 = best5_pls[n_t5] int32 (-1 = unmatched), f0 = chi2[n_t5]
+ */
+typedef struct {
+  int32_t capacity;
+  const int32_t* count;
+  const int32_t* i0;
+  const int32_t* i1;
+  const int32_t* i2;
+  const float* f0;
+  const float* f1;
+  const float* f2;
+} lst_view;
+
+/* Bytes of device workspace lst_create needs for these capacities.  Validates the geometry
+ * (LST_EINVAL on null pointers, non-monotone rowptr, column out of range / unsorted / duplicate /
+ * self-link, non-positive capacities). */
+int lst_workspace_bytes(const lst_geometry* geo, const lst_caps* caps, size_t* out_bytes);
+
+/* Build a context in `dev_workspace` (DEVICE, 256-byte aligned, >= lst_workspace_bytes) and upload
+ * the geometry, CSR and DNN weights (synchronous).  The workspace must outlive the context. */
+int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspace, size_t bytes, lst_ctx** out);
+
+/* Bind one event to a slot (SPEC.md 2).  DEVICE pointers; NOT copied: they must stay valid and
+ * unchanged until the lst_run that consumes them has completed.  n_hits <= max_hits,
+ * n_pls <= max_pls, else LST_EINVAL.  d_key[i] = 2*module + isUpper. */
+int lst_load_event(lst_ctx* ctx, int32_t slot, int32_t n_hits, const float* d_x, const float* d_y,
+                   const float* d_z, const uint32_t* d_key, int32_t n_pls, const float* d_px,
+                   const float* d_py, const float* d_pz, const float* d_z0, const int8_t* d_q,
+                   void* cuda_stream);
+
+/* Same with HOST pointers (pinned memory recommended): enqueues the host->device copies into the
+ * slot's staging area on `cuda_stream`.  Host buffers must stay valid until the copies complete. */
+int lst_load_event_host(lst_ctx* ctx, int32_t slot, int32_t n_hits, const float* h_x, const float* h_y,
+                        const float* h_z, const uint32_t* h_key, int32_t n_pls, const float* h_px,
+                        const float* h_py, const float* h_pz, const float* h_z0, const int8_t* h_q,
+                        void* cuda_stream);
+
+/* Enqueue the whole chain a0..a6 (SPEC.md 4.0-4.6) for one slot / for slots
+ * [first_slot, first_slot + n) in single batched launches (event index = a grid dimension). */
+int lst_run(lst_ctx* ctx, int32_t slot, void* cuda_stream);
+int lst_run_batch(lst_ctx* ctx, int32_t first_slot, int32_t n, void* cuda_stream);
+
+/* Device views of a slot's object lists. */
+int lst_get(lst_ctx* ctx, int32_t slot, int32_t objtype, lst_view* out);
+
+/* Synchronise `cuda_stream`, then return the slot's status bits and counts[LST_N_CNT] (HOST). */
+int lst_status(lst_ctx* ctx, int32_t slot, uint32_t* status_bits, int32_t* counts, void* cuda_stream);
+
+/* Enqueue device->host copies of the slot's counters (HOST int32[LST_N_CNT], then status word in
+ * h_counts[LST_N_CNT-1]) and of the first `max_rows` rows of its TC list (HOST int32[max_rows][3]). */
+int lst_read_tc_host(lst_ctx* ctx, int32_t slot, int32_t* h_counts, int32_t* h_tc, int32_t max_rows,
+                     void* cuda_stream);
+
+/* Number of kernel launches one lst_run / lst_run_batch enqueues (for the harness' accounting). */
+int lst_launches_per_run(void);
+
+void lst_destroy(lst_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LST_H_ */

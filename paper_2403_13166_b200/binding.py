@@ -1,0 +1,245 @@
+"""ctypes binding with the same names as include/lst.h (lst_create, lst_load_event, lst_run,
+lst_get, ...).  PyTorch supplies device memory and streams only."""
+import ctypes as C
+import os
+from dataclasses import dataclass, asdict
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBNAME = os.path.join(_HERE, "liblst_b200.so")
+
+LST_N_CNT = 32
+OBJ = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, match5=7)
+CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t3=9, raw_t5c=10,
+           raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16)
+STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
+EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
+           "lst_run_batch", "lst_get", "lst_status", "lst_read_tc_host", "lst_launches_per_run",
+           "lst_destroy"]
+
+
+class LstError(RuntimeError):
+    pass
+
+
+class _Geometry(C.Structure):
+    _fields_ = [("n_modules", C.c_int32), ("subdet", C.c_void_p), ("mtype", C.c_void_p),
+                ("conn_rowptr", C.c_void_p), ("conn_col", C.c_void_p), ("dnn_weights", C.c_void_p)]
+
+
+class _Caps(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("n_slots", "max_hits", "max_md", "max_ls", "max_t3", "max_t5c",
+                                         "max_t5", "max_pls")]
+
+
+class _View(C.Structure):
+    _fields_ = [("capacity", C.c_int32), ("count", C.c_void_p), ("i0", C.c_void_p), ("i1", C.c_void_p),
+                ("i2", C.c_void_p), ("f0", C.c_void_p), ("f1", C.c_void_p), ("f2", C.c_void_p)]
+
+
+@dataclass
+class Caps:
+    n_slots: int = 1
+    max_hits: int = 131072
+    max_md: int = 65536
+    max_ls: int = 65536
+    max_t3: int = 65536
+    max_t5c: int = 65536
+    max_t5: int = 65536
+    max_pls: int = 8192
+
+
+def default_caps(n_slots: int = 1) -> Caps:
+    """Capacities sized for configs[4]'s densest point (PU300 + 500 displaced) with head-room."""
+    return Caps(n_slots=n_slots)
+
+
+def library_path() -> str:
+    return _LIBNAME
+
+
+_lib = None
+
+
+def load_library():
+    """Load liblst_b200.so; raises LstError when it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBNAME):
+        raise LstError(f"{_LIBNAME} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                       "(nvcc, sm_100a). There is no CPU fallback.")
+    L = C.CDLL(_LIBNAME)
+    vp, i32 = C.c_void_p, C.c_int32
+    L.lst_workspace_bytes.argtypes = [C.POINTER(_Geometry), C.POINTER(_Caps), C.POINTER(C.c_size_t)]
+    L.lst_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Caps), vp, C.c_size_t, C.POINTER(vp)]
+    L.lst_load_event.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
+    L.lst_load_event_host.argtypes = L.lst_load_event.argtypes
+    L.lst_run.argtypes = [vp, i32, vp]
+    L.lst_run_batch.argtypes = [vp, i32, i32, vp]
+    L.lst_get.argtypes = [vp, i32, i32, C.POINTER(_View)]
+    L.lst_status.argtypes = [vp, i32, C.POINTER(C.c_uint32), vp, vp]
+    L.lst_read_tc_host.argtypes = [vp, i32, vp, vp, i32, vp]
+    L.lst_launches_per_run.argtypes = []
+    L.lst_destroy.argtypes = [vp]
+    L.lst_destroy.restype = None
+    for n in EXPORTS:
+        if n != "lst_destroy":
+            getattr(L, n).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise LstError(f"{what} failed with code {rc} "
+                       f"({ {-1: 'LST_EINVAL', -2: 'LST_ECUDA', -3: 'LST_ENOMEM'}.get(rc, '?') })")
+
+
+def _hp(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+# rows, dtype, columns of every view field (include/lst.h lst_view)
+_FIELDS = {
+    "hit": dict(i0=("orig", "i32", 1), f0=("xyzk", "f32", 4)),
+    "md": dict(i0=("hits", "i32", 2), i1=("modt", "i32", 1), f0=("anchor", "f32", 4), f1=("cw", "f32", 2)),
+    "ls": dict(i0=("ab", "i32", 2), f0=("c", "f32", 1)),
+    "t3": dict(i0=("abc", "i32", 4), i1=("l1", "i32", 1), f0=("k", "f32", 1)),
+    "t5c": dict(i0=("md", "i32", 5), i1=("t3", "i32", 2), i2=("pass", "i32", 1), f0=("curv", "f32", 3),
+                f1=("feat", "f32", 23), f2=("score", "f32", 1)),
+    "t5": dict(i0=("cand", "i32", 1)),
+    "tc": dict(i0=("tc", "i32", 3)),
+    "match5": dict(i0=("best5_pls", "i32", 1), f0=("chi2", "f32", 1)),
+}
+
+
+class LST:
+    """One context = one uploaded geometry + `caps.n_slots` event slots in a torch-owned workspace."""
+
+    def __init__(self, geo, weights, caps: Caps = None, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.lib = load_library()
+        self.caps = caps or default_caps()
+        self.device = torch.device(device)
+        self.n_modules = int(geo.n_modules)
+        self._keep = dict(subdet=np.ascontiguousarray(geo.subdet, np.uint8), mtype=np.ascontiguousarray(geo.mtype, np.uint8),
+                          rowptr=np.ascontiguousarray(geo.conn_rowptr, np.int32), col=np.ascontiguousarray(geo.conn_col, np.int32),
+                          w=np.ascontiguousarray(weights, np.float32))
+        if self._keep["w"].size != 1857:
+            raise LstError("dnn_weights must hold 1857 floats")
+        k = self._keep
+        self._g = _Geometry(self.n_modules, _hp(k["subdet"]), _hp(k["mtype"]), _hp(k["rowptr"]), _hp(k["col"]), _hp(k["w"]))
+        self._c = _Caps(**asdict(self.caps))
+        nbytes = C.c_size_t(0)
+        _chk(self.lib.lst_workspace_bytes(C.byref(self._g), C.byref(self._c), C.byref(nbytes)), "lst_workspace_bytes")
+        self.workspace_bytes = int(nbytes.value)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_off = (-base) % 256
+            self._ws_ptr = base + self._ws_off
+            ctx = C.c_void_p()
+            _chk(self.lib.lst_create(C.byref(self._g), C.byref(self._c), C.c_void_p(self._ws_ptr), nbytes, C.byref(ctx)), "lst_create")
+        self.ctx = ctx
+        self._bound = {}
+
+    # ---- entry points, same names as the C ABI -------------------------------------------------
+    def lst_load_event(self, slot, x, y, z, key, px, py, pz, z0, q, stream=None):
+        """Bind DEVICE tensors (float32 / int32-as-uint32 / int8) to a slot; they are not copied."""
+        t = self.torch
+        for a, dt in ((x, t.float32), (y, t.float32), (z, t.float32), (px, t.float32), (py, t.float32), (pz, t.float32), (z0, t.float32)):
+            assert a.is_cuda and a.dtype == dt and a.is_contiguous()
+        assert key.is_cuda and key.dtype in (t.int32, t.uint32) and key.is_contiguous()
+        assert q.is_cuda and q.dtype == t.int8 and q.is_contiguous()
+        self._bound[slot] = (x, y, z, key, px, py, pz, z0, q)
+        p = lambda a: C.c_void_p(a.data_ptr()) if a.numel() else C.c_void_p(0)
+        _chk(self.lib.lst_load_event(self.ctx, slot, x.numel(), p(x), p(y), p(z), p(key), px.numel(), p(px), p(py), p(pz), p(z0), p(q),
+                                     self._st(stream)), "lst_load_event")
+
+    def lst_load_event_host(self, slot, hx, hy, hz, hkey, hpx, hpy, hpz, hz0, hq, stream=None):
+        """HOST (ideally pinned) torch tensors or numpy arrays; enqueues the H2D copies."""
+        arrs = (hx, hy, hz, hkey, hpx, hpy, hpz, hz0, hq)
+        self._bound[slot] = arrs
+        def p(a):
+            if hasattr(a, "data_ptr"):
+                return C.c_void_p(a.data_ptr()) if a.numel() else C.c_void_p(0)
+            return _hp(a) if a.size else C.c_void_p(0)
+        n = lambda a: int(a.numel()) if hasattr(a, "numel") else int(a.size)
+        _chk(self.lib.lst_load_event_host(self.ctx, slot, n(hx), p(hx), p(hy), p(hz), p(hkey), n(hpx), p(hpx), p(hpy), p(hpz), p(hz0), p(hq),
+                                          self._st(stream)), "lst_load_event_host")
+
+    def lst_run(self, slot=0, stream=None):
+        _chk(self.lib.lst_run(self.ctx, slot, self._st(stream)), "lst_run")
+
+    def lst_run_batch(self, first_slot, n, stream=None):
+        _chk(self.lib.lst_run_batch(self.ctx, first_slot, n, self._st(stream)), "lst_run_batch")
+
+    def lst_status(self, slot=0, stream=None):
+        bits = C.c_uint32(0)
+        counts = np.zeros(LST_N_CNT, dtype=np.int32)
+        _chk(self.lib.lst_status(self.ctx, slot, C.byref(bits), _hp(counts), self._st(stream)), "lst_status")
+        return int(bits.value), {k: int(counts[v]) for k, v in CNT.items()}
+
+    def lst_get(self, slot, objtype, n=None):
+        """Device views (torch tensors aliasing the workspace) of one object list; `n` rows
+        (default: the clamped count, which costs a synchronising lst_status)."""
+        name = objtype if isinstance(objtype, str) else {v: k for k, v in OBJ.items()}[objtype]
+        v = _View()
+        _chk(self.lib.lst_get(self.ctx, slot, OBJ[name], C.byref(v)), "lst_get")
+        if n is None:
+            _, cnt = self.lst_status(slot)
+            n = cnt["t5" if name == "match5" else name]
+        out = {}
+        t = self.torch
+        for fld, (label, dt, cols) in _FIELDS[name].items():
+            ptr = getattr(v, fld)
+            off = ptr - self.workspace.data_ptr()
+            raw = self.workspace[off:off + 4 * n * cols]
+            out[label] = raw.view(t.int32 if dt == "i32" else t.float32).view(n, cols) if cols > 1 else \
+                raw.view(t.int32 if dt == "i32" else t.float32)
+        return out
+
+    def lst_read_tc_host(self, slot, h_counts, h_tc, stream=None):
+        """Enqueue D2H of counters and TC rows into HOST (pinned) int32 tensors."""
+        _chk(self.lib.lst_read_tc_host(self.ctx, slot, C.c_void_p(h_counts.data_ptr()), C.c_void_p(h_tc.data_ptr()),
+                                       int(h_tc.shape[0]), self._st(stream)), "lst_read_tc_host")
+
+    def launches_per_run(self):
+        return int(self.lib.lst_launches_per_run())
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            self.lib.lst_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- conveniences --------------------------------------------------------------------------
+    def _st(self, stream):
+        if stream is None:
+            stream = self.torch.cuda.current_stream(self.device)
+        return C.c_void_p(stream.cuda_stream)
+
+    def load_numpy_event(self, slot, ev, stream=None):
+        """Upload a lstgen.Event's arrays with torch and bind them (tests / smoke)."""
+        t = self.torch
+        dev = lambda a: t.from_numpy(np.ascontiguousarray(a)).to(self.device)
+        key = t.from_numpy(ev.key.view(np.int32).copy()).to(self.device)
+        self.lst_load_event(slot, dev(ev.x), dev(ev.y), dev(ev.z), key, dev(ev.pls_px), dev(ev.pls_py), dev(ev.pls_pz),
+                            dev(ev.pls_z0), dev(ev.pls_q), stream)
+
+    def fetch(self, slot):
+        """Copy every object list of a slot to numpy (one synchronising status call)."""
+        bits, cnt = self.lst_status(slot)
+        res = dict(status=bits, counts=cnt)
+        for name in _FIELDS:
+            n = cnt["t5" if name == "match5" else name]
+            res[name] = {k: v.cpu().numpy() for k, v in self.lst_get(slot, name, n).items()}
+        return res

@@ -1,0 +1,317 @@
+// lst_api.cu -- the C ABI of include/lst.h: workspace carving, geometry upload, launch sequence.
+// Host logic only; every step of the hot path runs in the kernels of lst_kernels.cuh.
+#include <cuda_runtime.h>
+#include <new>
+#include <vector>
+#include "lst_kernels.cuh"
+
+using namespace lst;
+
+struct lst_ctx {
+  int n_slots = 0;
+  int n_modules = 0;
+  Geo geo{};
+  Caps caps{};
+  Slot* d_slots = nullptr;        // device array [n_slots]
+  std::vector<Slot> h_slots;      // host mirror of the carved pointers (inputs not tracked)
+  char* zero_base = nullptr; size_t zero_stride = 0;
+  char* ones_base = nullptr; size_t ones_stride = 0;
+  bool sticky_cuda_error = false;
+};
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Carver {   // walks the workspace; with base == nullptr it only measures
+  char* base; size_t off = 0;
+  template <typename T> T* take(size_t n) {
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += up(n * sizeof(T));
+    return p;
+  }
+};
+
+int validate(const lst_geometry* g, const lst_caps* c) {
+  if (!g || !c || !g->subdet || !g->mtype || !g->conn_rowptr || !g->conn_col || !g->dnn_weights) return LST_EINVAL;
+  if (g->n_modules <= 0 || g->n_modules > (1 << 28)) return LST_EINVAL;
+  if (c->n_slots <= 0 || c->max_hits <= 0 || c->max_md <= 0 || c->max_ls <= 0 || c->max_t3 <= 0 || c->max_t5c <= 0 ||
+      c->max_t5 <= 0 || c->max_pls <= 0)
+    return LST_EINVAL;
+  if (c->max_pls > (1 << 28) / 5) return LST_EINVAL;
+  const int M = g->n_modules;
+  if (g->conn_rowptr[0] != 0) return LST_EINVAL;
+  for (int m = 0; m < M; ++m) {
+    const int b = g->conn_rowptr[m], e = g->conn_rowptr[m + 1];
+    if (e < b) return LST_EINVAL;
+    for (int i = b; i < e; ++i) {
+      const int col = g->conn_col[i];
+      if (col < 0 || col >= M || col == m) return LST_EINVAL;
+      if (i > b && g->conn_col[i - 1] >= col) return LST_EINVAL;
+    }
+    if (g->subdet[m] > 1 || g->mtype[m] > 1) return LST_EINVAL;
+  }
+  return LST_OK;
+}
+
+Caps make_caps(const lst_caps* c) {
+  Caps k;
+  k.max_hits = c->max_hits; k.max_md = c->max_md; k.max_ls = c->max_ls; k.max_t3 = c->max_t3;
+  k.max_t5c = c->max_t5c; k.max_t5 = c->max_t5; k.max_pls = c->max_pls; k.max_tc = c->max_pls + c->max_t5;
+  return k;
+}
+
+// One pass lays out the whole workspace; used both to measure and to carve.
+struct Layout {
+  Slot* slots; uint8_t* modt; int* rowptr; int* col; float* weights;
+  char* zero_base; size_t zero_stride; char* ones_base; size_t ones_stride;
+  size_t total;
+};
+
+Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vector<Slot>* out) {
+  Carver cv{base};
+  Layout L{};
+  L.slots = cv.take<Slot>(n_slots);
+  L.modt = cv.take<uint8_t>(M);
+  L.rowptr = cv.take<int>(M + 1);
+  L.col = cv.take<int>(nnz > 0 ? nnz : 1);
+  L.weights = cv.take<float>(N_W);
+  if (out) out->assign(n_slots, Slot{});
+  // zero region (contiguous over slots so one memset covers a batch)
+  {
+    Carver z{nullptr};
+    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(2 * M);
+    L.zero_stride = z.off;
+    L.zero_base = base ? base + cv.off : nullptr;
+    for (int s = 0; s < n_slots; ++s) {
+      Carver c2{base ? base + cv.off + s * L.zero_stride : nullptr};
+      int* cnt = c2.take<int>(LST_N_CNT);
+      int* ss = c2.take<int>(2 * M + 2);
+      int* cur = c2.take<int>(2 * M);
+      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].cursor = cur; }
+    }
+    cv.off += L.zero_stride * n_slots;
+  }
+  // 0xFF region
+  {
+    Carver z{nullptr};
+    z.take<unsigned long long>(k.max_pls); z.take<unsigned long long>(k.max_pls); z.take<int>(k.max_md);
+    L.ones_stride = z.off;
+    L.ones_base = base ? base + cv.off : nullptr;
+    for (int s = 0; s < n_slots; ++s) {
+      Carver c2{base ? base + cv.off + s * L.ones_stride : nullptr};
+      auto* w5 = c2.take<unsigned long long>(k.max_pls);
+      auto* w3 = c2.take<unsigned long long>(k.max_pls);
+      int* head = c2.take<int>(k.max_md);
+      if (out) { (*out)[s].win5 = w5; (*out)[s].win3 = w3; (*out)[s].md_head = head; }
+    }
+    cv.off += L.ones_stride * n_slots;
+  }
+  for (int s = 0; s < n_slots; ++s) {
+    Slot t{};
+    t.tmp_orig = cv.take<int>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
+    t.md_off = cv.take<int>(k.max_hits + 8); t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
+    t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_start = cv.take<int>(M + 1);
+    t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
+    t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
+    t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
+    t.t5_off = cv.take<int>(k.max_t3 + 8); t.t5c_md = cv.take<int>(5 * (size_t)k.max_t5c); t.t5c_t3 = cv.take<int2>(k.max_t5c);
+    t.t5c_curv = cv.take<float>(3 * (size_t)k.max_t5c); t.t5c_feat = cv.take<float>((size_t)N_FEAT * k.max_t5c);
+    t.t5c_score = cv.take<float>(k.max_t5c); t.t5c_pass = cv.take<int>(k.max_t5c); t.t5_scan = cv.take<int>(k.max_t5c + 8);
+    t.t5_list = cv.take<int>(k.max_t5);
+    t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.best5 = cv.take<int>(k.max_t5);
+    t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
+    t.chi3 = cv.take<float>(k.max_t3); t.tc = cv.take<int>(3 * (size_t)k.max_tc);
+    t.st_x = cv.take<float>(k.max_hits); t.st_y = cv.take<float>(k.max_hits); t.st_z = cv.take<float>(k.max_hits);
+    t.st_key = cv.take<uint32_t>(k.max_hits);
+    t.st_px = cv.take<float>(k.max_pls); t.st_py = cv.take<float>(k.max_pls); t.st_pz = cv.take<float>(k.max_pls);
+    t.st_z0 = cv.take<float>(k.max_pls); t.st_q = cv.take<int8_t>(k.max_pls);
+    if (out) {
+      Slot& d = (*out)[s];
+      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head;
+      d = t;
+    }
+  }
+  L.total = cv.off;
+  return L;
+}
+
+inline bool bad(lst_ctx* c, cudaError_t e) {
+  if (e != cudaSuccess) { c->sticky_cuda_error = true; return true; }
+  return false;
+}
+
+constexpr int N_LAUNCHES = 23;   // kernels per lst_run / lst_run_batch (plus two memsets)
+
+}  // namespace
+
+extern "C" {
+
+int lst_launches_per_run(void) { return N_LAUNCHES; }
+
+int lst_workspace_bytes(const lst_geometry* geo, const lst_caps* caps, size_t* out_bytes) {
+  if (!out_bytes) return LST_EINVAL;
+  const int rc = validate(geo, caps);
+  if (rc != LST_OK) return rc;
+  const Caps k = make_caps(caps);
+  const Layout L = lay_out(nullptr, geo->n_modules, geo->conn_rowptr[geo->n_modules], k, caps->n_slots, nullptr);
+  *out_bytes = L.total;
+  return LST_OK;
+}
+
+int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspace, size_t bytes, lst_ctx** out) {
+  if (!out || !dev_workspace) return LST_EINVAL;
+  if (reinterpret_cast<uintptr_t>(dev_workspace) % ALIGN) return LST_EINVAL;
+  const int rc = validate(geo, caps);
+  if (rc != LST_OK) return rc;
+  lst_ctx* c = new (std::nothrow) lst_ctx();
+  if (!c) return LST_ENOMEM;
+  const int M = geo->n_modules, nnz = geo->conn_rowptr[M];
+  c->caps = make_caps(caps);
+  c->n_slots = caps->n_slots;
+  c->n_modules = M;
+  const Layout L = lay_out(static_cast<char*>(dev_workspace), M, nnz, c->caps, c->n_slots, &c->h_slots);
+  if (L.total > bytes) { delete c; return LST_ENOMEM; }
+  c->d_slots = L.slots;
+  c->zero_base = L.zero_base; c->zero_stride = L.zero_stride;
+  c->ones_base = L.ones_base; c->ones_stride = L.ones_stride;
+  std::vector<uint8_t> modt(M);
+  for (int m = 0; m < M; ++m) modt[m] = uint8_t((geo->subdet[m] << 1) | geo->mtype[m]);
+  cudaError_t e = cudaMemcpy(L.modt, modt.data(), M, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(L.rowptr, geo->conn_rowptr, sizeof(int) * (M + 1), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && nnz > 0) e = cudaMemcpy(L.col, geo->conn_col, sizeof(int) * nnz, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(L.weights, geo->dnn_weights, sizeof(float) * N_W, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(L.slots, c->h_slots.data(), sizeof(Slot) * c->n_slots, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemset(c->zero_base, 0, c->zero_stride * c->n_slots);
+  if (e != cudaSuccess) { delete c; return LST_ECUDA; }
+  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
+  *out = c;
+  return LST_OK;
+}
+
+int lst_load_event(lst_ctx* c, int32_t slot, int32_t n_hits, const float* d_x, const float* d_y, const float* d_z,
+                   const uint32_t* d_key, int32_t n_pls, const float* d_px, const float* d_py, const float* d_pz,
+                   const float* d_z0, const int8_t* d_q, void* cuda_stream) {
+  if (!c || slot < 0 || slot >= c->n_slots || n_hits < 0 || n_pls < 0) return LST_EINVAL;
+  if (n_hits > c->caps.max_hits || n_pls > c->caps.max_pls) return LST_EINVAL;
+  if (n_hits > 0 && (!d_x || !d_y || !d_z || !d_key)) return LST_EINVAL;
+  if (n_pls > 0 && (!d_px || !d_py || !d_pz || !d_z0 || !d_q)) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  k_bind<<<1, 1, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->d_slots, slot, d_x, d_y, d_z, d_key, n_hits, d_px, d_py,
+                                                               d_pz, d_z0, d_q, n_pls);
+  return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
+}
+
+int lst_load_event_host(lst_ctx* c, int32_t slot, int32_t n_hits, const float* h_x, const float* h_y, const float* h_z,
+                        const uint32_t* h_key, int32_t n_pls, const float* h_px, const float* h_py, const float* h_pz,
+                        const float* h_z0, const int8_t* h_q, void* cuda_stream) {
+  if (!c || slot < 0 || slot >= c->n_slots || n_hits < 0 || n_pls < 0) return LST_EINVAL;
+  if (n_hits > c->caps.max_hits || n_pls > c->caps.max_pls) return LST_EINVAL;
+  if (n_hits > 0 && (!h_x || !h_y || !h_z || !h_key)) return LST_EINVAL;
+  if (n_pls > 0 && (!h_px || !h_py || !h_pz || !h_z0 || !h_q)) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const Slot& s = c->h_slots[slot];
+  cudaError_t e = cudaSuccess;
+  auto cp = [&](void* dst, const void* src, size_t n) {
+    if (e == cudaSuccess && n) e = cudaMemcpyAsync(dst, src, n, cudaMemcpyHostToDevice, st);
+  };
+  cp(s.st_x, h_x, sizeof(float) * n_hits); cp(s.st_y, h_y, sizeof(float) * n_hits); cp(s.st_z, h_z, sizeof(float) * n_hits);
+  cp(s.st_key, h_key, sizeof(uint32_t) * n_hits);
+  cp(s.st_px, h_px, sizeof(float) * n_pls); cp(s.st_py, h_py, sizeof(float) * n_pls); cp(s.st_pz, h_pz, sizeof(float) * n_pls);
+  cp(s.st_z0, h_z0, sizeof(float) * n_pls); cp(s.st_q, h_q, n_pls);
+  if (bad(c, e)) return LST_ECUDA;
+  return lst_load_event(c, slot, n_hits, s.st_x, s.st_y, s.st_z, s.st_key, n_pls, s.st_px, s.st_py, s.st_pz, s.st_z0,
+                        s.st_q, cuda_stream);
+}
+
+int lst_run_batch(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
+  if (!c || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const Slot* sl = c->d_slots + first;
+  const Geo g = c->geo;
+  const Caps k = c->caps;
+  if (bad(c, cudaMemsetAsync(c->zero_base + first * c->zero_stride, 0, c->zero_stride * n, st))) return LST_ECUDA;
+  if (bad(c, cudaMemsetAsync(c->ones_base + first * c->ones_stride, 0xFF, c->ones_stride * n, st))) return LST_ECUDA;
+  // x-extent of the grids: enough blocks to fill 148 SMs several times over across the whole batch
+  int gx = (148 * 8 + n - 1) / n;
+  if (gx < 8) gx = 8;
+  if (gx > 592) gx = 592;
+  const dim3 G(gx, n), G1(1, n);
+  k_hist<<<G, 256, 0, st>>>(sl, g);
+  k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
+  k_scatter<<<G, 256, 0, st>>>(sl, g);
+  k_rank<<<G, 256, 0, st>>>(sl);
+  k_md<false><<<G, 256, 0, st>>>(sl, g, k);
+  k_scan<SCAN_MD><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
+  k_md<true><<<G, 256, 0, st>>>(sl, g, k);
+  k_ls<false><<<G, 128, 0, st>>>(sl, g, k);
+  k_scan<SCAN_LS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
+  k_ls<true><<<G, 128, 0, st>>>(sl, g, k);
+  k_t3<false><<<G, 128, 0, st>>>(sl, k);
+  k_scan<SCAN_T3><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
+  k_t3<true><<<G, 128, 0, st>>>(sl, k);
+  k_t5<false><<<G, 128, 0, st>>>(sl, k);
+  k_scan<SCAN_T5C><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
+  k_t5<true><<<G, 128, 0, st>>>(sl, k);
+  k_dnn<<<G, 128, 0, st>>>(sl, g);
+  k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
+  k_pls<<<G, 128, 0, st>>>(sl);
+  k_match<5, false><<<G, 128, 0, st>>>(sl);
+  k_pt5_lists<<<G, 128, 0, st>>>(sl);
+  k_match<3, true><<<G, 128, 0, st>>>(sl);
+  k_tc_emit<<<G1, 1024, 0, st>>>(sl, k);
+  return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
+}
+
+int lst_run(lst_ctx* c, int32_t slot, void* cuda_stream) { return lst_run_batch(c, slot, 1, cuda_stream); }
+
+int lst_get(lst_ctx* c, int32_t slot, int32_t objtype, lst_view* v) {
+  if (!c || !v || slot < 0 || slot >= c->n_slots || objtype < 0 || objtype >= LST_N_OBJ) return LST_EINVAL;
+  const Slot& s = c->h_slots[slot];
+  *v = lst_view{};
+  auto I = [](const void* p) { return static_cast<const int32_t*>(p); };
+  switch (objtype) {
+    case LST_OBJ_HIT: v->capacity = c->caps.max_hits; v->count = s.cnt + LST_CNT_HIT; v->i0 = s.hit_orig; v->i1 = s.sensor_start;
+      v->f0 = reinterpret_cast<const float*>(s.hit); break;
+    case LST_OBJ_MD: v->capacity = c->caps.max_md; v->count = s.cnt + LST_CNT_MD; v->i0 = I(s.md_hits); v->i1 = s.md_modt;
+      v->i2 = s.md_start; v->f0 = reinterpret_cast<const float*>(s.md_pos); v->f1 = reinterpret_cast<const float*>(s.md_cw); break;
+    case LST_OBJ_LS: v->capacity = c->caps.max_ls; v->count = s.cnt + LST_CNT_LS; v->i0 = I(s.ls_ab); v->i1 = s.ls_start; v->f0 = s.ls_c; break;
+    case LST_OBJ_T3: v->capacity = c->caps.max_t3; v->count = s.cnt + LST_CNT_T3; v->i0 = I(s.t3_abc); v->i1 = s.t3_l1; v->i2 = s.t3_start;
+      v->f0 = s.t3_k; break;
+    case LST_OBJ_T5C: v->capacity = c->caps.max_t5c; v->count = s.cnt + LST_CNT_T5C; v->i0 = s.t5c_md; v->i1 = I(s.t5c_t3); v->i2 = s.t5c_pass;
+      v->f0 = s.t5c_curv; v->f1 = s.t5c_feat; v->f2 = s.t5c_score; break;
+    case LST_OBJ_T5: v->capacity = c->caps.max_t5; v->count = s.cnt + LST_CNT_T5; v->i0 = s.t5_list; break;
+    case LST_OBJ_TC: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TC; v->i0 = s.tc; break;
+    case LST_OBJ_MATCH5: v->capacity = c->caps.max_t5; v->count = s.cnt + LST_CNT_T5; v->i0 = s.best5; v->f0 = s.chi5; break;
+  }
+  return LST_OK;
+}
+
+int lst_status(lst_ctx* c, int32_t slot, uint32_t* status_bits, int32_t* counts, void* cuda_stream) {
+  if (!c || slot < 0 || slot >= c->n_slots) return LST_EINVAL;
+  int32_t tmp[LST_N_CNT];
+  if (bad(c, cudaStreamSynchronize(static_cast<cudaStream_t>(cuda_stream)))) return LST_ECUDA;
+  if (bad(c, cudaMemcpy(tmp, c->h_slots[slot].cnt, sizeof(tmp), cudaMemcpyDeviceToHost))) return LST_ECUDA;
+  if (status_bits) *status_bits = static_cast<uint32_t>(tmp[LST_N_CNT - 1]);
+  if (counts) for (int i = 0; i < LST_N_CNT; ++i) counts[i] = tmp[i];
+  return LST_OK;
+}
+
+int lst_read_tc_host(lst_ctx* c, int32_t slot, int32_t* h_counts, int32_t* h_tc, int32_t max_rows, void* cuda_stream) {
+  if (!c || slot < 0 || slot >= c->n_slots || !h_counts || max_rows < 0 || (max_rows > 0 && !h_tc)) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const Slot& s = c->h_slots[slot];
+  if (max_rows > c->caps.max_tc) max_rows = c->caps.max_tc;
+  if (bad(c, cudaMemcpyAsync(h_counts, s.cnt, sizeof(int32_t) * LST_N_CNT, cudaMemcpyDeviceToHost, st))) return LST_ECUDA;
+  if (max_rows > 0 && bad(c, cudaMemcpyAsync(h_tc, s.tc, sizeof(int32_t) * 3 * (size_t)max_rows, cudaMemcpyDeviceToHost, st)))
+    return LST_ECUDA;
+  return LST_OK;
+}
+
+void lst_destroy(lst_ctx* c) { delete c; }
+
+}  // extern "C"

@@ -1,0 +1,561 @@
+// lst_kernels.cuh -- sm_100a kernels of the LST chain (SPEC.md 4.0-4.6), batched over event slots.
+//
+// Launch geometry: every kernel takes the device array of slot descriptors and runs on a grid
+// (GX, n_events); blockIdx.y selects the slot, the x dimension grid-strides over that slot's items
+// (counts live in device memory -- lst_run never synchronises with the host).
+// Deterministic output order: every combinatorial stage is count -> exclusive scan -> fill, with one
+// thread owning one "inner" object (lower hit / inner MD / first LS / inner T3), so the object
+// order is the SPEC.md build order and capacity overflow is detected in the scan and flagged.
+#pragma once
+#include "lst_math.cuh"
+#include "../../include/lst.h"
+
+namespace lst {
+
+constexpr int N_FEAT = 23, N_HID = 32, N_W = 1857;
+constexpr int CNT_STATUS = LST_N_CNT - 1;
+constexpr unsigned long long WIN_EMPTY = 0xFFFFFFFFFFFFFFFFull;
+
+struct Geo {   // device copies, shared by all slots
+  int n_modules;
+  const uint8_t* modt;      // [M] subdet<<1 | mtype
+  const int* rowptr;        // [M+1]
+  const int* col;           // [nnz]
+  const float* weights;     // [1857]
+};
+
+struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
+
+struct Slot {
+  // bound inputs
+  const float *in_x, *in_y, *in_z; const uint32_t* in_key; int n_hits;
+  const float *in_px, *in_py, *in_pz, *in_z0; const int8_t* in_q; int n_pls;
+  // zero-initialised per run
+  int* cnt;                 // [LST_N_CNT]
+  int* sensor_start;        // [2M+1] histogram, then exclusive scan in place
+  int* cursor;              // [2M]
+  // 0xFF-initialised per run
+  unsigned long long* win5; // [max_pls]  (chi2 bits << 32 | T5 index)
+  unsigned long long* win3; // [max_pls]
+  int* md_head;             // [max_md]  head of the list of pT5 entries containing this MD
+  // a0
+  int* tmp_orig; float4* hit; int* hit_orig;
+  // a1
+  int* md_off; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; int* md_start;
+  // a2
+  int* ls_start; int2* ls_ab; float* ls_c;
+  // a3
+  int* t3_off; int4* t3_abc; int* t3_l1; float* t3_k; int* t3_start;
+  // a4 / a5
+  int* t5_off; int* t5c_md; int2* t5c_t3; float* t5c_curv; float* t5c_feat; float* t5c_score; int* t5c_pass;
+  int* t5_scan; int* t5_list;
+  // a6
+  float4* pls_a; float2* pls_b; int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
+  // host-load staging
+  float *st_x, *st_y, *st_z; uint32_t* st_key; float *st_px, *st_py, *st_pz, *st_z0; int8_t* st_q;
+};
+
+#define LST_FOR_ITEMS(i, n) \
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x, _st = gridDim.x * blockDim.x; i < (n); i += _st)
+
+// ------------------------------------------------------------------------------------------------
+// block-wide exclusive scan in place (one 1024-thread block): a[0..n) -> exclusive prefix clamped to
+// `cap`, a[n] = min(total, cap); returns the unclamped total to every thread.
+// ------------------------------------------------------------------------------------------------
+constexpr int SCAN_THREADS = 1024, SCAN_ITEMS = 8;
+
+__device__ __forceinline__ int block_scan_inplace(int* __restrict__ a, int n, int cap, int* sm /*[34]*/) {
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  int carry = 0;
+  for (int base = 0; base < n; base += SCAN_THREADS * SCAN_ITEMS) {
+    const int i0 = base + tid * SCAN_ITEMS;
+    int v[SCAN_ITEMS];
+    if (i0 + SCAN_ITEMS <= n) {
+      const int4 p = *reinterpret_cast<const int4*>(a + i0);
+      const int4 q = *reinterpret_cast<const int4*>(a + i0 + 4);
+      v[0] = p.x; v[1] = p.y; v[2] = p.z; v[3] = p.w; v[4] = q.x; v[5] = q.y; v[6] = q.z; v[7] = q.w;
+    } else {
+#pragma unroll
+      for (int k = 0; k < SCAN_ITEMS; ++k) v[k] = (i0 + k < n) ? a[i0 + k] : 0;
+    }
+    int tsum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) tsum += v[k];
+    int inc = tsum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, inc, d);
+      if (lane >= d) inc += t;
+    }
+    if (lane == 31) sm[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      int w = sm[lane];
+      int winc = w;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, winc, d);
+        if (lane >= d) winc += t;
+      }
+      sm[lane] = winc - w;            // exclusive prefix of warp totals
+      if (lane == 31) sm[32] = winc;  // block total
+    }
+    __syncthreads();
+    int run = carry + sm[wid] + (inc - tsum);
+    const int btot = sm[32];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+      const int e = min(run, cap);
+      run += v[k];
+      v[k] = e;
+    }
+    if (i0 + SCAN_ITEMS <= n) {
+      *reinterpret_cast<int4*>(a + i0) = make_int4(v[0], v[1], v[2], v[3]);
+      *reinterpret_cast<int4*>(a + i0 + 4) = make_int4(v[4], v[5], v[6], v[7]);
+    } else {
+#pragma unroll
+      for (int k = 0; k < SCAN_ITEMS; ++k)
+        if (i0 + k < n) a[i0 + k] = v[k];
+    }
+    carry += btot;
+    __syncthreads();
+  }
+  if (tid == 0) a[n] = min(carry, cap);
+  return carry;
+}
+
+enum { SCAN_SENSOR = 0, SCAN_MD, SCAN_LS, SCAN_T3, SCAN_T5C, SCAN_T5 };
+
+template <int MODE>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ int sm[34];
+  const Slot& s = slots[blockIdx.y];
+  int* cnt = s.cnt;
+  int* a; int n, cap, icnt, iraw; unsigned ovf;
+  if (MODE == SCAN_SENSOR) { a = s.sensor_start; n = 2 * geo.n_modules; cap = caps.max_hits; icnt = LST_CNT_HIT; iraw = -1; ovf = 0; }
+  else if (MODE == SCAN_MD) { a = s.md_off; n = cnt[LST_CNT_HIT]; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; }
+  else if (MODE == SCAN_LS) { a = s.ls_start; n = cnt[LST_CNT_MD]; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; }
+  else if (MODE == SCAN_T3) { a = s.t3_off; n = cnt[LST_CNT_LS]; cap = caps.max_t3; icnt = LST_CNT_T3; iraw = LST_CNT_RAW_T3; ovf = LST_ST_OVF_T3; }
+  else if (MODE == SCAN_T5C) { a = s.t5_off; n = cnt[LST_CNT_T3]; cap = caps.max_t5c; icnt = LST_CNT_T5C; iraw = LST_CNT_RAW_T5C; ovf = LST_ST_OVF_T5C; }
+  else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
+  __syncthreads();   // everyone has read n before thread 0 may overwrite counters below
+  const int total = block_scan_inplace(a, n, cap, sm);
+  if (threadIdx.x == 0) {
+    cnt[icnt] = min(total, cap);
+    if (iraw >= 0) cnt[iraw] = total;
+    if (total > cap) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), ovf);
+  }
+  __syncthreads();
+  // epilogues: range tables / compaction that fall out of the scan
+  if (MODE == SCAN_MD) {          // MDs of module m = [md_start[m], md_start[m+1])
+    for (int m = threadIdx.x; m <= geo.n_modules; m += SCAN_THREADS) s.md_start[m] = a[s.sensor_start[2 * m]];
+  } else if (MODE == SCAN_T3) {   // T3s whose inner MD is a = [t3_start[a], t3_start[a+1])
+    const int n_md = cnt[LST_CNT_MD];
+    for (int i = threadIdx.x; i <= n_md; i += SCAN_THREADS) s.t3_start[i] = a[s.ls_start[i]];
+  } else if (MODE == SCAN_T5) {   // T5 list = passing candidates in candidate order
+    for (int i = threadIdx.x; i < n; i += SCAN_THREADS)
+      if (s.t5c_pass[i] && a[i] < cap) s.t5_list[a[i]] = i;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a0: hit ingest (SPEC.md 4.0) -- histogram, scan (k_scan<SCAN_SENSOR>), scatter, in-sensor rank
+// ------------------------------------------------------------------------------------------------
+__global__ void k_hist(const Slot* __restrict__ slots, Geo geo) {
+  const Slot& s = slots[blockIdx.y];
+  const unsigned S = 2u * geo.n_modules;
+  LST_FOR_ITEMS(i, s.n_hits) {
+    const unsigned key = s.in_key[i];
+    if (key >= S) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_BAD_KEY);
+    else atomicAdd(s.sensor_start + key, 1);
+  }
+}
+__global__ void k_scatter(const Slot* __restrict__ slots, Geo geo) {
+  const Slot& s = slots[blockIdx.y];
+  const unsigned S = 2u * geo.n_modules;
+  LST_FOR_ITEMS(i, s.n_hits) {
+    const unsigned key = s.in_key[i];
+    if (key < S) s.tmp_orig[s.sensor_start[key] + atomicAdd(s.cursor + key, 1)] = i;
+  }
+}
+// stable order inside a sensor: rank of a hit = number of hits of the same sensor with a smaller
+// original index (sensors hold a handful of hits, so the quadratic count is cheap and exact)
+__global__ void k_rank(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = s.cnt[LST_CNT_HIT];
+  LST_FOR_ITEMS(p, n) {
+    const int o = s.tmp_orig[p];
+    const unsigned key = s.in_key[o];
+    const int b = s.sensor_start[key], e = s.sensor_start[key + 1];
+    int rank = 0;
+    for (int q = b; q < e; ++q) rank += (s.tmp_orig[q] < o);
+    const int d = b + rank;
+    s.hit[d] = make_float4(s.in_x[o], s.in_y[o], s.in_z[o], __int_as_float((int)key));
+    s.hit_orig[d] = o;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1: mini-doublets (SPEC.md 4.1).  One thread per lower-sensor hit; loops over the module's
+// upper-sensor hits (contiguous in the module-sorted store, L1-resident for the whole warp).
+// ------------------------------------------------------------------------------------------------
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_md(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = s.cnt[LST_CNT_HIT];
+  LST_FOR_ITEMS(p, n) {
+    const float4 h1 = s.hit[p];
+    const int key = __float_as_int(h1.w);
+    int count = 0;
+    if (!(key & 1)) {
+      const int m = key >> 1;
+      const int mt = geo.modt[m];
+      const int ub = s.sensor_start[key + 1], ue = s.sensor_start[key + 2];
+      const float r1 = fq(fa(fm(h1.x, h1.x), fm(h1.y, h1.y)));
+      int out = FILL ? s.md_off[p] : 0;
+      for (int j = ub; j < ue; ++j) {
+        const float4 h2 = s.hit[j];
+        float c, w;
+        if (!md_eval(h1.x, h1.y, h1.z, r1, h2.x, h2.y, h2.z, mt, c, w)) continue;
+        if (FILL) {
+          if (out < caps.max_md) {
+            s.md_hits[out] = make_int2(s.hit_orig[p], s.hit_orig[j]);
+            s.md_modt[out] = (m << 2) | mt;
+            s.md_pos[out] = make_float4(h1.x, h1.y, h1.z, r1);
+            s.md_cw[out] = make_float2(c, w);
+          }
+          ++out;
+        } else {
+          ++count;
+        }
+      }
+    }
+    if (!FILL) s.md_off[p] = count;
+  }
+}
+
+__device__ __forceinline__ Anchor load_anchor(const Slot& s, int i) {
+  const float4 p = s.md_pos[i];
+  const float2 cw = s.md_cw[i];
+  Anchor a; a.x = p.x; a.y = p.y; a.z = p.z; a.r = p.w; a.c = cw.x; a.w = cw.y; a.mt = s.md_modt[i] & 3;
+  return a;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2: line segments (SPEC.md 4.2).  One thread per inner MD; walks the CSR row of its module and
+// the MDs of each connected module.  Threads of a warp mostly share the module, so the inner loads
+// are warp-uniform (broadcast from L1).
+// ------------------------------------------------------------------------------------------------
+template <bool FILL>
+__global__ void __launch_bounds__(128) k_ls(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = s.cnt[LST_CNT_MD];
+  LST_FOR_ITEMS(a, n) {
+    const Anchor A = load_anchor(s, a);
+    const int m = s.md_modt[a] >> 2;
+    int out = FILL ? s.ls_start[a] : 0;
+    const int e1 = geo.rowptr[m + 1];
+    for (int e = geo.rowptr[m]; e < e1; ++e) {
+      const int m2 = geo.col[e];
+      const int b1 = s.md_start[m2 + 1];
+      for (int b = s.md_start[m2]; b < b1; ++b) {
+        const Anchor B = load_anchor(s, b);
+        float c;
+        if (!ls_eval(A, B, c)) continue;
+        if (FILL) {
+          if (out < caps.max_ls) { s.ls_ab[out] = make_int2(a, b); s.ls_c[out] = c; }
+        }
+        ++out;
+      }
+    }
+    if (!FILL) s.ls_start[a] = out;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3: triplets (SPEC.md 4.3).  One thread per first LS (a,b); loops over the LSs whose inner MD is b.
+// ------------------------------------------------------------------------------------------------
+template <bool FILL>
+__global__ void __launch_bounds__(128) k_t3(const Slot* __restrict__ slots, Caps caps) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = s.cnt[LST_CNT_LS];
+  LST_FOR_ITEMS(l0, n) {
+    const int2 ab = s.ls_ab[l0];
+    const int j1 = s.ls_start[ab.y + 1];
+    int j = s.ls_start[ab.y];
+    int out = FILL ? s.t3_off[l0] : 0;
+    if (j < j1) {
+      const Pt A = make_pt(s.md_pos[ab.x], s.md_modt[ab.x] & 3);
+      const Pt B = make_pt(s.md_pos[ab.y], s.md_modt[ab.y] & 3);
+      const float c0 = s.ls_c[l0];
+      for (; j < j1; ++j) {
+        const int cidx = s.ls_ab[j].y;
+        const Pt C = make_pt(s.md_pos[cidx], s.md_modt[cidx] & 3);
+        float k;
+        if (!triplet_eval(A, B, C, k)) continue;
+        if (!(fabsf(fs(c0, k)) <= LST_C_TOL3)) continue;                                  // T3
+        if (!(fabsf(fs(s.ls_c[j], k)) <= LST_C_TOL3)) continue;
+        if (FILL) {
+          if (out < caps.max_t3) { s.t3_abc[out] = make_int4(ab.x, ab.y, cidx, l0); s.t3_l1[out] = j; s.t3_k[out] = k; }
+        }
+        ++out;
+      }
+    }
+    if (!FILL) s.t3_off[l0] = out;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4: quintuplet candidates (SPEC.md 4.4).  One thread per inner T3 (a,b,c); loops over the T3s
+// whose inner MD is c and tests the bridge (b,c,d).
+// ------------------------------------------------------------------------------------------------
+template <bool FILL>
+__global__ void __launch_bounds__(128) k_t5(const Slot* __restrict__ slots, Caps caps) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = s.cnt[LST_CNT_T3];
+  LST_FOR_ITEMS(u, n) {
+    const int4 abc = s.t3_abc[u];
+    const int v1 = s.t3_start[abc.z + 1];
+    int v = s.t3_start[abc.z];
+    int out = FILL ? s.t5_off[u] : 0;
+    if (v < v1) {
+      const Pt B = make_pt(s.md_pos[abc.y], s.md_modt[abc.y] & 3);
+      const Pt C = make_pt(s.md_pos[abc.z], s.md_modt[abc.z] & 3);
+      for (; v < v1; ++v) {
+        const int4 cde = s.t3_abc[v];
+        const Pt D = make_pt(s.md_pos[cde.y], s.md_modt[cde.y] & 3);
+        float kbr;
+        if (!triplet_eval(B, C, D, kbr)) continue;                                        // Q1, Q2
+        if (FILL) {
+          if (out < caps.max_t5c) {
+            int* md = s.t5c_md + 5 * out;
+            md[0] = abc.x; md[1] = abc.y; md[2] = abc.z; md[3] = cde.y; md[4] = cde.z;
+            s.t5c_t3[out] = make_int2(u, v);
+            float* cv = s.t5c_curv + 3 * out;
+            cv[0] = s.t3_k[u]; cv[1] = kbr; cv[2] = s.t3_k[v];
+          }
+        }
+        ++out;
+      }
+    }
+    if (!FILL) s.t5_off[u] = out;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5: T5-DNN (SPEC.md 4.5).  One thread per candidate; features, hidden activations and the
+// running sums stay in registers, the 1857 weights sit in shared memory and are read as
+// warp-uniform (broadcast) float4s.  FMA is allowed here (scores agree with the oracle to 1e-5).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_dnn(const Slot* __restrict__ slots, Geo geo) {
+  __shared__ __align__(16) float W1[N_HID * 24];   // rows padded 23 -> 24 for float4 reads
+  __shared__ __align__(16) float W2[N_HID * N_HID];
+  __shared__ float B1[N_HID], B2[N_HID], W3[N_HID + 1];
+  for (int i = threadIdx.x; i < N_HID * 24; i += blockDim.x) {
+    const int j = i / 24, k = i - 24 * j;
+    W1[i] = (k < N_FEAT) ? geo.weights[j * N_FEAT + k] : 0.0f;
+  }
+  for (int i = threadIdx.x; i < N_HID * N_HID; i += blockDim.x) W2[i] = geo.weights[N_HID * N_FEAT + N_HID + i];
+  if (threadIdx.x < N_HID) {
+    B1[threadIdx.x] = geo.weights[N_HID * N_FEAT + threadIdx.x];
+    B2[threadIdx.x] = geo.weights[N_HID * N_FEAT + N_HID + N_HID * N_HID + threadIdx.x];
+    W3[threadIdx.x] = geo.weights[N_HID * N_FEAT + 2 * N_HID + N_HID * N_HID + threadIdx.x];
+  }
+  if (threadIdx.x == 0) W3[N_HID] = geo.weights[N_W - 1];
+  __syncthreads();
+  const Slot& s = slots[blockIdx.y];
+  const int n = s.cnt[LST_CNT_T5C];
+  LST_FOR_ITEMS(i, n) {
+    float x[24];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      const float4 p = s.md_pos[s.t5c_md[5 * i + q]];
+      x[4 * q + 0] = p.w * 0.01f;
+      x[4 * q + 1] = p.z * 0.01f;
+      x[4 * q + 2] = asinhf(__fdiv_rn(p.z, p.w));
+      x[4 * q + 3] = atan2f(p.y, p.x);
+    }
+#pragma unroll
+    for (int q = 0; q < 3; ++q) x[20 + q] = log10f(fminf(__fdiv_rn(1.0f, fabsf(s.t5c_curv[3 * i + q])), 1.0e5f));
+    x[23] = 0.0f;
+    float* fo = s.t5c_feat + (size_t)N_FEAT * i;
+#pragma unroll
+    for (int k = 0; k < N_FEAT; ++k) fo[k] = x[k];
+    float h1[N_HID];
+#pragma unroll
+    for (int j = 0; j < N_HID; ++j) {
+      float acc = B1[j];
+#pragma unroll
+      for (int k = 0; k < 24; k += 4) {
+        const float4 w = *reinterpret_cast<const float4*>(&W1[j * 24 + k]);
+        acc = fmaf(w.x, x[k], acc); acc = fmaf(w.y, x[k + 1], acc); acc = fmaf(w.z, x[k + 2], acc); acc = fmaf(w.w, x[k + 3], acc);
+      }
+      h1[j] = fmaxf(acc, 0.0f);
+    }
+    float y = W3[N_HID];
+#pragma unroll
+    for (int j = 0; j < N_HID; ++j) {
+      float acc = B2[j];
+#pragma unroll
+      for (int k = 0; k < N_HID; k += 4) {
+        const float4 w = *reinterpret_cast<const float4*>(&W2[j * N_HID + k]);
+        acc = fmaf(w.x, h1[k], acc); acc = fmaf(w.y, h1[k + 1], acc); acc = fmaf(w.z, h1[k + 2], acc); acc = fmaf(w.w, h1[k + 3], acc);
+      }
+      y = fmaf(W3[j], fmaxf(acc, 0.0f), y);
+    }
+    const float score = __fdiv_rn(1.0f, 1.0f + expf(-y));
+    const int pass = score > 0.5f;
+    s.t5c_score[i] = score;
+    s.t5c_pass[i] = pass;
+    s.t5_scan[i] = pass;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a6: track candidates (SPEC.md 4.6)
+// ------------------------------------------------------------------------------------------------
+__global__ void k_pls(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  LST_FOR_ITEMS(p, s.n_pls) {
+    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], (int)s.in_q[p]);
+    s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
+    s.pls_b[p] = make_float2(d.sec, d.z0);
+  }
+}
+
+__device__ __forceinline__ unsigned long long win_key(float chi2, int idx) {
+  return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned)idx;   // chi2 >= 0: bit order = value order
+}
+
+// match objects with NA anchors against every pLS: one thread per object, pLS loop in ascending p so
+// that a strict '<' keeps the smallest p on ties (argmin over (chi2, p)).
+template <int NA, bool IS_T3>
+__global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
+  const int n_pls = s.n_pls;
+  LST_FOR_ITEMS(t, n) {
+    int md[NA];
+    if (IS_T3) {
+      const int4 abc = s.t3_abc[t];
+      md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
+      // used iff {a,b,c} is contained in the five MDs of some pT5: walk the entries that contain a
+      bool used = false;
+      for (int e = s.md_head[abc.x]; e >= 0 && !used; e = s.pt5_next[e]) {
+        const int pp = e / 5;
+        const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(s.win5[pp] & 0xFFFFFFFFull)];
+        int found = 0;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) found += (m5[q] == abc.y) + (m5[q] == abc.z);
+        used = (found == 2);
+      }
+      if (used) { s.best3[t] = -1; continue; }
+    } else {
+      const int* m5 = s.t5c_md + 5 * s.t5_list[t];
+#pragma unroll
+      for (int q = 0; q < NA; ++q) md[q] = m5[q];
+    }
+    const float4 a0 = s.md_pos[md[0]];
+    const int mt0 = s.md_modt[md[0]] & 3;
+    int best = -1;
+    float bchi = 0.0f;
+    for (int p = 0; p < n_pls; ++p) {
+      const float4 pa = s.pls_a[p];
+      Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
+      float e, dT;
+      if (!pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT)) continue;       // cheap transverse early-out
+      if (IS_T3 && s.win5[p] != WIN_EMPTY) continue;                  // pLS already in a pT5
+      const float2 pb = s.pls_b[p];
+      P.sec = pb.x; P.z0 = pb.y;
+      float chi = 0.0f;
+      bool ok = pls_anchor(P, a0, mt0, chi);
+#pragma unroll
+      for (int q = 1; q < NA; ++q)
+        if (ok) ok = pls_anchor(P, s.md_pos[md[q]], s.md_modt[md[q]] & 3, chi);
+      if (!ok) continue;
+      if (best < 0 || chi < bchi) { best = p; bchi = chi; }
+    }
+    if (IS_T3) { s.best3[t] = best; s.chi3[t] = bchi; if (best >= 0) atomicMin(s.win3 + best, win_key(bchi, t)); }
+    else { s.best5[t] = best; s.chi5[t] = bchi; if (best >= 0) atomicMin(s.win5 + best, win_key(bchi, t)); }
+  }
+}
+
+// per-MD lists of the pT5 entries (p, q) that contain the MD, for the "T3 already in a pT5" test
+__global__ void k_pt5_lists(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  LST_FOR_ITEMS(p, s.n_pls) {
+    const unsigned long long w = s.win5[p];
+    if (w == WIN_EMPTY) continue;
+    const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(w & 0xFFFFFFFFull)];
+    for (int q = 0; q < 5; ++q) {
+      const int e = 5 * p + q;
+      s.pt5_next[e] = atomicExch(s.md_head + m5[q], e);
+    }
+  }
+}
+
+// ordered emission of the four candidate types: one block per event, four flag-scan-write sweeps
+__global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots, Caps caps) {
+  __shared__ int sm[34];
+  const Slot& s = slots[blockIdx.y];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int n_pls = s.n_pls, n_t5 = s.cnt[LST_CNT_T5];
+  int base_out = 0;
+  int n_type[4];
+  for (int type = 0; type < 4; ++type) {
+    const int n = (type == 1) ? n_t5 : n_pls;
+    const int start_out = base_out;
+    for (int base = 0; base < n; base += 1024) {
+      const int i = base + tid;
+      int flag = 0, obj = -1;
+      if (i < n) {
+        if (type == 1) { flag = s.best5[i] < 0; obj = i; }
+        else {
+          const unsigned long long w5 = s.win5[i], w3 = s.win3[i];
+          if (type == 0) { flag = w5 != WIN_EMPTY; obj = (int)(w5 & 0xFFFFFFFFull); }
+          else if (type == 2) { flag = (w5 == WIN_EMPTY) && (w3 != WIN_EMPTY); obj = (int)(w3 & 0xFFFFFFFFull); }
+          else { flag = (w5 == WIN_EMPTY) && (w3 == WIN_EMPTY); obj = -1; }
+        }
+      }
+      const unsigned bal = __ballot_sync(0xffffffffu, flag);
+      if (lane == 0) sm[wid] = __popc(bal);
+      __syncthreads();
+      if (wid == 0) {
+        const int w = sm[lane];
+        int winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const int t = __shfl_up_sync(0xffffffffu, winc, d);
+          if (lane >= d) winc += t;
+        }
+        sm[lane] = winc - w;
+        if (lane == 31) sm[32] = winc;
+      }
+      __syncthreads();
+      if (flag) {
+        const int o = base_out + sm[wid] + __popc(bal & ((1u << lane) - 1u));
+        if (o < caps.max_tc) { s.tc[3 * o] = type; s.tc[3 * o + 1] = (type == 1) ? -1 : i; s.tc[3 * o + 2] = obj; }
+      }
+      base_out += sm[32];
+      __syncthreads();
+    }
+    n_type[type] = base_out - start_out;
+  }
+  if (tid == 0) {
+    s.cnt[LST_CNT_PT5] = n_type[0]; s.cnt[LST_CNT_T5TC] = n_type[1]; s.cnt[LST_CNT_PT3] = n_type[2]; s.cnt[LST_CNT_PLSTC] = n_type[3];
+    s.cnt[LST_CNT_RAW_TC] = base_out;
+    s.cnt[LST_CNT_TC] = min(base_out, caps.max_tc);
+    if (base_out > caps.max_tc) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_TC);
+  }
+}
+
+// binds an event to a slot (stream-ordered, so a later lst_run on the same stream sees it)
+__global__ void k_bind(Slot* slots, int slot, const float* x, const float* y, const float* z, const uint32_t* key,
+                       int n_hits, const float* px, const float* py, const float* pz, const float* z0,
+                       const int8_t* q, int n_pls) {
+  Slot& s = slots[slot];
+  s.in_x = x; s.in_y = y; s.in_z = z; s.in_key = key; s.n_hits = n_hits;
+  s.in_px = px; s.in_py = py; s.in_pz = pz; s.in_z0 = z0; s.in_q = q; s.n_pls = n_pls;
+}
+
+}  // namespace lst

@@ -1,0 +1,170 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle.  `-m gpu` only."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from lstgen import build_geometry, make_event, config_event, xavier_weights
+import parity
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2403_13166_b200 as P
+    P.load_library()      # fails loudly if the extension is missing
+    return P
+
+
+def _run_one(P, geo, w, ev, caps=None):
+    lst = P.LST(geo, w, caps or P.default_caps(1))
+    lst.load_numpy_event(0, ev)
+    lst.lst_run(0)
+    out = lst.fetch(0)
+    lst.close()
+    return out
+
+
+def test_config0_barrel_toy(P, geo_barrel):
+    w = xavier_weights(1)
+    ev = config_event(geo_barrel, 0)
+    c = parity.compare(geo_barrel, w, ev, _run_one(P, geo_barrel, w, ev))
+    assert c["md"] == 60 and c["t5c"] == 20
+
+
+def test_config1_pu50(P, geo_full):
+    w = xavier_weights(2)
+    ev = config_event(geo_full, 1)
+    c = parity.compare(geo_full, w, ev, _run_one(P, geo_full, w, ev))
+    assert c["t5c"] > 500
+
+
+def test_config2_pu200_headline(P, geo_full):
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 2)
+    c = parity.compare(geo_full, w, ev, _run_one(P, geo_full, w, ev))
+    assert c["md"] > 10000 and c["tc"] > 2000
+
+
+@pytest.mark.parametrize("pileup", [0, 100, 300])
+def test_config4_displaced_stress(P, geo_full, pileup):
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 4, seed=200 + pileup // 100, pileup=pileup)
+    out = _run_one(P, geo_full, w, ev)
+    assert out["status"] == 0
+    parity.compare(geo_full, w, ev, out)
+
+
+def test_biased_weights_balanced_decisions(P, geo_full):
+    """Weights with biases put many scores on both sides of 0.5, so the decision comparison bites."""
+    w = xavier_weights(5, bias_scale=0.5)
+    w[-1] = -0.6
+    ev = config_event(geo_full, 2, seed=77)
+    out = _run_one(P, geo_full, w, ev)
+    frac = out["t5c"]["pass"].mean()
+    assert 0.05 < frac < 0.95
+    parity.compare(geo_full, w, ev, out)
+
+
+def test_empty_and_degenerate_events(P, geo_full):
+    w = xavier_weights(3)
+    ev = make_event(geo_full, 9)                                  # no hits, no pLS
+    out = _run_one(P, geo_full, w, ev)
+    assert out["status"] == 0 and all(out["counts"][k] == 0 for k in ("hit", "md", "ls", "t3", "t5c", "t5", "tc"))
+    ev = make_event(geo_full, 9, n_noise=500)                     # hits but nothing to build, no pLS
+    parity.compare(geo_full, w, ev, _run_one(P, geo_full, w, ev))
+    ev = config_event(geo_full, 1, seed=12)                       # pLS only: every seed becomes a pLS candidate
+    ev.x = ev.x[:0]; ev.y = ev.y[:0]; ev.z = ev.z[:0]; ev.key = ev.key[:0]
+    out = _run_one(P, geo_full, w, ev)
+    assert out["counts"]["plstc"] == ev.n_pls == out["counts"]["tc"]
+    parity.compare(geo_full, w, ev, out)
+
+
+def test_bad_key_is_flagged(P, geo_full):
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 1, seed=13)
+    ev.key[5] = 2 * geo_full.n_modules
+    ev.key[9] = 0xFFFFFFFF
+    out = _run_one(P, geo_full, w, ev)
+    assert out["status"] & P.STATUS_BITS["bad_key"]
+    assert out["counts"]["hit"] == ev.n_hits - 2
+    parity.compare(geo_full, w, ev, out)
+
+
+def test_every_overflow_flag(P, geo_full):
+    """configs[4]: shrink each capacity in turn; the stage keeps the first `cap` objects in build
+    order, flags the overflow and reports the unclamped total."""
+    from oracle import lst_oracle as O
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 1)
+    ref = O.run(geo_full, w, ev)
+    full = dict(max_md=ref.counts["md"], max_ls=ref.counts["ls"], max_t3=ref.counts["t3"], max_t5c=ref.counts["t5c"], max_t5=ref.counts["t5"])
+    for name, bit, cnt in [("max_md", "ovf_md", "md"), ("max_ls", "ovf_ls", "ls"), ("max_t3", "ovf_t3", "t3"),
+                           ("max_t5c", "ovf_t5c", "t5c"), ("max_t5", "ovf_t5", "t5")]:
+        kw = dict(n_slots=1, max_hits=32768, max_pls=2048, max_md=16384, max_ls=16384, max_t3=16384, max_t5c=16384, max_t5=16384)
+        kw[name] = full[name] // 2
+        out = _run_one(P, geo_full, w, ev, P.Caps(**kw))
+        assert out["status"] & P.STATUS_BITS[bit], name
+        assert out["counts"][cnt] == kw[name] and out["counts"]["raw_" + cnt] == full[name]
+        if name == "max_md":
+            assert np.array_equal(out["md"]["hits"], ref.md_hits[:kw[name]])
+        if name == "max_ls":
+            assert np.array_equal(out["ls"]["ab"], ref.ls[:kw[name]])
+    # exact fit: no flag
+    kw = dict(n_slots=1, max_hits=ev.n_hits, max_pls=ev.n_pls, **full)
+    out = _run_one(P, geo_full, w, ev, P.Caps(**kw))
+    assert out["status"] == 0
+    parity.compare(geo_full, w, ev, out)
+
+
+def test_batch_equals_single_and_is_deterministic(P, geo_full):
+    """configs[3] in small: a batched launch over several slots = each event alone; repeated runs
+    give identical bytes."""
+    import torch
+    w = xavier_weights(3)
+    evs = [config_event(geo_full, 2, seed=100 + i) for i in range(4)] + [make_event(geo_full, 1), config_event(geo_full, 1, seed=5)]
+    lst = P.LST(geo_full, w, P.default_caps(len(evs)))
+    for i, ev in enumerate(evs):
+        lst.load_numpy_event(i, ev)
+    lst.lst_run_batch(0, len(evs))
+    first = [lst.fetch(i) for i in range(len(evs))]
+    for i, ev in enumerate(evs):
+        parity.compare(geo_full, w, ev, first[i])
+    for _ in range(3):
+        lst.lst_run_batch(0, len(evs))
+        again = [lst.fetch(i) for i in range(len(evs))]
+        for a, b in zip(first, again):
+            for obj in ("md", "ls", "t3", "t5c", "t5", "tc", "match5"):
+                for k in a[obj]:
+                    assert np.array_equal(a[obj][k].view(np.int32) if a[obj][k].dtype == np.float32 else a[obj][k],
+                                          b[obj][k].view(np.int32) if b[obj][k].dtype == np.float32 else b[obj][k]), (obj, k)
+    # streams: two halves on two streams
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    lst.lst_run_batch(0, 3, s1); lst.lst_run_batch(3, 3, s2)
+    torch.cuda.synchronize()
+    for i, ev in enumerate(evs):
+        parity.compare(geo_full, w, ev, lst.fetch(i))
+    lst.close()
+
+
+def test_host_load_path(P, geo_full):
+    import torch
+    w = xavier_weights(2)
+    ev = config_event(geo_full, 1, seed=21)
+    lst = P.LST(geo_full, w, P.default_caps(1))
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    args = [pin(ev.x), pin(ev.y), pin(ev.z), pin(ev.key.view(np.int32)), pin(ev.pls_px), pin(ev.pls_py), pin(ev.pls_pz), pin(ev.pls_z0), pin(ev.pls_q)]
+    lst.lst_load_event_host(0, *args)
+    lst.lst_run(0)
+    h_cnt = torch.zeros(32, dtype=torch.int32).pin_memory()
+    h_tc = torch.zeros((lst.caps.max_pls + lst.caps.max_t5, 3), dtype=torch.int32).pin_memory()
+    lst.lst_read_tc_host(0, h_cnt, h_tc)
+    torch.cuda.synchronize()
+    out = lst.fetch(0)
+    parity.compare(geo_full, w, ev, out)
+    n = int(h_cnt[P.CNT["tc"]])
+    assert n == out["counts"]["tc"] and np.array_equal(h_tc[:n].numpy(), out["tc"]["tc"].reshape(-1, 3))
+    lst.close()
