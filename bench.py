@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of the whole LST hot path (a0 ingest -> MD -> LS -> T3 -> T5 + DNN -> TC) at PU200.
+
+Contract (one JSON line on stdout from rank 0):
+  python bench.py --gpus N --steps K --warmup W            our CUDA path through the C ABI
+  python bench.py --impl reference ...                     the CPU oracle, as it stands, on host cores
+
+A "step" = one pass of the whole hot path over one batch of `--events` synthetic PU200 events
+(BASELINE.json configs[2] recipe, the seeds of configs[3]); `value` = events/s with the inputs resident
+in HBM; `e2e` = the same through lst_load_event_host / lst_read_tc_host with pinned HOST buffers, copies
+inside the timed region.  Events are independent, so N GPUs run N replicas on different seeds (weak
+scaling, no collective on the data path -- DESIGN.md "Multi-GPU").
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "events/s at PU200 (MD->LS->T3->T5+DNN->TC)"
+UNIT = "events/s"
+WORKLOAD = "configs[2] HL-LHC PU200 events (6000 particles, 5% inefficiency, 10000 noise hits), seeds 100.. as in configs[3]"
+
+# ---- per-unit algorithmic work: un-fused fp32 operations per pair test and
+# compulsory bytes per object; FP32 non-fused peak = 148 SM x 128 lanes x sm_max_mhz.
+FLOPS = dict(md_pair=34, ls_pair=62, t3_pair=86, t5_pair=80, dnn_cand=3584 + 140, match_pair=10, match_full=45)
+SM_COUNT, LANES = 148, 128
+
+
+def shard_seeds(rank: int, world: int, n_events: int, base: int = 100):
+    """Event seeds of one rank: every rank gets its own `n_events` (weak scaling)."""
+    return [base + rank * n_events + i for i in range(n_events)]
+
+
+def aggregate(local_ms_per_step: float, local_events_per_step: int, world: int, reduce_max=None, reduce_sum=None):
+    """Whole-job throughput = all ranks' events / the slowest rank's time."""
+    t = local_ms_per_step if reduce_max is None else reduce_max(local_ms_per_step)
+    n = local_events_per_step * world if reduce_sum is None else reduce_sum(local_events_per_step)
+    return n / (t * 1e-3), t
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def make_events(geo, seeds):
+    from lstgen import config_event
+    return [config_event(geo, 2, seed=s) for s in seeds]
+
+
+# ------------------------------------------------------------------------------------------------
+def algorithmic_work(lst, geo, slots):
+    """Pair-test counts, bytes and flops per stage, summed over `slots`, from the device-side range
+    tables of a finished run (pure bookkeeping, never the oracle)."""
+    import torch
+    M = geo.n_modules
+    rowptr = torch.from_numpy(geo.conn_rowptr.astype(np.int64)).to(lst.device)
+    col = torch.from_numpy(geo.conn_col.astype(np.int64)).to(lst.device)
+    tot = dict(hits=0, md_pairs=0, md=0, ls_pairs=0, ls=0, t3_pairs=0, t3=0, t5_pairs=0, t5c=0, t5=0, pls=0, tc=0, match5=0, match3=0)
+    for s in slots:
+        _, c = lst.lst_status(s)
+        rg = lst.ranges(s, c)
+        ss = rg["sensor_start"].long()
+        n_lo, n_up = ss[1:2 * M:2] - ss[0:2 * M:2], ss[2:2 * M + 1:2] - ss[1:2 * M:2]
+        nmd = (rg["md_start"][1:] - rg["md_start"][:-1]).long()
+        cs = torch.cat([torch.zeros(1, dtype=torch.long, device=lst.device), torch.cumsum(nmd[col], 0)])
+        cand = cs[rowptr[1:]] - cs[rowptr[:-1]]
+        nls_in = (rg["ls_start"][1:] - rg["ls_start"][:-1]).long()
+        nt3_in = (rg["t3_start"][1:] - rg["t3_start"][:-1]).long()
+        ls_b = lst.lst_get(s, "ls", c["ls"])["ab"].view(-1, 2)[:, 1].long()
+        t3_c = lst.lst_get(s, "t3", c["t3"])["abc"].view(-1, 4)[:, 2].long()
+        n_pls = lst.n_pls[s]
+        tot["hits"] += c["hit"]; tot["md"] += c["md"]; tot["ls"] += c["ls"]; tot["t3"] += c["t3"]; tot["t5c"] += c["t5c"]
+        tot["t5"] += c["t5"]; tot["tc"] += c["tc"]; tot["pls"] += n_pls
+        tot["md_pairs"] += int((n_lo * n_up).sum()); tot["ls_pairs"] += int((nmd * cand).sum())
+        tot["t3_pairs"] += int(nls_in[ls_b].sum()) if c["ls"] else 0
+        tot["t5_pairs"] += int(nt3_in[t3_c].sum()) if c["t3"] else 0
+        tot["match5"] += c["t5"] * n_pls; tot["match3"] += c["t3"] * n_pls
+    nnz, nslot = int(geo.conn_col.size), len(slots)
+    stages = {
+        # compulsory bytes: each input once, each output once
+        "a0": dict(bytes=tot["hits"] * (16 + 16 + 4 + 4) + nslot * 2 * M * 4 * 2, flops=0),
+        "a1": dict(bytes=tot["hits"] * 20 + nslot * M * 8 + tot["md"] * 36, flops=FLOPS["md_pair"] * tot["md_pairs"]),
+        "a2": dict(bytes=tot["md"] * 28 + nslot * (nnz + M) * 4 + tot["ls"] * 12, flops=FLOPS["ls_pair"] * tot["ls_pairs"]),
+        "a3": dict(bytes=tot["ls"] * 12 + tot["md"] * 20 + tot["t3"] * 24, flops=FLOPS["t3_pair"] * tot["t3_pairs"]),
+        "a4": dict(bytes=tot["t3"] * 24 + tot["md"] * 20 + tot["t5c"] * 40, flops=FLOPS["t5_pair"] * tot["t5_pairs"]),
+        "a5": dict(bytes=tot["t5c"] * (32 + 80 + 92 + 12) + nslot * 7428, flops=FLOPS["dnn_cand"] * tot["t5c"]),
+        "a6": dict(bytes=tot["pls"] * 17 + tot["t5"] * 24 + tot["t3"] * 16 + tot["tc"] * 12,
+                   flops=FLOPS["match_pair"] * (tot["match5"] + tot["match3"]) + FLOPS["match_full"] * (5 * tot["t5"] + 3 * tot["t3"])),
+    }
+    return tot, stages
+
+
+def stage_of(name):
+    return name.split(".")[0]
+
+
+def run_ours(args):
+    import torch
+    import paper_2403_13166_b200 as P
+    from lstgen import build_geometry, xavier_weights
+    rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
+    assert world == args.gpus or world == 1, (world, args.gpus)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    P.load_library()
+    geo = build_geometry(True)
+    w = xavier_weights(3)
+    E, S = args.events, args.streams
+    assert E % S == 0
+    events = make_events(geo, shard_seeds(rank, world, E))
+    caps = P.Caps(n_slots=E, max_hits=114688, max_md=49152, max_ls=49152, max_t3=32768, max_t5c=16384, max_t5=16384, max_pls=4096)
+    lst = P.LST(geo, w, caps, device=dev)
+    lst.n_pls = [ev.n_pls for ev in events]
+    streams = [torch.cuda.Stream(device=dev) for _ in range(S)]
+    main = torch.cuda.current_stream(dev)
+    for i, ev in enumerate(events):
+        lst.load_numpy_event(i, ev)
+    torch.cuda.synchronize()
+    per = E // S
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        if S == 1:
+            lst.lst_run_batch(0, E, main)
+            return
+        ev0 = torch.cuda.Event(); ev0.record(main)
+        for si, st in enumerate(streams):
+            st.wait_event(ev0)
+            lst.lst_run_batch(si * per, per, st)
+            e = torch.cuda.Event(); e.record(st); main.wait_event(e)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    for i in range(E):     # a run with any status bit set is a failed run
+        bits, c = lst.lst_status(i)
+        assert bits == 0 and c["md"] > 0 and c["tc"] > 0, (i, bits, c)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: K steps, per-step CUDA events, L2 flushed (256 MiB write) between steps ----
+    sampler = ClockSampler(local); sampler.start()
+    barrier()
+    t_wall = time.perf_counter()
+    evs = []
+    for _ in range(args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(main); step(); b.record(main)
+        evs.append((a, b))
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    ms_local = float(np.mean(step_ms))
+
+    # ---- e2e: pinned host inputs -> H2D -> chain -> D2H of counters + TC rows, every step --------
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    host_in = [[pin(ev.x), pin(ev.y), pin(ev.z), pin(ev.key.view(np.int32)), pin(ev.pls_px), pin(ev.pls_py), pin(ev.pls_pz),
+                pin(ev.pls_z0), pin(ev.pls_q)] for ev in events]
+    TC_ROWS = 8192
+    h_cnt = [torch.zeros(32, dtype=torch.int32).pin_memory() for _ in range(E)]
+    h_tc = [torch.zeros((TC_ROWS, 3), dtype=torch.int32).pin_memory() for _ in range(E)]
+    h2d = sum(ev.n_hits * 16 + ev.n_pls * 17 for ev in events)
+    d2h = E * (32 * 4 + TC_ROWS * 12)
+    e2e_streams = streams if S > 1 else [main]
+
+    def e2e_step():
+        for si, st in enumerate(e2e_streams):
+            lo = si * (E // len(e2e_streams)); n = E // len(e2e_streams)
+            for i in range(lo, lo + n):
+                lst.lst_load_event_host(i, *host_in[i], stream=st)
+            lst.lst_run_batch(lo, n, st)
+            for i in range(lo, lo + n):
+                lst.lst_read_tc_host(i, h_cnt[i], h_tc[i], stream=st)
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    barrier()
+    e2e_ms_local = (time.perf_counter() - t0) * 1e3 / args.steps
+    for i in range(E):
+        assert int(h_cnt[i][31]) == 0 and 0 < int(h_cnt[i][P.CNT["tc"]]) <= TC_ROWS, "e2e run failed or TC rows truncated"
+    # rebind the resident inputs for the profile pass
+    for i, ev in enumerate(events):
+        lst.load_numpy_event(i, ev)
+    torch.cuda.synchronize()
+
+    # ---- per-kernel device times (same launch configuration as the timed region) ------------------
+    prof = {}
+    reps = 5
+    for r in range(reps + 1):
+        flush.zero_()
+        torch.cuda.synchronize()
+        if S == 1:
+            d = lst.lst_run_batch_profile(0, E, main)
+        else:       # one stream's share of the batch; the S streams run the same sequence concurrently
+            d = lst.lst_run_batch_profile(0, per, main)
+        if r:       # first one is warm-up
+            for k, v in d.items():
+                prof[k] = prof.get(k, 0.0) + v / reps
+    n_prof = E if S == 1 else per
+    tot, stages = algorithmic_work(lst, geo, range(n_prof))
+
+    def red_max(v):
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); return float(t.item())
+
+    value, ms = aggregate(ms_local, E, world, red_max)
+    e2e_value, e2e_ms = aggregate(e2e_ms_local, E, world, red_max)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    alu_peak = SM_COUNT * LANES * pk["sm_max_mhz"] * 1e6 / 1e12          # Tflop/s, un-fused mul/add
+    fma_peak = 2 * alu_peak
+    stage_ms = {}
+    for k, v in prof.items():
+        if k != "memset":
+            stage_ms[stage_of(k)] = stage_ms.get(stage_of(k), 0.0) + v
+    stage_ms["a0"] += prof.get("memset", 0.0)
+    stage_rows = {}
+    for st_name, wk in stages.items():
+        t_s = stage_ms[st_name] * 1e-3
+        peak_f = fma_peak if st_name == "a5" else alu_peak
+        t_hbm, t_alu = wk["bytes"] / (pk["hbm_gbs"] * 1e9), wk["flops"] / (peak_f * 1e12)
+        stage_rows[st_name] = dict(us_per_event=round(stage_ms[st_name] * 1e3 / n_prof, 3), bound="hbm" if t_hbm >= t_alu else "alu",
+                                   roofline_us_per_event=round(max(t_hbm, t_alu) * 1e6 / n_prof, 4),
+                                   frac=round(max(t_hbm, t_alu) / t_s, 4) if t_s > 0 else None,
+                                   gbs=round(wk["bytes"] / t_s / 1e9, 1), tflops=round(wk["flops"] / t_s / 1e12, 3))
+    # dominant kernel
+    kname = max((k for k in prof if k != "memset"), key=lambda k: prof[k])
+    kst = stage_of(kname)
+    share = {"a1": 0.5, "a2": 0.5, "a3": 0.5, "a4": 0.5}.get(kst, 1.0)   # count and fill passes each do the stage's pair tests once
+    wk = stages[kst]
+    k_s = prof[kname] * 1e-3
+    if kst in ("a0",) or wk["bytes"] / (pk["hbm_gbs"] * 1e9) >= wk["flops"] / (alu_peak * 1e12):
+        roof = dict(bound="hbm", achieved=round(wk["bytes"] / k_s / 1e9, 2), peak=pk["hbm_gbs"], unit="GB/s")
+    else:
+        peak_f = fma_peak if kst == "a5" else alu_peak
+        # each of the two passes evaluates every pair: per-launch algorithmic flops = the stage's
+        roof = dict(bound="alu", achieved=round(wk["flops"] / k_s / 1e12, 3), peak=round(peak_f, 2), unit="TFLOP/s")
+    roof.update(frac=round(roof["achieved"] / roof["peak"], 4), traffic=None, kernel=kname, kernel_ms=round(prof[kname], 4),
+                kernel_share_of_step=round(prof[kname] / sum(prof.values()), 3), peak_source=pk["source"],
+                note="ALU peak = 148 SM x 128 lanes x sm_max_mhz un-fused fp32 ops (cuts may not use FMA); DESIGN.md Rooflines")
+    del share
+
+    # ---- oracle on the host cores: bounded sample of the same workload ------------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import lst_oracle as O
+        O.build()
+        n_s = min(E, args.cpu_sample)
+        O.run(geo, w, events[0], counts_only=True)
+        t0 = time.perf_counter()
+        for ev in events[:n_s]:
+            O.run(geo, w, ev, counts_only=True)
+        dt = time.perf_counter() - t0
+        cpu = dict(value=round(n_s / dt, 3), unit=UNIT, cores=1, kind="oracle",
+                   sample=f"first {n_s} of the {E} PU200 events of one step, single thread, {dt:.1f} s")
+
+    out = dict(metric=METRIC, value=round(value, 1), unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+               ms_per_step=round(ms, 4), higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+               config=dict(workload=WORKLOAD, events_per_step_per_gpu=E, streams=S, events_per_launch=per,
+                           l2="flushed between steps (256 MiB write outside the per-step CUDA-event brackets)",
+                           timing="mean of per-step CUDA-event durations on the launching stream, max over ranks",
+                           parallelism=f"replicas x{world}" if world > 1 else "single GPU"),
+               e2e=dict(value=round(e2e_value, 1), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=round(e2e_ms, 4),
+                        timing="wall clock around K steps incl. pinned H2D of every input and D2H of counters + TC rows"),
+               gpu_launches=args.steps * S * lst.launches_per_run(),
+               clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows,
+               kernels_ms={k: round(v, 4) for k, v in prof.items()},
+               per_event=dict(us=round(ms * 1e3 / E, 2), objects={k: round(v / n_prof, 1) for k, v in tot.items()}),
+               wall_ms_per_step_incl_flush=round(t_wall * 1e3 / args.steps, 3))
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The CPU oracle as it stands, on the host cores, on the same config / metric / unit."""
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    from lstgen import build_geometry, xavier_weights
+    from oracle import lst_oracle as O
+    O.build()
+    geo = build_geometry(True)
+    w = xavier_weights(3)
+    n_s = args.ref_events
+    events = make_events(geo, shard_seeds(0, 1, n_s))
+    for _ in range(max(1, min(args.warmup, 2))):
+        O.run(geo, w, events[0], counts_only=True)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        for ev in events:
+            O.run(geo, w, ev, counts_only=True)
+    dt = time.perf_counter() - t0
+    v = args.steps * n_s / dt
+    sample = f"each step = the first {n_s} of the {args.events} PU200 events of our arm's step, single thread"
+    print(json.dumps(dict(impl="reference", metric=METRIC, value=round(v, 3), unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                          warmup=args.warmup, ms_per_step=round(dt * 1e3 / args.steps, 3), higher_is_better=True, scaling="weak",
+                          vs_baseline=None, dtype="f32", data="synthetic",
+                          config=dict(workload=WORKLOAD, events_per_step=n_s, sample=sample),
+                          cpu_baseline=dict(value=round(v, 3), unit=UNIT, cores=1, kind="oracle", sample=sample),
+                          e2e=dict(value=round(v, 3), unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                          gpu_launches=0)))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--events", type=int, default=64, help="PU200 events per step per GPU (configs[3]: 64)")
+    ap.add_argument("--streams", type=int, default=1, help="CUDA streams the batch is split over")
+    ap.add_argument("--cpu-sample", type=int, default=48)
+    ap.add_argument("--ref-events", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

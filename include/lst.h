@@ -141,6 +141,15 @@ int lst_read_tc_host(lst_ctx* ctx, int32_t slot, int32_t* h_counts, int32_t* h_t
 /* Number of kernel launches one lst_run / lst_run_batch enqueues (for the harness' accounting). */
 int lst_launches_per_run(void);
 
+/* Profiling variant of lst_run_batch: same launches with a CUDA event recorded on `cuda_stream`
+ * between them; synchronises, then writes the device time in ms of the memset pair and of each of
+ * the lst_launches_per_run() kernels to h_ms[0 .. lst_launches_per_run()] (HOST).  Not a bench
+ * path: the events serialise nothing but add launch gaps. */
+int lst_run_batch_profile(lst_ctx* ctx, int32_t first_slot, int32_t n, void* cuda_stream, float* h_ms);
+
+/* Name of entry i of h_ms ("memset", "a0.hist", ... , "a6.tc_emit"); NULL when out of range. */
+const char* lst_launch_name(int32_t i);
+
 void lst_destroy(lst_ctx* ctx);
 
 #ifdef __cplusplus

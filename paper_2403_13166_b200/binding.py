@@ -15,7 +15,7 @@ CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t
            raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
-           "lst_run_batch", "lst_get", "lst_status", "lst_read_tc_host", "lst_launches_per_run",
+           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_launches_per_run",
            "lst_destroy"]
 
 
@@ -82,11 +82,14 @@ def load_library():
     L.lst_status.argtypes = [vp, i32, C.POINTER(C.c_uint32), vp, vp]
     L.lst_read_tc_host.argtypes = [vp, i32, vp, vp, i32, vp]
     L.lst_launches_per_run.argtypes = []
+    L.lst_run_batch_profile.argtypes = [vp, i32, i32, vp, vp]
+    L.lst_launch_name.argtypes = [i32]
     L.lst_destroy.argtypes = [vp]
     L.lst_destroy.restype = None
     for n in EXPORTS:
-        if n != "lst_destroy":
+        if n not in ("lst_destroy", "lst_launch_name"):
             getattr(L, n).restype = C.c_int
+    L.lst_launch_name.restype = C.c_char_p
     _lib = L
     return L
 
@@ -202,10 +205,32 @@ class LST:
                 raw.view(t.int32 if dt == "i32" else t.float32)
         return out
 
+    def ranges(self, slot, counts=None):
+        """Device views of the range tables: sensor_start[2M+1], md_start[M+1], ls_start[n_md+1],
+        t3_start[n_md+1] (include/lst.h lst_view i1 / i2 entries)."""
+        if counts is None:
+            _, counts = self.lst_status(slot)
+        t, M = self.torch, self.n_modules
+        out = {}
+        for label, obj, fld, n in (("sensor_start", "hit", "i1", 2 * M + 1), ("md_start", "md", "i2", M + 1),
+                                   ("ls_start", "ls", "i1", counts["md"] + 1), ("t3_start", "t3", "i2", counts["md"] + 1)):
+            v = _View()
+            _chk(self.lib.lst_get(self.ctx, slot, OBJ[obj], C.byref(v)), "lst_get")
+            off = getattr(v, fld) - self.workspace.data_ptr()
+            out[label] = self.workspace[off:off + 4 * n].view(t.int32)
+        return out
+
     def lst_read_tc_host(self, slot, h_counts, h_tc, stream=None):
         """Enqueue D2H of counters and TC rows into HOST (pinned) int32 tensors."""
         _chk(self.lib.lst_read_tc_host(self.ctx, slot, C.c_void_p(h_counts.data_ptr()), C.c_void_p(h_tc.data_ptr()),
                                        int(h_tc.shape[0]), self._st(stream)), "lst_read_tc_host")
+
+    def lst_run_batch_profile(self, first_slot, n, stream=None):
+        """Per-launch device times in ms: dict name -> ms (memset + every kernel of one pass)."""
+        k = self.launches_per_run() + 1
+        ms = np.zeros(k, dtype=np.float32)
+        _chk(self.lib.lst_run_batch_profile(self.ctx, first_slot, n, self._st(stream), _hp(ms)), "lst_run_batch_profile")
+        return {self.lib.lst_launch_name(i).decode(): float(ms[i]) for i in range(k)}
 
     def launches_per_run(self):
         return int(self.lib.lst_launches_per_run())

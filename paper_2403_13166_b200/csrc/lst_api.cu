@@ -226,44 +226,78 @@ int lst_load_event_host(lst_ctx* c, int32_t slot, int32_t n_hits, const float* h
                         s.st_q, cuda_stream);
 }
 
-int lst_run_batch(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
-  if (!c || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
-  if (c->sticky_cuda_error) return LST_ECUDA;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+// The launch sequence of one pass over slots [first, first+n).  With `ev` != nullptr an event is
+// recorded before the first and after every launch (profiling entry point only).
+static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, cudaEvent_t* ev) {
   const Slot* sl = c->d_slots + first;
   const Geo g = c->geo;
   const Caps k = c->caps;
+  int li = 0;
+#define LST_MARK() do { if (ev && bad(c, cudaEventRecord(ev[li], st))) return LST_ECUDA; ++li; } while (0)
+  LST_MARK();
   if (bad(c, cudaMemsetAsync(c->zero_base + first * c->zero_stride, 0, c->zero_stride * n, st))) return LST_ECUDA;
   if (bad(c, cudaMemsetAsync(c->ones_base + first * c->ones_stride, 0xFF, c->ones_stride * n, st))) return LST_ECUDA;
+  LST_MARK();
   // x-extent of the grids: enough blocks to fill 148 SMs several times over across the whole batch
   int gx = (148 * 8 + n - 1) / n;
   if (gx < 8) gx = 8;
   if (gx > 592) gx = 592;
   const dim3 G(gx, n), G1(1, n);
-  k_hist<<<G, 256, 0, st>>>(sl, g);
-  k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
-  k_scatter<<<G, 256, 0, st>>>(sl, g);
-  k_rank<<<G, 256, 0, st>>>(sl);
-  k_md<false><<<G, 256, 0, st>>>(sl, g, k);
-  k_scan<SCAN_MD><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
-  k_md<true><<<G, 256, 0, st>>>(sl, g, k);
-  k_ls<false><<<G, 128, 0, st>>>(sl, g, k);
-  k_scan<SCAN_LS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
-  k_ls<true><<<G, 128, 0, st>>>(sl, g, k);
-  k_t3<false><<<G, 128, 0, st>>>(sl, k);
-  k_scan<SCAN_T3><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
-  k_t3<true><<<G, 128, 0, st>>>(sl, k);
-  k_t5<false><<<G, 128, 0, st>>>(sl, k);
-  k_scan<SCAN_T5C><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
-  k_t5<true><<<G, 128, 0, st>>>(sl, k);
-  k_dnn<<<G, 128, 0, st>>>(sl, g);
-  k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k);
-  k_pls<<<G, 128, 0, st>>>(sl);
-  k_match<5, false><<<G, 128, 0, st>>>(sl);
-  k_pt5_lists<<<G, 128, 0, st>>>(sl);
-  k_match<3, true><<<G, 128, 0, st>>>(sl);
-  k_tc_emit<<<G1, 1024, 0, st>>>(sl, k);
+  k_hist<<<G, 256, 0, st>>>(sl, g); LST_MARK();
+  k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_scatter<<<G, 256, 0, st>>>(sl, g); LST_MARK();
+  k_rank<<<G, 256, 0, st>>>(sl); LST_MARK();
+  k_md<false><<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan<SCAN_MD><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_md<true><<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls<false><<<G, 128, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan<SCAN_LS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls<true><<<G, 128, 0, st>>>(sl, g, k); LST_MARK();
+  k_t3<false><<<G, 128, 0, st>>>(sl, k); LST_MARK();
+  k_scan<SCAN_T3><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_t3<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
+  k_t5<false><<<G, 128, 0, st>>>(sl, k); LST_MARK();
+  k_scan<SCAN_T5C><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_t5<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
+  k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
+  k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_pls<<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_match<5, false><<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_pt5_lists<<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_match<3, true><<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_tc_emit<<<G1, 1024, 0, st>>>(sl, k); LST_MARK();
+#undef LST_MARK
+  if (li != N_LAUNCHES + 2) return LST_EINVAL;
   return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
+}
+
+int lst_run_batch(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
+  if (!c || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  return run_sequence(c, first, n, static_cast<cudaStream_t>(cuda_stream), nullptr);
+}
+
+int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream, float* h_ms) {
+  if (!c || !h_ms || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaEvent_t ev[N_LAUNCHES + 2];
+  for (auto& e : ev) if (bad(c, cudaEventCreate(&e))) return LST_ECUDA;
+  int rc = run_sequence(c, first, n, st, ev);
+  if (rc == LST_OK && bad(c, cudaStreamSynchronize(st))) rc = LST_ECUDA;
+  if (rc == LST_OK)
+    for (int i = 0; i <= N_LAUNCHES; ++i)
+      if (bad(c, cudaEventElapsedTime(&h_ms[i], ev[i], ev[i + 1]))) { rc = LST_ECUDA; break; }
+  for (auto& e : ev) cudaEventDestroy(e);
+  return rc;
+}
+
+const char* lst_launch_name(int32_t i) {
+  static const char* names[N_LAUNCHES + 1] = {
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_count", "a1.scan", "a1.md_fill", "a2.ls_count",
+      "a2.scan", "a2.ls_fill", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
+      "a5.scan", "a6.pls", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
+  return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 
 int lst_run(lst_ctx* c, int32_t slot, void* cuda_stream) { return lst_run_batch(c, slot, 1, cuda_stream); }
