@@ -110,7 +110,7 @@ def algorithmic_work(lst, geo, slots):
     M = geo.n_modules
     rowptr = torch.from_numpy(geo.conn_rowptr.astype(np.int64)).to(lst.device)
     col = torch.from_numpy(geo.conn_col.astype(np.int64)).to(lst.device)
-    tot = dict(hits=0, md_pairs=0, md=0, ls_pairs=0, ls=0, t3_pairs=0, t3=0, t5_pairs=0, t5c=0, t5=0, pls=0, tc=0, match5=0, match3=0)
+    tot = dict(hits=0, md_pairs=0, md=0, ls_pairs=0, ls=0, t3_pairs=0, t3=0, t5_pairs=0, t5c=0, t5=0, pls=0, tc=0, match5=0, match3=0, match_tests=0)
     for s in slots:
         _, c = lst.lst_status(s)
         rg = lst.ranges(s, c)
@@ -129,7 +129,7 @@ def algorithmic_work(lst, geo, slots):
         tot["md_pairs"] += int((n_lo * n_up).sum()); tot["ls_pairs"] += int((nmd * cand).sum())
         tot["t3_pairs"] += int(nls_in[ls_b].sum()) if c["ls"] else 0
         tot["t5_pairs"] += int(nt3_in[t3_c].sum()) if c["t3"] else 0
-        tot["match5"] += c["t5"] * n_pls; tot["match3"] += c["t3"] * n_pls
+        tot["match5"] += c["m5_cand"]; tot["match3"] += c["m3_cand"]; tot["match_tests"] += c["m5_tests"] + c["m3_tests"]
     nnz, nslot = int(geo.conn_col.size), len(slots)
     stages = {
         # compulsory bytes: each input once, each output once
@@ -139,8 +139,10 @@ def algorithmic_work(lst, geo, slots):
         "a3": dict(bytes=tot["ls"] * 12 + tot["md"] * 20 + tot["t3"] * 24, flops=FLOPS["t3_pair"] * tot["t3_pairs"]),
         "a4": dict(bytes=tot["t3"] * 24 + tot["md"] * 20 + tot["t5c"] * 40, flops=FLOPS["t5_pair"] * tot["t5_pairs"]),
         "a5": dict(bytes=tot["t5c"] * (32 + 80 + 92 + 12) + nslot * 7428, flops=FLOPS["dnn_cand"] * tot["t5c"]),
-        "a6": dict(bytes=tot["pls"] * 17 + tot["t5"] * 24 + tot["t3"] * 16 + tot["tc"] * 12,
-                   flops=FLOPS["match_pair"] * (tot["match5"] + tot["match3"]) + FLOPS["match_full"] * (5 * tot["t5"] + 3 * tot["t3"])),
+        # a6: the (pLS, object) pairs whose first anchor passes the transverse test must be tested by any exact
+        # method; the bucket walk's failed first-anchor tests are overhead, reported as per_event.match_tests
+        "a6": dict(bytes=tot["pls"] * (17 + 28) + tot["t5"] * (20 + 80 + 8) + tot["t3"] * (12 + 48 + 8) + tot["tc"] * 12,
+                   flops=FLOPS["match_full"] * (tot["match5"] + tot["match3"]) + FLOPS["match_pair"] * (tot["t5"] + tot["t3"])),
     }
     return tot, stages
 

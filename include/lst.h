@@ -49,7 +49,9 @@ enum { LST_OBJ_HIT = 0, LST_OBJ_MD = 1, LST_OBJ_LS = 2, LST_OBJ_T3 = 3, LST_OBJ_
  * then the UNCLAMPED totals (what the stage would have produced), then pair-test counts. */
 enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT_T5, LST_CNT_TC,
        LST_CNT_RAW_MD, LST_CNT_RAW_LS, LST_CNT_RAW_T3, LST_CNT_RAW_T5C, LST_CNT_RAW_T5, LST_CNT_RAW_TC,
-       LST_CNT_PT5, LST_CNT_T5TC, LST_CNT_PT3, LST_CNT_PLSTC, LST_N_CNT = 32 };
+       LST_CNT_PT5, LST_CNT_T5TC, LST_CNT_PT3, LST_CNT_PLSTC,
+       /* bookkeeping of the bucketed pLS matching: first-anchor tests executed / pairs fully tested */
+       LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
 

@@ -12,7 +12,7 @@ _LIBNAME = os.path.join(_HERE, "liblst_b200.so")
 LST_N_CNT = 32
 OBJ = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, match5=7)
 CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t3=9, raw_t5c=10,
-           raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16)
+           raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
            "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_launches_per_run",

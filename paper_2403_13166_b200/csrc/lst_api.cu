@@ -120,7 +120,9 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.t5c_curv = cv.take<float>(3 * (size_t)k.max_t5c); t.t5c_feat = cv.take<float>((size_t)N_FEAT * k.max_t5c);
     t.t5c_score = cv.take<float>(k.max_t5c); t.t5c_pass = cv.take<int>(k.max_t5c); t.t5_scan = cv.take<int>(k.max_t5c + 8);
     t.t5_list = cv.take<int>(k.max_t5);
-    t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.best5 = cv.take<int>(k.max_t5);
+    t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.pls_key = cv.take<int>(k.max_pls);
+    t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls);
+    t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc = cv.take<int>(3 * (size_t)k.max_tc);
     t.st_x = cv.take<float>(k.max_hits); t.st_y = cv.take<float>(k.max_hits); t.st_z = cv.take<float>(k.max_hits);
@@ -261,7 +263,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_t5<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
   k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_pls<<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_pls_bin<<<G1, 1024, 0, st>>>(sl); LST_MARK();
   k_match<5, false><<<G, 128, 0, st>>>(sl); LST_MARK();
   k_pt5_lists<<<G, 128, 0, st>>>(sl); LST_MARK();
   k_match<3, true><<<G, 128, 0, st>>>(sl); LST_MARK();
@@ -296,7 +298,7 @@ const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
       "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_count", "a1.scan", "a1.md_fill", "a2.ls_count",
       "a2.scan", "a2.ls_fill", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
-      "a5.scan", "a6.pls", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
+      "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 

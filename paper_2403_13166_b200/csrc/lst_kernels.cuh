@@ -50,7 +50,8 @@ struct Slot {
   int* t5_off; int* t5c_md; int2* t5c_t3; float* t5c_curv; float* t5c_feat; float* t5c_score; int* t5c_pass;
   int* t5_scan; int* t5_list;
   // a6
-  float4* pls_a; float2* pls_b; int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
+  float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_bin_start;
+  int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
   // host-load staging
   float *st_x, *st_y, *st_z; uint32_t* st_key; float *st_px, *st_py, *st_pz, *st_z0; int8_t* st_q;
 };
@@ -414,12 +415,77 @@ __global__ void __launch_bounds__(128) k_dnn(const Slot* __restrict__ slots, Geo
 // ------------------------------------------------------------------------------------------------
 // a6: track candidates (SPEC.md 4.6)
 // ------------------------------------------------------------------------------------------------
-__global__ void k_pls(const Slot* __restrict__ slots) {
+// pLS binning.  The matching of SPEC.md 4.6 is defined over all (pLS, object) pairs; to avoid the
+// all-pairs sweep the pLS are bucketed by (half-curvature h = 1/(2R), azimuth psi of the helix centre).
+// For an anchor at (r, phi) the transverse test |e| <= dT is, in exact arithmetic,
+//   |u - cos(phi - psi)| <= tau(u),  u = r*h,  tau(u) = 0.003 + 0.03*u + 0.02/r,
+// so for one h-bucket only two psi windows can hold a passing pLS.  The windows are widened by margins
+// (2e-3 in cos, 1e-3 rad) that exceed the fp32 rounding of every quantity involved by > 100x, so the
+// bucket walk is a conservative prefilter: every pair that passes the exact test is visited, and the
+// decisions themselves are still taken by the exact SPEC.md arithmetic.  pLS whose h is outside the
+// bucketed range (pT < ~0.76 GeV, NaN) or whose q is not +-1 go to an overflow bucket every object visits.
+constexpr int PLS_NB = 256, PLS_K = 8, PLS_NBINS = (PLS_K + 1) * PLS_NB;
+#define LST_PLS_HMAX 0.0075f
+#define LST_PI_F 3.14159265358979f
+
+__device__ __forceinline__ int psi_bin_raw(float ang) {   // unbounded bin index of an angle in radians
+  return (int)floorf((ang + LST_PI_F) * (PLS_NB / (2.0f * LST_PI_F)));
+}
+
+// one block per event: derive, histogram, scan, scatter (all in shared memory; ~2.6k pLS per event)
+__global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots) {
+  __shared__ int hist[PLS_NBINS + 1];
+  __shared__ int sm[34];
   const Slot& s = slots[blockIdx.y];
-  LST_FOR_ITEMS(p, s.n_pls) {
-    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], (int)s.in_q[p]);
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int n = s.n_pls;
+  for (int i = tid; i <= PLS_NBINS; i += 1024) hist[i] = 0;
+  __syncthreads();
+  for (int p = tid; p < n; p += 1024) {
+    const int q = (int)s.in_q[p];
+    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
     s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
     s.pls_b[p] = make_float2(d.sec, d.z0);
+    int kb = PLS_K, pb = 0;
+    if (d.h < LST_PLS_HMAX && (q == 1 || q == -1)) {
+      kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
+      pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
+    }
+    const int key = kb * PLS_NB + pb;
+    s.pls_key[p] = key;
+    atomicAdd(&hist[key], 1);
+  }
+  __syncthreads();
+  // exclusive scan of hist[0..PLS_NBINS] (3 items per thread)
+  constexpr int IT = (PLS_NBINS + 1 + 1023) / 1024;
+  int v[IT], tsum = 0;
+#pragma unroll
+  for (int k = 0; k < IT; ++k) { const int i = tid * IT + k; v[k] = (i <= PLS_NBINS) ? hist[i] : 0; tsum += v[k]; }
+  int inc = tsum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+  if (lane == 31) sm[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    const int w = sm[lane]; int winc = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, d); if (lane >= d) winc += t; }
+    sm[lane] = winc - w;
+  }
+  __syncthreads();
+  int run = sm[wid] + inc - tsum;
+#pragma unroll
+  for (int k = 0; k < IT; ++k) {
+    const int i = tid * IT + k;
+    if (i <= PLS_NBINS) { hist[i] = run; s.pls_bin_start[i] = run; }
+    run += v[k];
+  }
+  __syncthreads();
+  for (int p = tid; p < n; p += 1024) {
+    const int pos = atomicAdd(&hist[s.pls_key[p]], 1);   // order inside a bucket is free: argmin ties break on p
+    s.pls_sa[pos] = s.pls_a[p];
+    s.pls_sb[pos] = s.pls_b[p];
+    s.pls_sidx[pos] = p;
   }
 }
 
@@ -427,13 +493,14 @@ __device__ __forceinline__ unsigned long long win_key(float chi2, int idx) {
   return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned)idx;   // chi2 >= 0: bit order = value order
 }
 
-// match objects with NA anchors against every pLS: one thread per object, pLS loop in ascending p so
-// that a strict '<' keeps the smallest p on ties (argmin over (chi2, p)).
+// match objects with NA anchors against the pLS buckets their first anchor can reach: one thread per
+// object; best = argmin over (chi2, p) with an explicit tie-break on p (bucket order is arbitrary).
 template <int NA, bool IS_T3>
 __global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
   const Slot& s = slots[blockIdx.y];
   const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
-  const int n_pls = s.n_pls;
+  const int* __restrict__ bstart = s.pls_bin_start;
+  int n_tests = 0, n_cand = 0;
   LST_FOR_ITEMS(t, n) {
     int md[NA];
     if (IS_T3) {
@@ -459,24 +526,62 @@ __global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
     const int mt0 = s.md_modt[md[0]] & 3;
     int best = -1;
     float bchi = 0.0f;
-    for (int p = 0; p < n_pls; ++p) {
-      const float4 pa = s.pls_a[p];
-      Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
-      float e, dT;
-      if (!pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT)) continue;       // cheap transverse early-out
-      if (IS_T3 && s.win5[p] != WIN_EMPTY) continue;                  // pLS already in a pT5
-      const float2 pb = s.pls_b[p];
-      P.sec = pb.x; P.z0 = pb.y;
-      float chi = 0.0f;
-      bool ok = pls_anchor(P, a0, mt0, chi);
+    const float phi = atan2f(a0.y, a0.x);
+    const float r = a0.w;
+    const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
+    for (int kb = 0; kb <= PLS_K; ++kb) {
+      // up to four bucket ranges [rb[i], re[i]) of this h-bucket
+      int rb[4], re[4], nr = 0;
+      const int base = kb * PLS_NB;
+      if (kb == PLS_K) { rb[0] = base; re[0] = base + PLS_NB; nr = 1; }
+      else {
+        const float ulo = r * (kb * (LST_PLS_HMAX / PLS_K)), uhi = r * ((kb + 1) * (LST_PLS_HMAX / PLS_K));
+        const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
+        if (clo > 1.0f) { kb = PLS_K - 1; continue; }            // no circle of this or a larger curvature reaches r
+        const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
 #pragma unroll
-      for (int q = 1; q < NA; ++q)
-        if (ok) ok = pls_anchor(P, s.md_pos[md[q]], s.md_modt[md[q]] & 3, chi);
-      if (!ok) continue;
-      if (best < 0 || chi < bchi) { best = p; bchi = chi; }
+        for (int sgn = 0; sgn < 2; ++sgn) {
+          const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
+          const int blo = psi_bin_raw(lo);
+          const int nb = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
+          const int b0 = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
+          const int e0 = min(b0 + nb, PLS_NB);
+          rb[nr] = base + b0; re[nr] = base + e0; ++nr;
+          if (b0 + nb > PLS_NB) { rb[nr] = base; re[nr] = base + b0 + nb - PLS_NB; ++nr; }
+        }
+      }
+      for (int ir = 0; ir < nr; ++ir) {
+        const int j1 = bstart[re[ir]];
+        for (int j = bstart[rb[ir]]; j < j1; ++j) {
+          const float4 pa = s.pls_sa[j];
+          Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
+          float e, dT;
+          ++n_tests;
+          if (!pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT)) continue;       // transverse test of the first anchor
+          const int p = s.pls_sidx[j];
+          if (IS_T3 && s.win5[p] != WIN_EMPTY) continue;                  // pLS already in a pT5
+          ++n_cand;
+          const float2 pb = s.pls_sb[j];
+          P.sec = pb.x; P.z0 = pb.y;
+          float chi = 0.0f;
+          bool ok = pls_anchor(P, a0, mt0, chi);
+#pragma unroll
+          for (int q = 1; q < NA; ++q)
+            if (ok) ok = pls_anchor(P, s.md_pos[md[q]], s.md_modt[md[q]] & 3, chi);
+          if (!ok) continue;
+          if (best < 0 || chi < bchi || (chi == bchi && p < best)) { best = p; bchi = chi; }
+        }
+      }
     }
     if (IS_T3) { s.best3[t] = best; s.chi3[t] = bchi; if (best >= 0) atomicMin(s.win3 + best, win_key(bchi, t)); }
     else { s.best5[t] = best; s.chi5[t] = bchi; if (best >= 0) atomicMin(s.win5 + best, win_key(bchi, t)); }
+  }
+  // bookkeeping for the roofline accounting: prefilter tests executed / pairs that needed the full test
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) { n_tests += __shfl_xor_sync(0xffffffffu, n_tests, d); n_cand += __shfl_xor_sync(0xffffffffu, n_cand, d); }
+  if ((threadIdx.x & 31) == 0 && n_tests) {
+    atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_TESTS : LST_CNT_M5_TESTS), n_tests);
+    atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_CAND : LST_CNT_M5_CAND), n_cand);
   }
 }
 
