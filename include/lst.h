@@ -51,7 +51,9 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        LST_CNT_RAW_MD, LST_CNT_RAW_LS, LST_CNT_RAW_T3, LST_CNT_RAW_T5C, LST_CNT_RAW_T5, LST_CNT_RAW_TC,
        LST_CNT_PT5, LST_CNT_T5TC, LST_CNT_PT3, LST_CNT_PLSTC,
        /* bookkeeping of the bucketed pLS matching: first-anchor tests executed / pairs fully tested */
-       LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND, LST_N_CNT = 32 };
+       LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND,
+       /* internal: fill of the unordered MD / LS record buffers */
+       LST_CNT_TMP_MD, LST_CNT_TMP_LS, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
 

@@ -3,7 +3,7 @@
 #include <cuda_runtime.h>
 #include <new>
 #include <vector>
-#include "lst_kernels.cuh"
+#include "lst_pairs.cuh"
 
 using namespace lst;
 
@@ -111,9 +111,9 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   for (int s = 0; s < n_slots; ++s) {
     Slot t{};
     t.tmp_orig = cv.take<int>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
-    t.md_off = cv.take<int>(k.max_hits + 8); t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
+    t.md_off = cv.take<int>(k.max_hits + 8); t.md_item_off = cv.take<int>(M + 8); t.md_rec = cv.take<MdRec>(k.max_md); t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
     t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_start = cv.take<int>(M + 1);
-    t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
+    t.ls_start = cv.take<int>(k.max_md + 8); t.ls_L = cv.take<int>(M); t.ls_item_off = cv.take<int>(M + 8); t.ls_rec = cv.take<LsRec>(k.max_ls); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
     t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
     t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
     t.t5_off = cv.take<int>(k.max_t3 + 8); t.t5c_md = cv.take<int>(5 * (size_t)k.max_t5c); t.t5c_t3 = cv.take<int2>(k.max_t5c);
@@ -144,7 +144,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 23;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 26;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -249,12 +249,15 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_scatter<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_rank<<<G, 256, 0, st>>>(sl); LST_MARK();
-  k_md<false><<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
+  k_md_pairs<<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_scan<SCAN_MD><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_md<true><<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls<false><<<G, 128, 0, st>>>(sl, g, k); LST_MARK();
+  k_md_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan<SCAN_LSITEMS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_md<true><<<G, 256, 0, st>>>(sl, g, k); LST_MARK();          // overflow rescue (returns at once otherwise)
+  k_ls_pairs<<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_scan<SCAN_LS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls<true><<<G, 128, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_final<<<G, 256, 0, st>>>(sl, k); LST_MARK();
+  k_ls<true><<<G, 128, 0, st>>>(sl, g, k); LST_MARK();          // overflow rescue
   k_t3<false><<<G, 128, 0, st>>>(sl, k); LST_MARK();
   k_scan<SCAN_T3><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_t3<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
@@ -296,8 +299,8 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
-      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_count", "a1.scan", "a1.md_fill", "a2.ls_count",
-      "a2.scan", "a2.ls_fill", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_pairs", "a1.scan", "a1.md_final", "a2.item_scan", "a1.md_rescue", "a2.ls_pairs",
+      "a2.scan", "a2.ls_final", "a2.ls_rescue", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
       "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }

@@ -26,6 +26,9 @@ struct Geo {   // device copies, shared by all slots
 
 struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
 
+struct __align__(16) MdRec { int p_lo, p_up, rank, modt; float c, w, r1, pad; };   // lst_pairs.cuh
+struct __align__(16) LsRec { int a, b, rank; float c; };
+
 struct Slot {
   // bound inputs
   const float *in_x, *in_y, *in_z; const uint32_t* in_key; int n_hits;
@@ -41,9 +44,9 @@ struct Slot {
   // a0
   int* tmp_orig; float4* hit; int* hit_orig;
   // a1
-  int* md_off; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; int* md_start;
+  int* md_off; int* md_item_off; MdRec* md_rec; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; int* md_start;
   // a2
-  int* ls_start; int2* ls_ab; float* ls_c;
+  int* ls_start; int* ls_L; int* ls_item_off; LsRec* ls_rec; int2* ls_ab; float* ls_c;
   // a3
   int* t3_off; int4* t3_abc; int* t3_l1; float* t3_k; int* t3_start;
   // a4 / a5
@@ -125,7 +128,20 @@ __device__ __forceinline__ int block_scan_inplace(int* __restrict__ a, int n, in
   return carry;
 }
 
-enum { SCAN_SENSOR = 0, SCAN_MD, SCAN_LS, SCAN_T3, SCAN_T5C, SCAN_T5 };
+enum { SCAN_SENSOR = 0, SCAN_MD, SCAN_LS, SCAN_T3, SCAN_T5C, SCAN_T5, SCAN_LSITEMS };
+
+// Work items of the pair-parallel MD / LS sweeps (lst_pairs.cuh): a module's n_rows x L rectangle is cut
+// into items of about ITEM_SWEEPS warp sweeps.  Narrow rectangles (L <= 32) pack R = 32/W rows into one
+// sweep (W = L rounded up to a power of two); wide ones take S = ceil(L/32) sweeps per row.
+constexpr int ITEM_SWEEPS = 8;
+struct ItemPlan { int W, R, S, rows_per_item, n_items; };
+__device__ __forceinline__ ItemPlan item_plan(int n_rows, int L) {
+  ItemPlan p;
+  if (L <= 32) { p.W = L <= 1 ? 1 : 1 << (32 - __clz(L - 1)); p.R = 32 / p.W; p.S = 1; p.rows_per_item = ITEM_SWEEPS * p.R; }
+  else { p.W = 32; p.R = 1; p.S = (L + 31) >> 5; p.rows_per_item = max(1, ITEM_SWEEPS / p.S); }
+  p.n_items = (n_rows > 0 && L > 0) ? (n_rows + p.rows_per_item - 1) / p.rows_per_item : 0;
+  return p;
+}
 
 template <int MODE>
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
@@ -138,18 +154,30 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ 
   else if (MODE == SCAN_LS) { a = s.ls_start; n = cnt[LST_CNT_MD]; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; }
   else if (MODE == SCAN_T3) { a = s.t3_off; n = cnt[LST_CNT_LS]; cap = caps.max_t3; icnt = LST_CNT_T3; iraw = LST_CNT_RAW_T3; ovf = LST_ST_OVF_T3; }
   else if (MODE == SCAN_T5C) { a = s.t5_off; n = cnt[LST_CNT_T3]; cap = caps.max_t5c; icnt = LST_CNT_T5C; iraw = LST_CNT_RAW_T5C; ovf = LST_ST_OVF_T5C; }
-  else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
+  else if (MODE == SCAN_T5) { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
+  else { a = s.ls_item_off; n = geo.n_modules; cap = 0x7fffffff; icnt = -1; iraw = -1; ovf = 0; }
   __syncthreads();   // everyone has read n before thread 0 may overwrite counters below
   const int total = block_scan_inplace(a, n, cap, sm);
   if (threadIdx.x == 0) {
-    cnt[icnt] = min(total, cap);
+    if (icnt >= 0) cnt[icnt] = min(total, cap);
     if (iraw >= 0) cnt[iraw] = total;
     if (total > cap) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), ovf);
   }
   __syncthreads();
   // epilogues: range tables / compaction that fall out of the scan
-  if (MODE == SCAN_MD) {          // MDs of module m = [md_start[m], md_start[m+1])
+  if (MODE == SCAN_SENSOR) {      // row counts of the MD sweep start at zero; work items of the MD sweep
+    const int n_hits = min(total, cap);
+    for (int i = threadIdx.x; i < n_hits; i += SCAN_THREADS) s.md_off[i] = 0;
+    for (int m = threadIdx.x; m < geo.n_modules; m += SCAN_THREADS) {
+      const int lb = a[2 * m], ub = a[2 * m + 1], ue = a[2 * m + 2];
+      s.md_item_off[m] = item_plan(ub - lb, ue - ub).n_items;
+    }
+    __syncthreads();
+    block_scan_inplace(s.md_item_off, geo.n_modules, 0x7fffffff, sm);
+  } else if (MODE == SCAN_MD) {          // MDs of module m = [md_start[m], md_start[m+1])
     for (int m = threadIdx.x; m <= geo.n_modules; m += SCAN_THREADS) s.md_start[m] = a[s.sensor_start[2 * m]];
+    const int n_md = min(total, cap);
+    for (int i = threadIdx.x; i < n_md; i += SCAN_THREADS) s.ls_start[i] = 0;   // row counts of the LS sweep
   } else if (MODE == SCAN_T3) {   // T3s whose inner MD is a = [t3_start[a], t3_start[a+1])
     const int n_md = cnt[LST_CNT_MD];
     for (int i = threadIdx.x; i <= n_md; i += SCAN_THREADS) s.t3_start[i] = a[s.ls_start[i]];
@@ -203,6 +231,7 @@ __global__ void k_rank(const Slot* __restrict__ slots) {
 template <bool FILL>
 __global__ void __launch_bounds__(256) k_md(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   const Slot& s = slots[blockIdx.y];
+  if (FILL && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;   // fill = overflow rescue only (lst_pairs.cuh)
   const int n = s.cnt[LST_CNT_HIT];
   LST_FOR_ITEMS(p, n) {
     const float4 h1 = s.hit[p];
@@ -250,6 +279,7 @@ __device__ __forceinline__ Anchor load_anchor(const Slot& s, int i) {
 template <bool FILL>
 __global__ void __launch_bounds__(128) k_ls(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   const Slot& s = slots[blockIdx.y];
+  if (FILL && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;   // fill = overflow rescue only (lst_pairs.cuh)
   const int n = s.cnt[LST_CNT_MD];
   LST_FOR_ITEMS(a, n) {
     const Anchor A = load_anchor(s, a);
