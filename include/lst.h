@@ -52,8 +52,8 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        LST_CNT_PT5, LST_CNT_T5TC, LST_CNT_PT3, LST_CNT_PLSTC,
        /* bookkeeping of the bucketed pLS matching: first-anchor tests executed / pairs fully tested */
        LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND,
-       /* internal: fill of the unordered MD / LS record buffers */
-       LST_CNT_TMP_MD, LST_CNT_TMP_LS, LST_N_CNT = 32 };
+       /* internal: fill of the MD / LS record buffers; link tickets of the overflow re-run */
+       LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TICKET_MD, LST_CNT_TICKET_LS, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
 
@@ -77,7 +77,7 @@ typedef struct {
  * them completes and until the next lst_run on that slot.  `count` is a DEVICE pointer to the
  * clamped object count.  Unused entries are NULL.  Layouts (row-major, `capacity` rows):
  *  HIT   : i0 = orig[n] int32 (sorted position -> original hit index), i1 = sensor_start[2M+1],
- *          f0 = xyz as float4 (x, y, z, key as int bits)
+ *          f0 = xyzr as float4 (x, y, z, r = sqrt(x*x + y*y))
  *  MD    : i0 = hits[n][2] int32 (ORIGINAL lower, upper hit index), i1 = modt[n] int32 (module<<2 |
  *          subdet<<1 | mtype), f0 = anchor[n] float4 (x, y, z, r), f1 = cw[n] float2 (c, w),
  *          i2 = md_start[M+1]

@@ -106,7 +106,7 @@ def _hp(a):
 
 # rows, dtype, columns of every view field (include/lst.h lst_view)
 _FIELDS = {
-    "hit": dict(i0=("orig", "i32", 1), f0=("xyzk", "f32", 4)),
+    "hit": dict(i0=("orig", "i32", 1), f0=("xyzr", "f32", 4)),
     "md": dict(i0=("hits", "i32", 2), i1=("modt", "i32", 1), f0=("anchor", "f32", 4), f1=("cw", "f32", 2)),
     "ls": dict(i0=("ab", "i32", 2), f0=("c", "f32", 1)),
     "t3": dict(i0=("abc", "i32", 4), i1=("l1", "i32", 1), f0=("k", "f32", 1)),

@@ -17,6 +17,7 @@ struct lst_ctx {
   char* zero_base = nullptr; size_t zero_stride = 0;
   char* ones_base = nullptr; size_t ones_stride = 0;
   bool sticky_cuda_error = false;
+  unsigned epoch = 0;             // run counter carried in the look-back status words (lst_pairs.cuh)
 };
 
 namespace {
@@ -111,9 +112,14 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   for (int s = 0; s < n_slots; ++s) {
     Slot t{};
     t.tmp_orig = cv.take<int>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
-    t.md_off = cv.take<int>(k.max_hits + 8); t.md_item_off = cv.take<int>(M + 8); t.md_rec = cv.take<MdRec>(k.max_md); t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
-    t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_start = cv.take<int>(M + 1);
-    t.ls_start = cv.take<int>(k.max_md + 8); t.ls_L = cv.take<int>(M); t.ls_item_off = cv.take<int>(M + 8); t.ls_rec = cv.take<LsRec>(k.max_ls); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
+    t.md_pair_off = cv.take<int>(M + 8); t.md_link_mod = cv.take<int>(MAX_CELLS / MD_LP + 16); t.chain_md = cv.take<unsigned long long>(MAX_CELLS / MD_LP + 2);
+    t.md_link_cnt = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_link_soff = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_rec = cv.take<MdRec>(k.max_md);
+    t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
+    t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_aux = cv.take<float4>(k.max_md); t.md_start = cv.take<int>(M + 1);
+    t.ls_L = cv.take<int>(M); t.ls_off = cv.take<int>(M + 8); t.ls_coff = cv.take<int>(M + 8); t.ls_cand = cv.take<int>((size_t)CAND_PER_MD * k.max_md);
+    t.ls_link_mod = cv.take<int>(MAX_CELLS / LS_LP + 16); t.chain_ls = cv.take<unsigned long long>(MAX_CELLS / LS_LP + 2);
+    t.ls_link_cnt = cv.take<int>(MAX_CELLS / LS_LP + 16); t.ls_link_soff = cv.take<int>(MAX_CELLS / LS_LP + 16); t.ls_rec = cv.take<LsRec>(k.max_ls);
+    t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
     t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
     t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
     t.t5_off = cv.take<int>(k.max_t3 + 8); t.t5c_md = cv.take<int>(5 * (size_t)k.max_t5c); t.t5c_t3 = cv.take<int2>(k.max_t5c);
@@ -186,6 +192,10 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   if (e == cudaSuccess) e = cudaMemcpy(L.weights, geo->dnn_weights, sizeof(float) * N_W, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(L.slots, c->h_slots.data(), sizeof(Slot) * c->n_slots, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(c->zero_base, 0, c->zero_stride * c->n_slots);
+  for (int i = 0; i < c->n_slots && e == cudaSuccess; ++i) {   // status words start at epoch 0 (never a run's epoch)
+    e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (MAX_CELLS / MD_LP + 2));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (MAX_CELLS / LS_LP + 2));
+  }
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
   c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
   *out = c;
@@ -244,20 +254,21 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   int gx = (148 * 8 + n - 1) / n;
   if (gx < 8) gx = 8;
   if (gx > 592) gx = 592;
-  const dim3 G(gx, n), G1(1, n);
+  const dim3 G(gx, n), G1(1, n), GL(2 * gx, n);   // GL: the 128-thread link kernels
   k_hist<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_scatter<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_rank<<<G, 256, 0, st>>>(sl); LST_MARK();
-  k_md_pairs<<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
-  k_scan<SCAN_MD><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  const unsigned epoch = (c->epoch = (c->epoch % 0x3FFFFFFFu) + 1u);   // validates this run's look-back status words
+  k_md_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();
+  k_scan<SCAN_MDLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_md_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_scan<SCAN_LSITEMS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_md<true><<<G, 256, 0, st>>>(sl, g, k); LST_MARK();          // overflow rescue (returns at once otherwise)
-  k_ls_pairs<<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
-  k_scan<SCAN_LS><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_final<<<G, 256, 0, st>>>(sl, k); LST_MARK();
-  k_ls<true><<<G, 128, 0, st>>>(sl, g, k); LST_MARK();          // overflow rescue
+  k_md_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();     // overflow re-run (returns at once otherwise)
+  k_ls_plan<<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();
+  k_scan<SCAN_LSLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();     // overflow re-run
   k_t3<false><<<G, 128, 0, st>>>(sl, k); LST_MARK();
   k_scan<SCAN_T3><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_t3<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
@@ -299,8 +310,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
-      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_pairs", "a1.scan", "a1.md_final", "a2.item_scan", "a1.md_rescue", "a2.ls_pairs",
-      "a2.scan", "a2.ls_final", "a2.ls_rescue", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
       "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }

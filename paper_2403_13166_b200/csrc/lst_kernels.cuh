@@ -3,9 +3,9 @@
 // Launch geometry: every kernel takes the device array of slot descriptors and runs on a grid
 // (GX, n_events); blockIdx.y selects the slot, the x dimension grid-strides over that slot's items
 // (counts live in device memory -- lst_run never synchronises with the host).
-// Deterministic output order: every combinatorial stage is count -> exclusive scan -> fill, with one
-// thread owning one "inner" object (lower hit / inner MD / first LS / inner T3), so the object
-// order is the SPEC.md build order and capacity overflow is detected in the scan and flagged.
+// Deterministic output order: MD and LS are single-pass ordered compactions (lst_pairs.cuh); T3 / T5 are
+// count -> exclusive scan -> fill with one thread owning one inner object (first LS / inner T3).  Either
+// way the object order is the SPEC.md build order and capacity overflow is detected and flagged.
 #pragma once
 #include "lst_math.cuh"
 #include "../../include/lst.h"
@@ -26,8 +26,13 @@ struct Geo {   // device copies, shared by all slots
 
 struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
 
-struct __align__(16) MdRec { int p_lo, p_up, rank, modt; float c, w, r1, pad; };   // lst_pairs.cuh
-struct __align__(16) LsRec { int a, b, rank; float c; };
+// staged objects of the MD / LS links (lst_pairs.cuh): f = flat cell index relative to the link's first cell
+struct __align__(16) MdRec { int p_lo, p_up, mtm, f; float c, w; int link, pad; };
+struct __align__(16) LsRec { int a, b, lf; float c; };     // lf = link << LS_LP_BITS | f
+constexpr int MD_LP = 256;           // cells (hit pairs) per MD link = staging capacity, so staging cannot overflow
+constexpr int LS_LP_BITS = 8, LS_LP = 1 << LS_LP_BITS;   // cells (MD pairs) per LS link
+constexpr int CAND_PER_MD = 8;       // capacity of the per-slot candidate table = CAND_PER_MD * max_md entries
+constexpr int MAX_CELLS = 1 << 22;   // flat cell space per stage and slot (PU200: 0.35 M MD, 1.0 M LS cells)
 
 struct Slot {
   // bound inputs
@@ -44,9 +49,9 @@ struct Slot {
   // a0
   int* tmp_orig; float4* hit; int* hit_orig;
   // a1
-  int* md_off; int* md_item_off; MdRec* md_rec; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; int* md_start;
+  int* md_pair_off; int* md_link_mod; int* md_link_cnt; int* md_link_soff; MdRec* md_rec; unsigned long long* chain_md; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; float4* md_aux; int* md_start;
   // a2
-  int* ls_start; int* ls_L; int* ls_item_off; LsRec* ls_rec; int2* ls_ab; float* ls_c;
+  int* ls_L; int* ls_off; int* ls_coff; int* ls_cand; int* ls_link_mod; int* ls_link_cnt; int* ls_link_soff; LsRec* ls_rec; unsigned long long* chain_ls; int* ls_start; int2* ls_ab; float* ls_c;
   // a3
   int* t3_off; int4* t3_abc; int* t3_l1; float* t3_k; int* t3_start;
   // a4 / a5
@@ -128,20 +133,18 @@ __device__ __forceinline__ int block_scan_inplace(int* __restrict__ a, int n, in
   return carry;
 }
 
-enum { SCAN_SENSOR = 0, SCAN_MD, SCAN_LS, SCAN_T3, SCAN_T5C, SCAN_T5, SCAN_LSITEMS };
-
-// Work items of the pair-parallel MD / LS sweeps (lst_pairs.cuh): a module's n_rows x L rectangle is cut
-// into items of about ITEM_SWEEPS warp sweeps.  Narrow rectangles (L <= 32) pack R = 32/W rows into one
-// sweep (W = L rounded up to a power of two); wide ones take S = ceil(L/32) sweeps per row.
-constexpr int ITEM_SWEEPS = 8;
-struct ItemPlan { int W, R, S, rows_per_item, n_items; };
-__device__ __forceinline__ ItemPlan item_plan(int n_rows, int L) {
-  ItemPlan p;
-  if (L <= 32) { p.W = L <= 1 ? 1 : 1 << (32 - __clz(L - 1)); p.R = 32 / p.W; p.S = 1; p.rows_per_item = ITEM_SWEEPS * p.R; }
-  else { p.W = 32; p.R = 1; p.S = (L + 31) >> 5; p.rows_per_item = max(1, ITEM_SWEEPS / p.S); }
-  p.n_items = (n_rows > 0 && L > 0) ? (n_rows + p.rows_per_item - 1) / p.rows_per_item : 0;
-  return p;
+// link_mod[l] = the module that owns flat cell l*LP (off = exclusive scan of the per-module cell counts, off[M] =
+// total); entries of links that start at or beyond the total are M.  Called by a whole block after the scan.
+__device__ __forceinline__ void link_owner_table(const int* __restrict__ off, int M, int LP, int* __restrict__ link_mod) {
+  const int total = min(off[M], MAX_CELLS);
+  for (int m = threadIdx.x; m < M; m += blockDim.x) {
+    const int b = off[m], e = min(off[m + 1], total);
+    for (int l = (b + LP - 1) / LP; l * LP < e; ++l) link_mod[l] = m;
+  }
+  for (int l = (total + LP - 1) / LP + threadIdx.x; l <= total / LP + 1; l += blockDim.x) link_mod[l] = M;
 }
+
+enum { SCAN_SENSOR = 0, SCAN_MDLINK, SCAN_LSLINK, SCAN_T3, SCAN_T5C, SCAN_T5 };
 
 template <int MODE>
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
@@ -150,12 +153,11 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ 
   int* cnt = s.cnt;
   int* a; int n, cap, icnt, iraw; unsigned ovf;
   if (MODE == SCAN_SENSOR) { a = s.sensor_start; n = 2 * geo.n_modules; cap = caps.max_hits; icnt = LST_CNT_HIT; iraw = -1; ovf = 0; }
-  else if (MODE == SCAN_MD) { a = s.md_off; n = cnt[LST_CNT_HIT]; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; }
-  else if (MODE == SCAN_LS) { a = s.ls_start; n = cnt[LST_CNT_MD]; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; }
+  else if (MODE == SCAN_MDLINK) { a = s.md_link_cnt; n = min(s.md_pair_off[geo.n_modules], MAX_CELLS) / MD_LP + 1; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; }
+  else if (MODE == SCAN_LSLINK) { a = s.ls_link_cnt; n = min(s.ls_off[geo.n_modules], MAX_CELLS) / LS_LP + 1; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; }
   else if (MODE == SCAN_T3) { a = s.t3_off; n = cnt[LST_CNT_LS]; cap = caps.max_t3; icnt = LST_CNT_T3; iraw = LST_CNT_RAW_T3; ovf = LST_ST_OVF_T3; }
   else if (MODE == SCAN_T5C) { a = s.t5_off; n = cnt[LST_CNT_T3]; cap = caps.max_t5c; icnt = LST_CNT_T5C; iraw = LST_CNT_RAW_T5C; ovf = LST_ST_OVF_T5C; }
-  else if (MODE == SCAN_T5) { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
-  else { a = s.ls_item_off; n = geo.n_modules; cap = 0x7fffffff; icnt = -1; iraw = -1; ovf = 0; }
+  else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
   __syncthreads();   // everyone has read n before thread 0 may overwrite counters below
   const int total = block_scan_inplace(a, n, cap, sm);
   if (threadIdx.x == 0) {
@@ -165,19 +167,18 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ 
   }
   __syncthreads();
   // epilogues: range tables / compaction that fall out of the scan
-  if (MODE == SCAN_SENSOR) {      // row counts of the MD sweep start at zero; work items of the MD sweep
-    const int n_hits = min(total, cap);
-    for (int i = threadIdx.x; i < n_hits; i += SCAN_THREADS) s.md_off[i] = 0;
+  if (MODE == SCAN_SENSOR) {      // flat cell space of the MD stage: exclusive scan of n_lower * n_upper per module
     for (int m = threadIdx.x; m < geo.n_modules; m += SCAN_THREADS) {
       const int lb = a[2 * m], ub = a[2 * m + 1], ue = a[2 * m + 2];
-      s.md_item_off[m] = item_plan(ub - lb, ue - ub).n_items;
+      long long cells = (long long)(ub - lb) * (ue - ub);
+      if (cells > (1 << 22)) { cells = 0; atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), LST_ST_OVF_MD); }
+      s.md_pair_off[m] = (int)cells;
     }
     __syncthreads();
-    block_scan_inplace(s.md_item_off, geo.n_modules, 0x7fffffff, sm);
-  } else if (MODE == SCAN_MD) {          // MDs of module m = [md_start[m], md_start[m+1])
-    for (int m = threadIdx.x; m <= geo.n_modules; m += SCAN_THREADS) s.md_start[m] = a[s.sensor_start[2 * m]];
-    const int n_md = min(total, cap);
-    for (int i = threadIdx.x; i < n_md; i += SCAN_THREADS) s.ls_start[i] = 0;   // row counts of the LS sweep
+    const int cells_total = block_scan_inplace(s.md_pair_off, geo.n_modules, 0x7fffffff, sm);
+    if (threadIdx.x == 0 && cells_total > MAX_CELLS) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), LST_ST_OVF_MD);
+    __syncthreads();
+    link_owner_table(s.md_pair_off, geo.n_modules, MD_LP, s.md_link_mod);
   } else if (MODE == SCAN_T3) {   // T3s whose inner MD is a = [t3_start[a], t3_start[a+1])
     const int n_md = cnt[LST_CNT_MD];
     for (int i = threadIdx.x; i <= n_md; i += SCAN_THREADS) s.t3_start[i] = a[s.ls_start[i]];
@@ -219,87 +220,9 @@ __global__ void k_rank(const Slot* __restrict__ slots) {
     int rank = 0;
     for (int q = b; q < e; ++q) rank += (s.tmp_orig[q] < o);
     const int d = b + rank;
-    s.hit[d] = make_float4(s.in_x[o], s.in_y[o], s.in_z[o], __int_as_float((int)key));
+    const float x = s.in_x[o], y = s.in_y[o];
+    s.hit[d] = make_float4(x, y, s.in_z[o], fq(fa(fm(x, x), fm(y, y))));   // r as SPEC.md 4.1 computes it
     s.hit_orig[d] = o;
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// a1: mini-doublets (SPEC.md 4.1).  One thread per lower-sensor hit; loops over the module's
-// upper-sensor hits (contiguous in the module-sorted store, L1-resident for the whole warp).
-// ------------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(256) k_md(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  const Slot& s = slots[blockIdx.y];
-  if (FILL && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;   // fill = overflow rescue only (lst_pairs.cuh)
-  const int n = s.cnt[LST_CNT_HIT];
-  LST_FOR_ITEMS(p, n) {
-    const float4 h1 = s.hit[p];
-    const int key = __float_as_int(h1.w);
-    int count = 0;
-    if (!(key & 1)) {
-      const int m = key >> 1;
-      const int mt = geo.modt[m];
-      const int ub = s.sensor_start[key + 1], ue = s.sensor_start[key + 2];
-      const float r1 = fq(fa(fm(h1.x, h1.x), fm(h1.y, h1.y)));
-      int out = FILL ? s.md_off[p] : 0;
-      for (int j = ub; j < ue; ++j) {
-        const float4 h2 = s.hit[j];
-        float c, w;
-        if (!md_eval(h1.x, h1.y, h1.z, r1, h2.x, h2.y, h2.z, mt, c, w)) continue;
-        if (FILL) {
-          if (out < caps.max_md) {
-            s.md_hits[out] = make_int2(s.hit_orig[p], s.hit_orig[j]);
-            s.md_modt[out] = (m << 2) | mt;
-            s.md_pos[out] = make_float4(h1.x, h1.y, h1.z, r1);
-            s.md_cw[out] = make_float2(c, w);
-          }
-          ++out;
-        } else {
-          ++count;
-        }
-      }
-    }
-    if (!FILL) s.md_off[p] = count;
-  }
-}
-
-__device__ __forceinline__ Anchor load_anchor(const Slot& s, int i) {
-  const float4 p = s.md_pos[i];
-  const float2 cw = s.md_cw[i];
-  Anchor a; a.x = p.x; a.y = p.y; a.z = p.z; a.r = p.w; a.c = cw.x; a.w = cw.y; a.mt = s.md_modt[i] & 3;
-  return a;
-}
-
-// ------------------------------------------------------------------------------------------------
-// a2: line segments (SPEC.md 4.2).  One thread per inner MD; walks the CSR row of its module and
-// the MDs of each connected module.  Threads of a warp mostly share the module, so the inner loads
-// are warp-uniform (broadcast from L1).
-// ------------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(128) k_ls(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  const Slot& s = slots[blockIdx.y];
-  if (FILL && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;   // fill = overflow rescue only (lst_pairs.cuh)
-  const int n = s.cnt[LST_CNT_MD];
-  LST_FOR_ITEMS(a, n) {
-    const Anchor A = load_anchor(s, a);
-    const int m = s.md_modt[a] >> 2;
-    int out = FILL ? s.ls_start[a] : 0;
-    const int e1 = geo.rowptr[m + 1];
-    for (int e = geo.rowptr[m]; e < e1; ++e) {
-      const int m2 = geo.col[e];
-      const int b1 = s.md_start[m2 + 1];
-      for (int b = s.md_start[m2]; b < b1; ++b) {
-        const Anchor B = load_anchor(s, b);
-        float c;
-        if (!ls_eval(A, B, c)) continue;
-        if (FILL) {
-          if (out < caps.max_ls) { s.ls_ab[out] = make_int2(a, b); s.ls_c[out] = c; }
-        }
-        ++out;
-      }
-    }
-    if (!FILL) s.ls_start[a] = out;
   }
 }
 

@@ -45,9 +45,9 @@ __device__ __forceinline__ float arcfac(float u) {
 }
 
 // SPEC.md 4.1.  p1 = lower hit, p2 = upper hit.  Returns pass; fills r1, c, w.
-__device__ __forceinline__ bool md_eval(float x1, float y1, float z1, float r1, float x2, float y2, float z2, int mt,
+// r1, r2 = sqrt(x*x + y*y) of the two hits (computed once per hit by a0 with the same operations).
+__device__ __forceinline__ bool md_eval(float x1, float y1, float z1, float r1, float x2, float y2, float z2, float r2, int mt,
                                         float& c, float& w) {
-  const float r2 = fq(fa(fm(x2, x2), fm(y2, y2)));
   const float dx = fs(x2, x1), dy = fs(y2, y1), dz = fs(z2, z1);
   const float drho = fd(fa(fm(x1, dx), fm(y1, dy)), r1);
   const float dt = fd(fs(fm(x1, dy), fm(y1, dx)), r1);
@@ -72,6 +72,42 @@ __device__ __forceinline__ bool md_eval(float x1, float y1, float z1, float r1, 
   c = fd(fm(-2.0f, dt), den);
   w = fd(fm(2.0f, dtol), den);
   return true;
+}
+
+// approximate reciprocal / square roots (1-2 ulp, single MUFU instruction) for the prefilters only
+__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_fast(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sqrt_fast(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// Conservative prefilter of md_eval: exact pass  =>  prefilter pass (never the other way round is needed).
+// The numerators are formed with the same exactly-rounded operations as md_eval, so their cancellation
+// is shared; the divisions and the square root are replaced by approximations (a few ulp) and every
+// comparison gets a relative margin of 1e-4 plus an absolute one that exceeds the rounding of the exact
+// evaluation by >= 20x.  Non-finite intermediates pass (the exact test decides).
+__device__ __forceinline__ bool md_prefilter(float x1, float y1, float z1, float r1, float x2, float y2, float z2, float r2, int mt) {
+  const float dx = fs(x2, x1), dy = fs(y2, y1), dz = fs(z2, z1);
+  const float nrho = fa(fm(x1, dx), fm(y1, dy));
+  const float nt = fs(fm(x1, dy), fm(y1, dx));
+  const float S = fminf(1.0f, fm(r2, LST_C_HALF));
+  const float inv = rcp_fast(r1);
+  const float drho = nrho * inv, dt = nt * inv;
+  bool ok;
+  if (!(mt & 2)) {
+    const float t = drho * z1 * inv;
+    const float L = sqrt_fast(dt * dt + drho * drho);
+    const bool m1 = nrho > 0.0f;
+    const bool m2 = fabsf(dz - t) <= (drho * LST_Z0_MAX * inv + tol_dl2(mt)) * 1.0001f + 1.0e-5f * (fabsf(dz) + fabsf(t));
+    const bool m3 = fabsf(dt) <= (L * S + tol_dt(mt)) * 1.0001f;
+    ok = m1 && m2 && m3;
+    if (!(L < 1.0e30f) || !(fabsf(t) < 1.0e30f)) ok = true;
+  } else {
+    const float Ls = fabsf(dz) * r1 * rcp_fast(fabsf(z1));
+    const bool m2 = fabsf(drho - Ls) <= (0.15f * Ls + tol_dl2(mt)) * 1.0001f + 1.0e-5f * (fabsf(drho) + Ls);
+    const bool m3 = fabsf(dt) <= (1.3f * Ls * S + tol_dt(mt)) * 1.0001f;
+    ok = m2 && m3;
+    if (!(Ls < 1.0e30f) || !(fabsf(drho) < 1.0e30f) || !(fabsf(dt) < 1.0e30f)) ok = true;
+  }
+  return ok;
 }
 
 struct Anchor {   // what the later stages need of an MD
@@ -101,6 +137,22 @@ __device__ __forceinline__ bool ls_eval(const Anchor& A, const Anchor& B, float&
   if (!(lhs <= rhs)) return false;                                                       // L2
   c_out = c;
   return true;
+}
+
+// Conservative prefilter of ls_eval (L1 and both L3; L2 is left to the exact test).  `cr` is formed exactly
+// as in ls_eval; c is approximated to a few ulp (|c| <= 0.015 => absolute error < 2e-8) and the L3
+// comparisons carry an absolute margin of 3e-7 (w >= ~5e-4 for any real MD) -- DESIGN.md "Prefilters".
+// Rejections are positive comparisons, so a NaN anywhere lets the pair through to the exact test.
+// A2 / B2 = (c, w, f, -) of the two MDs (f = 0.3 for endcap MDs, else 0).
+__device__ __forceinline__ bool ls_prefilter(float4 A, float4 A2, float4 B, float4 B2) {
+  const float dx = fs(B.x, A.x), dy = fs(B.y, A.y);
+  const float cr = fs(fm(A.x, dy), fm(A.y, dx));
+  const float dd = dx * dx + dy * dy;
+  const float c = -2.0f * cr * rsqrt_fast(dd) * rcp_fast(A.w * B.w);
+  const float ac = fabsf(c);
+  const bool rej = (ac > LST_C_MAX105 * 1.0001f) | (fabsf(A2.x - c) > (A2.y + A2.z * ac) * 1.0001f + 3.0e-7f) |
+                   (fabsf(B2.x - c) > (B2.y + B2.z * ac) * 1.0001f + 3.0e-7f);
+  return !rej | (dd < 1.0e-30f);      // dd ~ 0: the approximations may overflow where the exact test does not
 }
 
 struct Pt {   // anchor position + long-direction tolerances

@@ -1,190 +1,359 @@
-// lst_pairs.cuh -- pair-parallel MD (a1) and LS (a2) kernels.
+// lst_pairs.cuh -- single-pass, order-preserving MD (a1) and LS (a2) kernels.
 //
-// Both stages test every cell of a per-module rectangle: rows = inner objects of module m (lower hits /
-// MDs of m), columns = the module's candidate partners (upper hits of m / MDs of the CSR-connected
-// modules), and the build order of SPEC.md 4.1-4.2 is row-major inside the module.  A warp sweeps the
-// rectangle 32 cells at a time (narrow rectangles pack several rows into one sweep), so all 32 lanes
-// evaluate a cut at once instead of one thread looping over its own row.
-//
-// Single evaluation, deterministic order:
-//   1. pairs:    every passing pair becomes a record (row, rank inside the row, payload) appended to an
-//                unordered per-slot record buffer (warp-staged in shared memory, one atomicAdd per flush);
-//                the row's pass count goes to the scan array (md_off / ls_start).
-//   2. scan:     exclusive scan of the row counts (k_scan), clamped to capacity, overflow flagged.
-//   3. finalize: one thread per record scatters it to scan[row] + rank -- the SPEC.md build order.
-// When a stage overflows its capacity the record buffer (same capacity) has dropped arbitrary records;
-// the thread-per-row fill kernels of lst_kernels.cuh then rewrite the first `cap` objects in build
-// order (they return immediately unless the stage's overflow bit is set).
+// Both stages test every cell of per-module rectangles (rows = inner objects of module m, columns = the
+// module's candidate partners) and must emit the passing cells in the build order of SPEC.md 4.1-4.2
+// (module, row, column).  The cells of all rectangles, in build order, form one flat index space (prefix scan
+// of the per-module cell counts); one warp owns one *link* = a fixed-size range of that space:
+//   1. prefilter:  all 32 lanes evaluate the cheap conservative form of the cuts (lst_math.cuh) on 32 cells;
+//                  survivors (a few %) are appended, in order, to a per-warp queue in shared memory;
+//   2. exact:      whenever the queue holds >= 32 cells a full warp evaluates the exact SPEC.md arithmetic
+//                  on them; passing cells are appended, in order, to the warp's staging buffer;
+//   3. place:      the link appends its objects (already in order) to an unordered per-slot record buffer and
+//                  stores its count; a block scan over the link counts (k_scan) gives every link its base,
+//                  and a per-link finalize warp copies the records to their final positions and writes the
+//                  range tables (md_start / ls_start) of the rows the link owns.
+// The output order depends only on the flat index, never on scheduling (bit-reproducible).  The staging
+// buffer holds as many objects as a link has cells, so it cannot overflow.
+// Capacity overflow: the record buffer (same capacity as the stage) may then have dropped records of early
+// links, so the CHAIN instantiation re-runs the stage: links are handed out by an atomic ticket, each obtains
+// the count of all earlier links by decoupled look-back and writes its first objects in place (a link only
+// waits for links that are already running: no deadlock).  It returns at once unless the overflow bit is set
+// (in-place waiting behind slow links makes it ~4x slower than the record path, measured r01).
 #pragma once
 #include "lst_kernels.cuh"
 
 namespace lst {
 
-constexpr int PAIR_WARPS = 8;        // warps per block
-constexpr int STAGE_CAP = 64;        // staged records per warp (flush at >= 32)
-constexpr int ITEMS_PER_WARP = 4;    // consecutive work items a warp takes at a time
-constexpr int CAND_CAP = 512;        // candidate-MD index table per warp (shared memory)
+constexpr int PAIR_WARPS = 4;        // warps per block
+constexpr int Q_CAP = 64;            // survivor queue per warp (drained at >= 32)
+constexpr int MD_WIN = 32;           // modules of a link cached in shared memory (one per lane)
 
 __device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
-template <typename Rec>
-__device__ __forceinline__ void flush_stage(Rec* __restrict__ stage, int& staged, int* counter, Rec* __restrict__ out, int cap, int lane) {
-  int base = 0;
-  if (lane == 0) base = atomicAdd(counter, staged);
-  base = __shfl_sync(0xffffffffu, base, 0);
-  for (int i = lane; i < staged; i += 32)
-    if (base + i < cap) out[base + i] = stage[i];
-  staged = 0;
-  __syncwarp();
+// ---- decoupled look-back over 64-bit status words: flag (2 bits) | run epoch (30 bits) | value (32 bits).
+// A word counts only if its epoch is the current run's (lst_api.cu increments it per launch sequence), so the
+// status arrays never need clearing.
+constexpr unsigned long long CH_AGG = 1ull << 62, CH_INC = 2ull << 62, CH_VAL = 0xFFFFFFFFull;
+__device__ __forceinline__ unsigned chain_flag(unsigned long long w, unsigned epoch) {
+  return (((unsigned)(w >> 32)) & 0x3FFFFFFFu) == epoch ? (unsigned)(w >> 62) : 0u;
+}
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// exclusive prefix of `count` over links [0, link); called by all 32 lanes, publishes the inclusive prefix
+__device__ __forceinline__ int chain_exclusive(unsigned long long* st, int link, int count, int lane, unsigned epoch) {
+  const unsigned long long ep = (unsigned long long)epoch << 32;
+  if (link == 0) {
+    if (lane == 0) st_status(st, CH_INC | ep | (unsigned long long)(unsigned)count);
+    return 0;
+  }
+  if (lane == 0) st_status(st + link, CH_AGG | ep | (unsigned long long)(unsigned)count);
+  int excl = 0;
+  int idx = link - 1 - lane;
+  while (true) {
+    unsigned long long w;
+    unsigned fl;
+    do {
+      w = (idx >= 0) ? ld_status(st + idx) : (CH_INC | ep);
+      fl = chain_flag(w, epoch);
+    } while (__any_sync(0xffffffffu, fl == 0u));
+    const unsigned inc = __ballot_sync(0xffffffffu, fl == 2u);
+    const int first = inc ? (__ffs(inc) - 1) : 31;     // nearest predecessor that holds an inclusive prefix
+    int v = (lane <= first) ? (int)(w & CH_VAL) : 0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    excl += v;
+    if (inc) break;
+    idx -= 32;
+  }
+  if (lane == 0) st_status(st + link, CH_INC | ep | (unsigned long long)(unsigned)(excl + count));
+  return excl;
 }
 
-// largest m in [0, M) with off[m] <= i (off non-decreasing, off[0] = 0 <= i < off[M]): 32-ary search, the
-// warp probes 32 positions per round
-__device__ __forceinline__ int find_module(const int* __restrict__ off, int M, int i, int lane) {
-  int lo = 0, n = M;
-  while (n > 1) {
-    const int step = (n + 31) >> 5;
-    const int idx = lo + lane * step;
-    const bool le = (idx < lo + n) && (off[idx] <= i);
-    const int j = __popc(__ballot_sync(0xffffffffu, le)) - 1;
-    const int nlo = lo + j * step;
-    n = min(step, lo + n - nlo);
-    lo = nlo;
+__device__ __forceinline__ int warp_ticket(int* counter, int lane) {
+  int t = 0;
+  if (lane == 0) t = atomicAdd(counter, 1);
+  return __shfl_sync(0xffffffffu, t, 0);
+}
+
+
+// first index i in [0, n] with off[i] > x (off non-decreasing); n + 1 if none
+__device__ __forceinline__ int upper_bound_g(const int* __restrict__ off, int n, int x) {
+  int lo = 0, hi = n + 1;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (off[mid] > x) hi = mid; else lo = mid + 1;
   }
   return lo;
 }
+// largest m in [mS, mE] with off[m] <= f (exists by construction); among equal offsets the last one, i.e. the
+// module that really owns cell f
+__device__ __forceinline__ int owner_module(const int* __restrict__ off, int mS, int mE, int f) {
+  int lo = mS, hi = mE;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (off[mid] <= f) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+__device__ __forceinline__ int lower_bound_s(const int* a, int n, int x) {   // first i with a[i] >= x
+  int lo = 0, hi = n;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (a[mid] < x) lo = mid + 1; else hi = mid;
+  }
+  return lo;
+}
+__device__ __forceinline__ void divmod_small(int v, int d, int& q, int& r) {   // 0 <= v < 2^22, d > 0
+  q = (int)(((float)v + 0.5f) * rcp_fast((float)d));
+  r = v - q * d;
+  if (r < 0) { --q; r += d; } else if (r >= d) { ++q; r -= d; }
+}
 
 // ------------------------------------------------------------------------------------------------
-// a1 pairs: rows = lower hits of m, columns = upper hits of m
+// a1: cells = (lower hit i, upper hit j) of module m, flat index md_pair_off[m] + i*n_up + j
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_pairs(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  __shared__ MdRec stage_all[PAIR_WARPS][STAGE_CAP];
+struct MdWarp {   // per-warp shared memory
+  int w_off[MD_WIN + 1], w_lb[MD_WIN], w_ub[MD_WIN], w_nup[MD_WIN], w_mt[MD_WIN];   // the link's first modules
+  int q_lo[Q_CAP], q_up[Q_CAP], q_mt[Q_CAP], q_f[Q_CAP];
+  int p_lo[MD_LP], p_up[MD_LP], p_mt[MD_LP], p_f[MD_LP];
+  float p_c[MD_LP], p_w[MD_LP];
+};
+
+// exact evaluation of `n` (<= 32) queued cells; appends the passing ones in order; returns the new count
+__device__ __forceinline__ int md_drain(const Slot& s, MdWarp& W, int n, int pn, int lane, unsigned lt) {
+  bool pass = false;
+  int p_lo = 0, p_up = 0, mtm = 0, f = 0;
+  float c = 0.f, w = 0.f;
+  if (lane < n) {
+    p_lo = W.q_lo[lane]; p_up = W.q_up[lane]; mtm = W.q_mt[lane]; f = W.q_f[lane];
+    const float4 h1 = s.hit[p_lo], h2 = s.hit[p_up];
+    pass = md_eval(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3, c, w);
+  }
+  const unsigned mask = __ballot_sync(0xffffffffu, pass);
+  if (pass) {
+    const int i = pn + __popc(mask & lt);
+    W.p_lo[i] = p_lo; W.p_up[i] = p_up; W.p_mt[i] = mtm; W.p_f[i] = f; W.p_c[i] = c; W.p_w[i] = w;
+  }
+  return pn + __popc(mask);
+}
+
+template <bool CHAIN>
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __restrict__ slots, Geo geo, Caps caps, unsigned epoch) {
+  __shared__ MdWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  MdRec* stage = stage_all[warp];
+  if (CHAIN && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;
+  const int lane = threadIdx.x & 31;
+  MdWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
-  int staged = 0;
   const int M = geo.n_modules;
-  const int* __restrict__ ioff = s.md_item_off;
+  const int* __restrict__ off = s.md_pair_off;
   const int* __restrict__ ss = s.sensor_start;
   const float4* __restrict__ hit = s.hit;
-  const int T = ioff[M];
-  const int n_chunks = (T + ITEMS_PER_WARP - 1) / ITEMS_PER_WARP;
-  for (int chunk = blockIdx.x * PAIR_WARPS + warp; chunk < n_chunks; chunk += gridDim.x * PAIR_WARPS) {
-    const int i_end = min(T, (chunk + 1) * ITEMS_PER_WARP);
-    int m_end = -1, m_beg = 0, m = 0;
-    int lb = 0, ub = 0, n_lo = 0, L = 0, mt = 0;
-    ItemPlan pl{};
-    for (int i = chunk * ITEMS_PER_WARP; i < i_end; ++i) {
-      if (i >= m_end) {   // next module
-        m = find_module(ioff, M, i, lane);
-        m_beg = ioff[m]; m_end = ioff[m + 1];
-        lb = ss[2 * m]; ub = ss[2 * m + 1];
-        n_lo = ub - lb; L = ss[2 * m + 2] - ub;
-        mt = geo.modt[m];
-        pl = item_plan(n_lo, L);
+  const int total_cells = min(off[M], MAX_CELLS);       // beyond: flagged by the scan that made `off`
+  const int n_links = total_cells / MD_LP + 1;
+  const int cap = caps.max_md;
+  int link = blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5);
+  while (true) {
+    if (CHAIN) link = warp_ticket(s.cnt + LST_CNT_TICKET_MD, lane);
+    if (link >= n_links) break;
+    const int lo = link * MD_LP, hi = min(total_cells, lo + MD_LP);
+    int qn = 0, pn = 0;
+    if (lo < hi) {
+      // cache the first MD_WIN modules of the link (normally all of them)
+      const int mS = s.md_link_mod[link];
+      __syncwarp();
+      {
+        const int m = mS + lane;
+        int o = 0x7fffffff, lb = 0, ub = 0, ue = 0, mt = 0;
+        if (m < M) { o = off[m]; lb = ss[2 * m]; ub = ss[2 * m + 1]; ue = ss[2 * m + 2]; mt = geo.modt[m]; }
+        W.w_off[lane] = o; W.w_lb[lane] = lb; W.w_ub[lane] = ub; W.w_nup[lane] = ue - ub; W.w_mt[lane] = (m << 2) | mt;
+        if (lane == 0) W.w_off[MD_WIN] = (mS + MD_WIN <= M) ? off[mS + MD_WIN] : 0x7fffffff;
       }
-      const int row0 = (i - m_beg) * pl.rows_per_item;
-      const int row1 = min(n_lo, row0 + pl.rows_per_item);
-      if (pl.S == 1) {
-        // narrow rectangle: W columns per row, R = 32/W rows per sweep; the lane's column is fixed
-        const int W = pl.W, lw = lane & (W - 1), rs = lane / W;
-        const bool vcol = lw < L;
-        const int pj = ub + min(lw, L - 1);
-        const float4 h2 = hit[pj];
-        const unsigned rowmask = (W == 32) ? 0xffffffffu : (((1u << W) - 1u) << (rs * W));
-        for (int r0 = row0; r0 < row1; r0 += pl.R) {
-          const int row = r0 + rs;
-          const int pi = lb + min(row, n_lo - 1);
-          const float4 h1 = hit[pi];
-          const float r1 = fq(fa(fm(h1.x, h1.x), fm(h1.y, h1.y)));
-          float c = 0.f, w = 0.f;
-          const bool pass = vcol && row < row1 && md_eval(h1.x, h1.y, h1.z, r1, h2.x, h2.y, h2.z, mt, c, w);
-          const unsigned mask = __ballot_sync(0xffffffffu, pass);
-          if (mask) {
-            const unsigned rm = mask & rowmask;
-            if (lw == 0 && row < row1 && rm) s.md_off[pi] = __popc(rm);
-            if (pass) {
-              MdRec rec; rec.p_lo = pi; rec.p_up = pj; rec.rank = __popc(rm & lt); rec.modt = (m << 2) | mt;
-              rec.c = c; rec.w = w; rec.r1 = r1; rec.pad = 0.f;
-              stage[staged + __popc(mask & lt)] = rec;
-            }
-            staged += __popc(mask);
+      __syncwarp();
+      const int win_end = W.w_off[MD_WIN];
+      for (int f0 = lo; f0 < hi; f0 += 32) {
+        const int f = f0 + lane;
+        bool pre = false;
+        int p_lo = 0, p_up = 0, mtm = 0;
+        if (f < hi) {
+          int loc, lb, ub, nup;
+          if (f < win_end) {
+            int k = 0;
+#pragma unroll
+            for (int step = MD_WIN / 2; step > 0; step >>= 1)
+              if (W.w_off[k + step] <= f) k += step;
+            loc = f - W.w_off[k]; lb = W.w_lb[k]; ub = W.w_ub[k]; nup = W.w_nup[k]; mtm = W.w_mt[k];
+          } else {     // sparse region: the link spans more than MD_WIN modules
+            const int m = owner_module(off, mS + MD_WIN, M - 1, f);
+            loc = f - off[m]; lb = ss[2 * m]; ub = ss[2 * m + 1]; nup = ss[2 * m + 2] - ub; mtm = (m << 2) | geo.modt[m];
+          }
+          int i, j;
+          divmod_small(loc, nup, i, j);
+          p_lo = lb + i; p_up = ub + j;
+          const float4 h1 = hit[p_lo], h2 = hit[p_up];
+          pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3);
+        }
+        const unsigned mask = __ballot_sync(0xffffffffu, pre);
+        if (mask) {
+          if (pre) { const int i = qn + __popc(mask & lt); W.q_lo[i] = p_lo; W.q_up[i] = p_up; W.q_mt[i] = mtm; W.q_f[i] = f - lo; }
+          qn += __popc(mask);
+          __syncwarp();
+          if (qn >= 32) {
+            pn = md_drain(s, W, 32, pn, lane, lt);
             __syncwarp();
-            if (staged >= 32) flush_stage(stage, staged, s.cnt + LST_CNT_TMP_MD, s.md_rec, caps.max_md, lane);
+            const int rest = qn - 32;
+            int a = 0, b = 0, c = 0, d = 0;
+            if (lane < rest) { a = W.q_lo[32 + lane]; b = W.q_up[32 + lane]; c = W.q_mt[32 + lane]; d = W.q_f[32 + lane]; }
+            __syncwarp();
+            if (lane < rest) { W.q_lo[lane] = a; W.q_up[lane] = b; W.q_mt[lane] = c; W.q_f[lane] = d; }
+            qn = rest;
+            __syncwarp();
           }
         }
-      } else {
-        // wide rectangle: one row at a time, S sweeps per row
-        for (int row = row0; row < row1; ++row) {
-          const int pi = lb + row;
-          const float4 h1 = hit[pi];
-          const float r1 = fq(fa(fm(h1.x, h1.x), fm(h1.y, h1.y)));
-          int running = 0;
-          for (int sw = 0; sw < pl.S; ++sw) {
-            const int col = sw * 32 + lane;
-            const int pj = ub + min(col, L - 1);
-            const float4 h2 = hit[pj];
-            float c = 0.f, w = 0.f;
-            const bool pass = col < L && md_eval(h1.x, h1.y, h1.z, r1, h2.x, h2.y, h2.z, mt, c, w);
-            const unsigned mask = __ballot_sync(0xffffffffu, pass);
-            if (mask) {
-              if (pass) {
-                MdRec rec; rec.p_lo = pi; rec.p_up = pj; rec.rank = running + __popc(mask & lt); rec.modt = (m << 2) | mt;
-                rec.c = c; rec.w = w; rec.r1 = r1; rec.pad = 0.f;
-                stage[staged + __popc(mask & lt)] = rec;
-              }
-              staged += __popc(mask);
-              running += __popc(mask);
-              __syncwarp();
-              if (staged >= 32) flush_stage(stage, staged, s.cnt + LST_CNT_TMP_MD, s.md_rec, caps.max_md, lane);
-            }
-          }
-          if (lane == 0 && running) s.md_off[pi] = running;
+      }
+      if (qn) pn = md_drain(s, W, qn, pn, lane, lt);
+      __syncwarp();
+    }
+    if (!CHAIN) {      // append the link's MDs to the record buffer, remember where and how many
+      int soff = 0;
+      if (lane == 0) { soff = pn ? atomicAdd(s.cnt + LST_CNT_FILL_MD, pn) : 0; s.md_link_cnt[link] = pn; s.md_link_soff[link] = soff; }
+      soff = __shfl_sync(0xffffffffu, soff, 0);
+      for (int i = lane; i < pn; i += 32)
+        if (soff + i < cap) {
+          MdRec r; r.p_lo = W.p_lo[i]; r.p_up = W.p_up[i]; r.mtm = W.p_mt[i]; r.f = W.p_f[i]; r.c = W.p_c[i]; r.w = W.p_w[i]; r.link = link; r.pad = 0;
+          s.md_rec[soff + i] = r;
         }
+      __syncwarp();
+      link += gridDim.x * PAIR_WARPS;
+      continue;
+    }
+    // CHAIN (overflow re-run): base by look-back, objects and range table written in place
+    const int base = chain_exclusive(s.chain_md, link, pn, lane, epoch);
+    for (int i = lane; i < pn; i += 32) {
+      const int pos = base + i;
+      if (pos < cap) {
+        const int p_lo = W.p_lo[i], p_up = W.p_up[i];
+        s.md_hits[pos] = make_int2(s.hit_orig[p_lo], s.hit_orig[p_up]);
+        s.md_modt[pos] = W.p_mt[i];
+        s.md_pos[pos] = hit[p_lo];              // (x, y, z, r1)
+        s.md_cw[pos] = make_float2(W.p_c[i], W.p_w[i]);
+        s.md_aux[pos] = make_float4(W.p_c[i], W.p_w[i], md_relf(W.p_mt[i] & 3), 0.f);
       }
     }
+    int sr = 0;
+    if (lane < 2) sr = upper_bound_g(off, M, lane == 0 ? lo - 1 : lo + MD_LP - 1);
+    const int mOwn0 = __shfl_sync(0xffffffffu, sr, 0), mOwn1 = min(M, __shfl_sync(0xffffffffu, sr, 1));
+    for (int m = mOwn0 + lane; m < mOwn1; m += 32) s.md_start[m] = min(base + lower_bound_s(W.p_f, pn, off[m] - lo), cap);
+    if (link == n_links - 1 && lane == 0) {
+      const int total = base + pn;
+      s.md_start[M] = min(total, cap);
+      s.cnt[LST_CNT_MD] = min(total, cap);
+      s.cnt[LST_CNT_RAW_MD] = total;
+    }
+    __syncwarp();
   }
-  if (staged) flush_stage(stage, staged, s.cnt + LST_CNT_TMP_MD, s.md_rec, caps.max_md, lane);
 }
 
-// a1 finalize: scatter the records to build order; candidate count L of every module for the LS sweep
+// a1 finalize (md_link_cnt holds the exclusive scan of the link counts by now): one thread per record copies it
+// to base[link] + its index inside the link; one thread per module writes md_start[m] = number of MDs before the
+// module's first cell
 __global__ void __launch_bounds__(256) k_md_final(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   const Slot& s = slots[blockIdx.y];
-  const int n_rec = min(s.cnt[LST_CNT_TMP_MD], caps.max_md);
-  LST_FOR_ITEMS(i, n_rec) {
-    const MdRec rec = s.md_rec[i];
-    const int pos = s.md_off[rec.p_lo] + rec.rank;
-    if (pos < caps.max_md) {
-      const float4 h1 = s.hit[rec.p_lo];
-      s.md_hits[pos] = make_int2(s.hit_orig[rec.p_lo], s.hit_orig[rec.p_up]);
-      s.md_modt[pos] = rec.modt;
-      s.md_pos[pos] = make_float4(h1.x, h1.y, h1.z, rec.r1);
-      s.md_cw[pos] = make_float2(rec.c, rec.w);
-    }
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) return;       // the CHAIN pass rewrites the stage
+  const int M = geo.n_modules;
+  const int* __restrict__ off = s.md_pair_off;
+  const int* __restrict__ base = s.md_link_cnt;
+  const int* __restrict__ soff = s.md_link_soff;
+  const int n_rec = min(s.cnt[LST_CNT_FILL_MD], caps.max_md);
+  LST_FOR_ITEMS(j, n_rec) {
+    const MdRec r = s.md_rec[j];
+    const int pos = base[r.link] + (j - soff[r.link]);
+    s.md_hits[pos] = make_int2(s.hit_orig[r.p_lo], s.hit_orig[r.p_up]);
+    s.md_modt[pos] = r.mtm;
+    s.md_pos[pos] = s.hit[r.p_lo];
+    s.md_cw[pos] = make_float2(r.c, r.w);
+    s.md_aux[pos] = make_float4(r.c, r.w, md_relf(r.mtm & 3), 0.f);     // (c, w, f, -): one load for the LS prefilter
   }
-  LST_FOR_ITEMS(m, geo.n_modules) {
-    int L = 0;
-    const int e1 = geo.rowptr[m + 1];
-    if (s.md_start[m + 1] > s.md_start[m])
-      for (int e = geo.rowptr[m]; e < e1; ++e) { const int m2 = geo.col[e]; L += s.md_start[m2 + 1] - s.md_start[m2]; }
-    s.ls_L[m] = L;
-    s.ls_item_off[m] = item_plan(s.md_start[m + 1] - s.md_start[m], L).n_items;
+  const int total_cells = min(off[M], MAX_CELLS);
+  LST_FOR_ITEMS(m, M + 1) {
+    const int x = min(off[m], total_cells);
+    const int link = x / MD_LP, rel = x - link * MD_LP;
+    const int b = base[link], pn = base[link + 1] - b;
+    const MdRec* __restrict__ rec = s.md_rec + soff[link];
+    int l = 0, h = pn;
+    while (l < h) { const int mid = (l + h) >> 1; if (rec[mid].f < rel) l = mid + 1; else h = mid; }
+    s.md_start[m] = b + l;
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2 pairs: rows = MDs of m, columns = MDs of the CSR-connected modules (ascending MD index)
+// a2: cells = (MD a of module m, candidate column) with flat index ls_off[m] + row*L[m] + col; the columns of m
+// are the MDs of its CSR-connected modules in ascending MD index (L[m] of them, listed in ls_cand)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ Anchor load_anchor2(const float4* __restrict__ pos, const float2* __restrict__ cw,
-                                               const int* __restrict__ modt, int i) {
-  const float4 p = pos[i];
-  const float2 q = cw[i];
-  Anchor a; a.x = p.x; a.y = p.y; a.z = p.z; a.r = p.w; a.c = q.x; a.w = q.y; a.mt = modt[i] & 3;
+// plan (one block per event): candidate count L[m], exclusive scans of the cell counts n_m * L[m] and of the
+// candidate-table offsets, the link -> module table and the candidate table itself
+__global__ void __launch_bounds__(SCAN_THREADS) k_ls_plan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ int sm[34];
+  const Slot& s = slots[blockIdx.y];
+  const int M = geo.n_modules;
+  const int* __restrict__ mds = s.md_start;
+  for (int m = threadIdx.x; m < M; m += SCAN_THREADS) {
+    const int n_m = mds[m + 1] - mds[m];
+    int L = 0;
+    if (n_m > 0) {
+      const int e1 = geo.rowptr[m + 1];
+      for (int e = geo.rowptr[m]; e < e1; ++e) { const int m2 = geo.col[e]; L += mds[m2 + 1] - mds[m2]; }
+    }
+    long long cells = (long long)n_m * L;
+    if (cells > MAX_CELLS) {      // beyond any event the capacities admit: drop the module's cells, flag the stage
+      cells = 0; L = 0;
+      atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_LS);
+    }
+    s.ls_L[m] = L;
+    s.ls_off[m] = (int)cells;
+    s.ls_coff[m] = L;
+  }
+  __syncthreads();
+  const int total = block_scan_inplace(s.ls_off, M, 0x7fffffff, sm);
+  __syncthreads();
+  block_scan_inplace(s.ls_coff, M, 0x7fffffff, sm);
+  __syncthreads();
+  if (threadIdx.x == 0 && total > MAX_CELLS) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_LS);
+  link_owner_table(s.ls_off, M, LS_LP, s.ls_link_mod);
+  const int cand_cap = CAND_PER_MD * caps.max_md;
+  for (int m = threadIdx.x; m < M; m += SCAN_THREADS) {
+    const int L = s.ls_L[m];
+    int o = s.ls_coff[m];
+    if (L == 0 || o + L > cand_cap) continue;        // modules beyond the table walk the CSR row instead
+    const int e1 = geo.rowptr[m + 1];
+    for (int e = geo.rowptr[m]; e < e1; ++e) {
+      const int m2 = geo.col[e];
+      const int b1 = mds[m2 + 1];
+      for (int b = mds[m2]; b < b1; ++b) s.ls_cand[o++] = b;
+    }
+  }
+}
+
+struct LsWarp {
+  int q_a[Q_CAP], q_b[Q_CAP], q_f[Q_CAP];
+  int p_a[LS_LP], p_b[LS_LP], p_f[LS_LP];
+  float p_c[LS_LP];
+};
+
+__device__ __forceinline__ Anchor load_anchor(const Slot& s, int i) {
+  const float4 p = s.md_pos[i];
+  const float2 q = s.md_cw[i];
+  Anchor a; a.x = p.x; a.y = p.y; a.z = p.z; a.r = p.w; a.c = q.x; a.w = q.y; a.mt = s.md_modt[i] & 3;
   return a;
 }
 
-// column -> MD index by walking the CSR row (only for rows with more than CAND_CAP candidates)
+// column -> MD index by walking the CSR row (only for modules beyond the candidate table)
 __device__ __noinline__ int cand_walk(const Slot& s, const Geo& geo, int m, int col) {
   const int e1 = geo.rowptr[m + 1];
   for (int e = geo.rowptr[m]; e < e1; ++e) {
@@ -196,114 +365,164 @@ __device__ __noinline__ int cand_walk(const Slot& s, const Geo& geo, int m, int 
   return 0;
 }
 
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_pairs(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  __shared__ LsRec stage_all[PAIR_WARPS][STAGE_CAP];
-  __shared__ int cand_all[PAIR_WARPS][CAND_CAP];
-  const Slot& s = slots[blockIdx.y];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  LsRec* stage = stage_all[warp];
-  int* cand = cand_all[warp];
-  const unsigned lt = lanemask_lt();
-  int staged = 0;
-  const int M = geo.n_modules;
-  const int* __restrict__ ioff = s.ls_item_off;
-  const int* __restrict__ mds = s.md_start;
-  const float4* __restrict__ mpos = s.md_pos;
-  const float2* __restrict__ mcw = s.md_cw;
-  const int* __restrict__ mmodt = s.md_modt;
-  const int T = ioff[M];
-  const int n_chunks = (T + ITEMS_PER_WARP - 1) / ITEMS_PER_WARP;
-  for (int chunk = blockIdx.x * PAIR_WARPS + warp; chunk < n_chunks; chunk += gridDim.x * PAIR_WARPS) {
-    const int i_end = min(T, (chunk + 1) * ITEMS_PER_WARP);
-    int m_end = -1, m_beg = 0, m = 0, a0 = 0, n_m = 0, L = 0;
-    bool tabled = false;
-    ItemPlan pl{};
-    for (int i = chunk * ITEMS_PER_WARP; i < i_end; ++i) {
-      if (i >= m_end) {   // next module: candidate table cand[col] = MD index over the connected modules' MD ranges
-        m = find_module(ioff, M, i, lane);
-        m_beg = ioff[m]; m_end = ioff[m + 1];
-        a0 = mds[m]; n_m = mds[m + 1] - a0;
-        L = s.ls_L[m];
-        pl = item_plan(n_m, L);
-        tabled = L <= CAND_CAP;
-        if (tabled) {
-          __syncwarp();
-          const int e0 = geo.rowptr[m], e1 = geo.rowptr[m + 1];
-          int cum = 0;
-          for (int eb = e0; eb < e1; eb += 32) {
-            const int e = eb + lane;
-            int b0 = 0, n = 0;
-            if (e < e1) { const int m2 = geo.col[e]; b0 = mds[m2]; n = mds[m2 + 1] - b0; }
-            int inc = n;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-            const int off = cum + inc - n;
-            for (int t = 0; t < n; ++t) cand[off + t] = b0 + t;        // a handful of MDs per connected module
-            cum += __shfl_sync(0xffffffffu, inc, 31);
-          }
-          __syncwarp();
-        }
-      }
-      const int row0 = (i - m_beg) * pl.rows_per_item;
-      const int row1 = min(n_m, row0 + pl.rows_per_item);
-      if (pl.S == 1) {
-        const int W = pl.W, lw = lane & (W - 1), rs = lane / W;
-        const bool vcol = lw < L;
-        const int b = cand[min(lw, L - 1)];
-        const Anchor B = load_anchor2(mpos, mcw, mmodt, b);
-        const unsigned rowmask = (W == 32) ? 0xffffffffu : (((1u << W) - 1u) << (rs * W));
-        for (int r0 = row0; r0 < row1; r0 += pl.R) {
-          const int row = r0 + rs;
-          const int a = a0 + min(row, n_m - 1);
-          const Anchor A = load_anchor2(mpos, mcw, mmodt, a);
-          float c = 0.f;
-          const bool pass = vcol && row < row1 && ls_eval(A, B, c);
-          const unsigned mask = __ballot_sync(0xffffffffu, pass);
-          if (mask) {
-            const unsigned rm = mask & rowmask;
-            if (lw == 0 && row < row1 && rm) s.ls_start[a] = __popc(rm);
-            if (pass) { LsRec rec; rec.a = a; rec.b = b; rec.rank = __popc(rm & lt); rec.c = c; stage[staged + __popc(mask & lt)] = rec; }
-            staged += __popc(mask);
-            __syncwarp();
-            if (staged >= 32) flush_stage(stage, staged, s.cnt + LST_CNT_TMP_LS, s.ls_rec, caps.max_ls, lane);
-          }
-        }
-      } else {
-        for (int row = row0; row < row1; ++row) {
-          const int a = a0 + row;
-          const Anchor A = load_anchor2(mpos, mcw, mmodt, a);
-          int running = 0;
-          for (int sw = 0; sw < pl.S; ++sw) {
-            const int col = sw * 32 + lane;
-            const int cc = min(col, L - 1);
-            const int b = tabled ? cand[cc] : cand_walk(s, geo, m, cc);
-            const Anchor B = load_anchor2(mpos, mcw, mmodt, b);
-            float c = 0.f;
-            const bool pass = col < L && ls_eval(A, B, c);
-            const unsigned mask = __ballot_sync(0xffffffffu, pass);
-            if (mask) {
-              if (pass) { LsRec rec; rec.a = a; rec.b = b; rec.rank = running + __popc(mask & lt); rec.c = c; stage[staged + __popc(mask & lt)] = rec; }
-              staged += __popc(mask);
-              running += __popc(mask);
-              __syncwarp();
-              if (staged >= 32) flush_stage(stage, staged, s.cnt + LST_CNT_TMP_LS, s.ls_rec, caps.max_ls, lane);
-            }
-          }
-          if (lane == 0 && running) s.ls_start[a] = running;
-        }
-      }
-    }
+__device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int pn, int lane, unsigned lt) {
+  bool pass = false;
+  int a = 0, b = 0, f = 0;
+  float c = 0.f;
+  if (lane < n) {
+    a = W.q_a[lane]; b = W.q_b[lane]; f = W.q_f[lane];
+    const Anchor A = load_anchor(s, a), B = load_anchor(s, b);
+    pass = ls_eval(A, B, c);
   }
-  if (staged) flush_stage(stage, staged, s.cnt + LST_CNT_TMP_LS, s.ls_rec, caps.max_ls, lane);
+  const unsigned mask = __ballot_sync(0xffffffffu, pass);
+  if (pass) {
+    const int i = pn + __popc(mask & lt);
+    W.p_a[i] = a; W.p_b[i] = b; W.p_f[i] = f; W.p_c[i] = c;
+  }
+  return pn + __popc(mask);
 }
 
-__global__ void __launch_bounds__(256) k_ls_final(const Slot* __restrict__ slots, Caps caps) {
+// first MD index whose row starts at a flat position >= x (rows are in MD order, positions non-decreasing)
+__device__ __forceinline__ int first_row_at(const Slot& s, const int* __restrict__ off, int M, int x) {
+  const int* __restrict__ mds = s.md_start;
+  if (x > off[M]) return mds[M];
+  const int mB = (x <= 0) ? 0 : upper_bound_g(off, M, x - 1);     // first module with off[m] >= x (<= M)
+  if (mB > 0) {
+    const int mP = mB - 1, L = s.ls_L[mP];                        // off[mP] < x: its later rows may still start >= x
+    if (L > 0) {
+      const int n_m = mds[mP + 1] - mds[mP];
+      const int r0 = (x - off[mP] + L - 1) / L;
+      if (r0 < n_m) return mds[mP] + r0;
+    }
+  }
+  return mds[mB];
+}
+
+template <bool CHAIN>
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __restrict__ slots, Geo geo, Caps caps, unsigned epoch) {
+  __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  const int n_rec = min(s.cnt[LST_CNT_TMP_LS], caps.max_ls);
-  LST_FOR_ITEMS(i, n_rec) {
-    const LsRec rec = s.ls_rec[i];
-    const int pos = s.ls_start[rec.a] + rec.rank;
-    if (pos < caps.max_ls) { s.ls_ab[pos] = make_int2(rec.a, rec.b); s.ls_c[pos] = rec.c; }
+  if (CHAIN && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;
+  const int lane = threadIdx.x & 31;
+  LsWarp& W = Wall[threadIdx.x >> 5];
+  const unsigned lt = lanemask_lt();
+  const int M = geo.n_modules;
+  const int* __restrict__ off = s.ls_off;
+  const int* __restrict__ mds = s.md_start;
+  const int* __restrict__ cand = s.ls_cand;
+  const int total_cells = min(off[M], MAX_CELLS);
+  const int n_links = total_cells / LS_LP + 1;
+  const int cap = caps.max_ls, cand_cap = CAND_PER_MD * caps.max_md;
+  int link = blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5);
+  while (true) {
+    if (CHAIN) link = warp_ticket(s.cnt + LST_CNT_TICKET_LS, lane);
+    if (link >= n_links) break;
+    const int lo = link * LS_LP, hi = min(total_cells, lo + LS_LP);
+    int qn = 0, pn = 0;
+    if (lo < hi) {
+      for (int m = s.ls_link_mod[link]; m < M; ++m) {
+        const int om = off[m];
+        if (om >= hi) break;
+        const int c0 = max(lo, om) - om, c1 = min(hi, off[m + 1]) - om;   // the link's cells of module m
+        if (c1 <= c0) continue;
+        const int a0 = mds[m], L = s.ls_L[m], co = s.ls_coff[m];
+        const bool tabled = co + L <= cand_cap;
+        int row, col, q32, r32;                       // the lane's cell (row, col); 32 cells further = (+q32, +r32)
+        divmod_small(c0 + lane, L, row, col);
+        divmod_small(32, L, q32, r32);
+        for (int cb = c0; cb < c1; cb += 32) {
+          const int cell = cb + lane;
+          bool pre = false;
+          int a = 0, b = 0;
+          if (cell < c1) {
+            a = a0 + row;
+            b = tabled ? cand[co + col] : cand_walk(s, geo, m, col);
+            pre = ls_prefilter(s.md_pos[a], s.md_aux[a], s.md_pos[b], s.md_aux[b]);
+          }
+          row += q32; col += r32;
+          if (col >= L) { col -= L; ++row; }
+          const unsigned mask = __ballot_sync(0xffffffffu, pre);
+          if (mask) {
+            if (pre) { const int i = qn + __popc(mask & lt); W.q_a[i] = a; W.q_b[i] = b; W.q_f[i] = om + cell - lo; }
+            qn += __popc(mask);
+            __syncwarp();
+            if (qn >= 32) {
+              pn = ls_drain(s, W, 32, pn, lane, lt);
+              __syncwarp();
+              const int rest = qn - 32;
+              int x = 0, y = 0, z = 0;
+              if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; z = W.q_f[32 + lane]; }
+              __syncwarp();
+              if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; W.q_f[lane] = z; }
+              qn = rest;
+              __syncwarp();
+            }
+          }
+        }
+      }
+      if (qn) pn = ls_drain(s, W, qn, pn, lane, lt);
+      __syncwarp();
+    }
+    if (!CHAIN) {
+      int soff = 0;
+      if (lane == 0) { soff = pn ? atomicAdd(s.cnt + LST_CNT_FILL_LS, pn) : 0; s.ls_link_cnt[link] = pn; s.ls_link_soff[link] = soff; }
+      soff = __shfl_sync(0xffffffffu, soff, 0);
+      for (int i = lane; i < pn; i += 32)
+        if (soff + i < cap) { LsRec r; r.a = W.p_a[i]; r.b = W.p_b[i]; r.lf = (link << LS_LP_BITS) | W.p_f[i]; r.c = W.p_c[i]; s.ls_rec[soff + i] = r; }
+      __syncwarp();
+      link += gridDim.x * PAIR_WARPS;
+      continue;
+    }
+    const int base = chain_exclusive(s.chain_ls, link, pn, lane, epoch);
+    for (int i = lane; i < pn; i += 32)
+      if (base + i < cap) { s.ls_ab[base + i] = make_int2(W.p_a[i], W.p_b[i]); s.ls_c[base + i] = W.p_c[i]; }
+    // LSs whose inner MD is a = [ls_start[a], ls_start[a+1]): the link owns the rows that start in its range
+    int sr = 0;
+    if (lane < 2) sr = first_row_at(s, off, M, lane == 0 ? lo : lo + LS_LP);
+    const int aLo = __shfl_sync(0xffffffffu, sr, 0), aHi = __shfl_sync(0xffffffffu, sr, 1);
+    for (int a = aLo + lane; a < aHi; a += 32) {
+      const int m = s.md_modt[a] >> 2;
+      const int rel = off[m] + (a - mds[m]) * s.ls_L[m] - lo;
+      s.ls_start[a] = min(base + lower_bound_s(W.p_f, pn, rel), cap);
+    }
+    if (link == n_links - 1 && lane == 0) {
+      const int total = base + pn;
+      s.ls_start[mds[M]] = min(total, cap);
+      s.cnt[LST_CNT_LS] = min(total, cap);
+      s.cnt[LST_CNT_RAW_LS] = total;
+    }
+    __syncwarp();
+  }
+}
+
+// a2 finalize: one thread per record; one thread per MD row for ls_start
+__global__ void __launch_bounds__(256) k_ls_final(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  const Slot& s = slots[blockIdx.y];
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) return;
+  const int M = geo.n_modules;
+  const int* __restrict__ off = s.ls_off;
+  const int* __restrict__ mds = s.md_start;
+  const int* __restrict__ base = s.ls_link_cnt;
+  const int* __restrict__ soff = s.ls_link_soff;
+  const int n_rec = min(s.cnt[LST_CNT_FILL_LS], caps.max_ls);
+  LST_FOR_ITEMS(j, n_rec) {
+    const LsRec r = s.ls_rec[j];
+    const int link = r.lf >> LS_LP_BITS;
+    const int pos = base[link] + (j - soff[link]);
+    s.ls_ab[pos] = make_int2(r.a, r.b);
+    s.ls_c[pos] = r.c;
+  }
+  const int total_cells = min(off[M], MAX_CELLS);
+  const int n_md = mds[M];
+  LST_FOR_ITEMS(a, n_md + 1) {
+    int x = total_cells;
+    if (a < n_md) { const int m = s.md_modt[a] >> 2; x = min(off[m] + (a - mds[m]) * s.ls_L[m], total_cells); }
+    const int link = x >> LS_LP_BITS, rel = x - (link << LS_LP_BITS);
+    const int b = base[link], pn = base[link + 1] - b;
+    const LsRec* __restrict__ rec = s.ls_rec + soff[link];
+    int l = 0, h = pn;
+    while (l < h) { const int mid = (l + h) >> 1; if ((rec[mid].lf & (LS_LP - 1)) < rel) l = mid + 1; else h = mid; }
+    s.ls_start[a] = b + l;
   }
 }
 
