@@ -150,7 +150,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 26;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 28;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -264,7 +264,9 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_scan<SCAN_MDLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_md_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
   k_md_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();     // overflow re-run (returns at once otherwise)
-  k_ls_plan<<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_plan1<<<G, 256, 0, st>>>(sl, g); LST_MARK();
+  k_ls_plan2<<<G1, SCAN_THREADS, 0, st>>>(sl, g); LST_MARK();
+  k_ls_plan3<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
   k_ls_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();
   k_scan<SCAN_LSLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_ls_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
@@ -310,7 +312,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
-      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan1", "a2.ls_plan2", "a2.ls_plan3", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
       "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }

@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __rest
           int i, j;
           divmod_small(loc, nup, i, j);
           p_lo = lb + i; p_up = ub + j;
-          const float4 h1 = hit[p_lo], h2 = hit[p_up];
+          const float4 h1 = __ldg(hit + p_lo), h2 = __ldg(hit + p_up);
           pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3);
         }
         const unsigned mask = __ballot_sync(0xffffffffu, pre);
@@ -296,14 +296,13 @@ __global__ void __launch_bounds__(256) k_md_final(const Slot* __restrict__ slots
 // a2: cells = (MD a of module m, candidate column) with flat index ls_off[m] + row*L[m] + col; the columns of m
 // are the MDs of its CSR-connected modules in ascending MD index (L[m] of them, listed in ls_cand)
 // ------------------------------------------------------------------------------------------------
-// plan (one block per event): candidate count L[m], exclusive scans of the cell counts n_m * L[m] and of the
-// candidate-table offsets, the link -> module table and the candidate table itself
-__global__ void __launch_bounds__(SCAN_THREADS) k_ls_plan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  __shared__ int sm[34];
+// plan, three small launches: (1) candidate count L[m] and cell count n_m * L[m] per module; (2) one block per
+// event: exclusive scans of the cell counts and of the candidate-table offsets, link -> module table; (3) the
+// candidate table itself
+__global__ void __launch_bounds__(256) k_ls_plan1(const Slot* __restrict__ slots, Geo geo) {
   const Slot& s = slots[blockIdx.y];
-  const int M = geo.n_modules;
   const int* __restrict__ mds = s.md_start;
-  for (int m = threadIdx.x; m < M; m += SCAN_THREADS) {
+  LST_FOR_ITEMS(m, geo.n_modules) {
     const int n_m = mds[m + 1] - mds[m];
     int L = 0;
     if (n_m > 0) {
@@ -319,23 +318,39 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_ls_plan(const Slot* __restrict
     s.ls_off[m] = (int)cells;
     s.ls_coff[m] = L;
   }
-  __syncthreads();
+}
+__global__ void __launch_bounds__(SCAN_THREADS) k_ls_plan2(const Slot* __restrict__ slots, Geo geo) {
+  __shared__ int sm[34];
+  const Slot& s = slots[blockIdx.y];
+  const int M = geo.n_modules;
   const int total = block_scan_inplace(s.ls_off, M, 0x7fffffff, sm);
   __syncthreads();
   block_scan_inplace(s.ls_coff, M, 0x7fffffff, sm);
   __syncthreads();
   if (threadIdx.x == 0 && total > MAX_CELLS) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_LS);
   link_owner_table(s.ls_off, M, LS_LP, s.ls_link_mod);
+}
+__global__ void __launch_bounds__(256) k_ls_plan3(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  const Slot& s = slots[blockIdx.y];
+  const int* __restrict__ mds = s.md_start;
   const int cand_cap = CAND_PER_MD * caps.max_md;
-  for (int m = threadIdx.x; m < M; m += SCAN_THREADS) {
+  const int lane = threadIdx.x & 31;
+  // one warp per module: the lanes take the CSR entries, a warp scan places each entry's MD range
+  for (int m = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; m < geo.n_modules; m += (gridDim.x * blockDim.x) >> 5) {
     const int L = s.ls_L[m];
     int o = s.ls_coff[m];
     if (L == 0 || o + L > cand_cap) continue;        // modules beyond the table walk the CSR row instead
-    const int e1 = geo.rowptr[m + 1];
-    for (int e = geo.rowptr[m]; e < e1; ++e) {
-      const int m2 = geo.col[e];
-      const int b1 = mds[m2 + 1];
-      for (int b = mds[m2]; b < b1; ++b) s.ls_cand[o++] = b;
+    const int e0 = geo.rowptr[m], e1 = geo.rowptr[m + 1];
+    for (int eb = e0; eb < e1; eb += 32) {
+      const int e = eb + lane;
+      int b0 = 0, n = 0;
+      if (e < e1) { const int m2 = geo.col[e]; b0 = mds[m2]; n = mds[m2 + 1] - b0; }
+      int inc = n;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+      const int w = o + inc - n;
+      for (int t = 0; t < n; ++t) s.ls_cand[w + t] = b0 + t;
+      o += __shfl_sync(0xffffffffu, inc, 31);
     }
   }
 }
@@ -410,6 +425,8 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __rest
   const int* __restrict__ off = s.ls_off;
   const int* __restrict__ mds = s.md_start;
   const int* __restrict__ cand = s.ls_cand;
+  const float4* __restrict__ mpos = s.md_pos;
+  const float4* __restrict__ maux = s.md_aux;
   const int total_cells = min(off[M], MAX_CELLS);
   const int n_links = total_cells / LS_LP + 1;
   const int cap = caps.max_ls, cand_cap = CAND_PER_MD * caps.max_md;
@@ -436,8 +453,8 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __rest
           int a = 0, b = 0;
           if (cell < c1) {
             a = a0 + row;
-            b = tabled ? cand[co + col] : cand_walk(s, geo, m, col);
-            pre = ls_prefilter(s.md_pos[a], s.md_aux[a], s.md_pos[b], s.md_aux[b]);
+            b = tabled ? __ldg(cand + co + col) : cand_walk(s, geo, m, col);
+            pre = ls_prefilter(__ldg(mpos + a), __ldg(maux + a), __ldg(mpos + b), __ldg(maux + b));
           }
           row += q32; col += r32;
           if (col >= L) { col -= L; ++row; }
