@@ -130,7 +130,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls);
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
-    t.chi3 = cv.take<float>(k.max_t3); t.tc = cv.take<int>(3 * (size_t)k.max_tc);
+    t.chi3 = cv.take<float>(k.max_t3); t.key5 = cv.take<unsigned long long>(k.max_t5); t.key3 = cv.take<unsigned long long>(k.max_t3); t.tc = cv.take<int>(3 * (size_t)k.max_tc);
     t.st_x = cv.take<float>(k.max_hits); t.st_y = cv.take<float>(k.max_hits); t.st_z = cv.take<float>(k.max_hits);
     t.st_key = cv.take<uint32_t>(k.max_hits);
     t.st_px = cv.take<float>(k.max_pls); t.st_py = cv.take<float>(k.max_pls); t.st_pz = cv.take<float>(k.max_pls);
@@ -150,7 +150,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 28;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 31;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -279,10 +279,13 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_t5<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
   k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_pls_bin<<<G1, 1024, 0, st>>>(sl); LST_MARK();
-  k_match<5, false><<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_pls_bin<false><<<G1, 1024, 0, st>>>(sl); LST_MARK();
+  k_match<5, false><<<GL, 128, 0, st>>>(sl); LST_MARK();
+  k_win<false><<<G, 256, 0, st>>>(sl); LST_MARK();
   k_pt5_lists<<<G, 128, 0, st>>>(sl); LST_MARK();
-  k_match<3, true><<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_pls_bin<true><<<G1, 1024, 0, st>>>(sl); LST_MARK();
+  k_match<3, true><<<GL, 128, 0, st>>>(sl); LST_MARK();
+  k_win<true><<<G, 256, 0, st>>>(sl); LST_MARK();
   k_tc_emit<<<G1, 1024, 0, st>>>(sl, k); LST_MARK();
 #undef LST_MARK
   if (li != N_LAUNCHES + 2) return LST_EINVAL;
@@ -313,7 +316,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
       "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan1", "a2.ls_plan2", "a2.ls_plan3", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
-      "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
+      "a5.scan", "a6.pls_bin", "a6.match5", "a6.win5", "a6.pt5_lists", "a6.pls_rebin", "a6.match3", "a6.win3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 

@@ -60,6 +60,7 @@ struct Slot {
   // a6
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_bin_start;
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
+  unsigned long long* key5; unsigned long long* key3;   // argmin (chi2, pLS) per T5 / T3
   // host-load staging
   float *st_x, *st_y, *st_z; uint32_t* st_key; float *st_px, *st_py, *st_pz, *st_z0; int8_t* st_q;
 };
@@ -385,7 +386,10 @@ __device__ __forceinline__ int psi_bin_raw(float ang) {   // unbounded bin index
   return (int)floorf((ang + LST_PI_F) * (PLS_NB / (2.0f * LST_PI_F)));
 }
 
-// one block per event: derive, histogram, scan, scatter (all in shared memory; ~2.6k pLS per event)
+// one block per event: derive, histogram, scan, scatter (all in shared memory; ~2.6k pLS per event).
+// SECOND = false: all pLS, for the T5 pass.  SECOND = true (after the pT5 are known): only the pLS without a pT5
+// are binned again for the T3 pass, and the T3s contained in a pT5 are marked used (best3 = -2).
+template <bool SECOND>
 __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots) {
   __shared__ int hist[PLS_NBINS + 1];
   __shared__ int sm[34];
@@ -393,20 +397,46 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int n = s.n_pls;
   for (int i = tid; i <= PLS_NBINS; i += 1024) hist[i] = 0;
+  {   // argmin keys of the pass that follows start empty
+    unsigned long long* key = SECOND ? s.key3 : s.key5;
+    const int nk = SECOND ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
+    for (int i = tid; i < nk; i += 1024) key[i] = WIN_EMPTY;
+  }
+  if (SECOND) {   // used iff {a,b,c} is contained in the five MDs of some pT5: walk the pT5 entries that contain a
+    const int n_t3 = s.cnt[LST_CNT_T3];
+    for (int t = tid; t < n_t3; t += 1024) {
+      const int4 abc = s.t3_abc[t];
+      bool used = false;
+      for (int e = s.md_head[abc.x]; e >= 0 && !used; e = s.pt5_next[e]) {
+        const int pp = e / 5;
+        const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(s.win5[pp] & 0xFFFFFFFFull)];
+        int found = 0;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) found += (m5[q] == abc.y) + (m5[q] == abc.z);
+        used = (found == 2);
+      }
+      s.best3[t] = used ? -2 : -1;
+    }
+  }
   __syncthreads();
   for (int p = tid; p < n; p += 1024) {
-    const int q = (int)s.in_q[p];
-    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
-    s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
-    s.pls_b[p] = make_float2(d.sec, d.z0);
-    int kb = PLS_K, pb = 0;
-    if (d.h < LST_PLS_HMAX && (q == 1 || q == -1)) {
-      kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
-      pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
+    int key = -1;
+    if (!SECOND) {
+      const int q = (int)s.in_q[p];
+      const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
+      s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
+      s.pls_b[p] = make_float2(d.sec, d.z0);
+      int kb = PLS_K, pb = 0;
+      if (d.h < LST_PLS_HMAX && (q == 1 || q == -1)) {
+        kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
+        pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
+      }
+      key = kb * PLS_NB + pb;
+      s.pls_key[p] = key;
+    } else if (s.win5[p] == WIN_EMPTY) {
+      key = s.pls_key[p];
     }
-    const int key = kb * PLS_NB + pb;
-    s.pls_key[p] = key;
-    atomicAdd(&hist[key], 1);
+    if (key >= 0) atomicAdd(&hist[key], 1);
   }
   __syncthreads();
   // exclusive scan of hist[0..PLS_NBINS] (3 items per thread)
@@ -435,6 +465,7 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
   }
   __syncthreads();
   for (int p = tid; p < n; p += 1024) {
+    if (SECOND && s.win5[p] != WIN_EMPTY) continue;
     const int pos = atomicAdd(&hist[s.pls_key[p]], 1);   // order inside a bucket is free: argmin ties break on p
     s.pls_sa[pos] = s.pls_a[p];
     s.pls_sb[pos] = s.pls_b[p];
@@ -446,30 +477,27 @@ __device__ __forceinline__ unsigned long long win_key(float chi2, int idx) {
   return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned)idx;   // chi2 >= 0: bit order = value order
 }
 
-// match objects with NA anchors against the pLS buckets their first anchor can reach: one thread per
-// object; best = argmin over (chi2, p) with an explicit tie-break on p (bucket order is arbitrary).
+// match objects with NA anchors against the pLS buckets their first anchor can reach.  One thread per (object,
+// h-bucket): the 32 lanes of a warp hold 32 consecutive objects and the SAME h-bucket, so the window arithmetic
+// is uniform and the bucket loops have similar lengths.  Every matching pLS is folded into the object's key with
+// a 64-bit atomicMin on (chi2 bits, p): argmin over (chi2, p), independent of the visiting order.
 template <int NA, bool IS_T3>
 __global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
   const Slot& s = slots[blockIdx.y];
   const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
+  const int n_pad = (n + 31) & ~31;
   const int* __restrict__ bstart = s.pls_bin_start;
+  unsigned long long* __restrict__ keys = IS_T3 ? s.key3 : s.key5;
   int n_tests = 0, n_cand = 0;
-  LST_FOR_ITEMS(t, n) {
+  LST_FOR_ITEMS(item, n_pad * (PLS_K + 1)) {
+    const int kb = item / n_pad, t = item - kb * n_pad;
+    if (t >= n) continue;
+    if (bstart[(kb + 1) * PLS_NB] == bstart[kb * PLS_NB]) continue;      // empty h-bucket (uniform over the warp)
     int md[NA];
     if (IS_T3) {
+      if (s.best3[t] == -2) continue;                                    // contained in a pT5
       const int4 abc = s.t3_abc[t];
       md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
-      // used iff {a,b,c} is contained in the five MDs of some pT5: walk the entries that contain a
-      bool used = false;
-      for (int e = s.md_head[abc.x]; e >= 0 && !used; e = s.pt5_next[e]) {
-        const int pp = e / 5;
-        const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(s.win5[pp] & 0xFFFFFFFFull)];
-        int found = 0;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) found += (m5[q] == abc.y) + (m5[q] == abc.z);
-        used = (found == 2);
-      }
-      if (used) { s.best3[t] = -1; continue; }
     } else {
       const int* m5 = s.t5c_md + 5 * s.t5_list[t];
 #pragma unroll
@@ -477,57 +505,52 @@ __global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
     }
     const float4 a0 = s.md_pos[md[0]];
     const int mt0 = s.md_modt[md[0]] & 3;
-    int best = -1;
-    float bchi = 0.0f;
-    const float phi = atan2f(a0.y, a0.x);
     const float r = a0.w;
-    const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
-    for (int kb = 0; kb <= PLS_K; ++kb) {
-      // up to four bucket ranges [rb[i], re[i]) of this h-bucket
-      int rb[4], re[4], nr = 0;
-      const int base = kb * PLS_NB;
-      if (kb == PLS_K) { rb[0] = base; re[0] = base + PLS_NB; nr = 1; }
-      else {
-        const float ulo = r * (kb * (LST_PLS_HMAX / PLS_K)), uhi = r * ((kb + 1) * (LST_PLS_HMAX / PLS_K));
-        const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
-        if (clo > 1.0f) { kb = PLS_K - 1; continue; }            // no circle of this or a larger curvature reaches r
-        const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
+    // up to four bucket ranges [rb[i], re[i]) of this h-bucket
+    int rb[4], re[4], nr = 0;
+    const int base = kb * PLS_NB;
+    if (kb == PLS_K) { rb[0] = base; re[0] = base + PLS_NB; nr = 1; }
+    else {
+      const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
+      const float ulo = r * (kb * (LST_PLS_HMAX / PLS_K)), uhi = r * ((kb + 1) * (LST_PLS_HMAX / PLS_K));
+      const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
+      if (clo > 1.0f) continue;                                          // no circle of this curvature reaches r
+      const float phi = atan2f(a0.y, a0.x);
+      const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
 #pragma unroll
-        for (int sgn = 0; sgn < 2; ++sgn) {
-          const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
-          const int blo = psi_bin_raw(lo);
-          const int nb = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
-          const int b0 = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
-          const int e0 = min(b0 + nb, PLS_NB);
-          rb[nr] = base + b0; re[nr] = base + e0; ++nr;
-          if (b0 + nb > PLS_NB) { rb[nr] = base; re[nr] = base + b0 + nb - PLS_NB; ++nr; }
-        }
-      }
-      for (int ir = 0; ir < nr; ++ir) {
-        const int j1 = bstart[re[ir]];
-        for (int j = bstart[rb[ir]]; j < j1; ++j) {
-          const float4 pa = s.pls_sa[j];
-          Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
-          float e, dT;
-          ++n_tests;
-          if (!pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT)) continue;       // transverse test of the first anchor
-          const int p = s.pls_sidx[j];
-          if (IS_T3 && s.win5[p] != WIN_EMPTY) continue;                  // pLS already in a pT5
-          ++n_cand;
-          const float2 pb = s.pls_sb[j];
-          P.sec = pb.x; P.z0 = pb.y;
-          float chi = 0.0f;
-          bool ok = pls_anchor(P, a0, mt0, chi);
-#pragma unroll
-          for (int q = 1; q < NA; ++q)
-            if (ok) ok = pls_anchor(P, s.md_pos[md[q]], s.md_modt[md[q]] & 3, chi);
-          if (!ok) continue;
-          if (best < 0 || chi < bchi || (chi == bchi && p < best)) { best = p; bchi = chi; }
-        }
+      for (int sgn = 0; sgn < 2; ++sgn) {
+        const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
+        const int blo = psi_bin_raw(lo);
+        const int nb = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
+        const int b0 = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
+        const int e0 = min(b0 + nb, PLS_NB);
+        rb[nr] = base + b0; re[nr] = base + e0; ++nr;
+        if (b0 + nb > PLS_NB) { rb[nr] = base; re[nr] = base + b0 + nb - PLS_NB; ++nr; }
       }
     }
-    if (IS_T3) { s.best3[t] = best; s.chi3[t] = bchi; if (best >= 0) atomicMin(s.win3 + best, win_key(bchi, t)); }
-    else { s.best5[t] = best; s.chi5[t] = bchi; if (best >= 0) atomicMin(s.win5 + best, win_key(bchi, t)); }
+    unsigned long long best = WIN_EMPTY;
+    for (int ir = 0; ir < nr; ++ir) {
+      const int j1 = bstart[re[ir]];
+      for (int j = bstart[rb[ir]]; j < j1; ++j) {
+        const float4 pa = s.pls_sa[j];
+        Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
+        float e, dT;
+        ++n_tests;
+        if (!pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT)) continue;       // transverse test of the first anchor
+        ++n_cand;
+        const float2 pb = s.pls_sb[j];
+        P.sec = pb.x; P.z0 = pb.y;
+        float chi = 0.0f;
+        bool ok = pls_anchor(P, a0, mt0, chi);
+#pragma unroll
+        for (int q = 1; q < NA; ++q)
+          if (ok) ok = pls_anchor(P, s.md_pos[md[q]], s.md_modt[md[q]] & 3, chi);
+        if (!ok) continue;
+        const unsigned long long k = ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j];
+        best = min(best, k);                                            // chi2 >= 0: bit order = value order
+      }
+    }
+    if (best != WIN_EMPTY) atomicMin(keys + t, best);
   }
   // bookkeeping for the roofline accounting: prefilter tests executed / pairs that needed the full test
 #pragma unroll
@@ -535,6 +558,20 @@ __global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
   if ((threadIdx.x & 31) == 0 && n_tests) {
     atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_TESTS : LST_CNT_M5_TESTS), n_tests);
     atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_CAND : LST_CNT_M5_CAND), n_cand);
+  }
+}
+
+// second reduction: winner per pLS = argmin over (chi2, object) among the objects whose best pLS it is
+template <bool IS_T3>
+__global__ void __launch_bounds__(256) k_win(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
+  LST_FOR_ITEMS(t, n) {
+    const unsigned long long k = IS_T3 ? s.key3[t] : s.key5[t];
+    const int best = (k == WIN_EMPTY) ? -1 : (int)(k & 0xFFFFFFFFull);
+    const float chi = (k == WIN_EMPTY) ? 0.0f : __uint_as_float((unsigned)(k >> 32));
+    if (IS_T3) { s.best3[t] = best; s.chi3[t] = chi; if (best >= 0) atomicMin(s.win3 + best, win_key(chi, t)); }
+    else { s.best5[t] = best; s.chi5[t] = chi; if (best >= 0) atomicMin(s.win5 + best, win_key(chi, t)); }
   }
 }
 
