@@ -221,12 +221,26 @@ def run_ours(args):
     ms_local = float(np.mean(step_ms))
 
     # ---- e2e: pinned host inputs -> H2D -> chain -> D2H of counters + TC rows, every step --------
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    host_in = [[pin(ev.x), pin(ev.y), pin(ev.z), pin(ev.key.view(np.int32)), pin(ev.pls_px), pin(ev.pls_py), pin(ev.pls_pz),
-                pin(ev.pls_z0), pin(ev.pls_q)] for ev in events]
+    # host events packed as the library stages them ([x|y|z|key], [px|py|pz|z0|q]) so each goes over in two copies,
+    # and counters + TC rows come back in one (lst.h: lst_load_event_host / lst_read_tc_host)
+    def pack(ev):
+        n, m = ev.n_hits, ev.n_pls
+        hb = torch.empty(4 * n, dtype=torch.float32).pin_memory()
+        hn = hb.numpy()
+        hn[0:n], hn[n:2 * n], hn[2 * n:3 * n] = ev.x, ev.y, ev.z
+        hn[3 * n:4 * n] = ev.key.view(np.float32)
+        pb = torch.empty(17 * m, dtype=torch.uint8).pin_memory()
+        pf = pb[:16 * m].view(torch.float32).numpy()
+        pf[0:m], pf[m:2 * m], pf[2 * m:3 * m], pf[3 * m:4 * m] = ev.pls_px, ev.pls_py, ev.pls_pz, ev.pls_z0
+        pb[16 * m:].numpy()[:] = ev.pls_q.view(np.uint8)
+        return [hb[0:n], hb[n:2 * n], hb[2 * n:3 * n], hb[3 * n:4 * n].view(torch.int32),
+                pb[0:4 * m].view(torch.float32), pb[4 * m:8 * m].view(torch.float32), pb[8 * m:12 * m].view(torch.float32),
+                pb[12 * m:16 * m].view(torch.float32), pb[16 * m:].view(torch.int8)]
+    host_in = [pack(ev) for ev in events]
     TC_ROWS = 8192
-    h_cnt = [torch.zeros(32, dtype=torch.int32).pin_memory() for _ in range(E)]
-    h_tc = [torch.zeros((TC_ROWS, 3), dtype=torch.int32).pin_memory() for _ in range(E)]
+    h_out = [torch.zeros(32 + 3 * TC_ROWS, dtype=torch.int32).pin_memory() for _ in range(E)]
+    h_cnt = [h[:32] for h in h_out]
+    h_tc = [h[32:].view(TC_ROWS, 3) for h in h_out]
     h2d = sum(ev.n_hits * 16 + ev.n_pls * 17 for ev in events)
     d2h = E * (32 * 4 + TC_ROWS * 12)
     e2e_streams = streams if S > 1 else [main]
@@ -386,7 +400,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=64, help="PU200 events per step per GPU (configs[3]: 64)")
-    ap.add_argument("--streams", type=int, default=1, help="CUDA streams the batch is split over")
+    ap.add_argument("--streams", type=int, default=4, help="CUDA streams the batch is split over (configs[3]: 4 x 16 events)")
     ap.add_argument("--cpu-sample", type=int, default=48)
     ap.add_argument("--ref-events", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")

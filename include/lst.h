@@ -53,7 +53,8 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        /* bookkeeping of the bucketed pLS matching: first-anchor tests executed / pairs fully tested */
        LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND,
        /* internal: fill of the MD / LS record buffers; link tickets of the overflow re-run */
-       LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TICKET_MD, LST_CNT_TICKET_LS, LST_N_CNT = 32 };
+       LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TICKET_MD, LST_CNT_TICKET_LS, LST_CNT_DYN_MD, LST_CNT_DYN_LS,
+       LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
 
@@ -120,7 +121,9 @@ int lst_load_event(lst_ctx* ctx, int32_t slot, int32_t n_hits, const float* d_x,
                    void* cuda_stream);
 
 /* Same with HOST pointers (pinned memory recommended): enqueues the host->device copies into the
- * slot's staging area on `cuda_stream`.  Host buffers must stay valid until the copies complete. */
+ * slot's staging area on `cuda_stream`.  Host buffers must stay valid until the copies complete.
+ * The staging area is packed [x|y|z|key] and [px|py|pz|z0|q]; when the host arrays are adjacent in
+ * memory in that order (h_y == h_x + n_hits, ...) each group is copied with ONE transfer. */
 int lst_load_event_host(lst_ctx* ctx, int32_t slot, int32_t n_hits, const float* h_x, const float* h_y,
                         const float* h_z, const uint32_t* h_key, int32_t n_pls, const float* h_px,
                         const float* h_py, const float* h_pz, const float* h_z0, const int8_t* h_q,
@@ -139,6 +142,7 @@ int lst_status(lst_ctx* ctx, int32_t slot, uint32_t* status_bits, int32_t* count
 
 /* Enqueue device->host copies of the slot's counters (HOST int32[LST_N_CNT], then status word in
  * h_counts[LST_N_CNT-1]) and of the first `max_rows` rows of its TC list (HOST int32[max_rows][3]). */
+/* When h_tc == h_counts + LST_N_CNT (one host buffer) both are read with ONE transfer. */
 int lst_read_tc_host(lst_ctx* ctx, int32_t slot, int32_t* h_counts, int32_t* h_tc, int32_t max_rows,
                      void* cuda_stream);
 

@@ -130,11 +130,8 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls);
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
-    t.chi3 = cv.take<float>(k.max_t3); t.key5 = cv.take<unsigned long long>(k.max_t5); t.key3 = cv.take<unsigned long long>(k.max_t3); t.tc = cv.take<int>(3 * (size_t)k.max_tc);
-    t.st_x = cv.take<float>(k.max_hits); t.st_y = cv.take<float>(k.max_hits); t.st_z = cv.take<float>(k.max_hits);
-    t.st_key = cv.take<uint32_t>(k.max_hits);
-    t.st_px = cv.take<float>(k.max_pls); t.st_py = cv.take<float>(k.max_pls); t.st_pz = cv.take<float>(k.max_pls);
-    t.st_z0 = cv.take<float>(k.max_pls); t.st_q = cv.take<int8_t>(k.max_pls);
+    t.chi3 = cv.take<float>(k.max_t3); t.key5 = cv.take<unsigned long long>(k.max_t5); t.key3 = cv.take<unsigned long long>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
+    t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
       t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head;
@@ -229,13 +226,16 @@ int lst_load_event_host(lst_ctx* c, int32_t slot, int32_t n_hits, const float* h
   auto cp = [&](void* dst, const void* src, size_t n) {
     if (e == cudaSuccess && n) e = cudaMemcpyAsync(dst, src, n, cudaMemcpyHostToDevice, st);
   };
-  cp(s.st_x, h_x, sizeof(float) * n_hits); cp(s.st_y, h_y, sizeof(float) * n_hits); cp(s.st_z, h_z, sizeof(float) * n_hits);
-  cp(s.st_key, h_key, sizeof(uint32_t) * n_hits);
-  cp(s.st_px, h_px, sizeof(float) * n_pls); cp(s.st_py, h_py, sizeof(float) * n_pls); cp(s.st_pz, h_pz, sizeof(float) * n_pls);
-  cp(s.st_z0, h_z0, sizeof(float) * n_pls); cp(s.st_q, h_q, n_pls);
+  // device staging is packed [x|y|z|key] and [px|py|pz|z0|q]; a host event packed the same way goes over in
+  // two copies instead of nine
+  float* dx = s.st_hits; float* dy = dx + n_hits; float* dz = dy + n_hits; uint32_t* dk = reinterpret_cast<uint32_t*>(dz + n_hits);
+  float* dpx = s.st_pls; float* dpy = dpx + n_pls; float* dpz = dpy + n_pls; float* dz0 = dpz + n_pls; int8_t* dq = reinterpret_cast<int8_t*>(dz0 + n_pls);
+  if (h_y == h_x + n_hits && h_z == h_y + n_hits && reinterpret_cast<const float*>(h_key) == h_z + n_hits) cp(dx, h_x, 16 * (size_t)n_hits);
+  else { cp(dx, h_x, 4 * (size_t)n_hits); cp(dy, h_y, 4 * (size_t)n_hits); cp(dz, h_z, 4 * (size_t)n_hits); cp(dk, h_key, 4 * (size_t)n_hits); }
+  if (h_py == h_px + n_pls && h_pz == h_py + n_pls && h_z0 == h_pz + n_pls && reinterpret_cast<const float*>(h_q) == h_z0 + n_pls) cp(dpx, h_px, 17 * (size_t)n_pls);
+  else { cp(dpx, h_px, 4 * (size_t)n_pls); cp(dpy, h_py, 4 * (size_t)n_pls); cp(dpz, h_pz, 4 * (size_t)n_pls); cp(dz0, h_z0, 4 * (size_t)n_pls); cp(dq, h_q, n_pls); }
   if (bad(c, e)) return LST_ECUDA;
-  return lst_load_event(c, slot, n_hits, s.st_x, s.st_y, s.st_z, s.st_key, n_pls, s.st_px, s.st_py, s.st_pz, s.st_z0,
-                        s.st_q, cuda_stream);
+  return lst_load_event(c, slot, n_hits, dx, dy, dz, dk, n_pls, dpx, dpy, dpz, dz0, dq, cuda_stream);
 }
 
 // The launch sequence of one pass over slots [first, first+n).  With `ev` != nullptr an event is
@@ -360,6 +360,10 @@ int lst_read_tc_host(lst_ctx* c, int32_t slot, int32_t* h_counts, int32_t* h_tc,
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const Slot& s = c->h_slots[slot];
   if (max_rows > c->caps.max_tc) max_rows = c->caps.max_tc;
+  if (max_rows > 0 && h_tc == h_counts + LST_N_CNT) {     // adjacent host buffers: counters (header copy) + rows in one copy
+    if (bad(c, cudaMemcpyAsync(h_counts, s.tc_hdr, sizeof(int32_t) * (LST_N_CNT + 3 * (size_t)max_rows), cudaMemcpyDeviceToHost, st))) return LST_ECUDA;
+    return LST_OK;
+  }
   if (bad(c, cudaMemcpyAsync(h_counts, s.cnt, sizeof(int32_t) * LST_N_CNT, cudaMemcpyDeviceToHost, st))) return LST_ECUDA;
   if (max_rows > 0 && bad(c, cudaMemcpyAsync(h_tc, s.tc, sizeof(int32_t) * 3 * (size_t)max_rows, cudaMemcpyDeviceToHost, st)))
     return LST_ECUDA;

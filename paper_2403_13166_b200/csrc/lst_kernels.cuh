@@ -62,7 +62,8 @@ struct Slot {
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
   unsigned long long* key5; unsigned long long* key3;   // argmin (chi2, pLS) per T5 / T3
   // host-load staging
-  float *st_x, *st_y, *st_z; uint32_t* st_key; float *st_px, *st_py, *st_pz, *st_z0; int8_t* st_q;
+  float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
+  int* tc_hdr;                       // copy of cnt[] in front of the TC rows, so one D2H copy reads both
 };
 
 #define LST_FOR_ITEMS(i, n) \
@@ -642,6 +643,8 @@ __global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots
     s.cnt[LST_CNT_TC] = min(base_out, caps.max_tc);
     if (base_out > caps.max_tc) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_TC);
   }
+  __syncthreads();
+  if (tid < LST_N_CNT) s.tc_hdr[tid] = s.cnt[tid];      // every counter is final here: last kernel of the chain
 }
 
 // binds an event to a slot (stream-ordered, so a later lst_run on the same stream sees it)

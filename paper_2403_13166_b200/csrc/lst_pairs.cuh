@@ -158,9 +158,9 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __rest
   const int total_cells = min(off[M], MAX_CELLS);       // beyond: flagged by the scan that made `off`
   const int n_links = total_cells / MD_LP + 1;
   const int cap = caps.max_md;
-  int link = blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5);
-  while (true) {
-    if (CHAIN) link = warp_ticket(s.cnt + LST_CNT_TICKET_MD, lane);
+  int link;
+  while (true) {      // links are handed out dynamically: their cost varies with the number of modules they span
+    link = warp_ticket(s.cnt + (CHAIN ? LST_CNT_TICKET_MD : LST_CNT_DYN_MD), lane);
     if (link >= n_links) break;
     const int lo = link * MD_LP, hi = min(total_cells, lo + MD_LP);
     int qn = 0, pn = 0;
@@ -230,7 +230,6 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __rest
           s.md_rec[soff + i] = r;
         }
       __syncwarp();
-      link += gridDim.x * PAIR_WARPS;
       continue;
     }
     // CHAIN (overflow re-run): base by look-back, objects and range table written in place
@@ -356,6 +355,7 @@ __global__ void __launch_bounds__(256) k_ls_plan3(const Slot* __restrict__ slots
 }
 
 struct LsWarp {
+  int w_off[MD_WIN + 1], w_a0[MD_WIN], w_L[MD_WIN], w_co[MD_WIN];      // the link's next modules
   int q_a[Q_CAP], q_b[Q_CAP], q_f[Q_CAP];
   int p_a[LS_LP], p_b[LS_LP], p_f[LS_LP];
   float p_c[LS_LP];
@@ -397,6 +397,26 @@ __device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int pn,
   return pn + __popc(mask);
 }
 
+// append the survivors of one sweep to the queue (in lane order); a full warp of queued cells is evaluated at once
+__device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int a, int b, int f, int& qn, int& pn, int lane, unsigned lt) {
+  const unsigned mask = __ballot_sync(0xffffffffu, pre);
+  if (!mask) return;
+  if (pre) { const int i = qn + __popc(mask & lt); W.q_a[i] = a; W.q_b[i] = b; W.q_f[i] = f; }
+  qn += __popc(mask);
+  __syncwarp();
+  if (qn >= 32) {
+    pn = ls_drain(s, W, 32, pn, lane, lt);
+    __syncwarp();
+    const int rest = qn - 32;
+    int x = 0, y = 0, z = 0;
+    if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; z = W.q_f[32 + lane]; }
+    __syncwarp();
+    if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; W.q_f[lane] = z; }
+    qn = rest;
+    __syncwarp();
+  }
+}
+
 // first MD index whose row starts at a flat position >= x (rows are in MD order, positions non-decreasing)
 __device__ __forceinline__ int first_row_at(const Slot& s, const int* __restrict__ off, int M, int x) {
   const int* __restrict__ mds = s.md_start;
@@ -430,51 +450,71 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __rest
   const int total_cells = min(off[M], MAX_CELLS);
   const int n_links = total_cells / LS_LP + 1;
   const int cap = caps.max_ls, cand_cap = CAND_PER_MD * caps.max_md;
-  int link = blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5);
+  int link;
   while (true) {
-    if (CHAIN) link = warp_ticket(s.cnt + LST_CNT_TICKET_LS, lane);
+    link = warp_ticket(s.cnt + (CHAIN ? LST_CNT_TICKET_LS : LST_CNT_DYN_LS), lane);
     if (link >= n_links) break;
     const int lo = link * LS_LP, hi = min(total_cells, lo + LS_LP);
     int qn = 0, pn = 0;
     if (lo < hi) {
-      for (int m = s.ls_link_mod[link]; m < M; ++m) {
-        const int om = off[m];
-        if (om >= hi) break;
-        const int c0 = max(lo, om) - om, c1 = min(hi, off[m + 1]) - om;   // the link's cells of module m
-        if (c1 <= c0) continue;
-        const int a0 = mds[m], L = s.ls_L[m], co = s.ls_coff[m];
-        const bool tabled = co + L <= cand_cap;
-        int row, col, q32, r32;                       // the lane's cell (row, col); 32 cells further = (+q32, +r32)
-        divmod_small(c0 + lane, L, row, col);
-        divmod_small(32, L, q32, r32);
-        for (int cb = c0; cb < c1; cb += 32) {
-          const int cell = cb + lane;
-          bool pre = false;
-          int a = 0, b = 0;
-          if (cell < c1) {
-            a = a0 + row;
-            b = tabled ? __ldg(cand + co + col) : cand_walk(s, geo, m, col);
-            pre = ls_prefilter(__ldg(mpos + a), __ldg(maux + a), __ldg(mpos + b), __ldg(maux + b));
-          }
-          row += q32; col += r32;
-          if (col >= L) { col -= L; ++row; }
-          const unsigned mask = __ballot_sync(0xffffffffu, pre);
-          if (mask) {
-            if (pre) { const int i = qn + __popc(mask & lt); W.q_a[i] = a; W.q_b[i] = b; W.q_f[i] = om + cell - lo; }
-            qn += __popc(mask);
-            __syncwarp();
-            if (qn >= 32) {
-              pn = ls_drain(s, W, 32, pn, lane, lt);
-              __syncwarp();
-              const int rest = qn - 32;
-              int x = 0, y = 0, z = 0;
-              if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; z = W.q_f[32 + lane]; }
-              __syncwarp();
-              if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; W.q_f[lane] = z; }
-              qn = rest;
-              __syncwarp();
+      int mW = s.ls_link_mod[link];      // module that owns the next unprocessed cell
+      int fc = lo;                       // next unprocessed cell
+      while (fc < hi) {
+        // cache the next MD_WIN modules (offsets, first MD, candidate count, candidate-table offset)
+        __syncwarp();
+        {
+          const int m = mW + lane;
+          int o = 0x7fffffff, a0 = 0, L = 1, co = 0;
+          if (m < M) { o = off[m]; a0 = mds[m]; L = s.ls_L[m]; co = s.ls_coff[m]; }
+          W.w_off[lane] = o; W.w_a0[lane] = a0; W.w_L[lane] = L; W.w_co[lane] = co;
+          if (lane == 0) W.w_off[MD_WIN] = (mW + MD_WIN <= M) ? off[mW + MD_WIN] : 0x7fffffff;
+        }
+        __syncwarp();
+        const int end = min(hi, W.w_off[MD_WIN]);
+        if (W.w_off[1] >= hi) {
+          // dense: the rest of the link lies in one module -- (row, col) advance incrementally
+          const int om = W.w_off[0], a0 = W.w_a0[0], L = W.w_L[0], co = W.w_co[0];
+          const bool tabled = co + L <= cand_cap;
+          const int c0 = fc - om, c1 = hi - om;
+          int row, col, q32, r32;                       // the lane's cell (row, col); 32 cells further = (+q32, +r32)
+          divmod_small(c0 + lane, L, row, col);
+          divmod_small(32, L, q32, r32);
+          for (int cb = c0; cb < c1; cb += 32) {
+            const int cell = cb + lane;
+            bool pre = false;
+            int a = 0, b = 0;
+            if (cell < c1) {
+              a = a0 + row;
+              b = tabled ? __ldg(cand + co + col) : cand_walk(s, geo, mW, col);
+              pre = ls_prefilter(__ldg(mpos + a), __ldg(maux + a), __ldg(mpos + b), __ldg(maux + b));
             }
+            row += q32; col += r32;
+            if (col >= L) { col -= L; ++row; }
+            ls_push(s, W, pre, a, b, om + cell - lo, qn, pn, lane, lt);
           }
+          fc = hi;
+        } else {
+          // several modules: every lane finds the module of its cell in the cached window
+          for (int f0 = fc; f0 < end; f0 += 32) {
+            const int f = f0 + lane;
+            bool pre = false;
+            int a = 0, b = 0;
+            if (f < end) {
+              int k = 0;
+#pragma unroll
+              for (int step = MD_WIN / 2; step > 0; step >>= 1)
+                if (W.w_off[k + step] <= f) k += step;
+              const int L = W.w_L[k], co = W.w_co[k];
+              int row, col;
+              divmod_small(f - W.w_off[k], L, row, col);
+              a = W.w_a0[k] + row;
+              b = (co + L <= cand_cap) ? __ldg(cand + co + col) : cand_walk(s, geo, mW + k, col);
+              pre = ls_prefilter(__ldg(mpos + a), __ldg(maux + a), __ldg(mpos + b), __ldg(maux + b));
+            }
+            ls_push(s, W, pre, a, b, f - lo, qn, pn, lane, lt);
+          }
+          fc = end;
+          mW += MD_WIN;          // off[mW + MD_WIN] <= fc: the owner of cell fc is at or after it
         }
       }
       if (qn) pn = ls_drain(s, W, qn, pn, lane, lt);
@@ -487,7 +527,6 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __rest
       for (int i = lane; i < pn; i += 32)
         if (soff + i < cap) { LsRec r; r.a = W.p_a[i]; r.b = W.p_b[i]; r.lf = (link << LS_LP_BITS) | W.p_f[i]; r.c = W.p_c[i]; s.ls_rec[soff + i] = r; }
       __syncwarp();
-      link += gridDim.x * PAIR_WARPS;
       continue;
     }
     const int base = chain_exclusive(s.chain_ls, link, pn, lane, epoch);
