@@ -111,7 +111,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   }
   for (int s = 0; s < n_slots; ++s) {
     Slot t{};
-    t.tmp_orig = cv.take<int>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
+    t.tmp_ok = cv.take<int2>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
     t.md_pair_off = cv.take<int>(M + 8); t.md_link_mod = cv.take<int>(MAX_CELLS / MD_LP + 16); t.chain_md = cv.take<unsigned long long>(MAX_CELLS / MD_LP + 2);
     t.md_link_cnt = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_link_soff = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_rec = cv.take<MdRec>(k.max_md);
     t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);

@@ -47,7 +47,7 @@ struct Slot {
   unsigned long long* win3; // [max_pls]
   int* md_head;             // [max_md]  head of the list of pT5 entries containing this MD
   // a0
-  int* tmp_orig; float4* hit; int* hit_orig;
+  int2* tmp_ok; float4* hit; int* hit_orig;
   // a1
   int* md_pair_off; int* md_link_mod; int* md_link_cnt; int* md_link_soff; MdRec* md_rec; unsigned long long* chain_md; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; float4* md_aux; int* md_start;
   // a2
@@ -207,7 +207,7 @@ __global__ void k_scatter(const Slot* __restrict__ slots, Geo geo) {
   const unsigned S = 2u * geo.n_modules;
   LST_FOR_ITEMS(i, s.n_hits) {
     const unsigned key = s.in_key[i];
-    if (key < S) s.tmp_orig[s.sensor_start[key] + atomicAdd(s.cursor + key, 1)] = i;
+    if (key < S) s.tmp_ok[s.sensor_start[key] + atomicAdd(s.cursor + key, 1)] = make_int2(i, (int)key);
   }
 }
 // stable order inside a sensor: rank of a hit = number of hits of the same sensor with a smaller
@@ -215,15 +215,16 @@ __global__ void k_scatter(const Slot* __restrict__ slots, Geo geo) {
 __global__ void k_rank(const Slot* __restrict__ slots) {
   const Slot& s = slots[blockIdx.y];
   const int n = s.cnt[LST_CNT_HIT];
+  const int2* __restrict__ ok = s.tmp_ok;
   LST_FOR_ITEMS(p, n) {
-    const int o = s.tmp_orig[p];
-    const unsigned key = s.in_key[o];
+    const int2 me = ok[p];
+    const int o = me.x, key = me.y;
+    const float x = s.in_x[o], y = s.in_y[o], z = s.in_z[o];        // independent of the rank: issued first
     const int b = s.sensor_start[key], e = s.sensor_start[key + 1];
     int rank = 0;
-    for (int q = b; q < e; ++q) rank += (s.tmp_orig[q] < o);
+    for (int q = b; q < e; ++q) rank += (ok[q].x < o);
     const int d = b + rank;
-    const float x = s.in_x[o], y = s.in_y[o];
-    s.hit[d] = make_float4(x, y, s.in_z[o], fq(fa(fm(x, x), fm(y, y))));   // r as SPEC.md 4.1 computes it
+    s.hit[d] = make_float4(x, y, z, fq(fa(fm(x, x), fm(y, y))));   // r as SPEC.md 4.1 computes it
     s.hit_orig[d] = o;
   }
 }
