@@ -237,7 +237,7 @@ def run_ours(args):
                 pb[0:4 * m].view(torch.float32), pb[4 * m:8 * m].view(torch.float32), pb[8 * m:12 * m].view(torch.float32),
                 pb[12 * m:16 * m].view(torch.float32), pb[16 * m:].view(torch.int8)]
     host_in = [pack(ev) for ev in events]
-    TC_ROWS = 8192
+    TC_ROWS = 4096
     h_out = [torch.zeros(32 + 3 * TC_ROWS, dtype=torch.int32).pin_memory() for _ in range(E)]
     h_cnt = [h[:32] for h in h_out]
     h_tc = [h[32:].view(TC_ROWS, 3) for h in h_out]
@@ -326,7 +326,14 @@ def run_ours(args):
         peak_f = fma_peak if kst == "a5" else alu_peak
         # each of the two passes evaluates every pair: per-launch algorithmic flops = the stage's
         roof = dict(bound="alu", achieved=round(wk["flops"] / k_s / 1e12, 3), peak=round(peak_f, 2), unit="TFLOP/s")
-    roof.update(frac=round(roof["achieved"] / roof["peak"], 4), traffic=None, kernel=kname, kernel_ms=round(prof[kname], 4),
+    traffic = None       # DRAM bytes per launch of this kernel from the committed ncu --set full capture
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    if os.path.exists(tpath):
+        for line in open(tpath).read().splitlines()[1:]:
+            f = line.split(",")
+            if f and f[0] == kname:
+                traffic = round((float(f[3]) + float(f[4])) * n_prof / float(f[2]))
+    roof.update(frac=round(roof["achieved"] / roof["peak"], 4), traffic=traffic, traffic_source="profiles/r01_traffic.csv", kernel=kname, kernel_ms=round(prof[kname], 4),
                 kernel_share_of_step=round(prof[kname] / sum(prof.values()), 3), peak_source=pk["source"],
                 note="ALU peak = 148 SM x 128 lanes x sm_max_mhz un-fused fp32 ops (cuts may not use FMA); DESIGN.md Rooflines")
     del share

@@ -168,3 +168,35 @@ def test_host_load_path(P, geo_full):
     n = int(h_cnt[P.CNT["tc"]])
     assert n == out["counts"]["tc"] and np.array_equal(h_tc[:n].numpy(), out["tc"]["tc"].reshape(-1, 3))
     lst.close()
+
+
+def test_packed_host_buffers_single_copies(P, geo_full):
+    """lst_load_event_host / lst_read_tc_host with adjacent host arrays ([x|y|z|key], [px|py|pz|z0|q], counters +
+    TC rows in one buffer) take the single-transfer path (include/lst.h); the result is the same event."""
+    import torch
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 1)
+    lst = P.LST(geo_full, w, P.default_caps(1), device="cuda:0")
+    n, m = ev.n_hits, ev.n_pls
+    hb = torch.empty(4 * n, dtype=torch.float32).pin_memory()
+    hn = hb.numpy()
+    hn[0:n], hn[n:2 * n], hn[2 * n:3 * n] = ev.x, ev.y, ev.z
+    hn[3 * n:4 * n] = ev.key.view(np.float32)
+    pb = torch.empty(17 * m, dtype=torch.uint8).pin_memory()
+    pf = pb[:16 * m].view(torch.float32).numpy()
+    pf[0:m], pf[m:2 * m], pf[2 * m:3 * m], pf[3 * m:4 * m] = ev.pls_px, ev.pls_py, ev.pls_pz, ev.pls_z0
+    pb[16 * m:].numpy()[:] = ev.pls_q.view(np.uint8)
+    lst.lst_load_event_host(0, hb[0:n], hb[n:2 * n], hb[2 * n:3 * n], hb[3 * n:4 * n].view(torch.int32),
+                            pb[0:4 * m].view(torch.float32), pb[4 * m:8 * m].view(torch.float32), pb[8 * m:12 * m].view(torch.float32),
+                            pb[12 * m:16 * m].view(torch.float32), pb[16 * m:].view(torch.int8))
+    lst.lst_run(0)
+    rows = 4096
+    h = torch.zeros(32 + 3 * rows, dtype=torch.int32).pin_memory()
+    lst.lst_read_tc_host(0, h[:32], h[32:].view(rows, 3))
+    torch.cuda.synchronize()
+    out = lst.fetch(0)
+    parity.compare(geo_full, w, ev, out)
+    assert int(h[31]) == 0 and int(h[P.CNT["tc"]]) == out["counts"]["tc"]
+    ntc = out["counts"]["tc"]
+    assert np.array_equal(h[32:32 + 3 * ntc].numpy().reshape(ntc, 3), out["tc"]["tc"].reshape(ntc, 3))
+    lst.close()
