@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(128) k_t5(const Slot* __restrict__ slots, Caps
 // running sums stay in registers, the 1857 weights sit in shared memory and are read as
 // warp-uniform (broadcast) float4s.  FMA is allowed here (scores agree with the oracle to 1e-5).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_dnn(const Slot* __restrict__ slots, Geo geo) {
+__global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, Geo geo) {
   __shared__ __align__(16) float W1[N_HID * 24];   // rows padded 23 -> 24 for float4 reads
   __shared__ __align__(16) float W2[N_HID * N_HID];
   __shared__ float B1[N_HID], B2[N_HID], W3[N_HID + 1];

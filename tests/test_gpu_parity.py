@@ -200,3 +200,30 @@ def test_packed_host_buffers_single_copies(P, geo_full):
     ntc = out["counts"]["tc"]
     assert np.array_equal(h[32:32 + 3 * ntc].numpy().reshape(ntc, 3), out["tc"]["tc"].reshape(ntc, 3))
     lst.close()
+
+
+def test_bench_launch_configuration_sampled(P, geo_full):
+    """The configuration bench.py times (configs[3]): 64 PU200 events, seeds 100-163, 4 streams x 16-event batched
+    launches, bench capacities.  Sampled events are compared with the oracle in full; every event must be
+    overflow-free and satisfy the TC partition identity n_pLS = pT5 + pT3 + pLS-TC."""
+    import torch
+    w = xavier_weights(3)
+    E, S = 64, 4
+    evs = [config_event(geo_full, 2, seed=100 + i) for i in range(E)]
+    caps = P.Caps(n_slots=E, max_hits=114688, max_md=49152, max_ls=49152, max_t3=32768, max_t5c=16384, max_t5=16384, max_pls=4096)
+    lst = P.LST(geo_full, w, caps)
+    for i, ev in enumerate(evs):
+        lst.load_numpy_event(i, ev)
+    streams = [torch.cuda.Stream() for _ in range(S)]
+    torch.cuda.synchronize()
+    for _ in range(2):                                    # second pass runs on warm state, as in the timed region
+        for si, st in enumerate(streams):
+            lst.lst_run_batch(si * (E // S), E // S, st)
+    torch.cuda.synchronize()
+    for i, ev in enumerate(evs):
+        bits, c = lst.lst_status(i)
+        assert bits == 0, (i, bits)
+        assert c["pt5"] + c["pt3"] + c["plstc"] == ev.n_pls and c["pt5"] + c["t5tc"] + c["pt3"] + c["plstc"] == c["tc"], (i, c)
+    for i in (0, 21, 42, 63):
+        parity.compare(geo_full, w, evs[i], lst.fetch(i))
+    lst.close()
