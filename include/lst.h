@@ -54,7 +54,7 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND,
        /* internal: fill of the MD / LS record buffers; link tickets of the overflow re-run */
        LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TICKET_MD, LST_CNT_TICKET_LS, LST_CNT_DYN_MD, LST_CNT_DYN_LS,
-       LST_N_CNT = 32 };
+       LST_CNT_DYN_T3, LST_CNT_DYN_T5, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
 

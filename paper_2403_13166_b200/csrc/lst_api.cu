@@ -3,7 +3,7 @@
 #include <cuda_runtime.h>
 #include <new>
 #include <vector>
-#include "lst_pairs.cuh"
+#include "lst_tuples.cuh"
 
 using namespace lst;
 
@@ -120,6 +120,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.ls_link_mod = cv.take<int>(MAX_CELLS / LS_LP + 16); t.chain_ls = cv.take<unsigned long long>(MAX_CELLS / LS_LP + 2);
     t.ls_link_cnt = cv.take<int>(MAX_CELLS / LS_LP + 16); t.ls_link_soff = cv.take<int>(MAX_CELLS / LS_LP + 16); t.ls_rec = cv.take<LsRec>(k.max_ls);
     t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
+    t.chain_t3 = cv.take<unsigned long long>(k.max_ls / TUPLE_TPB + 4); t.chain_t5 = cv.take<unsigned long long>(k.max_t3 / TUPLE_TPB + 4);
     t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
     t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
     t.t5_off = cv.take<int>(k.max_t3 + 8); t.t5c_md = cv.take<int>(5 * (size_t)k.max_t5c); t.t5c_t3 = cv.take<int2>(k.max_t5c);
@@ -147,7 +148,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 31;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 28;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -192,6 +193,8 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   for (int i = 0; i < c->n_slots && e == cudaSuccess; ++i) {   // status words start at epoch 0 (never a run's epoch)
     e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (MAX_CELLS / MD_LP + 2));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (MAX_CELLS / LS_LP + 2));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t3, 0, sizeof(unsigned long long) * (c->caps.max_ls / TUPLE_TPB + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
   }
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
   c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
@@ -271,12 +274,9 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_scan<SCAN_LSLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_ls_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
   k_ls_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();     // overflow re-run
-  k_t3<false><<<G, 128, 0, st>>>(sl, k); LST_MARK();
-  k_scan<SCAN_T3><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_t3<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
-  k_t5<false><<<G, 128, 0, st>>>(sl, k); LST_MARK();
-  k_scan<SCAN_T5C><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_t5<true><<<G, 128, 0, st>>>(sl, k); LST_MARK();
+  k_t3_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k, epoch); LST_MARK();
+  k_t3_start<<<G, 256, 0, st>>>(sl); LST_MARK();
+  k_t5_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k, epoch); LST_MARK();
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
   k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_pls_bin<false><<<G1, 1024, 0, st>>>(sl); LST_MARK();
@@ -315,7 +315,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
-      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan1", "a2.ls_plan2", "a2.ls_plan3", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3_count", "a3.scan", "a3.t3_fill", "a4.t5_count", "a4.scan", "a4.t5_fill", "a5.dnn",
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan1", "a2.ls_plan2", "a2.ls_plan3", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3", "a3.t3_start", "a4.t5", "a5.dnn",
       "a5.scan", "a6.pls_bin", "a6.match5", "a6.win5", "a6.pt5_lists", "a6.pls_rebin", "a6.match3", "a6.win3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }

@@ -53,6 +53,7 @@ struct Slot {
   // a2
   int* ls_L; int* ls_off; int* ls_coff; int* ls_cand; int* ls_link_mod; int* ls_link_cnt; int* ls_link_soff; LsRec* ls_rec; unsigned long long* chain_ls; int* ls_start; int2* ls_ab; float* ls_c;
   // a3
+  unsigned long long* chain_t3; unsigned long long* chain_t5;   // look-back status words of the a3 / a4 tiles
   int* t3_off; int4* t3_abc; int* t3_l1; float* t3_k; int* t3_start;
   // a4 / a5
   int* t5_off; int* t5c_md; int2* t5c_t3; float* t5c_curv; float* t5c_feat; float* t5c_score; int* t5c_pass;
@@ -146,7 +147,7 @@ __device__ __forceinline__ void link_owner_table(const int* __restrict__ off, in
   for (int l = (total + LP - 1) / LP + threadIdx.x; l <= total / LP + 1; l += blockDim.x) link_mod[l] = M;
 }
 
-enum { SCAN_SENSOR = 0, SCAN_MDLINK, SCAN_LSLINK, SCAN_T3, SCAN_T5C, SCAN_T5 };
+enum { SCAN_SENSOR = 0, SCAN_MDLINK, SCAN_LSLINK, SCAN_T5 };
 
 template <int MODE>
 __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
@@ -157,8 +158,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ 
   if (MODE == SCAN_SENSOR) { a = s.sensor_start; n = 2 * geo.n_modules; cap = caps.max_hits; icnt = LST_CNT_HIT; iraw = -1; ovf = 0; }
   else if (MODE == SCAN_MDLINK) { a = s.md_link_cnt; n = min(s.md_pair_off[geo.n_modules], MAX_CELLS) / MD_LP + 1; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; }
   else if (MODE == SCAN_LSLINK) { a = s.ls_link_cnt; n = min(s.ls_off[geo.n_modules], MAX_CELLS) / LS_LP + 1; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; }
-  else if (MODE == SCAN_T3) { a = s.t3_off; n = cnt[LST_CNT_LS]; cap = caps.max_t3; icnt = LST_CNT_T3; iraw = LST_CNT_RAW_T3; ovf = LST_ST_OVF_T3; }
-  else if (MODE == SCAN_T5C) { a = s.t5_off; n = cnt[LST_CNT_T3]; cap = caps.max_t5c; icnt = LST_CNT_T5C; iraw = LST_CNT_RAW_T5C; ovf = LST_ST_OVF_T5C; }
   else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
   __syncthreads();   // everyone has read n before thread 0 may overwrite counters below
   const int total = block_scan_inplace(a, n, cap, sm);
@@ -181,9 +180,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ 
     if (threadIdx.x == 0 && cells_total > MAX_CELLS) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), LST_ST_OVF_MD);
     __syncthreads();
     link_owner_table(s.md_pair_off, geo.n_modules, MD_LP, s.md_link_mod);
-  } else if (MODE == SCAN_T3) {   // T3s whose inner MD is a = [t3_start[a], t3_start[a+1])
-    const int n_md = cnt[LST_CNT_MD];
-    for (int i = threadIdx.x; i <= n_md; i += SCAN_THREADS) s.t3_start[i] = a[s.ls_start[i]];
   } else if (MODE == SCAN_T5) {   // T5 list = passing candidates in candidate order
     for (int i = threadIdx.x; i < n; i += SCAN_THREADS)
       if (s.t5c_pass[i] && a[i] < cap) s.t5_list[a[i]] = i;
@@ -226,76 +222,6 @@ __global__ void k_rank(const Slot* __restrict__ slots) {
     const int d = b + rank;
     s.hit[d] = make_float4(x, y, z, fq(fa(fm(x, x), fm(y, y))));   // r as SPEC.md 4.1 computes it
     s.hit_orig[d] = o;
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// a3: triplets (SPEC.md 4.3).  One thread per first LS (a,b); loops over the LSs whose inner MD is b.
-// ------------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(128) k_t3(const Slot* __restrict__ slots, Caps caps) {
-  const Slot& s = slots[blockIdx.y];
-  const int n = s.cnt[LST_CNT_LS];
-  LST_FOR_ITEMS(l0, n) {
-    const int2 ab = s.ls_ab[l0];
-    const int j1 = s.ls_start[ab.y + 1];
-    int j = s.ls_start[ab.y];
-    int out = FILL ? s.t3_off[l0] : 0;
-    if (j < j1) {
-      const Pt A = make_pt(s.md_pos[ab.x], s.md_modt[ab.x] & 3);
-      const Pt B = make_pt(s.md_pos[ab.y], s.md_modt[ab.y] & 3);
-      const float c0 = s.ls_c[l0];
-      for (; j < j1; ++j) {
-        const int cidx = s.ls_ab[j].y;
-        const Pt C = make_pt(s.md_pos[cidx], s.md_modt[cidx] & 3);
-        float k;
-        if (!triplet_eval(A, B, C, k)) continue;
-        if (!(fabsf(fs(c0, k)) <= LST_C_TOL3)) continue;                                  // T3
-        if (!(fabsf(fs(s.ls_c[j], k)) <= LST_C_TOL3)) continue;
-        if (FILL) {
-          if (out < caps.max_t3) { s.t3_abc[out] = make_int4(ab.x, ab.y, cidx, l0); s.t3_l1[out] = j; s.t3_k[out] = k; }
-        }
-        ++out;
-      }
-    }
-    if (!FILL) s.t3_off[l0] = out;
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// a4: quintuplet candidates (SPEC.md 4.4).  One thread per inner T3 (a,b,c); loops over the T3s
-// whose inner MD is c and tests the bridge (b,c,d).
-// ------------------------------------------------------------------------------------------------
-template <bool FILL>
-__global__ void __launch_bounds__(128) k_t5(const Slot* __restrict__ slots, Caps caps) {
-  const Slot& s = slots[blockIdx.y];
-  const int n = s.cnt[LST_CNT_T3];
-  LST_FOR_ITEMS(u, n) {
-    const int4 abc = s.t3_abc[u];
-    const int v1 = s.t3_start[abc.z + 1];
-    int v = s.t3_start[abc.z];
-    int out = FILL ? s.t5_off[u] : 0;
-    if (v < v1) {
-      const Pt B = make_pt(s.md_pos[abc.y], s.md_modt[abc.y] & 3);
-      const Pt C = make_pt(s.md_pos[abc.z], s.md_modt[abc.z] & 3);
-      for (; v < v1; ++v) {
-        const int4 cde = s.t3_abc[v];
-        const Pt D = make_pt(s.md_pos[cde.y], s.md_modt[cde.y] & 3);
-        float kbr;
-        if (!triplet_eval(B, C, D, kbr)) continue;                                        // Q1, Q2
-        if (FILL) {
-          if (out < caps.max_t5c) {
-            int* md = s.t5c_md + 5 * out;
-            md[0] = abc.x; md[1] = abc.y; md[2] = abc.z; md[3] = cde.y; md[4] = cde.z;
-            s.t5c_t3[out] = make_int2(u, v);
-            float* cv = s.t5c_curv + 3 * out;
-            cv[0] = s.t3_k[u]; cv[1] = kbr; cv[2] = s.t3_k[v];
-          }
-        }
-        ++out;
-      }
-    }
-    if (!FILL) s.t5_off[u] = out;
   }
 }
 
