@@ -221,38 +221,21 @@ def run_ours(args):
     ms_local = float(np.mean(step_ms))
 
     # ---- e2e: pinned host inputs -> H2D -> chain -> D2H of counters + TC rows, every step --------
-    # host events packed as the library stages them ([x|y|z|key], [px|py|pz|z0|q]) so each goes over in two copies,
-    # and counters + TC rows come back in one (lst.h: lst_load_event_host / lst_read_tc_host)
-    def pack(ev):
-        n, m = ev.n_hits, ev.n_pls
-        hb = torch.empty(4 * n, dtype=torch.float32).pin_memory()
-        hn = hb.numpy()
-        hn[0:n], hn[n:2 * n], hn[2 * n:3 * n] = ev.x, ev.y, ev.z
-        hn[3 * n:4 * n] = ev.key.view(np.float32)
-        pb = torch.empty(17 * m, dtype=torch.uint8).pin_memory()
-        pf = pb[:16 * m].view(torch.float32).numpy()
-        pf[0:m], pf[m:2 * m], pf[2 * m:3 * m], pf[3 * m:4 * m] = ev.pls_px, ev.pls_py, ev.pls_pz, ev.pls_z0
-        pb[16 * m:].numpy()[:] = ev.pls_q.view(np.uint8)
-        return [hb[0:n], hb[n:2 * n], hb[2 * n:3 * n], hb[3 * n:4 * n].view(torch.int32),
-                pb[0:4 * m].view(torch.float32), pb[4 * m:8 * m].view(torch.float32), pb[8 * m:12 * m].view(torch.float32),
-                pb[12 * m:16 * m].view(torch.float32), pb[16 * m:].view(torch.int8)]
-    host_in = [pack(ev) for ev in events]
+    # e2e: per stream ONE pinned blob in (all its events, lst_load_batch_host) and ONE pinned buffer out (counters +
+    # TC rows of its events, lst_read_tc_batch_host): 1 H2D + 1 D2H copy per 16-event batch
     TC_ROWS = 4096
-    h_out = [torch.zeros(32 + 3 * TC_ROWS, dtype=torch.int32).pin_memory() for _ in range(E)]
-    h_cnt = [h[:32] for h in h_out]
-    h_tc = [h[32:].view(TC_ROWS, 3) for h in h_out]
-    h2d = sum(ev.n_hits * 16 + ev.n_pls * 17 for ev in events)
-    d2h = E * (32 * 4 + TC_ROWS * 12)
     e2e_streams = streams if S > 1 else [main]
+    nb = E // len(e2e_streams)
+    blobs = [P.pack_batch(events[si * nb:(si + 1) * nb]) for si in range(len(e2e_streams))]
+    h_outs = [torch.zeros((nb, 32 + 3 * TC_ROWS), dtype=torch.int32).pin_memory() for _ in e2e_streams]
+    h2d = sum(int(b.numel()) for b in blobs)
+    d2h = E * (32 * 4 + TC_ROWS * 12)
 
     def e2e_step():
         for si, st in enumerate(e2e_streams):
-            lo = si * (E // len(e2e_streams)); n = E // len(e2e_streams)
-            for i in range(lo, lo + n):
-                lst.lst_load_event_host(i, *host_in[i], stream=st)
-            lst.lst_run_batch(lo, n, st)
-            for i in range(lo, lo + n):
-                lst.lst_read_tc_host(i, h_cnt[i], h_tc[i], stream=st)
+            lst.lst_load_batch_host(si * nb, nb, blobs[si], stream=st)
+            lst.lst_run_batch(si * nb, nb, st)
+            lst.lst_read_tc_batch_host(si * nb, nb, h_outs[si], stream=st)
 
     for _ in range(3):
         e2e_step()
@@ -262,8 +245,9 @@ def run_ours(args):
         e2e_step()
     barrier()
     e2e_ms_local = (time.perf_counter() - t0) * 1e3 / args.steps
-    for i in range(E):
-        assert int(h_cnt[i][31]) == 0 and 0 < int(h_cnt[i][P.CNT["tc"]]) <= TC_ROWS, "e2e run failed or TC rows truncated"
+    for h in h_outs:
+        for i in range(nb):
+            assert int(h[i, 31]) == 0 and 0 < int(h[i, P.CNT["tc"]]) <= TC_ROWS, "e2e run failed or TC rows truncated"
     # rebind the resident inputs for the profile pass
     for i, ev in enumerate(events):
         lst.load_numpy_event(i, ev)

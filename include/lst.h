@@ -129,6 +129,20 @@ int lst_load_event_host(lst_ctx* ctx, int32_t slot, int32_t n_hits, const float*
                         const float* h_py, const float* h_pz, const float* h_z0, const int8_t* h_q,
                         void* cuda_stream);
 
+/* Batched host load of slots [first_slot, first_slot + n): ONE host->device copy and one bind launch.
+ * `h_blob` (HOST, pinned recommended) = int32 desc[n][2] = (n_hits, n_pls) per event, padded to a multiple of
+ * 16 bytes, then per event one block padded to a multiple of 16 bytes: x[n_hits] y[n_hits] z[n_hits] (f32)
+ * key[n_hits] (u32) px[n_pls] py[n_pls] pz[n_pls] z0[n_pls] (f32) q[n_pls] (i8).  `blob_bytes` = size of the
+ * buffer (>= the packed size).  LST_EINVAL on sizes above the capacities or a short buffer. */
+int lst_load_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, const void* h_blob, size_t blob_bytes,
+                        void* cuda_stream);
+
+/* Batched read-back: h_out (HOST int32[n][LST_N_CNT + 3*max_rows]) receives, per slot, the counters (status word in
+ * entry LST_N_CNT-1) and the first min(max_rows, count) TC rows (the rest of a slot's rows is left untouched on
+ * the device side, i.e. undefined).  One pack launch + ONE device->host copy.  max_rows <= max_pls + max_t5. */
+int lst_read_tc_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, int32_t* h_out, int32_t max_rows,
+                           void* cuda_stream);
+
 /* Enqueue the whole chain a0..a6 (SPEC.md 4.0-4.6) for one slot / for slots
  * [first_slot, first_slot + n) in single batched launches (event index = a grid dimension). */
 int lst_run(lst_ctx* ctx, int32_t slot, void* cuda_stream);

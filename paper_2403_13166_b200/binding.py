@@ -15,7 +15,7 @@ CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t
            raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
-           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_launches_per_run",
+           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_launches_per_run",
            "lst_destroy"]
 
 
@@ -81,6 +81,8 @@ def load_library():
     L.lst_get.argtypes = [vp, i32, i32, C.POINTER(_View)]
     L.lst_status.argtypes = [vp, i32, C.POINTER(C.c_uint32), vp, vp]
     L.lst_read_tc_host.argtypes = [vp, i32, vp, vp, i32, vp]
+    L.lst_load_batch_host.argtypes = [vp, i32, i32, vp, C.c_size_t, vp]
+    L.lst_read_tc_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
     L.lst_launches_per_run.argtypes = []
     L.lst_run_batch_profile.argtypes = [vp, i32, i32, vp, vp]
     L.lst_launch_name.argtypes = [i32]
@@ -225,6 +227,17 @@ class LST:
         _chk(self.lib.lst_read_tc_host(self.ctx, slot, C.c_void_p(h_counts.data_ptr()), C.c_void_p(h_tc.data_ptr()),
                                        int(h_tc.shape[0]), self._st(stream)), "lst_read_tc_host")
 
+    def lst_load_batch_host(self, first_slot, n, h_blob, stream=None):
+        """h_blob: HOST (pinned) uint8 tensor packed as include/lst.h describes (see pack_batch)."""
+        _chk(self.lib.lst_load_batch_host(self.ctx, first_slot, n, C.c_void_p(h_blob.data_ptr()), C.c_size_t(h_blob.numel()),
+                                          self._st(stream)), "lst_load_batch_host")
+
+    def lst_read_tc_batch_host(self, first_slot, n, h_out, stream=None):
+        """h_out: HOST (pinned) int32 tensor [n, 32 + 3*max_rows]."""
+        rows = (int(h_out.shape[1]) - LST_N_CNT) // 3
+        _chk(self.lib.lst_read_tc_batch_host(self.ctx, first_slot, n, C.c_void_p(h_out.data_ptr()), rows, self._st(stream)),
+             "lst_read_tc_batch_host")
+
     def lst_run_batch_profile(self, first_slot, n, stream=None):
         """Per-launch device times in ms: dict name -> ms (memset + every kernel of one pass)."""
         k = self.launches_per_run() + 1
@@ -268,3 +281,29 @@ class LST:
             n = cnt["t5" if name == "match5" else name]
             res[name] = {k: v.cpu().numpy() for k, v in self.lst_get(slot, name, n).items()}
         return res
+
+
+def pack_batch(events, pin=True):
+    """Pack events (objects with x, y, z, key, pls_px, pls_py, pls_pz, pls_z0, pls_q numpy arrays) into the blob
+    layout of lst_load_batch_host: argument marshalling only."""
+    import torch
+    n = len(events)
+    hdr = (8 * n + 15) // 16 * 16
+    sizes = [((16 * ev.x.size + 17 * ev.pls_px.size + 15) // 16) * 16 for ev in events]
+    blob = torch.zeros(hdr + sum(sizes), dtype=torch.uint8)
+    if pin:
+        blob = blob.pin_memory()
+    b = blob.numpy()
+    desc = b[:8 * n].view(np.int32)
+    off = hdr
+    for i, ev in enumerate(events):
+        nh, npl = int(ev.x.size), int(ev.pls_px.size)
+        desc[2 * i], desc[2 * i + 1] = nh, npl
+        f = b[off:off + 16 * nh].view(np.float32)
+        f[0:nh], f[nh:2 * nh], f[2 * nh:3 * nh] = ev.x, ev.y, ev.z
+        f[3 * nh:4 * nh] = ev.key.view(np.float32)
+        g = b[off + 16 * nh:off + 16 * nh + 16 * npl].view(np.float32)
+        g[0:npl], g[npl:2 * npl], g[2 * npl:3 * npl], g[3 * npl:4 * npl] = ev.pls_px, ev.pls_py, ev.pls_pz, ev.pls_z0
+        b[off + 16 * nh + 16 * npl:off + 16 * nh + 17 * npl] = ev.pls_q.view(np.uint8)
+        off += sizes[i]
+    return blob

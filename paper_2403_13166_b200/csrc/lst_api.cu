@@ -14,6 +14,8 @@ struct lst_ctx {
   Caps caps{};
   Slot* d_slots = nullptr;        // device array [n_slots]
   std::vector<Slot> h_slots;      // host mirror of the carved pointers (inputs not tracked)
+  char* batch_in = nullptr; size_t batch_in_stride = 0;     // staging of lst_load_batch_host, one stride per slot
+  int* batch_out = nullptr; size_t batch_out_stride = 0;    // staging of lst_read_tc_batch_host (ints per slot)
   char* zero_base = nullptr; size_t zero_stride = 0;
   char* ones_base = nullptr; size_t ones_stride = 0;
   bool sticky_cuda_error = false;
@@ -65,6 +67,7 @@ Caps make_caps(const lst_caps* c) {
 
 // One pass lays out the whole workspace; used both to measure and to carve.
 struct Layout {
+  char* batch_in; size_t batch_in_stride; int* batch_out; size_t batch_out_stride;
   Slot* slots; uint8_t* modt; int* rowptr; int* col; float* weights;
   char* zero_base; size_t zero_stride; char* ones_base; size_t ones_stride;
   size_t total;
@@ -78,6 +81,10 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   L.rowptr = cv.take<int>(M + 1);
   L.col = cv.take<int>(nnz > 0 ? nnz : 1);
   L.weights = cv.take<float>(N_W);
+  L.batch_in_stride = blob_event_bytes(k.max_hits, k.max_pls) + 16;
+  L.batch_in = cv.take<char>(L.batch_in_stride * n_slots + 1024);
+  L.batch_out_stride = LST_N_CNT + 3 * (size_t)k.max_tc;
+  L.batch_out = cv.take<int>(L.batch_out_stride * n_slots);
   if (out) out->assign(n_slots, Slot{});
   // zero region (contiguous over slots so one memset covers a batch)
   {
@@ -181,6 +188,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   if (L.total > bytes) { delete c; return LST_ENOMEM; }
   c->d_slots = L.slots;
   c->zero_base = L.zero_base; c->zero_stride = L.zero_stride;
+  c->batch_in = L.batch_in; c->batch_in_stride = L.batch_in_stride; c->batch_out = L.batch_out; c->batch_out_stride = L.batch_out_stride;
   c->ones_base = L.ones_base; c->ones_stride = L.ones_stride;
   std::vector<uint8_t> modt(M);
   for (int m = 0; m < M; ++m) modt[m] = uint8_t((geo->subdet[m] << 1) | geo->mtype[m]);
@@ -368,6 +376,37 @@ int lst_read_tc_host(lst_ctx* c, int32_t slot, int32_t* h_counts, int32_t* h_tc,
   if (max_rows > 0 && bad(c, cudaMemcpyAsync(h_tc, s.tc, sizeof(int32_t) * 3 * (size_t)max_rows, cudaMemcpyDeviceToHost, st)))
     return LST_ECUDA;
   return LST_OK;
+}
+
+int lst_load_batch_host(lst_ctx* c, int32_t first, int32_t n, const void* h_blob, size_t blob_bytes, void* cuda_stream) {
+  if (!c || !h_blob || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  const int32_t* desc = static_cast<const int32_t*>(h_blob);
+  size_t need = blob_header_bytes(n);
+  if (blob_bytes < need) return LST_EINVAL;
+  for (int e = 0; e < n; ++e) {
+    const int nh = desc[2 * e], np = desc[2 * e + 1];
+    if (nh < 0 || np < 0 || nh > c->caps.max_hits || np > c->caps.max_pls) return LST_EINVAL;
+    need += blob_event_bytes(nh, np);
+  }
+  if (need > blob_bytes || need > c->batch_in_stride * n + 1024) return LST_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* dst = c->batch_in + c->batch_in_stride * first;
+  if (bad(c, cudaMemcpyAsync(dst, h_blob, need, cudaMemcpyHostToDevice, st))) return LST_ECUDA;
+  k_bind_batch<<<(n + 63) / 64, 64, 0, st>>>(c->d_slots, first, n, dst);
+  return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
+}
+
+int lst_read_tc_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out, int32_t max_rows, void* cuda_stream) {
+  if (!c || !h_out || first < 0 || n <= 0 || first + n > c->n_slots || max_rows < 0) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  if (max_rows > c->caps.max_tc) return LST_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int* dst = c->batch_out + c->batch_out_stride * first;
+  k_pack_tc<<<dim3(8, n), 256, 0, st>>>(c->d_slots + first, max_rows, dst);
+  if (bad(c, cudaGetLastError())) return LST_ECUDA;
+  const size_t bytes = sizeof(int32_t) * (LST_N_CNT + 3 * (size_t)max_rows) * n;
+  return bad(c, cudaMemcpyAsync(h_out, dst, bytes, cudaMemcpyDeviceToHost, st)) ? LST_ECUDA : LST_OK;
 }
 
 void lst_destroy(lst_ctx* c) { delete c; }

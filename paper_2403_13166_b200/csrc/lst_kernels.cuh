@@ -583,4 +583,33 @@ __global__ void k_bind(Slot* slots, int slot, const float* x, const float* y, co
   s.in_px = px; s.in_py = py; s.in_pz = pz; s.in_z0 = z0; s.in_q = q; s.n_pls = n_pls;
 }
 
+// batched bind: the staged blob starts with int32 desc[n][2] = (n_hits, n_pls) (padded to 16 bytes), followed by
+// one 16-byte aligned block per event: [x|y|z|key] (4 n_hits words), [px|py|pz|z0] (4 n_pls words), q (n_pls bytes)
+__host__ __device__ inline size_t blob_event_bytes(int n_hits, int n_pls) {
+  return ((size_t)16 * n_hits + (size_t)17 * n_pls + 15) / 16 * 16;
+}
+__host__ __device__ inline size_t blob_header_bytes(int n) { return ((size_t)8 * n + 15) / 16 * 16; }
+__global__ void k_bind_batch(Slot* slots, int first, int n, const char* blob) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const int* desc = reinterpret_cast<const int*>(blob);
+  size_t off = blob_header_bytes(n);
+  for (int i = 0; i < e; ++i) off += blob_event_bytes(desc[2 * i], desc[2 * i + 1]);
+  const int nh = desc[2 * e], np = desc[2 * e + 1];
+  const float* f = reinterpret_cast<const float*>(blob + off);
+  const float* g = f + 4 * (size_t)nh;
+  Slot& s = slots[first + e];
+  s.in_x = f; s.in_y = f + nh; s.in_z = f + 2 * (size_t)nh; s.in_key = reinterpret_cast<const uint32_t*>(f + 3 * (size_t)nh); s.n_hits = nh;
+  s.in_px = g; s.in_py = g + np; s.in_pz = g + 2 * (size_t)np; s.in_z0 = g + 3 * (size_t)np;
+  s.in_q = reinterpret_cast<const int8_t*>(g + 4 * (size_t)np); s.n_pls = np;
+}
+// packs counters + the first `rows` TC rows of n slots into one contiguous buffer [n][LST_N_CNT + 3 rows]
+__global__ void k_pack_tc(const Slot* __restrict__ slots, int rows, int* __restrict__ out) {
+  const Slot& s = slots[blockIdx.y];
+  const int w = LST_N_CNT + 3 * rows;
+  int* o = out + (size_t)blockIdx.y * w;
+  const int n = LST_N_CNT + 3 * min(rows, s.tc_hdr[LST_CNT_TC]);
+  LST_FOR_ITEMS(i, n) o[i] = s.tc_hdr[i];
+}
+
 }  // namespace lst

@@ -227,3 +227,32 @@ def test_bench_launch_configuration_sampled(P, geo_full):
     for i in (0, 21, 42, 63):
         parity.compare(geo_full, w, evs[i], lst.fetch(i))
     lst.close()
+
+
+def test_batched_host_load_and_read(P, geo_full):
+    """lst_load_batch_host (one blob, one H2D copy) + lst_read_tc_batch_host (one D2H copy) give the same events
+    and TC rows as the per-event path; malformed blobs are rejected."""
+    import torch
+    w = xavier_weights(3)
+    evs = [config_event(geo_full, 1, seed=7), make_event(geo_full, 3), config_event(geo_full, 2, seed=101)]
+    lst = P.LST(geo_full, w, P.default_caps(4))
+    blob = P.pack_batch(evs)
+    lst.lst_load_batch_host(1, 3, blob)                  # slots 1..3
+    lst.lst_run_batch(1, 3)
+    rows = 4096
+    h = torch.zeros((3, 32 + 3 * rows), dtype=torch.int32).pin_memory()
+    lst.lst_read_tc_batch_host(1, 3, h)
+    torch.cuda.synchronize()
+    for i, ev in enumerate(evs):
+        out = lst.fetch(1 + i)
+        parity.compare(geo_full, w, ev, out)
+        ntc = out["counts"]["tc"]
+        assert int(h[i, 31]) == 0 and int(h[i, P.CNT["tc"]]) == ntc
+        assert np.array_equal(h[i, 32:32 + 3 * ntc].numpy().reshape(ntc, 3), out["tc"]["tc"].reshape(ntc, 3))
+    with pytest.raises(P.LstError):                      # short buffer
+        lst.lst_load_batch_host(0, 3, blob[:1000])
+    bad = blob.clone()
+    bad.numpy()[:4].view(np.int32)[0] = 10 ** 8          # n_hits above the capacity
+    with pytest.raises(P.LstError):
+        lst.lst_load_batch_host(0, 3, bad)
+    lst.close()
