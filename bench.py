@@ -268,6 +268,18 @@ def run_ours(args):
                 prof[k] = prof.get(k, 0.0) + v / reps
     n_prof = E if S == 1 else per
     tot, stages = algorithmic_work(lst, geo, range(n_prof))
+    # launch floor: the smallest kernel of the library (a 1-thread bind), back to back on one stream -- the time
+    # below which no stage of a small batch can go (report it beside the per-stage fractions)
+    ev0 = events[0]
+    torch.cuda.synchronize()
+    fa, fb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    fa.record(main)
+    for _ in range(200):
+        lst.lib.lst_load_event(lst.ctx, 0, 0, None, None, None, None, 0, None, None, None, None, None, lst._st(main))
+    fb.record(main)
+    torch.cuda.synchronize()
+    launch_floor_us = fa.elapsed_time(fb) * 1e3 / 200
+    lst.load_numpy_event(0, ev0)
 
     def red_max(v):
         if dist is None:
@@ -344,7 +356,7 @@ def run_ours(args):
                            parallelism=f"replicas x{world}" if world > 1 else "single GPU"),
                e2e=dict(value=round(e2e_value, 1), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=round(e2e_ms, 4),
                         timing="wall clock around K steps incl. pinned H2D of every input and D2H of counters + TC rows"),
-               gpu_launches=args.steps * S * lst.launches_per_run(),
+               gpu_launches=args.steps * S * lst.launches_per_run(), launch_floor_us=round(launch_floor_us, 2),
                clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows,
                kernels_ms={k: round(v, 4) for k, v in prof.items()},
                per_event=dict(us=round(ms * 1e3 / E, 2), objects={k: round(v / n_prof, 1) for k, v in tot.items()}),
