@@ -2,6 +2,8 @@
 // Host logic only; every step of the hot path runs in the kernels of lst_kernels.cuh.
 #include <cuda_runtime.h>
 #include <new>
+#include <cstdlib>
+#include <map>
 #include <vector>
 #include "lst_tuples.cuh"
 
@@ -19,7 +21,8 @@ struct lst_ctx {
   char* zero_base = nullptr; size_t zero_stride = 0;
   char* ones_base = nullptr; size_t ones_stride = 0;
   bool sticky_cuda_error = false;
-  unsigned epoch = 0;             // run counter carried in the look-back status words (lst_pairs.cuh)
+  bool use_graphs = true;         // replay lst_run_batch as a CUDA graph on capturable streams (LST_GRAPHS=0 disables)
+  std::map<long long, cudaGraphExec_t> graphs;   // (first_slot, n) -> instantiated launch sequence
 };
 
 namespace {
@@ -118,7 +121,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   }
   for (int s = 0; s < n_slots; ++s) {
     Slot t{};
-    t.tmp_ok = cv.take<int2>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
+    t.epoch_dev = cv.take<unsigned>(4); t.tmp_ok = cv.take<int2>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
     t.md_pair_off = cv.take<int>(M + 8); t.md_link_mod = cv.take<int>(MAX_CELLS / MD_LP + 16); t.chain_md = cv.take<unsigned long long>(MAX_CELLS / MD_LP + 2);
     t.md_link_cnt = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_link_soff = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_rec = cv.take<MdRec>(k.max_md);
     t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
@@ -199,12 +202,14 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   if (e == cudaSuccess) e = cudaMemcpy(L.slots, c->h_slots.data(), sizeof(Slot) * c->n_slots, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(c->zero_base, 0, c->zero_stride * c->n_slots);
   for (int i = 0; i < c->n_slots && e == cudaSuccess; ++i) {   // status words start at epoch 0 (never a run's epoch)
-    e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (MAX_CELLS / MD_LP + 2));
+    e = cudaMemset(c->h_slots[i].epoch_dev, 0, 16);
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (MAX_CELLS / MD_LP + 2));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (MAX_CELLS / LS_LP + 2));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t3, 0, sizeof(unsigned long long) * (c->caps.max_ls / TUPLE_TPB + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
   }
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
+  if (const char* g = std::getenv("LST_GRAPHS")) c->use_graphs = !(g[0] == '0');
   c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
   *out = c;
   return LST_OK;
@@ -270,21 +275,20 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_scatter<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_rank<<<G, 256, 0, st>>>(sl); LST_MARK();
-  const unsigned epoch = (c->epoch = (c->epoch % 0x3FFFFFFFu) + 1u);   // validates this run's look-back status words
-  k_md_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();
+  k_md_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_scan<SCAN_MDLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_md_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_md_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();     // overflow re-run (returns at once otherwise)
+  k_md_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run (returns at once otherwise)
   k_ls_plan1<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_ls_plan2<<<G1, SCAN_THREADS, 0, st>>>(sl, g); LST_MARK();
   k_ls_plan3<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();
+  k_ls_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_scan<SCAN_LSLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_ls_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k, epoch); LST_MARK();     // overflow re-run
-  k_t3_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k, epoch); LST_MARK();
+  k_ls_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run
+  k_t3_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
   k_t3_start<<<G, 256, 0, st>>>(sl); LST_MARK();
-  k_t5_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k, epoch); LST_MARK();
+  k_t5_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
   k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
   k_pls_bin<false><<<G1, 1024, 0, st>>>(sl); LST_MARK();
@@ -303,7 +307,32 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
 int lst_run_batch(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
   if (!c || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
   if (c->sticky_cuda_error) return LST_ECUDA;
-  return run_sequence(c, first, n, static_cast<cudaStream_t>(cuda_stream), nullptr);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  // The launch sequence has no per-run arguments, so it is captured once per (first, n) and replayed as a CUDA graph
+  // (one submission instead of 26 launches + 2 memsets).  The legacy default stream cannot be captured: direct launches.
+  if (c->use_graphs && st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread) {
+    const long long key = ((long long)first << 32) | (unsigned)n;
+    auto it = c->graphs.find(key);
+    if (it == c->graphs.end()) {
+      cudaGraphExec_t exec = nullptr;
+      if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        const int rc = run_sequence(c, first, n, st, nullptr);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(st, &graph);
+        if (rc == LST_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
+        if (graph) cudaGraphDestroy(graph);
+      }
+      if (!exec) {                       // capture not possible here: stay with direct launches for this context
+        (void)cudaGetLastError();
+        c->use_graphs = false;
+        c->sticky_cuda_error = false;
+        return run_sequence(c, first, n, st, nullptr);
+      }
+      it = c->graphs.emplace(key, exec).first;
+    }
+    return bad(c, cudaGraphLaunch(it->second, st)) ? LST_ECUDA : LST_OK;
+  }
+  return run_sequence(c, first, n, st, nullptr);
 }
 
 int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream, float* h_ms) {
@@ -409,6 +438,10 @@ int lst_read_tc_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out,
   return bad(c, cudaMemcpyAsync(h_out, dst, bytes, cudaMemcpyDeviceToHost, st)) ? LST_ECUDA : LST_OK;
 }
 
-void lst_destroy(lst_ctx* c) { delete c; }
+void lst_destroy(lst_ctx* c) {
+  if (!c) return;
+  for (auto& kv : c->graphs) cudaGraphExecDestroy(kv.second);
+  delete c;
+}
 
 }  // extern "C"

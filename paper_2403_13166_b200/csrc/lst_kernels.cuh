@@ -39,6 +39,7 @@ struct Slot {
   const float *in_x, *in_y, *in_z; const uint32_t* in_key; int n_hits;
   const float *in_px, *in_py, *in_pz, *in_z0; const int8_t* in_q; int n_pls;
   // zero-initialised per run
+  unsigned* epoch_dev;      // run counter of the slot (not cleared): validates the look-back status words of a run
   int* cnt;                 // [LST_N_CNT]
   int* sensor_start;        // [2M+1] histogram, then exclusive scan in place
   int* cursor;              // [2M]
@@ -191,6 +192,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ 
 // ------------------------------------------------------------------------------------------------
 __global__ void k_hist(const Slot* __restrict__ slots, Geo geo) {
   const Slot& s = slots[blockIdx.y];
+  if (blockIdx.x == 0 && threadIdx.x == 0) *s.epoch_dev = (*s.epoch_dev % 0x3FFFFFFFu) + 1u;   // first kernel of a run
   const unsigned S = 2u * geo.n_modules;
   LST_FOR_ITEMS(i, s.n_hits) {
     const unsigned key = s.in_key[i];

@@ -31,8 +31,9 @@ constexpr int MD_WIN = 32;           // modules of a link cached in shared memor
 __device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
 // ---- decoupled look-back over 64-bit status words: flag (2 bits) | run epoch (30 bits) | value (32 bits).
-// A word counts only if its epoch is the current run's (lst_api.cu increments it per launch sequence), so the
-// status arrays never need clearing.
+// A word counts only if its epoch is the current run's (k_hist, the first kernel of a run, increments the slot's
+// device-side run counter), so the status arrays never need clearing and the launch sequence has no per-run
+// arguments (it can be replayed as a CUDA graph).
 constexpr unsigned long long CH_AGG = 1ull << 62, CH_INC = 2ull << 62, CH_VAL = 0xFFFFFFFFull;
 __device__ __forceinline__ unsigned chain_flag(unsigned long long w, unsigned epoch) {
   return (((unsigned)(w >> 32)) & 0x3FFFFFFFu) == epoch ? (unsigned)(w >> 62) : 0u;
@@ -144,9 +145,10 @@ __device__ __forceinline__ int md_drain(const Slot& s, MdWarp& W, int n, int pn,
 }
 
 template <bool CHAIN>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __restrict__ slots, Geo geo, Caps caps, unsigned epoch) {
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   __shared__ MdWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
   if (CHAIN && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;
   const int lane = threadIdx.x & 31;
   MdWarp& W = Wall[threadIdx.x >> 5];
@@ -434,9 +436,10 @@ __device__ __forceinline__ int first_row_at(const Slot& s, const int* __restrict
 }
 
 template <bool CHAIN>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __restrict__ slots, Geo geo, Caps caps, unsigned epoch) {
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
   if (CHAIN && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;
   const int lane = threadIdx.x & 31;
   LsWarp& W = Wall[threadIdx.x >> 5];

@@ -30,10 +30,11 @@ __device__ __forceinline__ int block_excl(int v, int* sm /*[TUPLE_TPB/32 + 1]*/,
 }
 
 // a3 (SPEC.md 4.3): rows = LS l0 = (a,b); partners = LSs whose inner MD is b
-__global__ void __launch_bounds__(TUPLE_TPB) k_t3_one(const Slot* __restrict__ slots, Caps caps, unsigned epoch) {
+__global__ void __launch_bounds__(TUPLE_TPB) k_t3_one(const Slot* __restrict__ slots, Caps caps) {
   __shared__ int sm[TUPLE_TPB / 32 + 1];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
   const int n = s.cnt[LST_CNT_LS];
   const int n_tiles = (n + TUPLE_TPB - 1) / TUPLE_TPB + (n == 0);
   const int cap = caps.max_t3;
@@ -117,10 +118,11 @@ __global__ void __launch_bounds__(256) k_t3_start(const Slot* __restrict__ slots
 }
 
 // a4 (SPEC.md 4.4): rows = T3 u = (a,b,c); partners = T3s whose inner MD is c; the bridge (b,c,d) must pass
-__global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ slots, Caps caps, unsigned epoch) {
+__global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ slots, Caps caps) {
   __shared__ int sm[TUPLE_TPB / 32 + 1];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
   const int n = s.cnt[LST_CNT_T3];
   const int n_tiles = (n + TUPLE_TPB - 1) / TUPLE_TPB + (n == 0);
   const int cap = caps.max_t5c;
