@@ -144,7 +144,10 @@ int lst_read_tc_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, int32_t*
                            void* cuda_stream);
 
 /* Enqueue the whole chain a0..a6 (SPEC.md 4.0-4.6) for one slot / for slots
- * [first_slot, first_slot + n) in single batched launches (event index = a grid dimension). */
+ * [first_slot, first_slot + n) in single batched launches (event index = a grid dimension).
+ * On a capturable stream (any stream but the legacy default stream 0) the launch sequence is captured once per
+ * (first_slot, n) and replayed as a CUDA graph; the environment variable LST_GRAPHS=0 (read by lst_create) keeps
+ * direct launches.  Results are identical either way. */
 int lst_run(lst_ctx* ctx, int32_t slot, void* cuda_stream);
 int lst_run_batch(lst_ctx* ctx, int32_t first_slot, int32_t n, void* cuda_stream);
 
