@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, 
 // bucket walk is a conservative prefilter: every pair that passes the exact test is visited, and the
 // decisions themselves are still taken by the exact SPEC.md arithmetic.  pLS whose h is outside the
 // bucketed range (pT < ~0.76 GeV, NaN) or whose q is not +-1 go to an overflow bucket every object visits.
-constexpr int PLS_NB = 256, PLS_K = 8, PLS_NBINS = (PLS_K + 1) * PLS_NB;
+constexpr int PLS_NB = 512, PLS_K = 8, PLS_NBINS = (PLS_K + 1) * PLS_NB;
 #define LST_PLS_HMAX 0.0075f
 #define LST_PI_F 3.14159265358979f
 
