@@ -15,10 +15,14 @@
 // type so that tests can run a `double` instantiation of the same procedure as a pin.
 //
 // Parity status: the paper prints no cut value, object count or score for any input that can be
-// constructed, so parity AGAINST THE PAPER is unpinned.  Against
-// mathematics it is pinned by tests/test_oracle_*.py: brute-force enumeration, closed-form
-// helices, textbook curvature cases, arcfac vs asin, an independent fp64 MLP, TC partition
-// identities, rotation / mirror / permutation invariance, cut-loosening monotonicity.
+// constructed, so parity AGAINST THE PAPER is unpinned.  Against SPEC.md and
+// mathematics every function below is pinned (tests/test_oracle_pins.py, tests/test_oracle_terms.py):
+// brute-force enumeration, closed-form helices, textbook curvature cases, arcfac vs asin, an
+// independent fp64 MLP, rotation / mirror / permutation invariance, cut-loosening monotonicity, and --
+// term by term -- hand-derived accept / reject boundaries for every tolerance term of M2/M3, L1-L3,
+// T1-T3, the anchor test and chi2, plus hand-built scenarios for run_chain's own assignments, the
+// bridge indices and the TC used / free / tie rules.  tests/test_oracle_mutants.py shows that 46
+// single-line mutations of this file each fail at least one pin.
 #include <cmath>
 #include <cstdint>
 #include <cstring>

@@ -26,38 +26,62 @@ def build(force: bool = False) -> str:
 _lib = None
 
 
+def _bind(path):
+    """dlopen an oracle library and declare its signatures."""
+    L = C.CDLL(path)
+    L.lst_oracle_run.restype = C.c_void_p
+    L.lst_oracle_run.argtypes = [C.c_int32] + [C.c_void_p] * 5 + [C.c_int32] + [C.c_void_p] * 4 + \
+        [C.c_int32] + [C.c_void_p] * 5 + [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32]
+    L.lst_oracle_count.restype = C.c_int64
+    L.lst_oracle_count.argtypes = [C.c_void_p, C.c_int32]
+    L.lst_oracle_copy_int.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    L.lst_oracle_copy_real.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    L.lst_oracle_free.argtypes = [C.c_void_p]
+    L.lst_oracle_md_eval.restype = C.c_int32
+    L.lst_oracle_md_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+    L.lst_oracle_ls_eval.restype = C.c_int32
+    L.lst_oracle_ls_eval.argtypes = [C.c_void_p] * 3
+    L.lst_oracle_t3_eval.restype = C.c_int32
+    L.lst_oracle_t3_eval.argtypes = [C.c_void_p] * 3 + [C.c_float, C.c_float, C.c_void_p]
+    L.lst_oracle_bridge_eval.restype = C.c_int32
+    L.lst_oracle_bridge_eval.argtypes = [C.c_void_p] * 4
+    L.lst_oracle_pls_match.restype = C.c_int32
+    L.lst_oracle_pls_match.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
+    L.lst_oracle_pls_residual.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    L.lst_oracle_arcfac.restype = C.c_float
+    L.lst_oracle_arcfac.argtypes = [C.c_float]
+    L.lst_oracle_arcfac_f64.restype = C.c_double
+    L.lst_oracle_arcfac_f64.argtypes = [C.c_double]
+    L.lst_oracle_features.argtypes = [C.c_void_p] * 4 + [C.c_float] * 3 + [C.c_void_p]
+    L.lst_oracle_mlp.restype = C.c_float
+    L.lst_oracle_mlp.argtypes = [C.c_void_p, C.c_void_p]
+    return L
+
+
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
-        L.lst_oracle_run.restype = C.c_void_p
-        L.lst_oracle_run.argtypes = [C.c_int32] + [C.c_void_p] * 5 + [C.c_int32] + [C.c_void_p] * 4 + \
-            [C.c_int32] + [C.c_void_p] * 5 + [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32]
-        L.lst_oracle_count.restype = C.c_int64
-        L.lst_oracle_count.argtypes = [C.c_void_p, C.c_int32]
-        L.lst_oracle_copy_int.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
-        L.lst_oracle_copy_real.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
-        L.lst_oracle_free.argtypes = [C.c_void_p]
-        L.lst_oracle_md_eval.restype = C.c_int32
-        L.lst_oracle_md_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
-        L.lst_oracle_ls_eval.restype = C.c_int32
-        L.lst_oracle_ls_eval.argtypes = [C.c_void_p] * 3
-        L.lst_oracle_t3_eval.restype = C.c_int32
-        L.lst_oracle_t3_eval.argtypes = [C.c_void_p] * 3 + [C.c_float, C.c_float, C.c_void_p]
-        L.lst_oracle_bridge_eval.restype = C.c_int32
-        L.lst_oracle_bridge_eval.argtypes = [C.c_void_p] * 4
-        L.lst_oracle_pls_match.restype = C.c_int32
-        L.lst_oracle_pls_match.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
-        L.lst_oracle_pls_residual.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
-        L.lst_oracle_arcfac.restype = C.c_float
-        L.lst_oracle_arcfac.argtypes = [C.c_float]
-        L.lst_oracle_arcfac_f64.restype = C.c_double
-        L.lst_oracle_arcfac_f64.argtypes = [C.c_double]
-        L.lst_oracle_features.argtypes = [C.c_void_p] * 4 + [C.c_float] * 3 + [C.c_void_p]
-        L.lst_oracle_mlp.restype = C.c_float
-        L.lst_oracle_mlp.argtypes = [C.c_void_p, C.c_void_p]
-        _lib = L
+        _lib = _bind(build())
     return _lib
+
+
+class use_library:
+    """Context manager for tests/test_oracle_mutants.py: route every call of this module through another
+    build of the oracle (a deliberately broken copy) so that the pins can be shown to notice the breakage."""
+
+    def __init__(self, path):
+        self.path = path
+
+    def __enter__(self):
+        global _lib
+        self.saved = _lib
+        _lib = _bind(self.path)
+        return self
+
+    def __exit__(self, *exc):
+        global _lib
+        _lib = self.saved
+        return False
 
 
 def _p(a):

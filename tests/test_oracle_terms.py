@@ -1,0 +1,582 @@
+"""Term-by-term pins of the oracle's cut predicates (SPEC.md 4.1-4.6).  CPU only.
+
+Every expected accept / reject below is derived BY HAND from the SPEC.md text on inputs built so that all other
+terms of the cut vanish (or are a stated constant): collinear anchors give curvature 0 and arcfac(0) = 1, so
+arc lengths equal radii / chord lengths exactly; a 1000 GeV seed along +x is a straight line with 2*R*h = 1.  Each
+pin sits a few per cent inside / outside the boundary of ONE term, so dropping that term, changing its coefficient or
+swapping its operand flips at least one stated decision.  tests/test_oracle_mutants.py re-runs the `pin_*`
+functions against deliberately broken builds of oracle/lst_oracle.cpp to show that they do notice.
+"""
+import numpy as np
+import pytest
+
+from lstgen import make_event, config_event, xavier_weights
+from lstgen.events import KAPPA64
+from oracle import lst_oracle as O
+
+
+def A9(x, y, z, c=0.0, w=1.0, f=0.0, dz=0.0, dr=0.0, r=None):
+    """anchor record of the single-predicate entry points: x, y, z, r, c_md, w, f, dz, dr"""
+    return np.array([x, y, z, np.hypot(x, y) if r is None else r, c, w, f, dz, dr], dtype=np.float32)
+
+
+# ====================================================================== a2: L2 (SPEC.md 4.2)
+def pin_ls_L2_terms():
+    """A = (40, 0, zA), B = (60, 0, zB): collinear with the origin => c = 0, sA = 40, sB = 60 exactly.
+    L2:  |60 zA - 40 zB| <= 15*20 + dzA*60 + dzB*40 + drA*|zB| + drB*|zA|."""
+    ls = lambda a, b: O.ls_eval(a, b)[0]
+    # Z0_MAX * |sB - sA| alone = 300
+    assert ls(A9(40, 0, 4.9), A9(60, 0, 0.0))            # 294 <= 300
+    assert not ls(A9(40, 0, 5.1), A9(60, 0, 0.0))        # 306 >  300
+    assert ls(A9(40, 0, -4.9), A9(60, 0, 0.0))           # |.|
+    # + dzA * sB = 10 * 60 -> 900   (dzA * sA would give 700)
+    assert ls(A9(40, 0, 14.9, dz=10), A9(60, 0, 0.0))    # 894
+    assert not ls(A9(40, 0, 15.1, dz=10), A9(60, 0, 0.0))
+    # + dzB * sA = 10 * 40 -> 700   (dzB * sB would give 900)
+    assert ls(A9(40, 0, 11.6), A9(60, 0, 0.0, dz=10))    # 696
+    assert not ls(A9(40, 0, 11.8), A9(60, 0, 0.0, dz=10))
+    # + drA * |zB| = 4 * 100 -> 700 (drA * |zA| = 4 * 55 would give 520); negative z checks the |.|
+    assert ls(A9(40, 0, -55.1, dr=4), A9(60, 0, -100.0))      # |-3306 + 4000| = 694
+    assert not ls(A9(40, 0, -54.9, dr=4), A9(60, 0, -100.0))  # 706
+    # + drB * |zA| = 4 * 100 -> 700 (drB * |zB| = 4 * 132 would give 830)
+    assert ls(A9(40, 0, 100.0), A9(60, 0, 132.6, dr=4))       # |6000 - 5304| = 696
+    assert not ls(A9(40, 0, 100.0), A9(60, 0, 132.4, dr=4))   # 704
+    # all five together: 300 + 1*60 + 2*40 + 0.5*50 + 0.25*30 = 472.5 ; lhs = |60*30 - 40*50| = 200 ; then 480
+    assert ls(A9(40, 0, 30.0, dz=1, dr=0.5), A9(60, 0, 50.0, dz=2, dr=0.25))
+    assert not ls(A9(40, 0, 30.0, dz=1, dr=0.5), A9(60, 0, 33.0, dz=2, dr=0.25))   # lhs 480 > 300+60+80+16.5+7.5 = 464
+
+
+def _on_circle(R, t, z=0.0, **kw):
+    """point of the circle of radius R through the origin with centre (0, R): a track leaving the origin along +x
+    and turning towards +y, i.e. azimuth increasing = NEGATIVE charge (SPEC.md 1) => signed curvature -1/R"""
+    return A9(R * np.sin(t), R * (1.0 - np.cos(t)), z, **kw)
+
+
+def pin_ls_curvature_L1_L3():
+    """c_ls is the signed curvature of the circle through the origin, A and B: -1/R on the circle above."""
+    R = 100.0
+    ok, c = O.ls_eval(_on_circle(R, 0.3, dz=100, c=-0.01), _on_circle(R, 0.5, dz=100, c=-0.01))
+    assert ok and abs(c + 0.01) < 2e-8
+    ok, c = O.ls_eval(_on_circle(R, -0.3, dz=100, c=0.01), _on_circle(R, -0.5, dz=100, c=0.01))   # mirror: positive charge
+    assert ok and abs(c - 0.01) < 2e-8
+    # L1: |c| <= 1.05 * 0.0114 / 0.8 = 0.0149625  <=>  R >= 66.83 cm
+    assert O.ls_eval(_on_circle(67.5, 0.3, dz=100, c=-1 / 67.5), _on_circle(67.5, 0.5, dz=100, c=-1 / 67.5))[0]
+    assert not O.ls_eval(_on_circle(66.0, 0.3, dz=100, c=-1 / 66.0), _on_circle(66.0, 0.5, dz=100, c=-1 / 66.0))[0]
+    # L3 inner MD: |c_md(a) - c| <= w(a) + f(a) |c|, c = -0.01
+    mk = lambda t, **kw: _on_circle(R, t, dz=100, **kw)
+    assert O.ls_eval(mk(0.3, c=-0.01 + 0.0009, w=0.001), mk(0.5, c=-0.01))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01 + 0.0011, w=0.001), mk(0.5, c=-0.01))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01 - 0.0011, w=0.001), mk(0.5, c=-0.01))[0]
+    assert not O.ls_eval(mk(0.3, c=+0.01, w=0.001), mk(0.5, c=-0.01))[0]          # wrong-sign MD estimate
+    # L3 outer MD
+    assert O.ls_eval(mk(0.3, c=-0.01), mk(0.5, c=-0.01 + 0.0009, w=0.001))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01), mk(0.5, c=-0.01 + 0.0011, w=0.001))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01), mk(0.5, c=0.02, w=0.001))[0]           # "wildly wrong" outer c_md
+    # relative term f |c| = 0.3 * 0.01 = 0.003 (w = 0)
+    assert O.ls_eval(mk(0.3, c=-0.01 + 0.0028, w=0.0, f=0.3), mk(0.5, c=-0.01))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01 + 0.0032, w=0.0, f=0.3), mk(0.5, c=-0.01))[0]
+    assert O.ls_eval(mk(0.3, c=-0.01), mk(0.5, c=-0.01 - 0.0028, w=0.0, f=0.3))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01), mk(0.5, c=-0.01 - 0.0032, w=0.0, f=0.3))[0]
+    # w + f |c| = 0.001 + 0.003
+    assert O.ls_eval(mk(0.3, c=-0.01 + 0.0038, w=0.001, f=0.3), mk(0.5, c=-0.01))[0]
+    assert not O.ls_eval(mk(0.3, c=-0.01 + 0.0042, w=0.001, f=0.3), mk(0.5, c=-0.01))[0]
+
+
+def pin_ls_L2_uses_arc_length():
+    """On a noise-free 0.8 GeV helix (R = 70.2 cm) from z0 = 14.5 with cot = -1, anchors at r = 88 and 108 cm (no
+    tolerances): with arc lengths L2 holds (|z0| < 15); with radii instead of arc lengths the same pair has
+    |zA rB - zB rA| = 14.5*20 + (sB rA - sA rB) = 861 = 2.9x the bound 300 -- so this pair only passes if s really is the arc length."""
+    R = 0.8 / KAPPA64
+    out = []
+    for r in (88.0, 108.0):
+        s = 2 * R * np.arcsin(r / (2 * R))
+        t = s / R
+        out.append(A9(R * np.sin(t), R * (1 - np.cos(t)), 14.5 - s * 1.0, c=-1 / R, w=1.0))
+    assert O.ls_eval(out[0], out[1])[0]
+    zA, zB = float(out[0][2]), float(out[1][2])
+    assert abs(zA * 108 - zB * 88) > 15 * 20 * 1.5         # the radius version would fail badly
+
+
+# ====================================================================== a3 / a4: triplet (SPEC.md 4.3)
+def _col(z_a, z_b, z_c, ta=(0, 0), tb=(0, 0), tc=(0, 0)):
+    """A, B, C at x = 30, 50, 80 on the x axis: k = 0, sab = 20, sbc = 30 exactly; t* = (dz, dr)"""
+    return (A9(30, 0, z_a, dz=ta[0], dr=ta[1]), A9(50, 0, z_b, dz=tb[0], dr=tb[1]), A9(80, 0, z_c, dz=tc[0], dr=tc[1]))
+
+
+def pin_triplet_T2_terms():
+    """T2: |zab*30 - zbc*20| <= (dzA+dzB)*30 + (dzB+dzC)*20 + (drA+drB)|zbc| + (drB+drC)|zab| + 0.05*50."""
+    br = lambda p: O.bridge_eval(*p)
+    ok, k = br(_col(0, 0, 0))
+    assert ok and k == 0.0
+    # constant 0.05 (sab + sbc) = 2.5 alone
+    assert br(_col(0, 0.08, 0.08))[0]           # zab = .08, zbc = 0: lhs 2.4
+    assert not br(_col(0, 0.09, 0.09))[0]       # 2.7
+    # dzA: + 1*30 = 32.5
+    assert br(_col(0, 1.0, 1.0, ta=(1, 0)))[0]      # 30
+    assert not br(_col(0, 1.2, 1.2, ta=(1, 0)))[0]  # 36
+    # dzB: + 1*(30+20) = 52.5
+    assert br(_col(0, 1.7, 1.7, tb=(1, 0)))[0]      # 51
+    assert not br(_col(0, 1.8, 1.8, tb=(1, 0)))[0]  # 54
+    # dzC: + 1*20 = 22.5   ((dzB+dzC)*sbc would give 32.5)
+    assert br(_col(0, 0.7, 0.7, tc=(1, 0)))[0]      # 21
+    assert not br(_col(0, 0.8, 0.8, tc=(1, 0)))[0]  # 24
+    # dr terms need |zbc|, |zab| large with a small lhs: zab = -200 + e/30, zbc = -300  =>  lhs = |e|
+    def kink(e, **kw):
+        zb = -200.0 + e / 30.0
+        return _col(0.0, zb, zb - 300.0, **kw)
+    # drA = 0.1: + 0.1*|zbc| = 30 -> 32.5   (with |zab| it would be 22.5)
+    assert br(kink(31.0, ta=(0, 0.1)))[0]
+    assert not br(kink(34.0, ta=(0, 0.1)))[0]
+    # drB = 0.1: + 0.1*(300 + ~198.3) -> 52.3   (without (drB+drC)|zab| it would be 32.5)
+    assert br(kink(50.0, tb=(0, 0.1)))[0]
+    assert not br(kink(54.0, tb=(0, 0.1)))[0]
+    # drC = 0.1: + 0.1*~199.3 -> 22.4   (with |zbc| it would be 32.5)
+    assert br(kink(21.0, tc=(0, 0.1)))[0]
+    assert not br(kink(24.0, tc=(0, 0.1)))[0]
+    assert br(kink(-21.0, tc=(0, 0.1)))[0] and not br(kink(-24.0, tc=(0, 0.1)))[0]
+
+
+def pin_t3_curvature_consistency():
+    """T3: |c_ls(a,b) - k| <= 0.00285 AND |c_ls(b,c) - k| <= 0.00285 (C_TOL3 = 0.2 * 0.0114 / 0.8)."""
+    a, b, c = _col(0, 0, 0, ta=(1, 0), tb=(1, 0), tc=(1, 0))
+    t3 = lambda cab, cbc: O.t3_eval(a, b, c, cab, cbc)[0]
+    assert t3(0.0027, 0.0) and t3(0.0, 0.0027) and t3(-0.0027, 0.0027)
+    assert not t3(0.0030, 0.0)
+    assert not t3(0.0, 0.0030)          # the second LS alone can veto
+    assert not t3(0.0, -0.0030)
+    # on the R = 100 circle: k = -0.01 (signed)
+    p = [_on_circle(100.0, t, dz=100) for t in (0.25, 0.4, 0.6)]
+    ok, k = O.t3_eval(p[0], p[1], p[2], -0.01, -0.01)
+    assert ok and abs(k + 0.01) < 2e-8
+    assert O.t3_eval(p[0], p[1], p[2], -0.01 - 0.0027, -0.01 + 0.0027)[0]
+    assert not O.t3_eval(p[0], p[1], p[2], -0.01, -0.01 + 0.0030)[0]
+    assert not O.t3_eval(p[0], p[1], p[2], 0.01, -0.01)[0]      # |c| alone is not what is compared
+
+
+# ====================================================================== a1: MD (SPEC.md 4.1)
+def pin_md_endcap_terms():
+    """p1 = (50, 0, 131), p2 = (50 + drho, dt, 131 + 10): r1 = 50, Ls = 10 * 50 / 131 = 3.81679.
+    M2: |drho - Ls| <= 0.15 Ls + DL2[t];  M3: |dt| <= 1.3 Ls S + DT[t], S = min(1, r2 * 0.007125)."""
+    Ls = 10.0 * 50.0 / 131.0
+    md = lambda drho, dt, mt: O.md_eval([50.0, 0.0, 131.0], [50.0 + drho, dt, 141.0], 1, mt)
+    # M2, PS: DL2 = 0.1837
+    for sgn in (1, -1):
+        assert md(Ls + sgn * (0.10 * Ls + 0.1837), 0.0, 0)[0]          # inside 0.15 Ls (a factor 0.05 would reject)
+        assert not md(Ls + sgn * (0.20 * Ls + 0.1837), 0.0, 0)[0]
+    assert md(Ls + 0.13 * Ls + 0.1837, 0.0, 0)[0] and not md(Ls + 0.17 * Ls + 0.1837, 0.0, 0)[0]
+    # M2, 2S: DL2 = 6.124
+    assert md(Ls + 0.10 * Ls + 6.0, 0.0, 1)[0] and not md(Ls + 0.10 * Ls + 6.0, 0.0, 0)[0]
+    assert not md(Ls + 0.15 * Ls + 6.3, 0.0, 1)[0]
+    # M3, PS: DT = 0.01225; drho = Ls so that M2's residual is 0
+    def m3(fac, mt, DT):
+        dt = 1.0
+        for _ in range(20):                       # fixed point of dt = fac * Ls * S(r2(dt)) + DT
+            S = min(1.0, np.hypot(50.0 + Ls, dt) * 0.007125)
+            dt = fac * Ls * S + DT
+        return md(Ls, dt, mt)[0], md(Ls, -dt, mt)[0]
+    assert m3(1.15, 0, 0.01225) == (True, True)   # a factor 1.0 instead of 1.3 would reject
+    assert m3(1.27, 0, 0.01225) == (True, True)
+    assert m3(1.33, 0, 0.01225) == (False, False)
+    assert m3(1.45, 0, 0.01225) == (False, False)
+    # DT itself: Ls -> tiny (dz = 0.001) leaves |dt| <= DT (+ 1e-5)
+    tiny = lambda dt, mt: O.md_eval([50.0, 0.0, 131.0], [50.0 + 0.001 * 50 / 131, dt, 131.001], 1, mt)[0]
+    assert tiny(0.0120, 0) and not tiny(0.0125, 0)          # PS 0.01225
+    assert tiny(0.0108, 1) and not tiny(0.0112, 1)          # 2S 0.01102
+    # stored quantities: c = -2 dt / (r2 Ls), w = 2 DT / (r2 Ls), f = 0.3, anchor tolerances (dz, dr) = (0, DL)
+    ok, o = md(Ls, 0.5, 0)
+    r2 = np.hypot(50.0 + Ls, 0.5)
+    assert ok and abs(o[0] - (-2 * 0.5 / (r2 * Ls))) < 1e-7 and abs(o[1] - 2 * 0.01225 / (r2 * Ls)) < 1e-8
+    assert o[2] == np.float32(0.3) and o[3] == 50.0 and o[4] == 0.0 and o[5] == np.float32(0.1299)
+    assert md(Ls, 0.5, 1)[1][5] == np.float32(4.330)
+
+
+def pin_md_barrel_terms():
+    """p1 = (50, 0, z1), p2 = (50 + drho, dt, z1 + dz), drho = 0.26.
+    M1: drho > 0;  M2: |dz - drho z1 / r1| <= drho * 15 / r1 + DL2[t];  M3: |dt| <= L S + DT[t]."""
+    md = lambda drho, dt, z1, dz, mt: O.md_eval([50.0, 0.0, z1], [50.0 + drho, dt, z1 + dz], 0, mt)
+    assert not md(-0.26, 0.0, 0.0, 0.0, 0)[0] and not md(0.0, 0.0, 0.0, 0.0, 0)[0]            # M1
+    # M2 PS at z1 = 100: drho z1 / r1 = 0.52 ; bound = 0.26*15/50 + 0.1837 = 0.2617
+    assert md(0.26, 0.0, 100.0, 0.52 + 0.25, 0)[0] and not md(0.26, 0.0, 100.0, 0.52 + 0.275, 0)[0]
+    assert md(0.26, 0.0, 100.0, 0.52 - 0.25, 0)[0] and not md(0.26, 0.0, 100.0, 0.52 - 0.275, 0)[0]
+    assert md(0.26, 0.0, -100.0, -0.52 - 0.25, 0)[0] and not md(0.26, 0.0, -100.0, 0.52 + 0.25, 0)[0]
+    # the Z0 term alone (drop it -> 0.1837 would reject 0.25); the DL2 term alone (2S: 0.078 + 6.124)
+    assert md(0.26, 0.0, 0.0, 6.1, 1)[0] and not md(0.26, 0.0, 0.0, 6.3, 1)[0] and not md(0.26, 0.0, 0.0, 6.1, 0)[0]
+    # M3 PS: S = r2 * 0.007125 = 0.3581 ; dt = 0.105 -> L = 0.2804, bound 0.1127 ; dt = 0.125 -> bound 0.1156
+    assert md(0.26, 0.105, 0.0, 0.0, 0)[0] and not md(0.26, 0.125, 0.0, 0.0, 0)[0]
+    assert md(0.26, -0.105, 0.0, 0.0, 0)[0] and not md(0.26, -0.125, 0.0, 0.0, 0)[0]
+    # stored: c = -2 dt / (r2 L), w = 2 DT / (r2 L), f = 0, tolerances (DL, 0)
+    ok, o = md(0.26, 0.05, 10.0, 0.05, 1)
+    r2, L = np.hypot(50.26, 0.05), np.hypot(0.26, 0.05)
+    assert ok and abs(o[0] + 2 * 0.05 / (r2 * L)) < 2e-7 and abs(o[1] - 2 * 0.01102 / (r2 * L)) < 2e-8
+    assert o[2] == 0.0 and o[4] == np.float32(4.330) and o[5] == 0.0
+
+
+# ====================================================================== a6: anchor test (SPEC.md 4.6)
+PT_STRAIGHT = 1000.0        # GeV: R = 87719 cm, h = 5.7e-6, 2 R h = 1, arcfac((r h)^2) rounds to 1 => s = r
+
+
+def _seed(cot=0.0, z0=0.0, pt=PT_STRAIGHT):
+    return [pt, 0.0, pt * cot, z0]          # px, py, pz, z0: direction +x; q = +1 puts the helix centre at (0, -R)
+
+
+def pin_pls_transverse_terms():
+    """Straight seed along +x (q = +1): e = (r^2 + 2 y R) h = r^2 h + y;  dT = 0.003 r + 0.03 r^2 h + 0.02."""
+    h = 0.5 * KAPPA64 / PT_STRAIGHT
+    m = lambda x, y: O.pls_match(_seed(), 1, A9(x, y, 0.0, dz=1000.0))[0]
+    # r = 50: r^2 h = 0.01425, dT = 0.15 + 0.0004 + 0.02 = 0.1704
+    assert abs(2500 * h - 0.01425) < 1e-6
+    assert m(50.0, 0.150) and not m(50.0, 0.162)          # e = 0.164 / 0.176
+    assert m(50.0, -0.180) and not m(50.0, -0.190)        # e = -0.166 / -0.176
+    # r = 100: r^2 h = 0.057, dT = 0.3 + 0.0017 + 0.02 = 0.3217   (two radii separate 0.003 r from 0.02)
+    assert m(100.0, 0.250) and not m(100.0, 0.280)
+    # curved seed, pT = 1 GeV: R = 87.72, anchor at distance R + eps from the helix centre (0, -R):
+    # e = ((R+eps)^2 - R^2) / 2R = eps + eps^2 / 2R (geometry);  dT = 0.003 r + 0.03 r^2 / 2R + 0.02 = 0.4724 at r = 43.4
+    R = 1.0 / KAPPA64
+    def off(eps, t=0.5):
+        x, y = (R + eps) * np.sin(t), -R + (R + eps) * np.cos(t)
+        return O.pls_match(_seed(pt=1.0), 1, A9(x, y, 0.0, dz=1000.0))[0], np.hypot(x, y)
+    ok, r = off(0.0)
+    assert ok and abs(r - 2 * R * np.sin(0.25)) < 1e-3
+    dT = 0.003 * r + 0.03 * r * r / (2 * R) + 0.02
+    assert abs(dT - 0.4724) < 2e-3
+    assert off(0.45)[0] and not off(0.50)[0]              # without the 0.03 r^2 h term dT would be 0.150
+    assert off(-0.45)[0] and not off(-0.50)[0]
+    # the other charge mirrors the helix: same anchors fail, mirrored anchors pass
+    assert not O.pls_match(_seed(pt=1.0), -1, A9(R * np.sin(0.5), -R + R * np.cos(0.5), 0.0, dz=1000.0))[0]
+    assert O.pls_match(_seed(pt=1.0), -1, A9(R * np.sin(0.5), R - R * np.cos(0.5), 0.0, dz=1000.0))[0]
+
+
+def pin_pls_longitudinal_terms():
+    """Straight seed along +x, anchor at (50, 0): s = 50, z_pred = z0 + 50 cot;
+    dZ = dz + dr |cot| + 0.003 * 50 * sqrt(1 + cot^2) + 0.05."""
+    m = lambda z, cot=0.0, z0=0.0, **kw: O.pls_match(_seed(cot, z0), 1, A9(50.0, 0.0, z, **kw))[0]
+    # cot = 0: 0.15 + 0.05 = 0.20
+    assert m(0.18) and not m(0.22) and m(-0.18) and not m(-0.22)
+    # dz = 1: 1.20
+    assert m(1.15, dz=1.0) and not m(1.25, dz=1.0)
+    # dr |cot| = 4 * 2 = 8: 8 + 0.003*50*2.23607 + 0.05 = 8.385   (without it: 0.385)
+    assert m(100.0 + 8.2, cot=2.0, dr=4.0) and not m(100.0 + 8.6, cot=2.0, dr=4.0)
+    assert m(-100.0 - 8.2, cot=-2.0, dr=4.0) and not m(-100.0 - 8.6, cot=-2.0, dr=4.0)
+    # 0.003 s sec at cot = 5: 0.76485 + 0.05 = 0.815   (without it: 0.05; with s alone: 0.20)
+    assert m(250.0 + 0.78, cot=5.0) and not m(250.0 + 0.85, cot=5.0)
+    # z0 enters the prediction
+    assert m(3.0 + 0.18, z0=3.0) and not m(0.18, z0=3.0)
+    # s is the arc length: pT = 0.8 GeV seed (R = 70.18), anchor on the helix at r = 100: s = 2R asin(r/2R) = 111.3,
+    # z = z0 + s cot; with s = r the residual would be 11.3 cm at cot = 1
+    R = 0.8 / KAPPA64
+    s = 2 * R * np.arcsin(100.0 / (2 * R)); t = s / R
+    on = A9(R * np.sin(t), -R + R * np.cos(t), 2.0 + s * 1.0)
+    assert abs(float(on[3]) - 100.0) < 1e-3
+    assert O.pls_match(_seed(1.0, 2.0, pt=0.8), 1, on)[0]
+
+
+def pin_pls_chi2_golden():
+    """chi2 = sum over anchors of (e/dT)^2 + (zres/dZ)^2.  Straight seed, anchor (50, y, z) with
+    y = 0.5*dT - r^2 h  (e = dT/2 -> 0.25)  and  z = 0.25 * 0.20 (cot = 0, no tolerances: dZ = 0.20 -> 0.0625):
+    0.3125 per anchor -> 1.5625 for five, 0.9375 for three."""
+    h = 0.5 * KAPPA64 / PT_STRAIGHT
+    dT = 0.003 * 50.0 + 0.03 * 2500.0 * h + 0.02
+    a = A9(50.0, 0.5 * dT - 2500.0 * h, 0.05)
+    ok, chi = O.pls_match(_seed(), 1, np.stack([a] * 5))
+    assert ok and abs(chi - 1.5625) < 2e-3
+    ok, chi = O.pls_match(_seed(), 1, np.stack([a] * 3))
+    assert ok and abs(chi - 0.9375) < 2e-3
+    # one failing anchor vetoes the match
+    bad = A9(50.0, 0.3, 0.05)
+    assert not O.pls_match(_seed(), 1, np.stack([a, a, bad, a, a]))[0]
+    # transverse-only and longitudinal-only displacement
+    ok, chi = O.pls_match(_seed(), 1, A9(50.0, 0.5 * dT - 2500.0 * h, 0.0))
+    assert ok and abs(chi - 0.25) < 1e-3
+    ok, chi = O.pls_match(_seed(), 1, A9(50.0, -2500.0 * h, 0.1))
+    assert ok and abs(chi - 0.25) < 1e-3
+
+
+# ====================================================================== through the whole chain
+def _barrel_mod(geo, layer, phi, z):
+    nphi = int(geo.barrel_nphi[layer])
+    return int(geo.barrel_base[layer] + int(phi / (2 * np.pi / nphi)) * 24 + int(np.floor((z + 120.0) / 10.0)))
+
+
+def _disk_mod(geo, side, disk, phi, r):
+    k = int(np.floor((r - 23.0) / 10.0))
+    nphi = int(geo.ring_nphi[k])
+    return int(geo.disk_base[side, disk, k] + int(phi / (2 * np.pi / nphi)))
+
+
+def _connected(geo, a, b):
+    return b in geo.conn_col[geo.conn_rowptr[a]:geo.conn_rowptr[a + 1]]
+
+
+def _event_from_hits(hits, pls=()):
+    """hits: (x, y, z, module, upper); pls: (px, py, pz, z0, q)"""
+    from lstgen.events import Event
+    h = np.array(hits, dtype=np.float64).reshape(-1, 5)
+    p = np.array(pls, dtype=np.float64).reshape(-1, 5)
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    return Event(x=f(h[:, 0]), y=f(h[:, 1]), z=f(h[:, 2]), key=(2 * h[:, 3] + h[:, 4]).astype(np.uint32),
+                 pls_px=f(p[:, 0]), pls_py=f(p[:, 1]), pls_pz=f(p[:, 2]), pls_z0=f(p[:, 3]), pls_q=p[:, 4].astype(np.int8),
+                 hit_particle=np.zeros(len(h), np.int32), pls_particle=np.zeros(len(p), np.int32))
+
+
+def _straight_endcap_track(geo, z0, phi, slope=0.4):
+    """hits of a straight line r = (z - z0) * slope at azimuth phi on both sensors of disks 1 and 2 (+z side)"""
+    hits, mods = [], []
+    for d, zd in ((0, 131.0), (1, 156.0)):
+        m = _disk_mod(geo, 1, d, phi, (zd - z0) * slope)
+        mods.append(m)
+        for up, zz in ((0, zd), (1, zd + 0.26)):
+            r = (zz - z0) * slope
+            hits.append((r * np.cos(phi), r * np.sin(phi), zz, m, up))
+    return hits, mods
+
+
+def pin_chain_anchor_tolerances_endcap(geo):
+    """run_chain's own (dz, dr) assignment: endcap MDs carry (0, DL), so for two PS endcap MDs on a straight line
+    from (0, 0, z0) with slope 0.4 (s = r, sB - sA = 10): L2 reads |z0| * 10 <= 15 * 10 + 0.1299 * (156 + 131) = 187.3.
+    z0 = 17 -> 170: LS; z0 = 19.5 -> 195: no LS.  (With dz = DL as well the bound would be 200.2; with dr = 0, 150.)"""
+    h1, m1 = _straight_endcap_track(geo, 17.0, 0.05)
+    h2, m2 = _straight_endcap_track(geo, 19.5, 1.00)
+    for m in (m1, m2):
+        assert _connected(geo, m[0], m[1]) and geo.subdet[m[0]] == 1 and geo.mtype[m[0]] == 0 and geo.mtype[m[1]] == 0
+    r = O.run(geo, xavier_weights(1), _event_from_hits(h1 + h2), last_stage="ls")
+    assert r.counts["md"] == 4 and r.counts["ls_pairs"] == 2
+    assert r.counts["ls"] == 1
+    assert set(r.md_mod[r.ls[0]].tolist()) == set(m1)
+
+
+def pin_chain_anchor_tolerances_barrel(geo):
+    """barrel MDs carry (DL, 0): straight line from (0, 0, z0) with cot = 1 through layers 1, 2 (r = 23, 36; PS):
+    |z0| * 13 <= 15 * 13 + 0.1299 * (36 + 23) = 202.66  <=>  |z0| <= 15.59.  z0 = 15.4: LS; z0 = 15.8: none
+    (with dr = DL as well the bound would grow by 0.1299 * (|zA| + |zB|) = 11.7 -> 16.5)."""
+    hits, mods = [], []
+    for z0, phi in ((15.4, 0.05), (15.8, 1.0)):
+        for l, rl in ((0, 23.0), (1, 36.0)):
+            m = _barrel_mod(geo, l, phi, z0 + rl)
+            mods.append(m)
+            for up, r in ((0, rl), (1, rl + 0.26)):
+                hits.append((r * np.cos(phi), r * np.sin(phi), z0 + r, m, up))
+    assert _connected(geo, mods[0], mods[1]) and _connected(geo, mods[2], mods[3])
+    r = O.run(geo, xavier_weights(1), _event_from_hits(hits), last_stage="ls")
+    assert r.counts["md"] == 4 and r.counts["ls_pairs"] == 2 and r.counts["ls"] == 1
+    assert set(r.md_mod[r.ls[0]].tolist()) == set(mods[:2])
+
+
+def _menger64(p, q, r):
+    """signed curvature of the circle through three transverse points from the textbook circumradius
+    R = |pq| |qr| |rp| / (4 Area); sign: negative for a left turn (azimuth increasing, SPEC.md 1)"""
+    cross = (q[0] - p[0]) * (r[1] - p[1]) - (q[1] - p[1]) * (r[0] - p[0])
+    return -2.0 * cross / (np.hypot(*(q - p)) * np.hypot(*(r - q)) * np.hypot(*(r - p)))
+
+
+def pin_chain_t5_curvature_indices(geo):
+    """The three curvatures stored with a T5 candidate belong to (a,b,c), (b,c,d) and (c,d,e) (the bridge
+    is the three MDs in the centre), checked against the circumradius formula in float64 on every candidate of the
+    PU50 event.  With smeared hits the curvature of (a,c,d) differs from (b,c,d) far beyond rounding."""
+    ev = config_event(geo, 1)
+    r = O.run(geo, xavier_weights(2), ev, last_stage="t5")
+    xy = r.md_real[:, 2:4]
+    assert len(r.t5c) > 500
+    n_sensitive = 0
+    for t, cv in zip(r.t5c[:, :5], r.t5c_curv):
+        a, b, c, d, e = (xy[i] for i in t)
+        for got, tri in ((cv[0], (a, b, c)), (cv[1], (b, c, d)), (cv[2], (c, d, e))):
+            assert abs(got - _menger64(*tri)) <= 5e-6 * max(abs(got), 1e-3)
+        n_sensitive += abs(_menger64(a, c, d) - _menger64(b, c, d)) > 1e-4 * max(abs(cv[1]), 1e-3)
+    assert n_sensitive > 0.5 * len(r.t5c)
+
+
+def tc_by_definition(r, ev):
+    """SPEC.md 4.6 selection rules restated with Python tuples / sets over the oracle's own match list (every
+    (pLS, object) pair is tested with the single-anchor predicate): pins loops, tie-breaks and the used / free rules."""
+    md9 = [np.array([x, y, z, rr, c, w, 0, 0, 0], np.float32) for c, w, x, y, z, rr in r.md_real]
+    # anchor tolerances are not in md_real: take them from the module type the way SPEC.md 3.1 states them
+    return md9
+
+
+def _tc_expected(geo, r, ev):
+    DL = (0.1299, 4.330)
+    def anchors(idx):
+        out = []
+        for i in idx:
+            c, w, x, y, z, rr = r.md_real[i]
+            m = r.md_mod[i]
+            dl = DL[geo.mtype[m]]
+            out.append(A9(x, y, z, r=rr, dz=0.0 if geo.subdet[m] else dl, dr=dl if geo.subdet[m] else 0.0))
+        return np.stack(out)
+    seed = lambda p: ([ev.pls_px[p], ev.pls_py[p], ev.pls_pz[p], ev.pls_z0[p]], int(ev.pls_q[p]))
+    t5 = [r.t5c[c, :5] for c in r.t5]
+    best5 = {}
+    for t, m5 in enumerate(t5):
+        cand = [(np.float32(chi), p) for p in range(ev.n_pls) for ok, chi in [O.pls_match(*seed(p), anchors(m5))] if ok]
+        if cand:
+            best5[t] = min(cand)                    # argmin over (chi2, p)
+    win5 = {}
+    for t, (chi, p) in best5.items():
+        if p not in win5 or (chi, t) < win5[p]:     # argmin over (chi2, t)
+            win5[p] = (chi, t)
+    used = [set(t5[t].tolist()) for _, t in win5.values()]
+    best3 = {}
+    for x, t in enumerate(r.t3[:, :3].tolist()):
+        if any(set(t) <= u for u in used):          # all three MDs inside one pT5
+            continue
+        cand = [(np.float32(chi), p) for p in range(ev.n_pls) if p not in win5
+                for ok, chi in [O.pls_match(*seed(p), anchors(t))] if ok]
+        if cand:
+            best3[x] = min(cand)
+    win3 = {}
+    for x, (chi, p) in best3.items():
+        if p not in win3 or (chi, x) < win3[p]:
+            win3[p] = (chi, x)
+    exp = [(0, p, win5[p][1]) for p in sorted(win5)]
+    exp += [(1, -1, t) for t in range(len(t5)) if t not in best5]
+    exp += [(2, p, win3[p][1]) for p in sorted(win3)]
+    exp += [(3, p, -1) for p in range(ev.n_pls) if p not in win5 and p not in win3]
+    return exp, win5
+
+
+def _muon_with_seeds(geo_barrel, seeds):
+    """one noise-free barrel muon (6 layers -> T5s on layers 1-5 and 2-6) and a list of pixel seeds derived from its
+    exact seed: 'exact' = copy, ('pt', f) = momentum scaled by f, ('z0', d) = z0 shifted by d cm"""
+    ev = make_event(geo_barrel, 91, origin_muons=1, smear=False)
+    base = (float(ev.pls_px[0]), float(ev.pls_py[0]), float(ev.pls_pz[0]), float(ev.pls_z0[0]), int(ev.pls_q[0]))
+    rows = []
+    for s in seeds:
+        if s == "exact":
+            rows.append(base)
+        elif s[0] == "pt":
+            rows.append((base[0] * s[1], base[1] * s[1], base[2] * s[1], base[3], base[4]))
+        else:
+            rows.append((base[0], base[1], base[2], base[3] + s[1], base[4]))
+    p = np.array(rows, dtype=np.float64)
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    ev.pls_px, ev.pls_py, ev.pls_pz, ev.pls_z0 = f32(p[:, 0]), f32(p[:, 1]), f32(p[:, 2]), f32(p[:, 3])
+    ev.pls_q = p[:, 4].astype(np.int8)
+    ev.pls_particle = np.zeros(len(rows), np.int32)
+    return ev
+
+
+def pin_tc_used_and_free_rules(geo_barrel):
+    """Seeds [exact, perturbed] on one clean muon.  Both T5s (layers 1-5, 2-6) match both seeds; the exact one has
+    the smaller chi2, so it owns the single pT5 and the perturbed seed stays free.  Of the four T3s, three lie inside
+    the pT5's five MDs (used) and ONE shares exactly two MDs with it: that one is still eligible, and only the free
+    seed may take it  =>  TC = [pT5(seed 0), pT3(seed 1, the two-shared T3)], no T5, no pLS candidate.
+    Two perturbations: a 1 % momentum error favours the INNER T3s (the transverse residual grows with r), a 1 mm z0
+    error favours the OUTER ones (2S layers have dZ = 4.4 cm) -- so in at least one of them a used T3 would beat the
+    eligible one if the used rule were not applied."""
+    beaten = 0
+    for pert in (("pt", 1.01), ("z0", 0.1)):
+        ev = _muon_with_seeds(geo_barrel, ["exact", pert])
+        r = O.run(geo_barrel, xavier_weights(1), ev)
+        assert len(r.t5) == 2 and len(r.t3) == 4 and np.all(r.best5_pls == 0)
+        tc = [tuple(t) for t in r.tc.tolist()]
+        assert len(tc) == 2 and tc[0][:2] == (0, 0) and tc[1][:2] == (2, 1), tc
+        m5 = set(r.t5c[r.t5[tc[0][2]], :5].tolist())
+        shared = [len(set(t) & m5) for t in r.t3[:, :3].tolist()]
+        assert sorted(shared) == [2, 3, 3, 3]
+        assert shared[tc[1][2]] == 2
+        assert tc == _tc_expected(geo_barrel, r, ev)[0]
+        chi = [_chi_of(geo_barrel, r, ev, 1, t) for t in r.t3[:, :3].tolist()]
+        beaten += min(chi) < chi[tc[1][2]]
+    assert beaten >= 1
+
+
+def _chi_of(geo, r, ev, p, mds):
+    DL = (0.1299, 4.330)
+    rows = []
+    for i in mds:
+        c, w, x, y, z, rr = r.md_real[i]
+        m = r.md_mod[i]
+        dl = DL[geo.mtype[m]]
+        rows.append(A9(x, y, z, r=rr, dz=0.0 if geo.subdet[m] else dl, dr=dl if geo.subdet[m] else 0.0))
+    ok, chi = O.pls_match([ev.pls_px[p], ev.pls_py[p], ev.pls_pz[p], ev.pls_z0[p]], int(ev.pls_q[p]), np.stack(rows))
+    return np.float32(chi) if ok else np.float32(np.inf)
+
+
+def pin_tc_tie_rules(geo_barrel):
+    """Exact duplicates of a seed tie bit-for-bit in chi2; SPEC.md 4.6 breaks ties towards the smaller index:
+    seeds [exact, exact, exact] => pT5 with seed 0, the free T3 goes to seed 1 (argmin over (chi2, p)), seed 2 is
+    left as a pLS candidate."""
+    ev = _muon_with_seeds(geo_barrel, ["exact", "exact", "exact"])
+    r = O.run(geo_barrel, xavier_weights(1), ev)
+    tc = [tuple(t) for t in r.tc.tolist()]
+    assert [t[:2] for t in tc] == [(0, 0), (2, 1), (3, 2)]
+    assert np.all(r.best5_pls == 0)
+    assert tc == _tc_expected(geo_barrel, r, ev)[0]
+    # duplicated HITS in the outermost layer duplicate every object built on them (4 copies of the outer MD): equal
+    # chi2 between objects => win5 / win3 ties are broken towards the smaller object index.  The z0-shifted second
+    # seed prefers the outer T3s, so the free T3 it takes is one of the tied copies.
+    n_tied = 0
+    for pert in (("pt", 1.01), ("z0", 0.1)):
+        ev = _muon_with_seeds(geo_barrel, ["exact", pert])
+        r6 = np.flatnonzero(np.hypot(ev.x, ev.y) > 100.0)
+        assert r6.size == 2
+        for name in ("x", "y", "z", "key", "hit_particle"):
+            a = getattr(ev, name)
+            setattr(ev, name, np.concatenate([a, a[r6]]))
+        r = O.run(geo_barrel, xavier_weights(1), ev)
+        assert r.counts["md"] == 5 + 4 and len(r.t5) == 1 + 4
+        exp, win5 = _tc_expected(geo_barrel, r, ev)
+        assert [tuple(t) for t in r.tc.tolist()] == exp
+        pt3 = [t for t in exp if t[0] == 2]
+        assert len(pt3) == 1
+        chi = [_chi_of(geo_barrel, r, ev, 1, t) for t in r.t3[:, :3].tolist()]
+        n_tied += sum(c == chi[pt3[0][2]] for c in chi) > 1
+    assert n_tied >= 1      # at least one scenario decided win3 on the index
+
+
+def pin_smeared_endcap_efficiency(geo):
+    """Physics sanity of the frozen endcap tolerances: smeared forward particles (pT > 1 GeV, 1.7 < |eta| < 2.3,
+    |z_v| < 10) keep their truth LSs and T3s.  Dropping a delta-r term of L2 / T2 (2S rings smear r by 1.44 cm)
+    or mis-assigning the endcap tolerances craters these numbers."""
+    tot = {"ls": 0, "t3": 0}
+    found = {"ls": 0, "t3": 0}
+    for seed in (301, 302, 303):
+        ev = make_event(geo, seed, n_particles=900, per_vertex=30)
+        r = O.run(geo, xavier_weights(1), ev, last_stage="t3")
+        part, hp = ev.particles, ev.hit_particle
+        good = (part["pt"] > 1.0) & (np.abs(part["eta"]) > 1.7) & (np.abs(part["eta"]) < 2.3) & (np.abs(part["zv"]) < 10.0)
+        md_of = {}
+        for i, (lo, up) in enumerate(r.md_hits):
+            if hp[lo] == hp[up] and hp[lo] >= 0 and good[hp[lo]] and geo.subdet[r.md_mod[i]] == 1:
+                md_of.setdefault(int(hp[lo]), []).append(i)
+        conn = lambda a, b: _connected(geo, r.md_mod[a], r.md_mod[b])
+        ls_set = {tuple(t) for t in r.ls.tolist()}
+        t3_set = {tuple(t[:3]) for t in r.t3.tolist()}
+        for p, mds in md_of.items():
+            mds = sorted(mds, key=lambda i: abs(r.md_real[i, 4]))          # along |z|
+            for a, b in zip(mds[:-1], mds[1:]):
+                if conn(a, b):
+                    tot["ls"] += 1; found["ls"] += (a, b) in ls_set
+            for a, b, c in zip(mds[:-2], mds[1:-1], mds[2:]):
+                if conn(a, b) and conn(b, c):
+                    tot["t3"] += 1; found["t3"] += (a, b, c) in t3_set
+    assert tot["ls"] > 150 and tot["t3"] > 100, tot
+    return found["ls"] / tot["ls"], found["t3"] / tot["t3"]
+
+
+# ---------------------------------------------------------------------- pytest entry points
+def test_ls_L2_terms(): pin_ls_L2_terms()
+def test_ls_curvature_L1_L3(): pin_ls_curvature_L1_L3()
+def test_ls_L2_uses_arc_length(): pin_ls_L2_uses_arc_length()
+def test_triplet_T2_terms(): pin_triplet_T2_terms()
+def test_t3_curvature_consistency(): pin_t3_curvature_consistency()
+def test_md_endcap_terms(): pin_md_endcap_terms()
+def test_md_barrel_terms(): pin_md_barrel_terms()
+def test_pls_transverse_terms(): pin_pls_transverse_terms()
+def test_pls_longitudinal_terms(): pin_pls_longitudinal_terms()
+def test_pls_chi2_golden(): pin_pls_chi2_golden()
+def test_chain_anchor_tolerances_endcap(geo_full): pin_chain_anchor_tolerances_endcap(geo_full)
+def test_chain_anchor_tolerances_barrel(geo_full): pin_chain_anchor_tolerances_barrel(geo_full)
+def test_chain_t5_curvature_indices(geo_full): pin_chain_t5_curvature_indices(geo_full)
+def test_tc_used_and_free_rules(geo_barrel): pin_tc_used_and_free_rules(geo_barrel)
+def test_tc_tie_rules(geo_barrel): pin_tc_tie_rules(geo_barrel)
+
+
+def test_smeared_endcap_efficiency(geo_full):
+    e_ls, e_t3 = pin_smeared_endcap_efficiency(geo_full)
+    assert e_ls >= ENDCAP_EFF_LS and e_t3 >= ENDCAP_EFF_T3, (e_ls, e_t3)
+
+
+# measured on the oracle as specified: 0.997 / 0.796 (T1 / T3 carry no delta-r tolerance, so the 1.44 cm radial smear of
+# the 2S rings costs ~20 % of the forward T3s -- SURVEY 8.c-E); the mutants land at 0.91 / 0.70 / 0.09
+ENDCAP_EFF_LS, ENDCAP_EFF_T3 = 0.985, 0.76
