@@ -52,8 +52,8 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        LST_CNT_PT5, LST_CNT_T5TC, LST_CNT_PT3, LST_CNT_PLSTC,
        /* bookkeeping of the bucketed pLS matching: first-anchor tests executed / pairs fully tested */
        LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND,
-       /* internal: fill of the MD / LS record buffers; link tickets of the overflow re-run */
-       LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TICKET_MD, LST_CNT_TICKET_LS, LST_CNT_DYN_MD, LST_CNT_DYN_LS,
+       /* internal: fill of the MD / LS record buffers; tile tickets of the row scans and of the T3 / T5 tiles */
+       LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TK_SENSOR, LST_CNT_TK_MD, LST_CNT_TK_LS, LST_CNT_TK_T5,
        LST_CNT_DYN_T3, LST_CNT_DYN_T5, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */

@@ -71,7 +71,7 @@ Caps make_caps(const lst_caps* c) {
 // One pass lays out the whole workspace; used both to measure and to carve.
 struct Layout {
   char* batch_in; size_t batch_in_stride; int* batch_out; size_t batch_out_stride;
-  Slot* slots; uint8_t* modt; int* rowptr; int* col; float* weights;
+  Slot* slots; uint8_t* modt; int* rowptr; int* col; float* weights; int* run_ptr; int* run_c0; int* run_c1;
   char* zero_base; size_t zero_stride; char* ones_base; size_t ones_stride;
   size_t total;
 };
@@ -84,6 +84,9 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   L.rowptr = cv.take<int>(M + 1);
   L.col = cv.take<int>(nnz > 0 ? nnz : 1);
   L.weights = cv.take<float>(N_W);
+  L.run_ptr = cv.take<int>(M + 1);
+  L.run_c0 = cv.take<int>(nnz > 0 ? nnz : 1);      // a row has at most as many runs as entries
+  L.run_c1 = cv.take<int>(nnz > 0 ? nnz : 1);
   L.batch_in_stride = blob_event_bytes(k.max_hits, k.max_pls) + 16;
   L.batch_in = cv.take<char>(L.batch_in_stride * n_slots + 1024);
   L.batch_out_stride = LST_N_CNT + 3 * (size_t)k.max_tc;
@@ -122,14 +125,13 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   for (int s = 0; s < n_slots; ++s) {
     Slot t{};
     t.epoch_dev = cv.take<unsigned>(4); t.tmp_ok = cv.take<int2>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
-    t.md_pair_off = cv.take<int>(M + 8); t.md_link_mod = cv.take<int>(MAX_CELLS / MD_LP + 16); t.chain_md = cv.take<unsigned long long>(MAX_CELLS / MD_LP + 2);
-    t.md_link_cnt = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_link_soff = cv.take<int>(MAX_CELLS / MD_LP + 16); t.md_rec = cv.take<MdRec>(k.max_md);
+    t.md_rec = cv.take<MdRec>(k.max_md);
     t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
-    t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_aux = cv.take<float4>(k.max_md); t.md_start = cv.take<int>(M + 1);
-    t.ls_L = cv.take<int>(M); t.ls_off = cv.take<int>(M + 8); t.ls_coff = cv.take<int>(M + 8); t.ls_cand = cv.take<int>((size_t)CAND_PER_MD * k.max_md);
-    t.ls_link_mod = cv.take<int>(MAX_CELLS / LS_LP + 16); t.chain_ls = cv.take<unsigned long long>(MAX_CELLS / LS_LP + 2);
-    t.ls_link_cnt = cv.take<int>(MAX_CELLS / LS_LP + 16); t.ls_link_soff = cv.take<int>(MAX_CELLS / LS_LP + 16); t.ls_rec = cv.take<LsRec>(k.max_ls);
+    t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_aux = cv.take<float4>(k.max_md); t.md_start = cv.take<int>(M + 8);
+    t.ls_rec = cv.take<LsRec>(k.max_ls);
     t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
+    t.chain_sensor = cv.take<unsigned long long>(2 * (size_t)M / SCAN_TILE + 4); t.chain_md = cv.take<unsigned long long>(M / SCAN_TILE + 4);
+    t.chain_ls = cv.take<unsigned long long>(k.max_md / SCAN_TILE + 4); t.chain_t5s = cv.take<unsigned long long>(k.max_t5c / SCAN_TILE + 4);
     t.chain_t3 = cv.take<unsigned long long>(k.max_ls / TUPLE_TPB + 4); t.chain_t5 = cv.take<unsigned long long>(k.max_t3 / TUPLE_TPB + 4);
     t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
     t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
@@ -158,7 +160,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 28;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 25;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -199,18 +201,36 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   if (e == cudaSuccess) e = cudaMemcpy(L.rowptr, geo->conn_rowptr, sizeof(int) * (M + 1), cudaMemcpyHostToDevice);
   if (e == cudaSuccess && nnz > 0) e = cudaMemcpy(L.col, geo->conn_col, sizeof(int) * nnz, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(L.weights, geo->dnn_weights, sizeof(float) * N_W, cudaMemcpyHostToDevice);
+  {   // CSR rows -> runs of consecutive module ids (one run = one contiguous MD range, lst_pairs.cuh)
+    std::vector<int> run_ptr(M + 1, 0), c0, c1;
+    for (int m = 0; m < M; ++m) {
+      for (int i = geo->conn_rowptr[m]; i < geo->conn_rowptr[m + 1]; ++i) {
+        const int col = geo->conn_col[i];
+        if (i > geo->conn_rowptr[m] && c1.back() == col) c1.back() = col + 1;
+        else { c0.push_back(col); c1.push_back(col + 1); }
+      }
+      run_ptr[m + 1] = (int)c0.size();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(L.run_ptr, run_ptr.data(), sizeof(int) * (M + 1), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !c0.empty()) e = cudaMemcpy(L.run_c0, c0.data(), sizeof(int) * c0.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !c0.empty()) e = cudaMemcpy(L.run_c1, c1.data(), sizeof(int) * c1.size(), cudaMemcpyHostToDevice);
+  }
   if (e == cudaSuccess) e = cudaMemcpy(L.slots, c->h_slots.data(), sizeof(Slot) * c->n_slots, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(c->zero_base, 0, c->zero_stride * c->n_slots);
   for (int i = 0; i < c->n_slots && e == cudaSuccess; ++i) {   // status words start at epoch 0 (never a run's epoch)
     e = cudaMemset(c->h_slots[i].epoch_dev, 0, 16);
-    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (MAX_CELLS / MD_LP + 2));
-    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (MAX_CELLS / LS_LP + 2));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_sensor, 0, sizeof(unsigned long long) * (2 * (size_t)M / SCAN_TILE + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (M / SCAN_TILE + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (c->caps.max_md / SCAN_TILE + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5s, 0, sizeof(unsigned long long) * (c->caps.max_t5c / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t3, 0, sizeof(unsigned long long) * (c->caps.max_ls / TUPLE_TPB + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
   }
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();       // the memsets above are asynchronous on device memory
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
   if (const char* g = std::getenv("LST_GRAPHS")) c->use_graphs = !(g[0] == '0');
   c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
+  c->geo.run_ptr = L.run_ptr; c->geo.run_c0 = L.run_c0; c->geo.run_c1 = L.run_c1;
   *out = c;
   return LST_OK;
 }
@@ -271,26 +291,24 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   if (gx < 8) gx = 8;
   if (gx > 592) gx = 592;
   const dim3 G(gx, n), G1(1, n), GL(2 * gx, n);   // GL: the 128-thread link kernels
+  const dim3 GS(gx < 16 ? gx : 16, n);            // look-back scans: tiles of 2048 entries by ticket
   k_hist<<<G, 256, 0, st>>>(sl, g); LST_MARK();
-  k_scan<SCAN_SENSOR><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan_lb<SCAN_SENSOR><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
   k_scatter<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_rank<<<G, 256, 0, st>>>(sl); LST_MARK();
-  k_md_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
-  k_scan<SCAN_MDLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_md_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_md_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run (returns at once otherwise)
-  k_ls_plan1<<<G, 256, 0, st>>>(sl, g); LST_MARK();
-  k_ls_plan2<<<G1, SCAN_THREADS, 0, st>>>(sl, g); LST_MARK();
-  k_ls_plan3<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_links<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
-  k_scan<SCAN_LSLINK><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_final<<<G, 256, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_links<true><<<G, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run
+  k_md_sweep<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan_lb<SCAN_MDROW><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
+  k_md_scatter<<<G, 256, 0, st>>>(sl, k); LST_MARK();
+  k_md_sweep<true><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run (returns at once otherwise)
+  k_ls_sweep<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan_lb<SCAN_LSROW><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_scatter<<<G, 256, 0, st>>>(sl, k); LST_MARK();
+  k_ls_sweep<true><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run
   k_t3_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
   k_t3_start<<<G, 256, 0, st>>>(sl); LST_MARK();
   k_t5_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
-  k_scan<SCAN_T5><<<G1, SCAN_THREADS, 0, st>>>(sl, g, k); LST_MARK();
+  k_scan_lb<SCAN_T5><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
   k_pls_bin<false><<<G1, 1024, 0, st>>>(sl); LST_MARK();
   k_match<5, false><<<GL, 128, 0, st>>>(sl); LST_MARK();
   k_win<false><<<G, 256, 0, st>>>(sl); LST_MARK();
@@ -352,7 +370,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
-      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_links", "a1.scan", "a1.md_final", "a1.md_rerun", "a2.ls_plan1", "a2.ls_plan2", "a2.ls_plan3", "a2.ls_links", "a2.scan", "a2.ls_final", "a2.ls_rerun", "a3.t3", "a3.t3_start", "a4.t5", "a5.dnn",
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_sweep", "a1.scan", "a1.md_scatter", "a1.md_rerun", "a2.ls_sweep", "a2.scan", "a2.ls_scatter", "a2.ls_rerun", "a3.t3", "a3.t3_start", "a4.t5", "a5.dnn",
       "a5.scan", "a6.pls_bin", "a6.match5", "a6.win5", "a6.pt5_lists", "a6.pls_rebin", "a6.match3", "a6.win3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }

@@ -3,9 +3,9 @@
 // Launch geometry: every kernel takes the device array of slot descriptors and runs on a grid
 // (GX, n_events); blockIdx.y selects the slot, the x dimension grid-strides over that slot's items
 // (counts live in device memory -- lst_run never synchronises with the host).
-// Deterministic output order: MD and LS are single-pass ordered compactions (lst_pairs.cuh); T3 / T5 are
-// count -> exclusive scan -> fill with one thread owning one inner object (first LS / inner T3).  Either
-// way the object order is the SPEC.md build order and capacity overflow is detected and flagged.
+// Deterministic output order: MD and LS are row sweeps that emit (row, rank-in-row) records, placed by a look-back
+// scan of the row counts (lst_pairs.cuh); T3 / T5 are single-pass tiles with the same look-back (lst_tuples.cuh).
+// Either way the object order is the SPEC.md build order and capacity overflow is detected and flagged.
 #pragma once
 #include "lst_math.cuh"
 #include "../../include/lst.h"
@@ -22,17 +22,18 @@ struct Geo {   // device copies, shared by all slots
   const int* rowptr;        // [M+1]
   const int* col;           // [nnz]
   const float* weights;     // [1857]
+  // CSR rows compressed into runs of consecutive module ids (built by lst_create): row m = runs [run_ptr[m], run_ptr[m+1]),
+  // run e = modules [run_c0[e], run_c1[e]).  MDs are stored in module order, so a run is one contiguous MD range.
+  const int* run_ptr;       // [M+1]
+  const int* run_c0;        // [n_runs]
+  const int* run_c1;        // [n_runs]
 };
 
 struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
 
-// staged objects of the MD / LS links (lst_pairs.cuh): f = flat cell index relative to the link's first cell
-struct __align__(16) MdRec { int p_lo, p_up, mtm, f; float c, w; int link, pad; };
-struct __align__(16) LsRec { int a, b, lf; float c; };     // lf = link << LS_LP_BITS | f
-constexpr int MD_LP = 256;           // cells (hit pairs) per MD link = staging capacity, so staging cannot overflow
-constexpr int LS_LP_BITS = 8, LS_LP = 1 << LS_LP_BITS;   // cells (MD pairs) per LS link
-constexpr int CAND_PER_MD = 8;       // capacity of the per-slot candidate table = CAND_PER_MD * max_md entries
-constexpr int MAX_CELLS = 1 << 22;   // flat cell space per stage and slot (PU200: 0.35 M MD, 1.0 M LS cells)
+// records of the MD / LS sweeps (lst_pairs.cuh): seq = rank of the object among the objects of its row
+struct __align__(16) MdRec { int p_lo, p_up, mtm, seq; float c, w; int pad0, pad1; };    // mtm = module << 2 | type
+struct __align__(16) LsRec { int a, b, seq; float c; };
 
 struct Slot {
   // bound inputs
@@ -50,9 +51,11 @@ struct Slot {
   // a0
   int2* tmp_ok; float4* hit; int* hit_orig;
   // a1
-  int* md_pair_off; int* md_link_mod; int* md_link_cnt; int* md_link_soff; MdRec* md_rec; unsigned long long* chain_md; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; float4* md_aux; int* md_start;
+  MdRec* md_rec; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; float4* md_aux; int* md_start;
   // a2
-  int* ls_L; int* ls_off; int* ls_coff; int* ls_cand; int* ls_link_mod; int* ls_link_cnt; int* ls_link_soff; LsRec* ls_rec; unsigned long long* chain_ls; int* ls_start; int2* ls_ab; float* ls_c;
+  LsRec* ls_rec; int* ls_start; int2* ls_ab; float* ls_c;
+  // look-back status words of the row scans (sensor counts, MDs per module, LSs per MD, T5 pass flags)
+  unsigned long long *chain_sensor, *chain_md, *chain_ls, *chain_t5s;
   // a3
   unsigned long long* chain_t3; unsigned long long* chain_t5;   // look-back status words of the a3 / a4 tiles
   int* t3_off; int4* t3_abc; int* t3_l1; float* t3_k; int* t3_start;
@@ -72,16 +75,84 @@ struct Slot {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x, _st = gridDim.x * blockDim.x; i < (n); i += _st)
 
 // ------------------------------------------------------------------------------------------------
-// block-wide exclusive scan in place (one 1024-thread block): a[0..n) -> exclusive prefix clamped to
-// `cap`, a[n] = min(total, cap); returns the unclamped total to every thread.
+// decoupled look-back over 64-bit status words: flag (2 bits) | run epoch (30 bits) | value (32 bits).
+// A word counts only if its epoch is the current run's (k_hist, the first kernel of a run, increments the slot's
+// device-side run counter), so the status arrays never need clearing and the launch sequence has no per-run
+// arguments (it can be replayed as a CUDA graph).  Tiles are handed out by an atomic ticket, so a tile only ever
+// waits for tiles that are already running.
 // ------------------------------------------------------------------------------------------------
-constexpr int SCAN_THREADS = 1024, SCAN_ITEMS = 8;
+constexpr unsigned long long CH_AGG = 1ull << 62, CH_INC = 2ull << 62, CH_VAL = 0xFFFFFFFFull;
+__device__ __forceinline__ unsigned chain_flag(unsigned long long w, unsigned epoch) {
+  return (((unsigned)(w >> 32)) & 0x3FFFFFFFu) == epoch ? (unsigned)(w >> 62) : 0u;
+}
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// exclusive prefix of `count` over tiles [0, tile); called by all 32 lanes of one warp, publishes the inclusive prefix
+__device__ __forceinline__ int chain_exclusive(unsigned long long* st, int tile, int count, int lane, unsigned epoch) {
+  const unsigned long long ep = (unsigned long long)epoch << 32;
+  if (tile == 0) {
+    if (lane == 0) st_status(st, CH_INC | ep | (unsigned long long)(unsigned)count);
+    return 0;
+  }
+  if (lane == 0) st_status(st + tile, CH_AGG | ep | (unsigned long long)(unsigned)count);
+  int excl = 0;
+  int idx = tile - 1 - lane;
+  while (true) {
+    unsigned long long w;
+    unsigned fl;
+    do {
+      w = (idx >= 0) ? ld_status(st + idx) : (CH_INC | ep);
+      fl = chain_flag(w, epoch);
+    } while (__any_sync(0xffffffffu, fl == 0u));
+    const unsigned inc = __ballot_sync(0xffffffffu, fl == 2u);
+    const int first = inc ? (__ffs(inc) - 1) : 31;     // nearest predecessor that holds an inclusive prefix
+    int v = (lane <= first) ? (int)(w & CH_VAL) : 0;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    excl += v;
+    if (inc) break;
+    idx -= 32;
+  }
+  if (lane == 0) st_status(st + tile, CH_INC | ep | (unsigned long long)(unsigned)(excl + count));
+  return excl;
+}
 
-__device__ __forceinline__ int block_scan_inplace(int* __restrict__ a, int n, int cap, int* sm /*[34]*/) {
+// ------------------------------------------------------------------------------------------------
+// k_scan_lb: exclusive scan IN PLACE of a per-slot int table a[0..n) -> prefix clamped to `cap`, a[n] = min(total, cap),
+// as a multi-block single pass (tiles of SCAN_TILE entries, look-back across tiles).  The unclamped total and the
+// overflow bit go to the slot's counters.
+//   SENSOR: hits per sensor -> sensor_start            MDROW: MDs per module -> md_start
+//   LSROW : LSs per inner MD -> ls_start               T5   : pass flags -> positions in the T5 list (+ the list itself)
+// ------------------------------------------------------------------------------------------------
+constexpr int SCAN_TPB = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_TPB * SCAN_ITEMS;
+enum { SCAN_SENSOR = 0, SCAN_MDROW, SCAN_LSROW, SCAN_T5 };
+
+template <int MODE>
+__global__ void __launch_bounds__(SCAN_TPB) k_scan_lb(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ int sm[SCAN_TPB / 32];
+  __shared__ int s_tile, s_base;
+  const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
+  int* cnt = s.cnt;
+  int* a; int n, cap, icnt, iraw, itk; unsigned ovf; unsigned long long* chain;
+  if (MODE == SCAN_SENSOR) { a = s.sensor_start; n = 2 * geo.n_modules; cap = caps.max_hits; icnt = LST_CNT_HIT; iraw = -1; ovf = 0; itk = LST_CNT_TK_SENSOR; chain = s.chain_sensor; }
+  else if (MODE == SCAN_MDROW) { a = s.md_start; n = geo.n_modules; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; itk = LST_CNT_TK_MD; chain = s.chain_md; }
+  else if (MODE == SCAN_LSROW) { a = s.ls_start; n = cnt[LST_CNT_MD]; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; itk = LST_CNT_TK_LS; chain = s.chain_ls; }
+  else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; itk = LST_CNT_TK_T5; chain = s.chain_t5s; }
+  const int n_tiles = (n + SCAN_TILE - 1) / SCAN_TILE + (n == 0);
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  int carry = 0;
-  for (int base = 0; base < n; base += SCAN_THREADS * SCAN_ITEMS) {
-    const int i0 = base + tid * SCAN_ITEMS;
+  while (true) {
+    if (tid == 0) s_tile = atomicAdd(cnt + itk, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int i0 = tile * SCAN_TILE + tid * SCAN_ITEMS;
     int v[SCAN_ITEMS];
     if (i0 + SCAN_ITEMS <= n) {
       const int4 p = *reinterpret_cast<const int4*>(a + i0);
@@ -96,94 +167,43 @@ __device__ __forceinline__ int block_scan_inplace(int* __restrict__ a, int n, in
     for (int k = 0; k < SCAN_ITEMS; ++k) tsum += v[k];
     int inc = tsum;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, inc, d);
-      if (lane >= d) inc += t;
-    }
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
     if (lane == 31) sm[wid] = inc;
     __syncthreads();
-    if (wid == 0) {
-      int w = sm[lane];
-      int winc = w;
+    int wbase = 0, btot = 0;
 #pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, winc, d);
-        if (lane >= d) winc += t;
-      }
-      sm[lane] = winc - w;            // exclusive prefix of warp totals
-      if (lane == 31) sm[32] = winc;  // block total
+    for (int w = 0; w < SCAN_TPB / 32; ++w) { const int c = sm[w]; if (w < wid) wbase += c; btot += c; }
+    if (wid == 0) {
+      const int b = chain_exclusive(chain, tile, btot, lane, epoch);
+      if (lane == 0) s_base = b;
     }
     __syncthreads();
-    int run = carry + sm[wid] + (inc - tsum);
-    const int btot = sm[32];
+    const int base = s_base;
+    int run = base + wbase + inc - tsum;
+    int o[SCAN_ITEMS];
 #pragma unroll
-    for (int k = 0; k < SCAN_ITEMS; ++k) {
-      const int e = min(run, cap);
-      run += v[k];
-      v[k] = e;
+    for (int k = 0; k < SCAN_ITEMS; ++k) { o[k] = min(run, cap); run += v[k]; }
+    if (MODE == SCAN_T5) {        // T5 list = passing candidates in candidate order
+#pragma unroll
+      for (int k = 0; k < SCAN_ITEMS; ++k)
+        if (v[k] && i0 + k < n && o[k] < cap) s.t5_list[o[k]] = i0 + k;
     }
     if (i0 + SCAN_ITEMS <= n) {
-      *reinterpret_cast<int4*>(a + i0) = make_int4(v[0], v[1], v[2], v[3]);
-      *reinterpret_cast<int4*>(a + i0 + 4) = make_int4(v[4], v[5], v[6], v[7]);
+      *reinterpret_cast<int4*>(a + i0) = make_int4(o[0], o[1], o[2], o[3]);
+      *reinterpret_cast<int4*>(a + i0 + 4) = make_int4(o[4], o[5], o[6], o[7]);
     } else {
 #pragma unroll
       for (int k = 0; k < SCAN_ITEMS; ++k)
-        if (i0 + k < n) a[i0 + k] = v[k];
+        if (i0 + k < n) a[i0 + k] = o[k];
     }
-    carry += btot;
-    __syncthreads();
-  }
-  if (tid == 0) a[n] = min(carry, cap);
-  return carry;
-}
-
-// link_mod[l] = the module that owns flat cell l*LP (off = exclusive scan of the per-module cell counts, off[M] =
-// total); entries of links that start at or beyond the total are M.  Called by a whole block after the scan.
-__device__ __forceinline__ void link_owner_table(const int* __restrict__ off, int M, int LP, int* __restrict__ link_mod) {
-  const int total = min(off[M], MAX_CELLS);
-  for (int m = threadIdx.x; m < M; m += blockDim.x) {
-    const int b = off[m], e = min(off[m + 1], total);
-    for (int l = (b + LP - 1) / LP; l * LP < e; ++l) link_mod[l] = m;
-  }
-  for (int l = (total + LP - 1) / LP + threadIdx.x; l <= total / LP + 1; l += blockDim.x) link_mod[l] = M;
-}
-
-enum { SCAN_SENSOR = 0, SCAN_MDLINK, SCAN_LSLINK, SCAN_T5 };
-
-template <int MODE>
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  __shared__ int sm[34];
-  const Slot& s = slots[blockIdx.y];
-  int* cnt = s.cnt;
-  int* a; int n, cap, icnt, iraw; unsigned ovf;
-  if (MODE == SCAN_SENSOR) { a = s.sensor_start; n = 2 * geo.n_modules; cap = caps.max_hits; icnt = LST_CNT_HIT; iraw = -1; ovf = 0; }
-  else if (MODE == SCAN_MDLINK) { a = s.md_link_cnt; n = min(s.md_pair_off[geo.n_modules], MAX_CELLS) / MD_LP + 1; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; }
-  else if (MODE == SCAN_LSLINK) { a = s.ls_link_cnt; n = min(s.ls_off[geo.n_modules], MAX_CELLS) / LS_LP + 1; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; }
-  else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; }
-  __syncthreads();   // everyone has read n before thread 0 may overwrite counters below
-  const int total = block_scan_inplace(a, n, cap, sm);
-  if (threadIdx.x == 0) {
-    if (icnt >= 0) cnt[icnt] = min(total, cap);
-    if (iraw >= 0) cnt[iraw] = total;
-    if (total > cap) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), ovf);
-  }
-  __syncthreads();
-  // epilogues: range tables / compaction that fall out of the scan
-  if (MODE == SCAN_SENSOR) {      // flat cell space of the MD stage: exclusive scan of n_lower * n_upper per module
-    for (int m = threadIdx.x; m < geo.n_modules; m += SCAN_THREADS) {
-      const int lb = a[2 * m], ub = a[2 * m + 1], ue = a[2 * m + 2];
-      long long cells = (long long)(ub - lb) * (ue - ub);
-      if (cells > (1 << 22)) { cells = 0; atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), LST_ST_OVF_MD); }
-      s.md_pair_off[m] = (int)cells;
+    if (tile == n_tiles - 1 && tid == 0) {
+      const int total = base + btot;
+      a[n] = min(total, cap);
+      cnt[icnt] = min(total, cap);
+      if (iraw >= 0) cnt[iraw] = total;
+      if (total > cap) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), ovf);
     }
     __syncthreads();
-    const int cells_total = block_scan_inplace(s.md_pair_off, geo.n_modules, 0x7fffffff, sm);
-    if (threadIdx.x == 0 && cells_total > MAX_CELLS) atomicOr(reinterpret_cast<unsigned*>(cnt + CNT_STATUS), LST_ST_OVF_MD);
-    __syncthreads();
-    link_owner_table(s.md_pair_off, geo.n_modules, MD_LP, s.md_link_mod);
-  } else if (MODE == SCAN_T5) {   // T5 list = passing candidates in candidate order
-    for (int i = threadIdx.x; i < n; i += SCAN_THREADS)
-      if (s.t5c_pass[i] && a[i] < cap) s.t5_list[a[i]] = i;
   }
 }
 

@@ -139,19 +139,20 @@ __device__ __forceinline__ bool ls_eval(const Anchor& A, const Anchor& B, float&
   return true;
 }
 
-// Conservative prefilter of ls_eval (L1 and both L3; L2 is left to the exact test).  `cr` is formed exactly
-// as in ls_eval; c is approximated to a few ulp (|c| <= 0.015 => absolute error < 2e-8) and the L3
-// comparisons carry an absolute margin of 3e-7 (w >= ~5e-4 for any real MD) -- DESIGN.md "Prefilters".
-// Rejections are positive comparisons, so a NaN anywhere lets the pair through to the exact test.
-// A2 / B2 = (c, w, f, -) of the two MDs (f = 0.3 for endcap MDs, else 0).
-__device__ __forceinline__ bool ls_prefilter(float4 A, float4 A2, float4 B, float4 B2) {
-  const float dx = fs(B.x, A.x), dy = fs(B.y, A.y);
-  const float cr = fs(fm(A.x, dy), fm(A.y, dx));
-  const float dd = dx * dx + dy * dy;
-  const float c = -2.0f * cr * rsqrt_fast(dd) * rcp_fast(A.w * B.w);
+// Conservative prefilter of ls_eval (L1 and both L3; L2 is left to the exact test): exact pass => prefilter pass.
+// c is formed from the same quantities as in ls_eval but with fused / approximate operations: cr by one FMA
+// (|error| <= 2^-23 rA d, i.e. < 1e-8 in c), 1/sqrt by MUFU (2 ulp), 1/r precomputed per MD -- in all a few ulp of
+// |c| <= 0.015, i.e. < 1e-8 absolute.  Margins: L1 1e-4 relative; L3 1e-4 relative + 3e-7 absolute, folded into the
+// per-MD record by k_md_scatter: *a = (c_md, w*1.0001 + 3e-7, f*1.0001 | module-type bits, 1/r).  Rejections are positive
+// comparisons, so a NaN anywhere lets the pair through to the exact test.
+// kinvA = -2 / rA.
+__device__ __forceinline__ bool ls_prefilter(float4 Ap, float4 Aa, float kinvA, float4 Bp, float4 Ba) {
+  const float dx = Bp.x - Ap.x, dy = Bp.y - Ap.y;
+  const float cr = fmaf(Ap.x, dy, -(Ap.y * dx));
+  const float dd = fmaf(dx, dx, dy * dy);
+  const float c = (cr * rsqrt_fast(dd)) * (kinvA * Ba.w);
   const float ac = fabsf(c);
-  const bool rej = (ac > LST_C_MAX105 * 1.0001f) | (fabsf(A2.x - c) > (A2.y + A2.z * ac) * 1.0001f + 3.0e-7f) |
-                   (fabsf(B2.x - c) > (B2.y + B2.z * ac) * 1.0001f + 3.0e-7f);
+  const bool rej = (ac > LST_C_MAX105 * 1.0001f) | (fabsf(Aa.x - c) > fmaf(Aa.z, ac, Aa.y)) | (fabsf(Ba.x - c) > fmaf(Ba.z, ac, Ba.y));
   return !rej | (dd < 1.0e-30f);      // dd ~ 0: the approximations may overflow where the exact test does not
 }
 

@@ -1,366 +1,219 @@
-// lst_pairs.cuh -- single-pass, order-preserving MD (a1) and LS (a2) kernels.
+// lst_pairs.cuh -- a1 (mini-doublets) and a2 (line segments): order-preserving row sweeps.
 //
 // Both stages test every cell of per-module rectangles (rows = inner objects of module m, columns = the
 // module's candidate partners) and must emit the passing cells in the build order of SPEC.md 4.1-4.2
-// (module, row, column).  The cells of all rectangles, in build order, form one flat index space (prefix scan
-// of the per-module cell counts); one warp owns one *link* = a fixed-size range of that space:
+// (module, row, column).  A warp owns whole rows and walks their columns 32 at a time:
 //   1. prefilter:  all 32 lanes evaluate the cheap conservative form of the cuts (lst_math.cuh) on 32 cells;
 //                  survivors (a few %) are appended, in order, to a per-warp queue in shared memory;
 //   2. exact:      whenever the queue holds >= 32 cells a full warp evaluates the exact SPEC.md arithmetic
-//                  on them; passing cells are appended, in order, to the warp's staging buffer;
-//   3. place:      the link appends its objects (already in order) to an unordered per-slot record buffer and
-//                  stores its count; a block scan over the link counts (k_scan) gives every link its base,
-//                  and a per-link finalize warp copies the records to their final positions and writes the
-//                  range tables (md_start / ls_start) of the rows the link owns.
-// The output order depends only on the flat index, never on scheduling (bit-reproducible).  The staging
-// buffer holds as many objects as a link has cells, so it cannot overflow.
-// Capacity overflow: the record buffer (same capacity as the stage) may then have dropped records of early
-// links, so the CHAIN instantiation re-runs the stage: links are handed out by an atomic ticket, each obtains
-// the count of all earlier links by decoupled look-back and writes its first objects in place (a link only
-// waits for links that are already running: no deadlock).  It returns at once unless the overflow bit is set
-// (in-place waiting behind slow links makes it ~4x slower than the record path, measured r01).
+//                  on them; a passing cell becomes a record (row, seq = its rank among the row's objects, payload);
+//   3. place:      records go to an unordered per-slot buffer (one atomic per 32 records), the row's object
+//                  count goes to the row table.  A multi-block look-back scan of the row table
+//                  (k_scan_lb, lst_kernels.cuh) gives every row its first output position, and a scatter
+//                  kernel writes record -> start[row] + seq.
+// A row is never split between warps and a warp visits its rows and columns in ascending order, so `seq`
+// depends only on the input (bit-reproducible output order), whatever the scheduling.
+// a1: row = module (cells = lower x upper hits of the module, both contiguous in the sorted hit store).
+// a2: row = MD a; its columns are the MDs of the modules connected to module(a), which are a few contiguous MD
+//     ranges: lst_create compresses every CSR row into runs of consecutive module ids (Geo::run_*), and MDs are
+//     stored in module order, so one run = one contiguous slice of md_pos / md_aux.
+// Capacity overflow (more objects than the record buffer holds): the scan flags it, and the DIRECT instantiation
+// of the sweep runs the stage again, writing start[row] + seq in place for positions below the capacity ("first
+// cap objects in build order").  It returns at once unless the overflow bit is set.
 #pragma once
 #include "lst_kernels.cuh"
 
 namespace lst {
 
 constexpr int PAIR_WARPS = 4;        // warps per block
-constexpr int Q_CAP = 64;            // survivor queue per warp (drained at >= 32)
-constexpr int MD_WIN = 32;           // modules of a link cached in shared memory (one per lane)
+constexpr int Q_CAP = 64;            // survivor queue / record staging per warp (drained / flushed at >= 32)
+constexpr int LS_ROWS = 8;           // consecutive MD rows a warp takes at a time
+constexpr int RUN_CAP = 32;          // runs of a CSR row cached per warp at a time
 
 __device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
-// ---- decoupled look-back over 64-bit status words: flag (2 bits) | run epoch (30 bits) | value (32 bits).
-// A word counts only if its epoch is the current run's (k_hist, the first kernel of a run, increments the slot's
-// device-side run counter), so the status arrays never need clearing and the launch sequence has no per-run
-// arguments (it can be replayed as a CUDA graph).
-constexpr unsigned long long CH_AGG = 1ull << 62, CH_INC = 2ull << 62, CH_VAL = 0xFFFFFFFFull;
-__device__ __forceinline__ unsigned chain_flag(unsigned long long w, unsigned epoch) {
-  return (((unsigned)(w >> 32)) & 0x3FFFFFFFu) == epoch ? (unsigned)(w >> 62) : 0u;
-}
-__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
-  unsigned long long v;
-  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
-  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-// exclusive prefix of `count` over links [0, link); called by all 32 lanes, publishes the inclusive prefix
-__device__ __forceinline__ int chain_exclusive(unsigned long long* st, int link, int count, int lane, unsigned epoch) {
-  const unsigned long long ep = (unsigned long long)epoch << 32;
-  if (link == 0) {
-    if (lane == 0) st_status(st, CH_INC | ep | (unsigned long long)(unsigned)count);
-    return 0;
-  }
-  if (lane == 0) st_status(st + link, CH_AGG | ep | (unsigned long long)(unsigned)count);
-  int excl = 0;
-  int idx = link - 1 - lane;
-  while (true) {
-    unsigned long long w;
-    unsigned fl;
-    do {
-      w = (idx >= 0) ? ld_status(st + idx) : (CH_INC | ep);
-      fl = chain_flag(w, epoch);
-    } while (__any_sync(0xffffffffu, fl == 0u));
-    const unsigned inc = __ballot_sync(0xffffffffu, fl == 2u);
-    const int first = inc ? (__ffs(inc) - 1) : 31;     // nearest predecessor that holds an inclusive prefix
-    int v = (lane <= first) ? (int)(w & CH_VAL) : 0;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-    excl += v;
-    if (inc) break;
-    idx -= 32;
-  }
-  if (lane == 0) st_status(st + link, CH_INC | ep | (unsigned long long)(unsigned)(excl + count));
-  return excl;
-}
-
-__device__ __forceinline__ int warp_ticket(int* counter, int lane) {
-  int t = 0;
-  if (lane == 0) t = atomicAdd(counter, 1);
-  return __shfl_sync(0xffffffffu, t, 0);
-}
-
-
-// first index i in [0, n] with off[i] > x (off non-decreasing); n + 1 if none
-__device__ __forceinline__ int upper_bound_g(const int* __restrict__ off, int n, int x) {
-  int lo = 0, hi = n + 1;
-  while (lo < hi) {
-    const int mid = (lo + hi) >> 1;
-    if (off[mid] > x) hi = mid; else lo = mid + 1;
-  }
-  return lo;
-}
-// largest m in [mS, mE] with off[m] <= f (exists by construction); among equal offsets the last one, i.e. the
-// module that really owns cell f
-__device__ __forceinline__ int owner_module(const int* __restrict__ off, int mS, int mE, int f) {
-  int lo = mS, hi = mE;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if (off[mid] <= f) lo = mid; else hi = mid - 1;
-  }
-  return lo;
-}
-__device__ __forceinline__ int lower_bound_s(const int* a, int n, int x) {   // first i with a[i] >= x
-  int lo = 0, hi = n;
-  while (lo < hi) {
-    const int mid = (lo + hi) >> 1;
-    if (a[mid] < x) lo = mid + 1; else hi = mid;
-  }
-  return lo;
-}
 __device__ __forceinline__ void divmod_small(int v, int d, int& q, int& r) {   // 0 <= v < 2^22, d > 0
   q = (int)(((float)v + 0.5f) * rcp_fast((float)d));
   r = v - q * d;
   if (r < 0) { --q; r += d; } else if (r >= d) { ++q; r -= d; }
 }
 
+// rank of every passing lane among the passing lanes with the same row, continued from the previous batch
+// (carry = row and running count of the last object emitted so far).  Returns seq; updates the carry.
+__device__ __forceinline__ int row_sequence(int row, bool pass, unsigned mask, unsigned lt, int lane, int& carry_row, int& carry_n,
+                                            bool& last_of_row) {
+  const unsigned peers = __match_any_sync(0xffffffffu, row) & mask;
+  const int seq = __popc(peers & lt) + (row == carry_row ? carry_n : 0);
+  last_of_row = pass && ((peers >> lane) >> 1) == 0u;
+  if (mask) {
+    const int hl = 31 - __clz(mask);
+    carry_row = __shfl_sync(0xffffffffu, row, hl);
+    carry_n = __shfl_sync(0xffffffffu, seq, hl) + 1;
+  }
+  return seq;
+}
+
 // ------------------------------------------------------------------------------------------------
-// a1: cells = (lower hit i, upper hit j) of module m, flat index md_pair_off[m] + i*n_up + j
+// a1: row = module m; cells = (lower hit i, upper hit j), i-major
 // ------------------------------------------------------------------------------------------------
 struct MdWarp {   // per-warp shared memory
-  int w_off[MD_WIN + 1], w_lb[MD_WIN], w_ub[MD_WIN], w_nup[MD_WIN], w_mt[MD_WIN];   // the link's first modules
-  int q_lo[Q_CAP], q_up[Q_CAP], q_mt[Q_CAP], q_f[Q_CAP];
-  int p_lo[MD_LP], p_up[MD_LP], p_mt[MD_LP], p_f[MD_LP];
-  float p_c[MD_LP], p_w[MD_LP];
+  int q_lo[Q_CAP], q_up[Q_CAP], q_mt[Q_CAP];
+  MdRec st[Q_CAP];
 };
 
-// exact evaluation of `n` (<= 32) queued cells; appends the passing ones in order; returns the new count
-__device__ __forceinline__ int md_drain(const Slot& s, MdWarp& W, int n, int pn, int lane, unsigned lt) {
+template <bool DIRECT>
+__device__ __forceinline__ void md_emit(const Slot& s, const MdRec& r, int cap) {      // final arrays of one MD
+  const int pos = s.md_start[r.mtm >> 2] + r.seq;
+  if (pos >= cap) return;
+  const float4 h = s.hit[r.p_lo];
+  const int mt = r.mtm & 3;
+  s.md_hits[pos] = make_int2(s.hit_orig[r.p_lo], s.hit_orig[r.p_up]);
+  s.md_modt[pos] = r.mtm;
+  s.md_pos[pos] = h;                                  // anchor (x, y, z, r1)
+  s.md_cw[pos] = make_float2(r.c, r.w);
+  // (c, w and f with the prefilter margins folded in, 1/r): one load for the LS prefilter; the low two mantissa bits of f
+  // carry the module type (they only widen the tolerance)
+  const float fm_ = __int_as_float(__float_as_int(md_relf(mt) * 1.0001f) | mt);
+  s.md_aux[pos] = make_float4(r.c, fmaf(r.w, 1.0001f, 3.0e-7f), fm_, 1.0f / h.w);
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ void md_flush(const Slot& s, MdWarp& W, int n, int lane, int cap) {
+  if (DIRECT) {
+    if (lane < n) md_emit<true>(s, W.st[lane], cap);
+    return;
+  }
+  int base = 0;
+  if (lane == 0) base = atomicAdd(s.cnt + LST_CNT_FILL_MD, n);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (lane < n && base + lane < cap) s.md_rec[base + lane] = W.st[lane];
+}
+
+// exact evaluation of the first `n` (<= 32) queued cells; passing ones become staged records; returns the new staging count
+template <bool DIRECT>
+__device__ __forceinline__ int md_drain(const Slot& s, MdWarp& W, int n, int sn, int lane, unsigned lt, int& carry_row, int& carry_n) {
   bool pass = false;
-  int p_lo = 0, p_up = 0, mtm = 0, f = 0;
+  int p_lo = 0, p_up = 0, mtm = -1 - lane;
   float c = 0.f, w = 0.f;
   if (lane < n) {
-    p_lo = W.q_lo[lane]; p_up = W.q_up[lane]; mtm = W.q_mt[lane]; f = W.q_f[lane];
+    p_lo = W.q_lo[lane]; p_up = W.q_up[lane]; mtm = W.q_mt[lane];
     const float4 h1 = s.hit[p_lo], h2 = s.hit[p_up];
     pass = md_eval(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3, c, w);
   }
   const unsigned mask = __ballot_sync(0xffffffffu, pass);
+  bool last;
+  const int seq = row_sequence(mtm, pass, mask, lt, lane, carry_row, carry_n, last);
   if (pass) {
-    const int i = pn + __popc(mask & lt);
-    W.p_lo[i] = p_lo; W.p_up[i] = p_up; W.p_mt[i] = mtm; W.p_f[i] = f; W.p_c[i] = c; W.p_w[i] = w;
+    MdRec r; r.p_lo = p_lo; r.p_up = p_up; r.mtm = mtm; r.seq = seq; r.c = c; r.w = w; r.pad0 = 0; r.pad1 = 0;
+    W.st[sn + __popc(mask & lt)] = r;
+    if (!DIRECT && last) s.md_start[mtm >> 2] = seq + 1;        // objects of this module so far
   }
-  return pn + __popc(mask);
+  return sn + __popc(mask);
 }
 
-template <bool CHAIN>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_links(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+template <bool DIRECT>
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   __shared__ MdWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  const unsigned epoch = *s.epoch_dev;
-  if (CHAIN && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;
+  if (DIRECT && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;
   const int lane = threadIdx.x & 31;
   MdWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
   const int M = geo.n_modules;
-  const int* __restrict__ off = s.md_pair_off;
   const int* __restrict__ ss = s.sensor_start;
   const float4* __restrict__ hit = s.hit;
-  const int total_cells = min(off[M], MAX_CELLS);       // beyond: flagged by the scan that made `off`
-  const int n_links = total_cells / MD_LP + 1;
   const int cap = caps.max_md;
-  int link;
-  while (true) {      // links are handed out dynamically: their cost varies with the number of modules they span
-    link = warp_ticket(s.cnt + (CHAIN ? LST_CNT_TICKET_MD : LST_CNT_DYN_MD), lane);
-    if (link >= n_links) break;
-    const int lo = link * MD_LP, hi = min(total_cells, lo + MD_LP);
-    int qn = 0, pn = 0;
-    if (lo < hi) {
-      // cache the first MD_WIN modules of the link (normally all of them)
-      const int mS = s.md_link_mod[link];
-      __syncwarp();
-      {
-        const int m = mS + lane;
-        int o = 0x7fffffff, lb = 0, ub = 0, ue = 0, mt = 0;
-        if (m < M) { o = off[m]; lb = ss[2 * m]; ub = ss[2 * m + 1]; ue = ss[2 * m + 2]; mt = geo.modt[m]; }
-        W.w_off[lane] = o; W.w_lb[lane] = lb; W.w_ub[lane] = ub; W.w_nup[lane] = ue - ub; W.w_mt[lane] = (m << 2) | mt;
-        if (lane == 0) W.w_off[MD_WIN] = (mS + MD_WIN <= M) ? off[mS + MD_WIN] : 0x7fffffff;
-      }
-      __syncwarp();
-      const int win_end = W.w_off[MD_WIN];
-      for (int f0 = lo; f0 < hi; f0 += 32) {
-        const int f = f0 + lane;
+  const int n_warps = gridDim.x * PAIR_WARPS;
+  int qn = 0, sn = 0, carry_row = -1, carry_n = 0;
+  // modules are interleaved over the warps (heavy inner-layer modules have consecutive ids); a warp fetches the ranges of
+  // its next 32 modules with one round of loads
+  const int wid = blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5);
+  for (int mb = wid; mb < M; mb += n_warps * 32) {
+    const int my_m = mb + lane * n_warps;
+    int my_lb = 0, my_ub = 0, my_ue = 0, my_mt = 0;
+    if (my_m < M) {
+      my_lb = ss[2 * my_m]; my_ub = ss[2 * my_m + 1]; my_ue = ss[2 * my_m + 2]; my_mt = geo.modt[my_m];
+      if (!DIRECT) s.md_start[my_m] = 0;
+    }
+    __syncwarp();
+    unsigned todo = __ballot_sync(0xffffffffu, my_ub > my_lb && my_ue > my_ub);
+    while (todo) {
+      const int k = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const int lb = __shfl_sync(0xffffffffu, my_lb, k), ub = __shfl_sync(0xffffffffu, my_ub, k), ue = __shfl_sync(0xffffffffu, my_ue, k);
+      const int mtm = ((mb + k * n_warps) << 2) | __shfl_sync(0xffffffffu, my_mt, k);
+      const int n_lo = ub - lb, n_up = ue - ub;
+      int i, j, q32, r32;                       // the lane's cell (i, j); 32 cells further = (+q32, +r32)
+      divmod_small(lane, n_up, i, j);
+      divmod_small(32, n_up, q32, r32);
+      const long long n_sweeps = ((long long)n_lo * n_up + 31) >> 5;
+      for (long long sw = 0; sw < n_sweeps; ++sw) {
         bool pre = false;
-        int p_lo = 0, p_up = 0, mtm = 0;
-        if (f < hi) {
-          int loc, lb, ub, nup;
-          if (f < win_end) {
-            int k = 0;
-#pragma unroll
-            for (int step = MD_WIN / 2; step > 0; step >>= 1)
-              if (W.w_off[k + step] <= f) k += step;
-            loc = f - W.w_off[k]; lb = W.w_lb[k]; ub = W.w_ub[k]; nup = W.w_nup[k]; mtm = W.w_mt[k];
-          } else {     // sparse region: the link spans more than MD_WIN modules
-            const int m = owner_module(off, mS + MD_WIN, M - 1, f);
-            loc = f - off[m]; lb = ss[2 * m]; ub = ss[2 * m + 1]; nup = ss[2 * m + 2] - ub; mtm = (m << 2) | geo.modt[m];
-          }
-          int i, j;
-          divmod_small(loc, nup, i, j);
-          p_lo = lb + i; p_up = ub + j;
+        const int p_lo = lb + i, p_up = ub + j;
+        if (i < n_lo) {
           const float4 h1 = __ldg(hit + p_lo), h2 = __ldg(hit + p_up);
           pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3);
         }
+        i += q32; j += r32;
+        if (j >= n_up) { j -= n_up; ++i; }
         const unsigned mask = __ballot_sync(0xffffffffu, pre);
         if (mask) {
-          if (pre) { const int i = qn + __popc(mask & lt); W.q_lo[i] = p_lo; W.q_up[i] = p_up; W.q_mt[i] = mtm; W.q_f[i] = f - lo; }
+          if (pre) { const int q = qn + __popc(mask & lt); W.q_lo[q] = p_lo; W.q_up[q] = p_up; W.q_mt[q] = mtm; }
           qn += __popc(mask);
           __syncwarp();
           if (qn >= 32) {
-            pn = md_drain(s, W, 32, pn, lane, lt);
+            sn = md_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
             __syncwarp();
             const int rest = qn - 32;
-            int a = 0, b = 0, c = 0, d = 0;
-            if (lane < rest) { a = W.q_lo[32 + lane]; b = W.q_up[32 + lane]; c = W.q_mt[32 + lane]; d = W.q_f[32 + lane]; }
+            int a = 0, b = 0, c = 0;
+            if (lane < rest) { a = W.q_lo[32 + lane]; b = W.q_up[32 + lane]; c = W.q_mt[32 + lane]; }
             __syncwarp();
-            if (lane < rest) { W.q_lo[lane] = a; W.q_up[lane] = b; W.q_mt[lane] = c; W.q_f[lane] = d; }
+            if (lane < rest) { W.q_lo[lane] = a; W.q_up[lane] = b; W.q_mt[lane] = c; }
             qn = rest;
+            if (sn >= 32) {
+              md_flush<DIRECT>(s, W, 32, lane, cap);
+              __syncwarp();
+              MdRec t{};
+              if (lane < sn - 32) t = W.st[32 + lane];
+              __syncwarp();
+              if (lane < sn - 32) W.st[lane] = t;
+              sn -= 32;
+            }
             __syncwarp();
           }
         }
       }
-      if (qn) pn = md_drain(s, W, qn, pn, lane, lt);
-      __syncwarp();
     }
-    if (!CHAIN) {      // append the link's MDs to the record buffer, remember where and how many
-      int soff = 0;
-      if (lane == 0) { soff = pn ? atomicAdd(s.cnt + LST_CNT_FILL_MD, pn) : 0; s.md_link_cnt[link] = pn; s.md_link_soff[link] = soff; }
-      soff = __shfl_sync(0xffffffffu, soff, 0);
-      for (int i = lane; i < pn; i += 32)
-        if (soff + i < cap) {
-          MdRec r; r.p_lo = W.p_lo[i]; r.p_up = W.p_up[i]; r.mtm = W.p_mt[i]; r.f = W.p_f[i]; r.c = W.p_c[i]; r.w = W.p_w[i]; r.link = link; r.pad = 0;
-          s.md_rec[soff + i] = r;
-        }
-      __syncwarp();
-      continue;
-    }
-    // CHAIN (overflow re-run): base by look-back, objects and range table written in place
-    const int base = chain_exclusive(s.chain_md, link, pn, lane, epoch);
-    for (int i = lane; i < pn; i += 32) {
-      const int pos = base + i;
-      if (pos < cap) {
-        const int p_lo = W.p_lo[i], p_up = W.p_up[i];
-        s.md_hits[pos] = make_int2(s.hit_orig[p_lo], s.hit_orig[p_up]);
-        s.md_modt[pos] = W.p_mt[i];
-        s.md_pos[pos] = hit[p_lo];              // (x, y, z, r1)
-        s.md_cw[pos] = make_float2(W.p_c[i], W.p_w[i]);
-        s.md_aux[pos] = make_float4(W.p_c[i], W.p_w[i], md_relf(W.p_mt[i] & 3), 0.f);
-      }
-    }
-    int sr = 0;
-    if (lane < 2) sr = upper_bound_g(off, M, lane == 0 ? lo - 1 : lo + MD_LP - 1);
-    const int mOwn0 = __shfl_sync(0xffffffffu, sr, 0), mOwn1 = min(M, __shfl_sync(0xffffffffu, sr, 1));
-    for (int m = mOwn0 + lane; m < mOwn1; m += 32) s.md_start[m] = min(base + lower_bound_s(W.p_f, pn, off[m] - lo), cap);
-    if (link == n_links - 1 && lane == 0) {
-      const int total = base + pn;
-      s.md_start[M] = min(total, cap);
-      s.cnt[LST_CNT_MD] = min(total, cap);
-      s.cnt[LST_CNT_RAW_MD] = total;
-    }
+  }
+  if (qn) { sn = md_drain<DIRECT>(s, W, qn, sn, lane, lt, carry_row, carry_n); __syncwarp(); }
+  if (sn >= 32) {
+    md_flush<DIRECT>(s, W, 32, lane, cap);
+    __syncwarp();
+    MdRec t{};
+    if (lane < sn - 32) t = W.st[32 + lane];
+    __syncwarp();
+    if (lane < sn - 32) W.st[lane] = t;
+    sn -= 32;
     __syncwarp();
   }
+  if (sn) md_flush<DIRECT>(s, W, sn, lane, cap);
 }
 
-// a1 finalize (md_link_cnt holds the exclusive scan of the link counts by now): one thread per record copies it
-// to base[link] + its index inside the link; one thread per module writes md_start[m] = number of MDs before the
-// module's first cell
-__global__ void __launch_bounds__(256) k_md_final(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+// a1 scatter (md_start holds the exclusive scan of the per-module counts by now): record -> md_start[module] + seq
+__global__ void __launch_bounds__(256) k_md_scatter(const Slot* __restrict__ slots, Caps caps) {
   const Slot& s = slots[blockIdx.y];
-  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) return;       // the CHAIN pass rewrites the stage
-  const int M = geo.n_modules;
-  const int* __restrict__ off = s.md_pair_off;
-  const int* __restrict__ base = s.md_link_cnt;
-  const int* __restrict__ soff = s.md_link_soff;
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) return;       // the DIRECT pass rewrites the stage
   const int n_rec = min(s.cnt[LST_CNT_FILL_MD], caps.max_md);
-  LST_FOR_ITEMS(j, n_rec) {
-    const MdRec r = s.md_rec[j];
-    const int pos = base[r.link] + (j - soff[r.link]);
-    s.md_hits[pos] = make_int2(s.hit_orig[r.p_lo], s.hit_orig[r.p_up]);
-    s.md_modt[pos] = r.mtm;
-    s.md_pos[pos] = s.hit[r.p_lo];
-    s.md_cw[pos] = make_float2(r.c, r.w);
-    s.md_aux[pos] = make_float4(r.c, r.w, md_relf(r.mtm & 3), 0.f);     // (c, w, f, -): one load for the LS prefilter
-  }
-  const int total_cells = min(off[M], MAX_CELLS);
-  LST_FOR_ITEMS(m, M + 1) {
-    const int x = min(off[m], total_cells);
-    const int link = x / MD_LP, rel = x - link * MD_LP;
-    const int b = base[link], pn = base[link + 1] - b;
-    const MdRec* __restrict__ rec = s.md_rec + soff[link];
-    int l = 0, h = pn;
-    while (l < h) { const int mid = (l + h) >> 1; if (rec[mid].f < rel) l = mid + 1; else h = mid; }
-    s.md_start[m] = b + l;
-  }
+  LST_FOR_ITEMS(j, n_rec) md_emit<false>(s, s.md_rec[j], caps.max_md);
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2: cells = (MD a of module m, candidate column) with flat index ls_off[m] + row*L[m] + col; the columns of m
-// are the MDs of its CSR-connected modules in ascending MD index (L[m] of them, listed in ls_cand)
+// a2: row = MD a of module m; columns = the MDs of the runs of CSR row m, ascending
 // ------------------------------------------------------------------------------------------------
-// plan, three small launches: (1) candidate count L[m] and cell count n_m * L[m] per module; (2) one block per
-// event: exclusive scans of the cell counts and of the candidate-table offsets, link -> module table; (3) the
-// candidate table itself
-__global__ void __launch_bounds__(256) k_ls_plan1(const Slot* __restrict__ slots, Geo geo) {
-  const Slot& s = slots[blockIdx.y];
-  const int* __restrict__ mds = s.md_start;
-  LST_FOR_ITEMS(m, geo.n_modules) {
-    const int n_m = mds[m + 1] - mds[m];
-    int L = 0;
-    if (n_m > 0) {
-      const int e1 = geo.rowptr[m + 1];
-      for (int e = geo.rowptr[m]; e < e1; ++e) { const int m2 = geo.col[e]; L += mds[m2 + 1] - mds[m2]; }
-    }
-    long long cells = (long long)n_m * L;
-    if (cells > MAX_CELLS) {      // beyond any event the capacities admit: drop the module's cells, flag the stage
-      cells = 0; L = 0;
-      atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_LS);
-    }
-    s.ls_L[m] = L;
-    s.ls_off[m] = (int)cells;
-    s.ls_coff[m] = L;
-  }
-}
-__global__ void __launch_bounds__(SCAN_THREADS) k_ls_plan2(const Slot* __restrict__ slots, Geo geo) {
-  __shared__ int sm[34];
-  const Slot& s = slots[blockIdx.y];
-  const int M = geo.n_modules;
-  const int total = block_scan_inplace(s.ls_off, M, 0x7fffffff, sm);
-  __syncthreads();
-  block_scan_inplace(s.ls_coff, M, 0x7fffffff, sm);
-  __syncthreads();
-  if (threadIdx.x == 0 && total > MAX_CELLS) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_LS);
-  link_owner_table(s.ls_off, M, LS_LP, s.ls_link_mod);
-}
-__global__ void __launch_bounds__(256) k_ls_plan3(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  const Slot& s = slots[blockIdx.y];
-  const int* __restrict__ mds = s.md_start;
-  const int cand_cap = CAND_PER_MD * caps.max_md;
-  const int lane = threadIdx.x & 31;
-  // one warp per module: the lanes take the CSR entries, a warp scan places each entry's MD range
-  for (int m = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; m < geo.n_modules; m += (gridDim.x * blockDim.x) >> 5) {
-    const int L = s.ls_L[m];
-    int o = s.ls_coff[m];
-    if (L == 0 || o + L > cand_cap) continue;        // modules beyond the table walk the CSR row instead
-    const int e0 = geo.rowptr[m], e1 = geo.rowptr[m + 1];
-    for (int eb = e0; eb < e1; eb += 32) {
-      const int e = eb + lane;
-      int b0 = 0, n = 0;
-      if (e < e1) { const int m2 = geo.col[e]; b0 = mds[m2]; n = mds[m2 + 1] - b0; }
-      int inc = n;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-      const int w = o + inc - n;
-      for (int t = 0; t < n; ++t) s.ls_cand[w + t] = b0 + t;
-      o += __shfl_sync(0xffffffffu, inc, 31);
-    }
-  }
-}
-
 struct LsWarp {
-  int w_off[MD_WIN + 1], w_a0[MD_WIN], w_L[MD_WIN], w_co[MD_WIN];      // the link's next modules
-  int q_a[Q_CAP], q_b[Q_CAP], q_f[Q_CAP];
-  int p_a[LS_LP], p_b[LS_LP], p_f[LS_LP];
-  float p_c[LS_LP];
+  int r_off[RUN_CAP + 1], r_b0[RUN_CAP];      // non-empty runs of the current module: first column, first MD
+  int q_a[Q_CAP], q_b[Q_CAP];
+  LsRec st[Q_CAP];
 };
 
 __device__ __forceinline__ Anchor load_anchor(const Slot& s, int i) {
@@ -370,218 +223,152 @@ __device__ __forceinline__ Anchor load_anchor(const Slot& s, int i) {
   return a;
 }
 
-// column -> MD index by walking the CSR row (only for modules beyond the candidate table)
-__device__ __noinline__ int cand_walk(const Slot& s, const Geo& geo, int m, int col) {
-  const int e1 = geo.rowptr[m + 1];
-  for (int e = geo.rowptr[m]; e < e1; ++e) {
-    const int m2 = geo.col[e];
-    const int b0 = s.md_start[m2], n = s.md_start[m2 + 1] - b0;
-    if (col < n) return b0 + col;
-    col -= n;
+template <bool DIRECT>
+__device__ __forceinline__ void ls_flush(const Slot& s, LsWarp& W, int n, int lane, int cap) {
+  if (DIRECT) {
+    if (lane < n) {
+      const LsRec r = W.st[lane];
+      const int pos = s.ls_start[r.a] + r.seq;
+      if (pos < cap) { s.ls_ab[pos] = make_int2(r.a, r.b); s.ls_c[pos] = r.c; }
+    }
+    return;
   }
-  return 0;
+  int base = 0;
+  if (lane == 0) base = atomicAdd(s.cnt + LST_CNT_FILL_LS, n);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (lane < n && base + lane < cap) s.ls_rec[base + lane] = W.st[lane];
 }
 
-__device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int pn, int lane, unsigned lt) {
+template <bool DIRECT>
+__device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int sn, int lane, unsigned lt, int& carry_row, int& carry_n) {
   bool pass = false;
-  int a = 0, b = 0, f = 0;
+  int a = -1 - lane, b = 0;
   float c = 0.f;
   if (lane < n) {
-    a = W.q_a[lane]; b = W.q_b[lane]; f = W.q_f[lane];
+    a = W.q_a[lane]; b = W.q_b[lane];
     const Anchor A = load_anchor(s, a), B = load_anchor(s, b);
     pass = ls_eval(A, B, c);
   }
   const unsigned mask = __ballot_sync(0xffffffffu, pass);
+  bool last;
+  const int seq = row_sequence(a, pass, mask, lt, lane, carry_row, carry_n, last);
   if (pass) {
-    const int i = pn + __popc(mask & lt);
-    W.p_a[i] = a; W.p_b[i] = b; W.p_f[i] = f; W.p_c[i] = c;
+    LsRec r; r.a = a; r.b = b; r.seq = seq; r.c = c;
+    W.st[sn + __popc(mask & lt)] = r;
+    if (!DIRECT && last) s.ls_start[a] = seq + 1;              // LSs of this row so far
   }
-  return pn + __popc(mask);
+  return sn + __popc(mask);
 }
 
-// append the survivors of one sweep to the queue (in lane order); a full warp of queued cells is evaluated at once
-__device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int a, int b, int f, int& qn, int& pn, int lane, unsigned lt) {
-  const unsigned mask = __ballot_sync(0xffffffffu, pre);
-  if (!mask) return;
-  if (pre) { const int i = qn + __popc(mask & lt); W.q_a[i] = a; W.q_b[i] = b; W.q_f[i] = f; }
-  qn += __popc(mask);
+// non-empty runs [e, e + 32) of CSR row m -> the warp's run table; returns the number of columns they hold
+__device__ __forceinline__ int ls_load_runs(const Geo& geo, const int* __restrict__ mds, LsWarp& W, int e0, int e1, int lane, unsigned lt) {
+  const int e = e0 + lane;
+  int b0 = 0, n = 0;
+  if (e < e1) { b0 = mds[geo.run_c0[e]]; n = mds[geo.run_c1[e]] - b0; }
+  int inc = n;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+  const unsigned nz = __ballot_sync(0xffffffffu, n > 0);
+  const int total = __shfl_sync(0xffffffffu, inc, 31);
   __syncwarp();
-  if (qn >= 32) {
-    pn = ls_drain(s, W, 32, pn, lane, lt);
-    __syncwarp();
-    const int rest = qn - 32;
-    int x = 0, y = 0, z = 0;
-    if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; z = W.q_f[32 + lane]; }
-    __syncwarp();
-    if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; W.q_f[lane] = z; }
-    qn = rest;
-    __syncwarp();
-  }
+  if (n > 0) { const int i = __popc(nz & lt); W.r_off[i] = inc - n; W.r_b0[i] = b0; }
+  if (lane == 0) W.r_off[__popc(nz)] = total;
+  __syncwarp();
+  return total;
 }
 
-// first MD index whose row starts at a flat position >= x (rows are in MD order, positions non-decreasing)
-__device__ __forceinline__ int first_row_at(const Slot& s, const int* __restrict__ off, int M, int x) {
-  const int* __restrict__ mds = s.md_start;
-  if (x > off[M]) return mds[M];
-  const int mB = (x <= 0) ? 0 : upper_bound_g(off, M, x - 1);     // first module with off[m] >= x (<= M)
-  if (mB > 0) {
-    const int mP = mB - 1, L = s.ls_L[mP];                        // off[mP] < x: its later rows may still start >= x
-    if (L > 0) {
-      const int n_m = mds[mP + 1] - mds[mP];
-      const int r0 = (x - off[mP] + L - 1) / L;
-      if (r0 < n_m) return mds[mP] + r0;
-    }
-  }
-  return mds[mB];
-}
-
-template <bool CHAIN>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_links(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+template <bool DIRECT>
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  const unsigned epoch = *s.epoch_dev;
-  if (CHAIN && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;
+  if (DIRECT && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;
   const int lane = threadIdx.x & 31;
   LsWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
-  const int M = geo.n_modules;
-  const int* __restrict__ off = s.ls_off;
   const int* __restrict__ mds = s.md_start;
-  const int* __restrict__ cand = s.ls_cand;
   const float4* __restrict__ mpos = s.md_pos;
   const float4* __restrict__ maux = s.md_aux;
-  const int total_cells = min(off[M], MAX_CELLS);
-  const int n_links = total_cells / LS_LP + 1;
-  const int cap = caps.max_ls, cand_cap = CAND_PER_MD * caps.max_md;
-  int link;
-  while (true) {
-    link = warp_ticket(s.cnt + (CHAIN ? LST_CNT_TICKET_LS : LST_CNT_DYN_LS), lane);
-    if (link >= n_links) break;
-    const int lo = link * LS_LP, hi = min(total_cells, lo + LS_LP);
-    int qn = 0, pn = 0;
-    if (lo < hi) {
-      int mW = s.ls_link_mod[link];      // module that owns the next unprocessed cell
-      int fc = lo;                       // next unprocessed cell
-      while (fc < hi) {
-        // cache the next MD_WIN modules (offsets, first MD, candidate count, candidate-table offset)
-        __syncwarp();
-        {
-          const int m = mW + lane;
-          int o = 0x7fffffff, a0 = 0, L = 1, co = 0;
-          if (m < M) { o = off[m]; a0 = mds[m]; L = s.ls_L[m]; co = s.ls_coff[m]; }
-          W.w_off[lane] = o; W.w_a0[lane] = a0; W.w_L[lane] = L; W.w_co[lane] = co;
-          if (lane == 0) W.w_off[MD_WIN] = (mW + MD_WIN <= M) ? off[mW + MD_WIN] : 0x7fffffff;
-        }
-        __syncwarp();
-        const int end = min(hi, W.w_off[MD_WIN]);
-        if (W.w_off[1] >= hi) {
-          // dense: the rest of the link lies in one module -- (row, col) advance incrementally
-          const int om = W.w_off[0], a0 = W.w_a0[0], L = W.w_L[0], co = W.w_co[0];
-          const bool tabled = co + L <= cand_cap;
-          const int c0 = fc - om, c1 = hi - om;
-          int row, col, q32, r32;                       // the lane's cell (row, col); 32 cells further = (+q32, +r32)
-          divmod_small(c0 + lane, L, row, col);
-          divmod_small(32, L, q32, r32);
-          for (int cb = c0; cb < c1; cb += 32) {
-            const int cell = cb + lane;
-            bool pre = false;
-            int a = 0, b = 0;
-            if (cell < c1) {
-              a = a0 + row;
-              b = tabled ? __ldg(cand + co + col) : cand_walk(s, geo, mW, col);
-              pre = ls_prefilter(__ldg(mpos + a), __ldg(maux + a), __ldg(mpos + b), __ldg(maux + b));
+  const int n_md = s.cnt[LST_CNT_MD];
+  const int cap = caps.max_ls;
+  const int n_warps = gridDim.x * PAIR_WARPS;
+  int qn = 0, sn = 0, carry_row = -1, carry_n = 0;
+  for (int a0 = (blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5)) * LS_ROWS; a0 < n_md; a0 += n_warps * LS_ROWS) {
+    const int a1 = min(a0 + LS_ROWS, n_md);
+    if (!DIRECT && a0 + lane < a1) s.ls_start[a0 + lane] = 0;
+    __syncwarp();
+    int cur_m = -1, L = 0, e0 = 0, e1 = 0;
+    for (int a = a0; a < a1; ++a) {
+      const int m = s.md_modt[a] >> 2;
+      if (m != cur_m) {
+        cur_m = m;
+        e0 = geo.run_ptr[m]; e1 = geo.run_ptr[m + 1];
+        if (e1 - e0 <= RUN_CAP) L = ls_load_runs(geo, mds, W, e0, e1, lane, lt);
+      }
+      const float4 Ap = __ldg(mpos + a), Aa = __ldg(maux + a);
+      const float kinvA = -2.0f * Aa.w;
+      for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
+        if (e1 - e0 > RUN_CAP) L = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
+        int r = 0;
+        for (int t0 = 0; t0 < L; t0 += 32) {
+          const int t = min(t0 + lane, L - 1);
+          while (t >= W.r_off[r + 1]) ++r;
+          const int b = W.r_b0[r] + (t - W.r_off[r]);
+          const float4 Bp = __ldg(mpos + b), Ba = __ldg(maux + b);
+          const bool pre = ls_prefilter(Ap, Aa, kinvA, Bp, Ba) && (t0 + lane < L);
+          const unsigned mask = __ballot_sync(0xffffffffu, pre);
+          if (mask) {
+            if (pre) { const int q = qn + __popc(mask & lt); W.q_a[q] = a; W.q_b[q] = b; }
+            qn += __popc(mask);
+            __syncwarp();
+            if (qn >= 32) {
+              sn = ls_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
+              __syncwarp();
+              const int rest = qn - 32;
+              int x = 0, y = 0;
+              if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; }
+              __syncwarp();
+              if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; }
+              qn = rest;
+              if (sn >= 32) {
+                ls_flush<DIRECT>(s, W, 32, lane, cap);
+                __syncwarp();
+                LsRec tr{};
+                if (lane < sn - 32) tr = W.st[32 + lane];
+                __syncwarp();
+                if (lane < sn - 32) W.st[lane] = tr;
+                sn -= 32;
+              }
+              __syncwarp();
             }
-            row += q32; col += r32;
-            if (col >= L) { col -= L; ++row; }
-            ls_push(s, W, pre, a, b, om + cell - lo, qn, pn, lane, lt);
           }
-          fc = hi;
-        } else {
-          // several modules: every lane finds the module of its cell in the cached window
-          for (int f0 = fc; f0 < end; f0 += 32) {
-            const int f = f0 + lane;
-            bool pre = false;
-            int a = 0, b = 0;
-            if (f < end) {
-              int k = 0;
-#pragma unroll
-              for (int step = MD_WIN / 2; step > 0; step >>= 1)
-                if (W.w_off[k + step] <= f) k += step;
-              const int L = W.w_L[k], co = W.w_co[k];
-              int row, col;
-              divmod_small(f - W.w_off[k], L, row, col);
-              a = W.w_a0[k] + row;
-              b = (co + L <= cand_cap) ? __ldg(cand + co + col) : cand_walk(s, geo, mW + k, col);
-              pre = ls_prefilter(__ldg(mpos + a), __ldg(maux + a), __ldg(mpos + b), __ldg(maux + b));
-            }
-            ls_push(s, W, pre, a, b, f - lo, qn, pn, lane, lt);
-          }
-          fc = end;
-          mW += MD_WIN;          // off[mW + MD_WIN] <= fc: the owner of cell fc is at or after it
         }
       }
-      if (qn) pn = ls_drain(s, W, qn, pn, lane, lt);
-      __syncwarp();
     }
-    if (!CHAIN) {
-      int soff = 0;
-      if (lane == 0) { soff = pn ? atomicAdd(s.cnt + LST_CNT_FILL_LS, pn) : 0; s.ls_link_cnt[link] = pn; s.ls_link_soff[link] = soff; }
-      soff = __shfl_sync(0xffffffffu, soff, 0);
-      for (int i = lane; i < pn; i += 32)
-        if (soff + i < cap) { LsRec r; r.a = W.p_a[i]; r.b = W.p_b[i]; r.lf = (link << LS_LP_BITS) | W.p_f[i]; r.c = W.p_c[i]; s.ls_rec[soff + i] = r; }
-      __syncwarp();
-      continue;
-    }
-    const int base = chain_exclusive(s.chain_ls, link, pn, lane, epoch);
-    for (int i = lane; i < pn; i += 32)
-      if (base + i < cap) { s.ls_ab[base + i] = make_int2(W.p_a[i], W.p_b[i]); s.ls_c[base + i] = W.p_c[i]; }
-    // LSs whose inner MD is a = [ls_start[a], ls_start[a+1]): the link owns the rows that start in its range
-    int sr = 0;
-    if (lane < 2) sr = first_row_at(s, off, M, lane == 0 ? lo : lo + LS_LP);
-    const int aLo = __shfl_sync(0xffffffffu, sr, 0), aHi = __shfl_sync(0xffffffffu, sr, 1);
-    for (int a = aLo + lane; a < aHi; a += 32) {
-      const int m = s.md_modt[a] >> 2;
-      const int rel = off[m] + (a - mds[m]) * s.ls_L[m] - lo;
-      s.ls_start[a] = min(base + lower_bound_s(W.p_f, pn, rel), cap);
-    }
-    if (link == n_links - 1 && lane == 0) {
-      const int total = base + pn;
-      s.ls_start[mds[M]] = min(total, cap);
-      s.cnt[LST_CNT_LS] = min(total, cap);
-      s.cnt[LST_CNT_RAW_LS] = total;
-    }
+  }
+  if (qn) { sn = ls_drain<DIRECT>(s, W, qn, sn, lane, lt, carry_row, carry_n); __syncwarp(); }
+  if (sn >= 32) {
+    ls_flush<DIRECT>(s, W, 32, lane, cap);
+    __syncwarp();
+    LsRec tr{};
+    if (lane < sn - 32) tr = W.st[32 + lane];
+    __syncwarp();
+    if (lane < sn - 32) W.st[lane] = tr;
+    sn -= 32;
     __syncwarp();
   }
+  if (sn) ls_flush<DIRECT>(s, W, sn, lane, cap);
 }
 
-// a2 finalize: one thread per record; one thread per MD row for ls_start
-__global__ void __launch_bounds__(256) k_ls_final(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+// a2 scatter (ls_start holds the exclusive scan of the per-row counts by now): record -> ls_start[a] + seq
+__global__ void __launch_bounds__(256) k_ls_scatter(const Slot* __restrict__ slots, Caps caps) {
   const Slot& s = slots[blockIdx.y];
   if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) return;
-  const int M = geo.n_modules;
-  const int* __restrict__ off = s.ls_off;
-  const int* __restrict__ mds = s.md_start;
-  const int* __restrict__ base = s.ls_link_cnt;
-  const int* __restrict__ soff = s.ls_link_soff;
   const int n_rec = min(s.cnt[LST_CNT_FILL_LS], caps.max_ls);
   LST_FOR_ITEMS(j, n_rec) {
     const LsRec r = s.ls_rec[j];
-    const int link = r.lf >> LS_LP_BITS;
-    const int pos = base[link] + (j - soff[link]);
+    const int pos = s.ls_start[r.a] + r.seq;
     s.ls_ab[pos] = make_int2(r.a, r.b);
     s.ls_c[pos] = r.c;
-  }
-  const int total_cells = min(off[M], MAX_CELLS);
-  const int n_md = mds[M];
-  LST_FOR_ITEMS(a, n_md + 1) {
-    int x = total_cells;
-    if (a < n_md) { const int m = s.md_modt[a] >> 2; x = min(off[m] + (a - mds[m]) * s.ls_L[m], total_cells); }
-    const int link = x >> LS_LP_BITS, rel = x - (link << LS_LP_BITS);
-    const int b = base[link], pn = base[link + 1] - b;
-    const LsRec* __restrict__ rec = s.ls_rec + soff[link];
-    int l = 0, h = pn;
-    while (l < h) { const int mid = (l + h) >> 1; if ((rec[mid].lf & (LS_LP - 1)) < rel) l = mid + 1; else h = mid; }
-    s.ls_start[a] = b + l;
   }
 }
 
