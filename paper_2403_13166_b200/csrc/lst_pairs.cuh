@@ -27,8 +27,10 @@ namespace lst {
 
 constexpr int PAIR_WARPS = 4;        // warps per block
 constexpr int Q_CAP = 64;            // survivor queue / record staging per warp (drained / flushed at >= 32)
-constexpr int LS_ROWS = 8;           // consecutive MD rows a warp takes at a time
 constexpr int RUN_CAP = 32;          // runs of a CSR row cached per warp at a time
+constexpr int LS_ROWS = 8;           // consecutive MD rows a warp takes at a time
+constexpr int LS_BC = 4;             // sweeps of a module whose column -> MD mapping a lane keeps in registers
+constexpr int MD_BIG = 1 << 20;      // modules with more cells than this are swept alone (64-bit sweep counter)
 
 __device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
@@ -57,6 +59,7 @@ __device__ __forceinline__ int row_sequence(int row, bool pass, unsigned mask, u
 // a1: row = module m; cells = (lower hit i, upper hit j), i-major
 // ------------------------------------------------------------------------------------------------
 struct MdWarp {   // per-warp shared memory
+  int P[33]; int4 par[32]; float inv[32];     // non-empty modules of the warp's current group: first flat cell, (lb, ub, n_up, mtm), 1/n_up
   int q_lo[Q_CAP], q_up[Q_CAP], q_mt[Q_CAP];
   MdRec st[Q_CAP];
 };
@@ -111,6 +114,37 @@ __device__ __forceinline__ int md_drain(const Slot& s, MdWarp& W, int n, int sn,
   return sn + __popc(mask);
 }
 
+// queue the prefilter survivors of one sweep (in lane order); a full warp of queued cells is evaluated at once and full
+// warps of records are flushed
+template <bool DIRECT>
+__device__ __forceinline__ void md_push(const Slot& s, MdWarp& W, bool pre, int p_lo, int p_up, int mtm, int& qn, int& sn, int lane,
+                                        unsigned lt, int& carry_row, int& carry_n, int cap) {
+  const unsigned mask = __ballot_sync(0xffffffffu, pre);
+  if (!mask) return;
+  if (pre) { const int q = qn + __popc(mask & lt); W.q_lo[q] = p_lo; W.q_up[q] = p_up; W.q_mt[q] = mtm; }
+  qn += __popc(mask);
+  __syncwarp();
+  if (qn < 32) return;
+  sn = md_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
+  __syncwarp();
+  const int rest = qn - 32;
+  int a = 0, b = 0, c = 0;
+  if (lane < rest) { a = W.q_lo[32 + lane]; b = W.q_up[32 + lane]; c = W.q_mt[32 + lane]; }
+  __syncwarp();
+  if (lane < rest) { W.q_lo[lane] = a; W.q_up[lane] = b; W.q_mt[lane] = c; }
+  qn = rest;
+  if (sn >= 32) {
+    md_flush<DIRECT>(s, W, 32, lane, cap);
+    __syncwarp();
+    MdRec t{};
+    if (lane < sn - 32) t = W.st[32 + lane];
+    __syncwarp();
+    if (lane < sn - 32) W.st[lane] = t;
+    sn -= 32;
+  }
+  __syncwarp();
+}
+
 template <bool DIRECT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   __shared__ MdWarp Wall[PAIR_WARPS];
@@ -125,63 +159,72 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __rest
   const int cap = caps.max_md;
   const int n_warps = gridDim.x * PAIR_WARPS;
   int qn = 0, sn = 0, carry_row = -1, carry_n = 0;
-  // modules are interleaved over the warps (heavy inner-layer modules have consecutive ids); a warp fetches the ranges of
-  // its next 32 modules with one round of loads
+  // modules are interleaved over the warps (heavy inner-layer modules have consecutive ids).  A warp takes 32 of its modules
+  // at a time (one round of range loads) and sweeps their cells as ONE flat index space, 32 cells per step: most modules
+  // hold fewer than 32 cells, so per-module sweeps would leave most lanes idle.
   const int wid = blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5);
   for (int mb = wid; mb < M; mb += n_warps * 32) {
     const int my_m = mb + lane * n_warps;
-    int my_lb = 0, my_ub = 0, my_ue = 0, my_mt = 0;
+    int lb = 0, ub = 0, ue = 0, mt = 0;
     if (my_m < M) {
-      my_lb = ss[2 * my_m]; my_ub = ss[2 * my_m + 1]; my_ue = ss[2 * my_m + 2]; my_mt = geo.modt[my_m];
+      lb = ss[2 * my_m]; ub = ss[2 * my_m + 1]; ue = ss[2 * my_m + 2]; mt = geo.modt[my_m];
       if (!DIRECT) s.md_start[my_m] = 0;
     }
+    const int n_lo = ub - lb, n_up = ue - ub;
+    const long long cells64 = (long long)n_lo * n_up;
+    const bool big = cells64 > MD_BIG;
+    const int cells = big ? 0 : (int)cells64;
+    int inc = cells;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+    const int total = __shfl_sync(0xffffffffu, inc, 31);
+    const unsigned nz = __ballot_sync(0xffffffffu, cells > 0);
     __syncwarp();
-    unsigned todo = __ballot_sync(0xffffffffu, my_ub > my_lb && my_ue > my_ub);
+    W.P[lane + 1] = total;                       // padding: the search never runs past the last non-empty module
+    __syncwarp();
+    if (cells > 0) {
+      const int i = __popc(nz & lt);
+      W.P[i] = inc - cells; W.par[i] = make_int4(lb, ub, n_up, (my_m << 2) | mt); W.inv[i] = rcp_fast((float)n_up);
+    }
+    __syncwarp();
+    for (int F = 0; F < total; F += 32) {
+      const int f = min(F + lane, total - 1);
+      int k = 0;
+#pragma unroll
+      for (int step = 16; step > 0; step >>= 1)
+        if (W.P[k + step] <= f) k += step;
+      const int4 pr = W.par[k];
+      const int loc = f - W.P[k];
+      int i = (int)(((float)loc + 0.5f) * W.inv[k]);
+      int j = loc - i * pr.z;
+      if (j < 0) { --i; j += pr.z; } else if (j >= pr.z) { ++i; j -= pr.z; }
+      const int p_lo = pr.x + i, p_up = pr.y + j;
+      const float4 h1 = __ldg(hit + p_lo), h2 = __ldg(hit + p_up);
+      const bool pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, pr.w & 3) && (F + lane < total);
+      md_push<DIRECT>(s, W, pre, p_lo, p_up, pr.w, qn, sn, lane, lt, carry_row, carry_n, cap);
+    }
+    // modules too large for the flat space (only in pathological events): alone, (i, j) advanced incrementally
+    unsigned todo = __ballot_sync(0xffffffffu, big);
     while (todo) {
-      const int k = __ffs(todo) - 1;
+      const int kk = __ffs(todo) - 1;
       todo &= todo - 1;
-      const int lb = __shfl_sync(0xffffffffu, my_lb, k), ub = __shfl_sync(0xffffffffu, my_ub, k), ue = __shfl_sync(0xffffffffu, my_ue, k);
-      const int mtm = ((mb + k * n_warps) << 2) | __shfl_sync(0xffffffffu, my_mt, k);
-      const int n_lo = ub - lb, n_up = ue - ub;
+      const int blb = __shfl_sync(0xffffffffu, lb, kk), bub = __shfl_sync(0xffffffffu, ub, kk), bue = __shfl_sync(0xffffffffu, ue, kk);
+      const int mtm = ((mb + kk * n_warps) << 2) | __shfl_sync(0xffffffffu, mt, kk);
+      const int bn_lo = bub - blb, bn_up = bue - bub;
       int i, j, q32, r32;                       // the lane's cell (i, j); 32 cells further = (+q32, +r32)
-      divmod_small(lane, n_up, i, j);
-      divmod_small(32, n_up, q32, r32);
-      const long long n_sweeps = ((long long)n_lo * n_up + 31) >> 5;
+      divmod_small(lane, bn_up, i, j);
+      divmod_small(32, bn_up, q32, r32);
+      const long long n_sweeps = ((long long)bn_lo * bn_up + 31) >> 5;
       for (long long sw = 0; sw < n_sweeps; ++sw) {
         bool pre = false;
-        const int p_lo = lb + i, p_up = ub + j;
-        if (i < n_lo) {
+        const int p_lo = blb + i, p_up = bub + j;
+        if (i < bn_lo) {
           const float4 h1 = __ldg(hit + p_lo), h2 = __ldg(hit + p_up);
           pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3);
         }
         i += q32; j += r32;
-        if (j >= n_up) { j -= n_up; ++i; }
-        const unsigned mask = __ballot_sync(0xffffffffu, pre);
-        if (mask) {
-          if (pre) { const int q = qn + __popc(mask & lt); W.q_lo[q] = p_lo; W.q_up[q] = p_up; W.q_mt[q] = mtm; }
-          qn += __popc(mask);
-          __syncwarp();
-          if (qn >= 32) {
-            sn = md_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
-            __syncwarp();
-            const int rest = qn - 32;
-            int a = 0, b = 0, c = 0;
-            if (lane < rest) { a = W.q_lo[32 + lane]; b = W.q_up[32 + lane]; c = W.q_mt[32 + lane]; }
-            __syncwarp();
-            if (lane < rest) { W.q_lo[lane] = a; W.q_up[lane] = b; W.q_mt[lane] = c; }
-            qn = rest;
-            if (sn >= 32) {
-              md_flush<DIRECT>(s, W, 32, lane, cap);
-              __syncwarp();
-              MdRec t{};
-              if (lane < sn - 32) t = W.st[32 + lane];
-              __syncwarp();
-              if (lane < sn - 32) W.st[lane] = t;
-              sn -= 32;
-            }
-            __syncwarp();
-          }
-        }
+        if (j >= bn_up) { j -= bn_up; ++i; }
+        md_push<DIRECT>(s, W, pre, p_lo, p_up, mtm, qn, sn, lane, lt, carry_row, carry_n, cap);
       }
     }
   }
@@ -271,10 +314,48 @@ __device__ __forceinline__ int ls_load_runs(const Geo& geo, const int* __restric
   const unsigned nz = __ballot_sync(0xffffffffu, n > 0);
   const int total = __shfl_sync(0xffffffffu, inc, 31);
   __syncwarp();
+  W.r_off[lane + 1] = total;                    // padding for the search
+  __syncwarp();
   if (n > 0) { const int i = __popc(nz & lt); W.r_off[i] = inc - n; W.r_b0[i] = b0; }
-  if (lane == 0) W.r_off[__popc(nz)] = total;
   __syncwarp();
   return total;
+}
+// column t of the run table -> MD index
+__device__ __forceinline__ int ls_column(const LsWarp& W, int t) {
+  int r = 0;
+#pragma unroll
+  for (int step = RUN_CAP / 2; step > 0; step >>= 1)
+    if (W.r_off[r + step] <= t) r += step;
+  return W.r_b0[r] + (t - W.r_off[r]);
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int a, int b, int& qn, int& sn, int lane, unsigned lt,
+                                        int& carry_row, int& carry_n, int cap) {
+  const unsigned mask = __ballot_sync(0xffffffffu, pre);
+  if (!mask) return;
+  if (pre) { const int q = qn + __popc(mask & lt); W.q_a[q] = a; W.q_b[q] = b; }
+  qn += __popc(mask);
+  __syncwarp();
+  if (qn < 32) return;
+  sn = ls_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
+  __syncwarp();
+  const int rest = qn - 32;
+  int x = 0, y = 0;
+  if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; }
+  __syncwarp();
+  if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; }
+  qn = rest;
+  if (sn >= 32) {
+    ls_flush<DIRECT>(s, W, 32, lane, cap);
+    __syncwarp();
+    LsRec tr{};
+    if (lane < sn - 32) tr = W.st[32 + lane];
+    __syncwarp();
+    if (lane < sn - 32) W.st[lane] = tr;
+    sn -= 32;
+  }
+  __syncwarp();
 }
 
 template <bool DIRECT>
@@ -297,50 +378,42 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __rest
     if (!DIRECT && a0 + lane < a1) s.ls_start[a0 + lane] = 0;
     __syncwarp();
     int cur_m = -1, L = 0, e0 = 0, e1 = 0;
+    int bc[LS_BC];                              // the lane's columns of the first LS_BC sweeps of the current module
+    float4 Ap = __ldg(mpos + a0), Aa = __ldg(maux + a0);
+    int m = s.md_modt[a0] >> 2;
     for (int a = a0; a < a1; ++a) {
-      const int m = s.md_modt[a] >> 2;
       if (m != cur_m) {
         cur_m = m;
         e0 = geo.run_ptr[m]; e1 = geo.run_ptr[m + 1];
-        if (e1 - e0 <= RUN_CAP) L = ls_load_runs(geo, mds, W, e0, e1, lane, lt);
+        if (e1 - e0 <= RUN_CAP) {
+          L = ls_load_runs(geo, mds, W, e0, e1, lane, lt);
+#pragma unroll
+          for (int j = 0; j < LS_BC; ++j) bc[j] = (32 * j < L) ? ls_column(W, min(32 * j + lane, L - 1)) : 0;
+        }
       }
-      const float4 Ap = __ldg(mpos + a), Aa = __ldg(maux + a);
-      const float kinvA = -2.0f * Aa.w;
+      const float4 Apc = Ap, Aac = Aa;
+      if (a + 1 < a1) { Ap = __ldg(mpos + a + 1); Aa = __ldg(maux + a + 1); m = s.md_modt[a + 1] >> 2; }     // next row, ahead of use
+      const float kinvA = -2.0f * Aac.w;
       for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
-        if (e1 - e0 > RUN_CAP) L = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
-        int r = 0;
-        for (int t0 = 0; t0 < L; t0 += 32) {
-          const int t = min(t0 + lane, L - 1);
-          while (t >= W.r_off[r + 1]) ++r;
-          const int b = W.r_b0[r] + (t - W.r_off[r]);
-          const float4 Bp = __ldg(mpos + b), Ba = __ldg(maux + b);
-          const bool pre = ls_prefilter(Ap, Aa, kinvA, Bp, Ba) && (t0 + lane < L);
-          const unsigned mask = __ballot_sync(0xffffffffu, pre);
-          if (mask) {
-            if (pre) { const int q = qn + __popc(mask & lt); W.q_a[q] = a; W.q_b[q] = b; }
-            qn += __popc(mask);
-            __syncwarp();
-            if (qn >= 32) {
-              sn = ls_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
-              __syncwarp();
-              const int rest = qn - 32;
-              int x = 0, y = 0;
-              if (lane < rest) { x = W.q_a[32 + lane]; y = W.q_b[32 + lane]; }
-              __syncwarp();
-              if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; }
-              qn = rest;
-              if (sn >= 32) {
-                ls_flush<DIRECT>(s, W, 32, lane, cap);
-                __syncwarp();
-                LsRec tr{};
-                if (lane < sn - 32) tr = W.st[32 + lane];
-                __syncwarp();
-                if (lane < sn - 32) W.st[lane] = tr;
-                sn -= 32;
-              }
-              __syncwarp();
-            }
+        const bool one_pass = e1 - e0 <= RUN_CAP;
+        if (!one_pass) L = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
+#pragma unroll
+        for (int j = 0; j < LS_BC; j += 2) {       // two sweeps in flight: their loads and prefilter chains are independent
+          if (32 * j < L) {
+            const bool two = 32 * (j + 1) < L;
+            const int b0 = one_pass ? bc[j] : ls_column(W, min(32 * j + lane, L - 1));
+            const int b1 = two ? (one_pass ? bc[j + 1] : ls_column(W, min(32 * (j + 1) + lane, L - 1))) : b0;
+            const float4 Bp0 = __ldg(mpos + b0), Ba0 = __ldg(maux + b0), Bp1 = __ldg(mpos + b1), Ba1 = __ldg(maux + b1);
+            const bool pre0 = ls_prefilter(Apc, Aac, kinvA, Bp0, Ba0) && (32 * j + lane < L);
+            const bool pre1 = ls_prefilter(Apc, Aac, kinvA, Bp1, Ba1) && (32 * (j + 1) + lane < L);
+            ls_push<DIRECT>(s, W, pre0, a, b0, qn, sn, lane, lt, carry_row, carry_n, cap);
+            ls_push<DIRECT>(s, W, pre1, a, b1, qn, sn, lane, lt, carry_row, carry_n, cap);
           }
+        }
+        for (int t0 = 32 * LS_BC; t0 < L; t0 += 32) {
+          const int b = ls_column(W, min(t0 + lane, L - 1));
+          const bool pre = ls_prefilter(Apc, Aac, kinvA, __ldg(mpos + b), __ldg(maux + b)) && (t0 + lane < L);
+          ls_push<DIRECT>(s, W, pre, a, b, qn, sn, lane, lt, carry_row, carry_n, cap);
         }
       }
     }
