@@ -21,8 +21,11 @@ struct lst_ctx {
   char* zero_base = nullptr; size_t zero_stride = 0;
   char* ones_base = nullptr; size_t ones_stride = 0;
   bool sticky_cuda_error = false;
+  bool capturing = false;         // run_sequence is being recorded into a graph
   bool use_graphs = true;         // replay lst_run_batch as a CUDA graph on capturable streams (LST_GRAPHS=0 disables)
   std::map<long long, cudaGraphExec_t> graphs;   // (first_slot, n) -> instantiated launch sequence
+  cudaStream_t side = nullptr;                   // capture-time side branch (pLS binning runs beside a0..a5)
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 namespace {
@@ -143,7 +146,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls);
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
-    t.chi3 = cv.take<float>(k.max_t3); t.key5 = cv.take<unsigned long long>(k.max_t5); t.key3 = cv.take<unsigned long long>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
+    t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
@@ -160,7 +163,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 25;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 19;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -229,6 +232,14 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   if (e == cudaSuccess) e = cudaDeviceSynchronize();       // the memsets above are asynchronous on device memory
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
   if (const char* g = std::getenv("LST_GRAPHS")) c->use_graphs = !(g[0] == '0');
+  if (c->use_graphs) {            // host-side objects only; without them the binning simply stays in line
+    if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess) c->side = nullptr;
+    if (c->side && (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                    cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess)) {
+      cudaStreamDestroy(c->side); c->side = nullptr;
+    }
+    (void)cudaGetLastError();
+  }
   c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
   c->geo.run_ptr = L.run_ptr; c->geo.run_c0 = L.run_c0; c->geo.run_c1 = L.run_c1;
   *out = c;
@@ -292,30 +303,33 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   if (gx > 592) gx = 592;
   const dim3 G(gx, n), G1(1, n), GL(2 * gx, n);   // GL: the 128-thread link kernels
   const dim3 GS(gx < 16 ? gx : 16, n);            // look-back scans: tiles of 2048 entries by ticket
+  // the pLS binning depends on the inputs only: under stream capture it becomes a side branch of the graph
+  const bool fork = c->capturing && c->side;
+  if (fork) {
+    if (bad(c, cudaEventRecord(c->ev_fork, st)) || bad(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0))) return LST_ECUDA;
+    k_pls_bin<<<G1, 1024, 0, c->side>>>(sl);
+    if (bad(c, cudaEventRecord(c->ev_join, c->side))) return LST_ECUDA;
+  }
   k_hist<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_scan_lb<SCAN_SENSOR><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
   k_scatter<<<G, 256, 0, st>>>(sl, g); LST_MARK();
   k_rank<<<G, 256, 0, st>>>(sl); LST_MARK();
-  k_md_sweep<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
+  k_md_sweep<<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_scan_lb<SCAN_MDROW><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
-  k_md_scatter<<<G, 256, 0, st>>>(sl, k); LST_MARK();
-  k_md_sweep<true><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run (returns at once otherwise)
-  k_ls_sweep<false><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
+  k_md_finish<<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
+  k_ls_sweep<<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_scan_lb<SCAN_LSROW><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
-  k_ls_scatter<<<G, 256, 0, st>>>(sl, k); LST_MARK();
-  k_ls_sweep<true><<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();     // overflow re-run
+  k_ls_finish<<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_t3_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
-  k_t3_start<<<G, 256, 0, st>>>(sl); LST_MARK();
   k_t5_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
   k_scan_lb<SCAN_T5><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
-  k_pls_bin<false><<<G1, 1024, 0, st>>>(sl); LST_MARK();
-  k_match<5, false><<<GL, 128, 0, st>>>(sl); LST_MARK();
-  k_win<false><<<G, 256, 0, st>>>(sl); LST_MARK();
+  if (fork) { if (bad(c, cudaStreamWaitEvent(st, c->ev_join, 0))) return LST_ECUDA; }
+  else k_pls_bin<<<G1, 1024, 0, st>>>(sl);
+  LST_MARK();
+  k_match<5, false><<<G, MATCH_WARPS * 32, 0, st>>>(sl); LST_MARK();
   k_pt5_lists<<<G, 128, 0, st>>>(sl); LST_MARK();
-  k_pls_bin<true><<<G1, 1024, 0, st>>>(sl); LST_MARK();
-  k_match<3, true><<<GL, 128, 0, st>>>(sl); LST_MARK();
-  k_win<true><<<G, 256, 0, st>>>(sl); LST_MARK();
+  k_match<3, true><<<G, MATCH_WARPS * 32, 0, st>>>(sl); LST_MARK();
   k_tc_emit<<<G1, 1024, 0, st>>>(sl, k); LST_MARK();
 #undef LST_MARK
   if (li != N_LAUNCHES + 2) return LST_EINVAL;
@@ -334,7 +348,9 @@ int lst_run_batch(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
     if (it == c->graphs.end()) {
       cudaGraphExec_t exec = nullptr;
       if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        c->capturing = true;
         const int rc = run_sequence(c, first, n, st, nullptr);
+        c->capturing = false;
         cudaGraph_t graph = nullptr;
         const cudaError_t e = cudaStreamEndCapture(st, &graph);
         if (rc == LST_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) exec = nullptr;
@@ -370,8 +386,8 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
-      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_sweep", "a1.scan", "a1.md_scatter", "a1.md_rerun", "a2.ls_sweep", "a2.scan", "a2.ls_scatter", "a2.ls_rerun", "a3.t3", "a3.t3_start", "a4.t5", "a5.dnn",
-      "a5.scan", "a6.pls_bin", "a6.match5", "a6.win5", "a6.pt5_lists", "a6.pls_rebin", "a6.match3", "a6.win3", "a6.tc_emit"};
+      "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_sweep", "a1.scan", "a1.md_finish", "a2.ls_sweep", "a2.scan", "a2.ls_finish",
+      "a3.t3", "a4.t5", "a5.dnn", "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 
@@ -459,6 +475,9 @@ int lst_read_tc_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out,
 void lst_destroy(lst_ctx* c) {
   if (!c) return;
   for (auto& kv : c->graphs) cudaGraphExecDestroy(kv.second);
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
+  if (c->side) cudaStreamDestroy(c->side);
   delete c;
 }
 

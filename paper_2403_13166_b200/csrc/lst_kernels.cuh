@@ -65,7 +65,6 @@ struct Slot {
   // a6
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_bin_start;
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
-  unsigned long long* key5; unsigned long long* key3;   // argmin (chi2, pLS) per T5 / T3
   // host-load staging
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
   int* tc_hdr;                       // copy of cnt[] in front of the TC rows, so one D2H copy reads both
@@ -336,10 +335,8 @@ __device__ __forceinline__ int psi_bin_raw(float ang) {   // unbounded bin index
   return (int)floorf((ang + LST_PI_F) * (PLS_NB / (2.0f * LST_PI_F)));
 }
 
-// one block per event: derive, histogram, scan, scatter (all in shared memory; ~2.6k pLS per event).
-// SECOND = false: all pLS, for the T5 pass.  SECOND = true (after the pT5 are known): only the pLS without a pT5
-// are binned again for the T3 pass, and the T3s contained in a pT5 are marked used (best3 = -2).
-template <bool SECOND>
+// one block per event: derive, histogram, scan, scatter (all in shared memory; ~2.6k pLS per event).  Depends only on
+// the event's inputs, so lst_run puts it on a side branch of the launch graph, off the critical path.
 __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots) {
   __shared__ int hist[PLS_NBINS + 1];
   __shared__ int sm[34];
@@ -347,49 +344,23 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int n = s.n_pls;
   for (int i = tid; i <= PLS_NBINS; i += 1024) hist[i] = 0;
-  {   // argmin keys of the pass that follows start empty
-    unsigned long long* key = SECOND ? s.key3 : s.key5;
-    const int nk = SECOND ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
-    for (int i = tid; i < nk; i += 1024) key[i] = WIN_EMPTY;
-  }
-  if (SECOND) {   // used iff {a,b,c} is contained in the five MDs of some pT5: walk the pT5 entries that contain a
-    const int n_t3 = s.cnt[LST_CNT_T3];
-    for (int t = tid; t < n_t3; t += 1024) {
-      const int4 abc = s.t3_abc[t];
-      bool used = false;
-      for (int e = s.md_head[abc.x]; e >= 0 && !used; e = s.pt5_next[e]) {
-        const int pp = e / 5;
-        const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(s.win5[pp] & 0xFFFFFFFFull)];
-        int found = 0;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) found += (m5[q] == abc.y) + (m5[q] == abc.z);
-        used = (found == 2);
-      }
-      s.best3[t] = used ? -2 : -1;
-    }
-  }
   __syncthreads();
   for (int p = tid; p < n; p += 1024) {
-    int key = -1;
-    if (!SECOND) {
-      const int q = (int)s.in_q[p];
-      const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
-      s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
-      s.pls_b[p] = make_float2(d.sec, d.z0);
-      int kb = PLS_K, pb = 0;
-      if (d.h < LST_PLS_HMAX && (q == 1 || q == -1)) {
-        kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
-        pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
-      }
-      key = kb * PLS_NB + pb;
-      s.pls_key[p] = key;
-    } else if (s.win5[p] == WIN_EMPTY) {
-      key = s.pls_key[p];
+    const int q = (int)s.in_q[p];
+    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
+    s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
+    s.pls_b[p] = make_float2(d.sec, d.z0);
+    int kb = PLS_K, pb = 0;
+    if (d.h < LST_PLS_HMAX && (q == 1 || q == -1)) {
+      kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
+      pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
     }
-    if (key >= 0) atomicAdd(&hist[key], 1);
+    const int key = kb * PLS_NB + pb;
+    s.pls_key[p] = key;
+    atomicAdd(&hist[key], 1);
   }
   __syncthreads();
-  // exclusive scan of hist[0..PLS_NBINS] (3 items per thread)
+  // exclusive scan of hist[0..PLS_NBINS] (5 items per thread)
   constexpr int IT = (PLS_NBINS + 1 + 1023) / 1024;
   int v[IT], tsum = 0;
 #pragma unroll
@@ -415,7 +386,6 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
   }
   __syncthreads();
   for (int p = tid; p < n; p += 1024) {
-    if (SECOND && s.win5[p] != WIN_EMPTY) continue;
     const int pos = atomicAdd(&hist[s.pls_key[p]], 1);   // order inside a bucket is free: argmin ties break on p
     s.pls_sa[pos] = s.pls_a[p];
     s.pls_sb[pos] = s.pls_b[p];
@@ -427,101 +397,192 @@ __device__ __forceinline__ unsigned long long win_key(float chi2, int idx) {
   return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned)idx;   // chi2 >= 0: bit order = value order
 }
 
-// match objects with NA anchors against the pLS buckets their first anchor can reach.  One thread per (object,
-// h-bucket): the 32 lanes of a warp hold 32 consecutive objects and the SAME h-bucket, so the window arithmetic
-// is uniform and the bucket loops have similar lengths.  Every matching pLS is folded into the object's key with
-// a 64-bit atomicMin on (chi2 bits, p): argmin over (chi2, p), independent of the visiting order.
+// Match objects with NA anchors against the pLS buckets their first anchor can reach, and reduce to the winners.
+// One thread per object (T5 of the T5 list / T3); it visits the nine h-buckets in turn (so all lanes of a warp are in the
+// same h-bucket: uniform window arithmetic, similar loop lengths) and applies the cheap transverse test of the first
+// anchor to every pLS of its windows.  Survivors are queued per warp, and whenever 32 are queued the warp evaluates them
+// densely: first the full test of the first anchor, then -- queued again -- the remaining anchors.  The object's best
+// match is argmin over (chi2, p), kept as a 64-bit key in shared memory (independent of the visiting order); when the
+// object is done its thread folds it into the pLS's winner with a 64-bit atomicMin on (chi2, object): argmin over
+// (chi2, object) among the objects whose best pLS it is (SPEC.md 4.6).  T3 pass: T3s contained in a pT5 are skipped
+// (walk of the pT5 entries that hold the T3's first MD), and so are pLS that own a pT5.
+constexpr int MATCH_WARPS = 4, MQ_CAP = 64;
+struct MatchWarp {
+  unsigned long long key[32];                    // best (chi2, p) per lane's object
+  int o_md[32][5];                               // the objects' MDs
+  int q1_o[MQ_CAP], q1_j[MQ_CAP];                // queue 1: (lane of the object, sorted pLS index) passing the transverse test
+  int q2_o[MQ_CAP], q2_j[MQ_CAP]; float q2_c[MQ_CAP];     // queue 2: first anchor fully passed; chi2 so far
+};
+
 template <int NA, bool IS_T3>
-__global__ void __launch_bounds__(128) k_match(const Slot* __restrict__ slots) {
-  const Slot& s = slots[blockIdx.y];
-  const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
-  const int n_pad = (n + 31) & ~31;
-  const int* __restrict__ bstart = s.pls_bin_start;
-  unsigned long long* __restrict__ keys = IS_T3 ? s.key3 : s.key5;
-  int n_tests = 0, n_cand = 0;
-  LST_FOR_ITEMS(item, n_pad * (PLS_K + 1)) {
-    const int kb = item / n_pad, t = item - kb * n_pad;
-    if (t >= n) continue;
-    if (bstart[(kb + 1) * PLS_NB] == bstart[kb * PLS_NB]) continue;      // empty h-bucket (uniform over the warp)
-    int md[NA];
-    if (IS_T3) {
-      if (s.best3[t] == -2) continue;                                    // contained in a pT5
-      const int4 abc = s.t3_abc[t];
-      md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
-    } else {
-      const int* m5 = s.t5c_md + 5 * s.t5_list[t];
+__device__ __forceinline__ void match_drain2(const Slot& s, MatchWarp& W, int n, int lane) {
+  if (lane < n) {
+    const int o = W.q2_o[lane], j = W.q2_j[lane];
+    float chi = W.q2_c[lane];
+    const float4 pa = s.pls_sa[j];
+    const float2 pb = s.pls_sb[j];
+    Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w; P.sec = pb.x; P.z0 = pb.y;
+    bool ok = true;
 #pragma unroll
-      for (int q = 0; q < NA; ++q) md[q] = m5[q];
-    }
-    const float4 a0 = s.md_pos[md[0]];
-    const int mt0 = s.md_modt[md[0]] & 3;
-    const float r = a0.w;
-    // up to four bucket ranges [rb[i], re[i]) of this h-bucket
-    int rb[4], re[4], nr = 0;
-    const int base = kb * PLS_NB;
-    if (kb == PLS_K) { rb[0] = base; re[0] = base + PLS_NB; nr = 1; }
-    else {
-      const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
-      const float ulo = r * (kb * (LST_PLS_HMAX / PLS_K)), uhi = r * ((kb + 1) * (LST_PLS_HMAX / PLS_K));
-      const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
-      if (clo > 1.0f) continue;                                          // no circle of this curvature reaches r
-      const float phi = atan2f(a0.y, a0.x);
-      const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
-#pragma unroll
-      for (int sgn = 0; sgn < 2; ++sgn) {
-        const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
-        const int blo = psi_bin_raw(lo);
-        const int nb = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
-        const int b0 = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
-        const int e0 = min(b0 + nb, PLS_NB);
-        rb[nr] = base + b0; re[nr] = base + e0; ++nr;
-        if (b0 + nb > PLS_NB) { rb[nr] = base; re[nr] = base + b0 + nb - PLS_NB; ++nr; }
-      }
-    }
-    unsigned long long best = WIN_EMPTY;
-    for (int ir = 0; ir < nr; ++ir) {
-      const int j1 = bstart[re[ir]];
-      for (int j = bstart[rb[ir]]; j < j1; ++j) {
-        const float4 pa = s.pls_sa[j];
-        Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
-        float e, dT;
-        ++n_tests;
-        if (!pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT)) continue;       // transverse test of the first anchor
-        ++n_cand;
-        const float2 pb = s.pls_sb[j];
-        P.sec = pb.x; P.z0 = pb.y;
-        float chi = 0.0f;
-        bool ok = pls_anchor(P, a0, mt0, chi);
-#pragma unroll
-        for (int q = 1; q < NA; ++q)
-          if (ok) ok = pls_anchor(P, s.md_pos[md[q]], s.md_modt[md[q]] & 3, chi);
-        if (!ok) continue;
-        const unsigned long long k = ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j];
-        best = min(best, k);                                            // chi2 >= 0: bit order = value order
-      }
-    }
-    if (best != WIN_EMPTY) atomicMin(keys + t, best);
+    for (int q = 1; q < NA; ++q)
+      if (ok) { const int m = W.o_md[o][q]; ok = pls_anchor(P, s.md_pos[m], s.md_modt[m] & 3, chi); }
+    if (ok) atomicMin(&W.key[o], ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j]);   // chi2 >= 0: bit order = value order
   }
-  // bookkeeping for the roofline accounting: prefilter tests executed / pairs that needed the full test
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) { n_tests += __shfl_xor_sync(0xffffffffu, n_tests, d); n_cand += __shfl_xor_sync(0xffffffffu, n_cand, d); }
-  if ((threadIdx.x & 31) == 0 && n_tests) {
-    atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_TESTS : LST_CNT_M5_TESTS), n_tests);
-    atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_CAND : LST_CNT_M5_CAND), n_cand);
+}
+template <int NA, bool IS_T3>
+__device__ __forceinline__ void match_drain1(const Slot& s, MatchWarp& W, int n, int& q2n, int lane, unsigned lt, int& n_cand) {
+  bool ok = false;
+  int o = 0, j = 0;
+  float chi = 0.0f;
+  if (lane < n) {
+    o = W.q1_o[lane]; j = W.q1_j[lane];
+    ok = !IS_T3 || s.win5[s.pls_sidx[j]] == WIN_EMPTY;             // T3 pass: only pLS without a pT5
+    if (ok) {
+      const float4 pa = s.pls_sa[j];
+      const float2 pb = s.pls_sb[j];
+      Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w; P.sec = pb.x; P.z0 = pb.y;
+      const int m = W.o_md[o][0];
+      ok = pls_anchor(P, s.md_pos[m], s.md_modt[m] & 3, chi);
+    }
+  }
+  n_cand += n;
+  const unsigned mask = __ballot_sync(0xffffffffu, ok);
+  if (ok) { const int i = q2n + __popc(mask & lt); W.q2_o[i] = o; W.q2_j[i] = j; W.q2_c[i] = chi; }
+  q2n += __popc(mask);
+  __syncwarp();
+  if (q2n >= 32) {
+    match_drain2<NA, IS_T3>(s, W, 32, lane);
+    __syncwarp();
+    const int rest = q2n - 32;
+    int a = 0, b = 0; float c = 0.f;
+    if (lane < rest) { a = W.q2_o[32 + lane]; b = W.q2_j[32 + lane]; c = W.q2_c[32 + lane]; }
+    __syncwarp();
+    if (lane < rest) { W.q2_o[lane] = a; W.q2_j[lane] = b; W.q2_c[lane] = c; }
+    q2n = rest;
+    __syncwarp();
   }
 }
 
-// second reduction: winner per pLS = argmin over (chi2, object) among the objects whose best pLS it is
-template <bool IS_T3>
-__global__ void __launch_bounds__(256) k_win(const Slot* __restrict__ slots) {
+template <int NA, bool IS_T3>
+__global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restrict__ slots) {
+  __shared__ MatchWarp Wall[MATCH_WARPS];
   const Slot& s = slots[blockIdx.y];
   const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
-  LST_FOR_ITEMS(t, n) {
-    const unsigned long long k = IS_T3 ? s.key3[t] : s.key5[t];
-    const int best = (k == WIN_EMPTY) ? -1 : (int)(k & 0xFFFFFFFFull);
-    const float chi = (k == WIN_EMPTY) ? 0.0f : __uint_as_float((unsigned)(k >> 32));
-    if (IS_T3) { s.best3[t] = best; s.chi3[t] = chi; if (best >= 0) atomicMin(s.win3 + best, win_key(chi, t)); }
-    else { s.best5[t] = best; s.chi5[t] = chi; if (best >= 0) atomicMin(s.win5 + best, win_key(chi, t)); }
+  const int lane = threadIdx.x & 31;
+  MatchWarp& W = Wall[threadIdx.x >> 5];
+  const unsigned lt = (1u << lane) - 1u;
+  const int* __restrict__ bstart = s.pls_bin_start;
+  const float4* __restrict__ psa = s.pls_sa;
+  int n_tests = 0, n_cand = 0;
+  const int n_warps = gridDim.x * MATCH_WARPS;
+  for (int t0 = (blockIdx.x * MATCH_WARPS + (threadIdx.x >> 5)) * 32; t0 < n; t0 += n_warps * 32) {
+    const int t = t0 + lane;
+    bool act = t < n;
+    int md0 = 0;
+    __syncwarp();
+    W.key[lane] = WIN_EMPTY;
+    if (act) {
+      if (IS_T3) {
+        const int4 abc = s.t3_abc[t];
+        W.o_md[lane][0] = abc.x; W.o_md[lane][1] = abc.y; W.o_md[lane][2] = abc.z;
+        md0 = abc.x;
+        // used iff {a,b,c} is contained in the five MDs of some pT5: walk the pT5 entries that contain a
+        bool used = false;
+        for (int e = s.md_head[abc.x]; e >= 0 && !used; e = s.pt5_next[e]) {
+          const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(s.win5[e / 5] & 0xFFFFFFFFull)];
+          int found = 0;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) found += (m5[q] == abc.y) + (m5[q] == abc.z);
+          used = (found == 2);
+        }
+        if (used) { act = false; s.best3[t] = -2; }
+      } else {
+        const int* m5 = s.t5c_md + 5 * s.t5_list[t];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) W.o_md[lane][q] = m5[q];
+        md0 = m5[0];
+      }
+    }
+    float4 a0 = make_float4(1.f, 0.f, 0.f, 1.f);
+    if (act) a0 = s.md_pos[md0];
+    const float r = a0.w;
+    const float phi = atan2f(a0.y, a0.x);
+    const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
+    int q1n = 0, q2n = 0;
+    __syncwarp();
+    for (int kb = 0; kb <= PLS_K; ++kb) {
+      const int base = kb * PLS_NB;
+      if (bstart[base + PLS_NB] == bstart[base]) continue;               // empty h-bucket (uniform)
+      // up to four index ranges [js, je) of sorted pLS for this object in this h-bucket
+      int js[4] = {0, 0, 0, 0}, len[4] = {0, 0, 0, 0};
+      if (act) {
+        if (kb == PLS_K) { js[0] = bstart[base]; len[0] = bstart[base + PLS_NB] - js[0]; }
+        else {
+          const float ulo = r * (kb * (LST_PLS_HMAX / PLS_K)), uhi = r * ((kb + 1) * (LST_PLS_HMAX / PLS_K));
+          const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
+          if (clo <= 1.0f) {                                             // else no circle of this curvature reaches r
+            const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
+#pragma unroll
+            for (int sgn = 0; sgn < 2; ++sgn) {
+              const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
+              const int blo = psi_bin_raw(lo);
+              const int nb = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
+              const int b0 = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
+              const int e0 = min(b0 + nb, PLS_NB);
+              js[2 * sgn] = bstart[base + b0]; len[2 * sgn] = bstart[base + e0] - js[2 * sgn];
+              if (b0 + nb > PLS_NB) { js[2 * sgn + 1] = bstart[base]; len[2 * sgn + 1] = bstart[base + b0 + nb - PLS_NB] - js[2 * sgn + 1]; }
+            }
+          }
+        }
+      }
+      const int c1 = len[0], c2 = c1 + len[1], c3 = c2 + len[2], total = c3 + len[3];
+      for (int q = 0; __any_sync(0xffffffffu, q < total); ++q) {
+        bool pass = false;
+        int j = 0;
+        if (q < total) {
+          j = q < c1 ? js[0] + q : q < c2 ? js[1] + (q - c1) : q < c3 ? js[2] + (q - c2) : js[3] + (q - c3);
+          const float4 pa = __ldg(psa + j);
+          Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
+          float e, dT;
+          pass = pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT);                 // transverse test of the first anchor
+          ++n_tests;
+        }
+        const unsigned mask = __ballot_sync(0xffffffffu, pass);
+        if (mask) {
+          if (pass) { const int i = q1n + __popc(mask & lt); W.q1_o[i] = lane; W.q1_j[i] = j; }
+          q1n += __popc(mask);
+          __syncwarp();
+          if (q1n >= 32) {
+            match_drain1<NA, IS_T3>(s, W, 32, q2n, lane, lt, n_cand);
+            const int rest = q1n - 32;
+            int a = 0, b = 0;
+            if (lane < rest) { a = W.q1_o[32 + lane]; b = W.q1_j[32 + lane]; }
+            __syncwarp();
+            if (lane < rest) { W.q1_o[lane] = a; W.q1_j[lane] = b; }
+            q1n = rest;
+            __syncwarp();
+          }
+        }
+      }
+    }
+    if (q1n) match_drain1<NA, IS_T3>(s, W, q1n, q2n, lane, lt, n_cand);
+    __syncwarp();
+    if (q2n) match_drain2<NA, IS_T3>(s, W, q2n, lane);
+    __syncwarp();
+    if (act) {
+      const unsigned long long k = W.key[lane];
+      const int best = (k == WIN_EMPTY) ? -1 : (int)(k & 0xFFFFFFFFull);
+      const float chi = (k == WIN_EMPTY) ? 0.0f : __uint_as_float((unsigned)(k >> 32));
+      if (IS_T3) { s.best3[t] = best; s.chi3[t] = chi; if (best >= 0) atomicMin(s.win3 + best, win_key(chi, t)); }
+      else { s.best5[t] = best; s.chi5[t] = chi; if (best >= 0) atomicMin(s.win5 + best, win_key(chi, t)); }
+    }
+  }
+  // bookkeeping for the roofline accounting: first-anchor transverse tests executed / pairs that went on to the full test
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) n_tests += __shfl_xor_sync(0xffffffffu, n_tests, d);
+  if (lane == 0 && n_tests) {
+    atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_TESTS : LST_CNT_M5_TESTS), n_tests);
+    atomicAdd(s.cnt + (IS_T3 ? LST_CNT_M3_CAND : LST_CNT_M5_CAND), n_cand);
   }
 }
 

@@ -18,8 +18,8 @@
 //     ranges: lst_create compresses every CSR row into runs of consecutive module ids (Geo::run_*), and MDs are
 //     stored in module order, so one run = one contiguous slice of md_pos / md_aux.
 // Capacity overflow (more objects than the record buffer holds): the scan flags it, and the DIRECT instantiation
-// of the sweep runs the stage again, writing start[row] + seq in place for positions below the capacity ("first
-// cap objects in build order").  It returns at once unless the overflow bit is set.
+// of the sweep runs the stage again (inside the finish kernel), writing start[row] + seq in place for positions below the
+// capacity ("first cap objects in build order").
 #pragma once
 #include "lst_kernels.cuh"
 
@@ -146,10 +146,7 @@ __device__ __forceinline__ void md_push(const Slot& s, MdWarp& W, bool pre, int 
 }
 
 template <bool DIRECT>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  __shared__ MdWarp Wall[PAIR_WARPS];
-  const Slot& s = slots[blockIdx.y];
-  if (DIRECT && !(s.cnt[CNT_STATUS] & LST_ST_OVF_MD)) return;
+__device__ __forceinline__ void md_sweep_body(const Slot& s, const Geo& geo, const Caps& caps, MdWarp* Wall) {
   const int lane = threadIdx.x & 31;
   MdWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
@@ -242,10 +239,17 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __rest
   if (sn) md_flush<DIRECT>(s, W, sn, lane, cap);
 }
 
-// a1 scatter (md_start holds the exclusive scan of the per-module counts by now): record -> md_start[module] + seq
-__global__ void __launch_bounds__(256) k_md_scatter(const Slot* __restrict__ slots, Caps caps) {
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ MdWarp Wall[PAIR_WARPS];
+  md_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
+}
+
+// a1 finish (md_start holds the exclusive scan of the per-module counts by now): record -> md_start[module] + seq.
+// If the stage overflowed its capacity the record buffer is incomplete: run the sweep again, writing in place.
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ MdWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) return;       // the DIRECT pass rewrites the stage
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) { md_sweep_body<true>(s, geo, caps, Wall); return; }
   const int n_rec = min(s.cnt[LST_CNT_FILL_MD], caps.max_md);
   LST_FOR_ITEMS(j, n_rec) md_emit<false>(s, s.md_rec[j], caps.max_md);
 }
@@ -359,10 +363,7 @@ __device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int 
 }
 
 template <bool DIRECT>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
-  __shared__ LsWarp Wall[PAIR_WARPS];
-  const Slot& s = slots[blockIdx.y];
-  if (DIRECT && !(s.cnt[CNT_STATUS] & LST_ST_OVF_LS)) return;
+__device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, const Caps& caps, LsWarp* Wall) {
   const int lane = threadIdx.x & 31;
   LsWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
@@ -432,10 +433,17 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __rest
   if (sn) ls_flush<DIRECT>(s, W, sn, lane, cap);
 }
 
-// a2 scatter (ls_start holds the exclusive scan of the per-row counts by now): record -> ls_start[a] + seq
-__global__ void __launch_bounds__(256) k_ls_scatter(const Slot* __restrict__ slots, Caps caps) {
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ LsWarp Wall[PAIR_WARPS];
+  ls_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
+}
+
+// a2 finish (ls_start holds the exclusive scan of the per-row counts by now): record -> ls_start[a] + seq; on capacity
+// overflow the sweep runs again, in place
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_finish(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) return;
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) { ls_sweep_body<true>(s, geo, caps, Wall); return; }
   const int n_rec = min(s.cnt[LST_CNT_FILL_LS], caps.max_ls);
   LST_FOR_ITEMS(j, n_rec) {
     const LsRec r = s.ls_rec[j];

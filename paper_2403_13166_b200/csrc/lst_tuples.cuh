@@ -111,12 +111,6 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t3_one(const Slot* __restrict__ s
   }
 }
 
-// T3s whose inner MD is a = [t3_start[a], t3_start[a+1])
-__global__ void __launch_bounds__(256) k_t3_start(const Slot* __restrict__ slots) {
-  const Slot& s = slots[blockIdx.y];
-  LST_FOR_ITEMS(a, s.cnt[LST_CNT_MD] + 1) s.t3_start[a] = s.t3_off[s.ls_start[a]];
-}
-
 // a4 (SPEC.md 4.4): rows = T3 u = (a,b,c); partners = T3s whose inner MD is c; the bridge (b,c,d) must pass
 __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ slots, Caps caps) {
   __shared__ int sm[TUPLE_TPB / 32 + 1];
@@ -126,6 +120,9 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ s
   const int n = s.cnt[LST_CNT_T3];
   const int n_tiles = (n + TUPLE_TPB - 1) / TUPLE_TPB + (n == 0);
   const int cap = caps.max_t5c;
+  // T3s whose inner MD is a = [t3_start[a], t3_start[a+1]) with t3_start[a] = t3_off[ls_start[a]]: the table is an output
+  // (lst_get); this kernel itself goes through t3_off / ls_start so that it need not wait for it
+  LST_FOR_ITEMS(a, s.cnt[LST_CNT_MD] + 1) s.t3_start[a] = s.t3_off[s.ls_start[a]];
   while (true) {
     if (threadIdx.x == 0) s_tile = atomicAdd(s.cnt + LST_CNT_DYN_T5, 1);
     __syncthreads();
@@ -140,7 +137,7 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ s
     Pt B{}, C{};
     if (u < n) {
       abc = s.t3_abc[u];
-      v0 = s.t3_start[abc.z]; v1 = s.t3_start[abc.z + 1];
+      v0 = s.t3_off[s.ls_start[abc.z]]; v1 = s.t3_off[s.ls_start[abc.z + 1]];
       if (v0 < v1) {
         B = make_pt(s.md_pos[abc.y], s.md_modt[abc.y] & 3);
         C = make_pt(s.md_pos[abc.z], s.md_modt[abc.z] & 3);
