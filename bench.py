@@ -7,8 +7,8 @@ Contract (one JSON line on stdout from rank 0):
 
 A "step" = one pass of the whole hot path over one batch of `--events` synthetic PU200 events
 (BASELINE.json configs[2] recipe, the seeds of configs[3]); `value` = events/s with the inputs resident
-in HBM; `e2e` = the same through lst_load_event_host / lst_read_tc_host with pinned HOST buffers, copies
-inside the timed region.  Events are independent, so N GPUs run N replicas on different seeds (weak
+in HBM; `e2e` = the same through lst_load_batch_host / lst_read_tc_hits_batch_host with pinned HOST buffers, copies
+inside the timed region; `single_event` = configs[2] exactly (one event, seed 3); `--config 4` = the occupancy sweep.  Events are independent, so N GPUs run N replicas on different seeds (weak
 scaling, no collective on the data path -- DESIGN.md "Multi-GPU").
 """
 import argparse
@@ -30,8 +30,9 @@ WORKLOAD = "configs[2] HL-LHC PU200 events (6000 particles, 5% inefficiency, 100
 
 # ---- per-unit algorithmic work: un-fused fp32 operations per pair test and
 # compulsory bytes per object; FP32 non-fused peak = 148 SM x 128 lanes x sm_max_mhz.
-FLOPS = dict(md_pair=34, ls_pair=62, t3_pair=86, t5_pair=80, dnn_cand=3584 + 140, match_pair=10, match_full=45)
+FLOPS = dict(md_pair=34, ls_pair=60, t3_pair=86, t5_pair=80, dnn_cand=3584 + 140, match_pair=10, match_full=45)   # ls_pair: SURVEY.md 8.d
 SM_COUNT, LANES = 148, 128
+TC_ROWS = 4096          # TC rows per event read back by the e2e leg (a PU200 event has ~3.3 k)
 
 
 def shard_seeds(rank: int, world: int, n_events: int, base: int = 100):
@@ -151,12 +152,106 @@ def stage_of(name):
     return name.split(".")[0]
 
 
+_CPU_EVENTS = None
+
+
+def _cpu_worker(args):
+    """one oracle process: runs its share of the events, returns (events, seconds)"""
+    idx, reps = args
+    from oracle import lst_oracle as O
+    geo, w, events = _CPU_EVENTS
+    O.run(geo, w, events[idx[0]], counts_only=True)
+    t0 = time.perf_counter()
+    n = 0
+    for _ in range(reps):
+        for i in idx:
+            O.run(geo, w, events[i], counts_only=True)
+            n += 1
+    return n, time.perf_counter() - t0
+
+
+def cpu_baseline(geo, w, events, n_single, budget_s=8.0):
+    """The oracle as it stands on the host cores: one core, all cores (one process per core, different events), and the
+    per-stage split of one event.  Runs BEFORE CUDA is initialised (the workers are forked)."""
+    import multiprocessing as mp
+    from oracle import lst_oracle as O
+    global _CPU_EVENTS
+    O.build()
+    O.run(geo, w, events[0], counts_only=True)
+    t0 = time.perf_counter()
+    for ev in events[:n_single]:
+        O.run(geo, w, ev, counts_only=True)
+    dt1 = time.perf_counter() - t0
+    per_core = n_single / dt1
+    # per-stage: cumulative runs that stop after each stage
+    names = ["sort", "md", "ls", "t3", "t5", "tc"]
+    cum = []
+    for st in names:
+        t0 = time.perf_counter()
+        for ev in events[:2]:
+            O.run(geo, w, ev, last_stage=st, counts_only=True)
+        cum.append((time.perf_counter() - t0) / 2 * 1e3)
+    stage_ms = {"a0": cum[0], "a1": cum[1] - cum[0], "a2": cum[2] - cum[1], "a3": cum[3] - cum[2], "a4+a5": cum[4] - cum[3], "a6": cum[5] - cum[4]}
+    ncpu = os.cpu_count() or 1
+    per_proc = max(1, int(round(budget_s * per_core)))
+    _CPU_EVENTS = (geo, w, events)
+    jobs = [([(p * per_proc + k) % len(events) for k in range(per_proc)], 1) for p in range(ncpu)]
+    try:
+        with mp.get_context("fork").Pool(ncpu) as pool:
+            res = pool.map(_cpu_worker, jobs)
+        all_cores = sum(n for n, _ in res) / max(t for _, t in res)
+    except Exception as e:      # a box that cannot fork: report the single-core number only
+        all_cores, ncpu = None, 1
+    model = "?"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip(); break
+    except OSError:
+        pass
+    return dict(value=round(per_core, 3), unit=UNIT, cores=1, kind="oracle",
+                sample=f"first {n_single} of the PU200 events of one step, single thread, {dt1:.1f} s",
+                all_cores=dict(value=None if all_cores is None else round(all_cores, 2), cores=ncpu,
+                               sample=f"{ncpu} oracle processes x {per_proc} events each, events / slowest process"),
+                cpu_model=model, nproc=os.cpu_count(),
+                stage_ms_per_event={k: round(v, 2) for k, v in stage_ms.items()})
+
+
+def stage_table(prof, stages, n_events, pk, alu_peak, fma_peak):
+    """per-stage us / event, bound and achieved fraction of the stage's own roofline"""
+    stage_ms = {}
+    for k, v in prof.items():
+        st_name = "a0" if k == "memset" else stage_of(k)
+        stage_ms[st_name] = stage_ms.get(st_name, 0.0) + v
+    rows = {}
+    for st_name, wk in stages.items():
+        t_s = stage_ms[st_name] * 1e-3
+        peak_f = fma_peak if st_name == "a5" else alu_peak
+        t_hbm, t_alu = wk["bytes"] / (pk["hbm_gbs"] * 1e9), wk["flops"] / (peak_f * 1e12)
+        rows[st_name] = dict(us_per_event=round(stage_ms[st_name] * 1e3 / n_events, 3), bound="hbm" if t_hbm >= t_alu else "alu",
+                             roofline_us_per_event=round(max(t_hbm, t_alu) * 1e6 / n_events, 4),
+                             frac=round(max(t_hbm, t_alu) / t_s, 4) if t_s > 0 else None,
+                             gbs=round(wk["bytes"] / t_s / 1e9, 1), tflops=round(wk["flops"] / t_s / 1e12, 3))
+    return rows
+
+
 def run_ours(args):
-    import torch
-    import paper_2403_13166_b200 as P
-    from lstgen import build_geometry, xavier_weights
     rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
     assert world == args.gpus or world == 1, (world, args.gpus)
+    from lstgen import build_geometry, xavier_weights, config_event
+    geo = build_geometry(True)
+    w = xavier_weights(3)
+    E, S = args.events, args.streams
+    assert E % S == 0
+    events = make_events(geo, shard_seeds(rank, world, E))
+    ev_c2 = config_event(geo, 2)                    # configs[2] exactly: seed 3, the single-event headline
+    # ---- oracle on the host cores (rank 0, N = 1), before CUDA is initialised: the workers are forked
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(geo, w, events, min(E, args.cpu_sample))
+
+    import torch
+    import paper_2403_13166_b200 as P
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
@@ -166,11 +261,6 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     P.load_library()
-    geo = build_geometry(True)
-    w = xavier_weights(3)
-    E, S = args.events, args.streams
-    assert E % S == 0
-    events = make_events(geo, shard_seeds(rank, world, E))
     caps = P.Caps(n_slots=E, max_hits=114688, max_md=49152, max_ls=49152, max_t3=32768, max_t5c=16384, max_t5=16384, max_pls=4096)
     lst = P.LST(geo, w, caps, device=dev)
     lst.n_pls = [ev.n_pls for ev in events]
@@ -220,22 +310,20 @@ def run_ours(args):
     step_ms = [a.elapsed_time(b) for a, b in evs]
     ms_local = float(np.mean(step_ms))
 
-    # ---- e2e: pinned host inputs -> H2D -> chain -> D2H of counters + TC rows, every step --------
-    # e2e: per stream ONE pinned blob in (all its events, lst_load_batch_host) and ONE pinned buffer out (counters +
-    # TC rows of its events, lst_read_tc_batch_host): 1 H2D + 1 D2H copy per 16-event batch
-    TC_ROWS = 4096
+    # ---- e2e: per stream ONE pinned blob in (all its events, lst_load_batch_host) and ONE pinned buffer out (counters + TC
+    # rows WITH their original hit indices, lst_read_tc_hits_batch_host): 1 H2D + 1 D2H copy per 16-event batch, every step
     e2e_streams = streams if S > 1 else [main]
     nb = E // len(e2e_streams)
     blobs = [P.pack_batch(events[si * nb:(si + 1) * nb]) for si in range(len(e2e_streams))]
-    h_outs = [torch.zeros((nb, 32 + 3 * TC_ROWS), dtype=torch.int32).pin_memory() for _ in e2e_streams]
+    h_outs = [torch.zeros((nb, 32 + 13 * TC_ROWS), dtype=torch.int32).pin_memory() for _ in e2e_streams]
     h2d = sum(int(b.numel()) for b in blobs)
-    d2h = E * (32 * 4 + TC_ROWS * 12)
+    d2h = E * (32 * 4 + TC_ROWS * 13 * 4)
 
     def e2e_step():
         for si, st in enumerate(e2e_streams):
             lst.lst_load_batch_host(si * nb, nb, blobs[si], stream=st)
             lst.lst_run_batch(si * nb, nb, st)
-            lst.lst_read_tc_batch_host(si * nb, nb, h_outs[si], stream=st)
+            lst.lst_read_tc_hits_batch_host(si * nb, nb, h_outs[si], stream=st)
 
     for _ in range(3):
         e2e_step()
@@ -247,30 +335,66 @@ def run_ours(args):
     e2e_ms_local = (time.perf_counter() - t0) * 1e3 / args.steps
     for h in h_outs:
         for i in range(nb):
-            assert int(h[i, 31]) == 0 and 0 < int(h[i, P.CNT["tc"]]) <= TC_ROWS, "e2e run failed or TC rows truncated"
+            ntc = int(h[i, P.CNT["tc"]])
+            assert int(h[i, 31]) == 0 and 0 < ntc <= TC_ROWS, "e2e run failed or TC rows truncated"
+            rows = h[i, 32:32 + 13 * ntc].view(ntc, 13)
+            t5 = rows[rows[:, 0] <= 1]
+            assert bool((t5[:, 3:] >= 0).all()), "a T5-based candidate came back without its ten hits"
     # rebind the resident inputs for the profile pass
     for i, ev in enumerate(events):
         lst.load_numpy_event(i, ev)
     torch.cuda.synchronize()
 
     # ---- per-kernel device times (same launch configuration as the timed region) ------------------
-    prof = {}
-    reps = 5
-    for r in range(reps + 1):
-        flush.zero_()
-        torch.cuda.synchronize()
-        if S == 1:
-            d = lst.lst_run_batch_profile(0, E, main)
-        else:       # one stream's share of the batch; the S streams run the same sequence concurrently
-            d = lst.lst_run_batch_profile(0, per, main)
-        if r:       # first one is warm-up
-            for k, v in d.items():
-                prof[k] = prof.get(k, 0.0) + v / reps
-    n_prof = E if S == 1 else per
+    def profile(first, n, reps=5):
+        acc = {}
+        for r in range(reps + 1):
+            flush.zero_()
+            torch.cuda.synchronize()
+            d = lst.lst_run_batch_profile(first, n, main)
+            if r:       # first one is warm-up
+                for k, v in d.items():
+                    acc[k] = acc.get(k, 0.0) + v / reps
+        return acc
+
+    n_prof = E if S == 1 else per       # one stream's share of the batch; the S streams run the same sequence concurrently
+    prof = profile(0, n_prof)
     tot, stages = algorithmic_work(lst, geo, range(n_prof))
+
+    # ---- single event: configs[2] exactly (seed 3), one event, one stream ---------------------------------------------
+    lst.load_numpy_event(0, ev_c2)
+    torch.cuda.synchronize()
+    one = streams[0]
+    for _ in range(5):
+        lst.lst_run_batch(0, 1, one)
+    torch.cuda.synchronize()
+    bits1, c1 = lst.lst_status(0)
+    assert bits1 == 0
+    lat = []
+    for _ in range(args.single_reps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        one.wait_stream(main)
+        a.record(one); lst.lst_run_batch(0, 1, one); b.record(one)
+        main.wait_stream(one)
+        lat.append((a, b))
+    torch.cuda.synchronize()
+    lat_ms = float(np.median([a.elapsed_time(b) for a, b in lat]))
+    # back to back, L2 warm (no flush): the steady-state rate of a stream that keeps feeding single events
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(one)
+    for _ in range(args.single_reps):
+        lst.lst_run_batch(0, 1, one)
+    b.record(one)
+    torch.cuda.synchronize()
+    warm_ms = a.elapsed_time(b) / args.single_reps
+    prof1 = profile(0, 1)
+    lst.n_pls[0] = ev_c2.n_pls
+    tot1, stages1 = algorithmic_work(lst, geo, [0])
+    lst.n_pls[0] = events[0].n_pls
+
     # launch floor: the smallest kernel of the library (a 1-thread bind), back to back on one stream -- the time
     # below which no stage of a small batch can go (report it beside the per-stage fractions)
-    ev0 = events[0]
     torch.cuda.synchronize()
     fa, fb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     fa.record(main)
@@ -279,7 +403,9 @@ def run_ours(args):
     fb.record(main)
     torch.cuda.synchronize()
     launch_floor_us = fa.elapsed_time(fb) * 1e3 / 200
-    lst.load_numpy_event(0, ev0)
+    lst.load_numpy_event(0, events[0])
+    # fp32 throughput of this GPU, measured with the library's probe kernels
+    alu_meas, fma_meas = lst.lst_measure_fp32(False, main), lst.lst_measure_fp32(True, main)
 
     def red_max(v):
         if dist is None:
@@ -294,59 +420,42 @@ def run_ours(args):
         return
 
     pk = peaks()
-    alu_peak = SM_COUNT * LANES * pk["sm_max_mhz"] * 1e6 / 1e12          # Tflop/s, un-fused mul/add
-    fma_peak = 2 * alu_peak
-    stage_ms = {}
-    for k, v in prof.items():
-        if k != "memset":
-            stage_ms[stage_of(k)] = stage_ms.get(stage_of(k), 0.0) + v
-    stage_ms["a0"] += prof.get("memset", 0.0)
-    stage_rows = {}
-    for st_name, wk in stages.items():
-        t_s = stage_ms[st_name] * 1e-3
-        peak_f = fma_peak if st_name == "a5" else alu_peak
-        t_hbm, t_alu = wk["bytes"] / (pk["hbm_gbs"] * 1e9), wk["flops"] / (peak_f * 1e12)
-        stage_rows[st_name] = dict(us_per_event=round(stage_ms[st_name] * 1e3 / n_prof, 3), bound="hbm" if t_hbm >= t_alu else "alu",
-                                   roofline_us_per_event=round(max(t_hbm, t_alu) * 1e6 / n_prof, 4),
-                                   frac=round(max(t_hbm, t_alu) / t_s, 4) if t_s > 0 else None,
-                                   gbs=round(wk["bytes"] / t_s / 1e9, 1), tflops=round(wk["flops"] / t_s / 1e12, 3))
+    alu_nominal = SM_COUNT * LANES * pk["sm_max_mhz"] * 1e6 / 1e12        # one op per lane per clock
+    alu_peak = alu_meas if alu_meas > 0 else alu_nominal
+    fma_peak = fma_meas if fma_meas > 0 else 2 * alu_nominal
+    stage_rows = stage_table(prof, stages, n_prof, pk, alu_peak, fma_peak)
     # dominant kernel
     kname = max((k for k in prof if k != "memset"), key=lambda k: prof[k])
     kst = stage_of(kname)
-    share = {"a1": 0.5, "a2": 0.5, "a3": 0.5, "a4": 0.5}.get(kst, 1.0)   # count and fill passes each do the stage's pair tests once
     wk = stages[kst]
     k_s = prof[kname] * 1e-3
-    if kst in ("a0",) or wk["bytes"] / (pk["hbm_gbs"] * 1e9) >= wk["flops"] / (alu_peak * 1e12):
-        roof = dict(bound="hbm", achieved=round(wk["bytes"] / k_s / 1e9, 2), peak=pk["hbm_gbs"], unit="GB/s")
+    if kst == "a0" or wk["bytes"] / (pk["hbm_gbs"] * 1e9) >= wk["flops"] / (alu_peak * 1e12):
+        roof = dict(bound="hbm", achieved=round(wk["bytes"] / k_s / 1e9, 2), peak=pk["hbm_gbs"], unit="GB/s", peak_source=f"MEASURED_PEAKS.json ({pk['source']})")
     else:
         peak_f = fma_peak if kst == "a5" else alu_peak
-        # each of the two passes evaluates every pair: per-launch algorithmic flops = the stage's
-        roof = dict(bound="alu", achieved=round(wk["flops"] / k_s / 1e12, 3), peak=round(peak_f, 2), unit="TFLOP/s")
-    traffic = None       # DRAM bytes per launch of this kernel from the committed ncu --set full capture
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    if os.path.exists(tpath):
-        for line in open(tpath).read().splitlines()[1:]:
-            f = line.split(",")
-            if f and f[0] == kname:
-                traffic = round((float(f[3]) + float(f[4])) * n_prof / float(f[2]))
-    roof.update(frac=round(roof["achieved"] / roof["peak"], 4), traffic=traffic, traffic_source="profiles/r01_traffic.csv", kernel=kname, kernel_ms=round(prof[kname], 4),
-                kernel_share_of_step=round(prof[kname] / sum(prof.values()), 3), peak_source=pk["source"],
-                note="ALU peak = 148 SM x 128 lanes x sm_max_mhz un-fused fp32 ops (cuts may not use FMA); DESIGN.md Rooflines")
-    del share
-
-    # ---- oracle on the host cores: bounded sample of the same workload ------------------------------
-    cpu = None
-    if world == 1 and not args.no_cpu_baseline:
-        from oracle import lst_oracle as O
-        O.build()
-        n_s = min(E, args.cpu_sample)
-        O.run(geo, w, events[0], counts_only=True)
-        t0 = time.perf_counter()
-        for ev in events[:n_s]:
-            O.run(geo, w, ev, counts_only=True)
-        dt = time.perf_counter() - t0
-        cpu = dict(value=round(n_s / dt, 3), unit=UNIT, cores=1, kind="oracle",
-                   sample=f"first {n_s} of the {E} PU200 events of one step, single thread, {dt:.1f} s")
+        roof = dict(bound="alu", achieved=round(wk["flops"] / k_s / 1e12, 3), peak=round(peak_f, 2), unit="TFLOP/s",
+                    peak_source="measured in this run by lst_measure_fp32 (separately rounded multiply + add)")
+    traffic, tsrc = None, None       # DRAM bytes per launch of this kernel from the committed ncu --set full capture
+    for tname in ("r02_traffic.csv", "r01_traffic.csv"):
+        tpath = os.path.join(ROOT, "profiles", tname)
+        if traffic is None and os.path.exists(tpath):
+            for line in open(tpath).read().splitlines()[1:]:
+                f = line.split(",")
+                if f and f[0] == kname:
+                    traffic, tsrc = round((float(f[3]) + float(f[4])) * n_prof / float(f[2])), "profiles/" + tname
+    roof.update(frac=round(roof["achieved"] / roof["peak"], 4), traffic=traffic, traffic_source=tsrc, kernel=kname, kernel_ms=round(prof[kname], 4),
+                kernel_share_of_step=round(prof[kname] / sum(prof.values()), 3), algorithmic_per_unit="60 flop per LS pair test (SURVEY.md 8.d)" if kst == "a2" else None,
+                fp32_tflops=dict(unfused_measured=round(alu_meas, 2), fma_measured=round(fma_meas, 2), unfused_nominal=round(alu_nominal, 2),
+                                 note="nominal = 148 SM x 128 lanes x sm_max_mhz, one op per lane per clock; the cut kernels may not fuse (north_star)"))
+    single = dict(workload="configs[2] exactly: one HL-LHC PU200 event, seed 3, one stream, one lst_run (CUDA-graph replay)",
+                  value=round(1e3 / lat_ms, 1), unit=UNIT, us_per_event=round(lat_ms * 1e3, 1),
+                  timing=f"median of {args.single_reps} runs, CUDA events on the launching stream, L2 flushed before every run",
+                  back_to_back=dict(value=round(1e3 / warm_ms, 1), us_per_event=round(warm_ms * 1e3, 1), note="same event resubmitted without flush (L2 warm)"),
+                  launches=lst.launches_per_run(), launch_floor_us=round(launch_floor_us, 2),
+                  launch_floor_total_us=round(launch_floor_us * lst.launches_per_run(), 1),
+                  stages=stage_table(prof1, stages1, 1, pk, alu_peak, fma_peak),
+                  kernels_us={k: round(v * 1e3, 2) for k, v in prof1.items()},
+                  objects={k: v for k, v in tot1.items()})
 
     out = dict(metric=METRIC, value=round(value, 1), unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                ms_per_step=round(ms, 4), higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
@@ -355,15 +464,55 @@ def run_ours(args):
                            timing="mean of per-step CUDA-event durations on the launching stream, max over ranks",
                            parallelism=f"replicas x{world}" if world > 1 else "single GPU"),
                e2e=dict(value=round(e2e_value, 1), unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, ms_per_step=round(e2e_ms, 4),
-                        timing="wall clock around K steps incl. pinned H2D of every input and D2H of counters + TC rows"),
+                        timing="wall clock around K steps incl. pinned H2D of every input and D2H of counters + TC rows with their hit indices",
+                        host_link_gbs=round((h2d + d2h) / (e2e_ms * 1e-3) / 1e9, 1)),
                gpu_launches=args.steps * S * lst.launches_per_run(), launch_floor_us=round(launch_floor_us, 2),
-               clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows,
+               clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows, single_event=single,
                kernels_ms={k: round(v, 4) for k, v in prof.items()},
                per_event=dict(us=round(ms * 1e3 / E, 2), objects={k: round(v / n_prof, 1) for k, v in tot.items()}),
                wall_ms_per_step_incl_flush=round(t_wall * 1e3 / args.steps, 3))
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def run_sweep(args):
+    """configs[4]: displaced-track and occupancy stress.  config 2 recipe scaled to pile-up 0 / 100 / 200 / 300 plus 500
+    displaced particles, 8 events per point (seeds 200-231): events/s, object counts and the overflow status per point."""
+    import torch
+    import paper_2403_13166_b200 as P
+    from lstgen import build_geometry, config_event, xavier_weights
+    if not torch.cuda.is_available():
+        raise SystemExit("needs a CUDA device (no CPU fallback)")
+    geo, w = build_geometry(True), xavier_weights(3)
+    caps = P.Caps(n_slots=8, max_hits=196608, max_md=98304, max_ls=98304, max_t3=65536, max_t5c=32768, max_t5=32768, max_pls=8192)
+    lst = P.LST(geo, w, caps)
+    st = torch.cuda.Stream()
+    points, seed = [], 200
+    for pu in (0, 100, 200, 300):
+        evs = [config_event(geo, 4, seed=seed + i, pileup=pu) for i in range(8)]
+        seed += 8
+        for i, ev in enumerate(evs):
+            lst.load_numpy_event(i, ev)
+        torch.cuda.synchronize()
+        for _ in range(3):
+            lst.lst_run_batch(0, 8, st)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(st)
+        for _ in range(args.steps):
+            lst.lst_run_batch(0, 8, st)
+        b.record(st)
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / args.steps
+        stat, cs = zip(*[lst.lst_status(i) for i in range(8)])
+        mean = lambda k: round(float(np.mean([c[k] for c in cs])), 1)
+        points.append(dict(pileup=pu, events_per_s=round(8 / ms * 1e3, 1), us_per_event=round(ms * 1e3 / 8, 1), status_or=int(np.bitwise_or.reduce(stat)),
+                           hits=mean("hit"), md=mean("md"), ls=mean("ls"), t3=mean("t3"), t5c=mean("t5c"), t5=mean("t5"),
+                           pls=round(float(np.mean([ev.n_pls for ev in evs])), 1), tc=mean("tc")))
+    lst.close()
+    print(json.dumps(dict(metric="events/s vs occupancy (configs[4]: PU-scaled config 2 + 500 displaced, 8 events per point, seeds 200-231)",
+                          unit=UNIT, n_gpus=1, steps=args.steps, data="synthetic", dtype="f32", points=points,
+                          timing="8-event batched launches back to back on one stream (CUDA-graph replay), CUDA events, L2 warm")))
 
 
 def run_reference(args):
@@ -407,9 +556,13 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=48)
     ap.add_argument("--ref-events", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--single-reps", type=int, default=50, help="timed runs of the single-event (configs[2]) block")
+    ap.add_argument("--config", type=int, default=3, choices=[3, 4], help="3: the batched PU200 throughput line; 4: the occupancy sweep")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == 4:
+        run_sweep(args)
     else:
         run_ours(args)
 

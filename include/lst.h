@@ -143,6 +143,12 @@ int lst_load_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, const void*
 int lst_read_tc_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, int32_t* h_out, int32_t max_rows,
                            void* cuda_stream);
 
+/* The same with self-contained rows: h_out (HOST int32[n][LST_N_CNT + 13*max_rows]); a row is (type, pLS, object index)
+ * followed by the candidate's ten ORIGINAL hit indices (SPEC.md 5: lower, upper hit of each of its MDs in order; the five
+ * MDs of a pT5 / T5, the three of a pT3, -1 padded; a pLS candidate has none). */
+int lst_read_tc_hits_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, int32_t* h_out, int32_t max_rows,
+                                void* cuda_stream);
+
 /* Enqueue the whole chain a0..a6 (SPEC.md 4.0-4.6) for one slot / for slots
  * [first_slot, first_slot + n) in single batched launches (event index = a grid dimension).
  * On a capturable stream (any stream but the legacy default stream 0) the launch sequence is captured once per
@@ -171,6 +177,12 @@ int lst_launches_per_run(void);
  * the lst_launches_per_run() kernels to h_ms[0 .. lst_launches_per_run()] (HOST).  Not a bench
  * path: the events serialise nothing but add launch gaps. */
 int lst_run_batch_profile(lst_ctx* ctx, int32_t first_slot, int32_t n, void* cuda_stream, float* h_ms);
+
+/* Measurement only: sustained fp32 throughput of this GPU in Tflop/s (HOST *h_tflops), counted as one multiply + one add
+ * per chain step, with separately rounded multiply and add (fused = 0: the form the cut arithmetic must use) or with fused
+ * multiply-add (fused = 1: allowed in the DNN).  Runs a few ms of a register-only kernel on `cuda_stream` and synchronises.
+ * These are the denominators of the ALU-bound rooflines in bench.py. */
+int lst_measure_fp32(lst_ctx* ctx, int32_t fused, float* h_tflops, void* cuda_stream);
 
 /* Name of entry i of h_ms ("memset", "a0.hist", ... , "a6.tc_emit"); NULL when out of range. */
 const char* lst_launch_name(int32_t i);

@@ -15,7 +15,7 @@ CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t
            raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
-           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_launches_per_run",
+           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_measure_fp32", "lst_launches_per_run",
            "lst_destroy"]
 
 
@@ -83,6 +83,8 @@ def load_library():
     L.lst_read_tc_host.argtypes = [vp, i32, vp, vp, i32, vp]
     L.lst_load_batch_host.argtypes = [vp, i32, i32, vp, C.c_size_t, vp]
     L.lst_read_tc_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
+    L.lst_read_tc_hits_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
+    L.lst_measure_fp32.argtypes = [vp, i32, C.POINTER(C.c_float), vp]
     L.lst_launches_per_run.argtypes = []
     L.lst_run_batch_profile.argtypes = [vp, i32, i32, vp, vp]
     L.lst_launch_name.argtypes = [i32]
@@ -237,6 +239,18 @@ class LST:
         rows = (int(h_out.shape[1]) - LST_N_CNT) // 3
         _chk(self.lib.lst_read_tc_batch_host(self.ctx, first_slot, n, C.c_void_p(h_out.data_ptr()), rows, self._st(stream)),
              "lst_read_tc_batch_host")
+
+    def lst_read_tc_hits_batch_host(self, first_slot, n, h_out, stream=None):
+        """h_out: HOST (pinned) int32 tensor [n, 32 + 13*max_rows]: rows = (type, pLS, object, 10 original hit indices)."""
+        rows = (int(h_out.shape[1]) - LST_N_CNT) // 13
+        _chk(self.lib.lst_read_tc_hits_batch_host(self.ctx, first_slot, n, C.c_void_p(h_out.data_ptr()), rows, self._st(stream)),
+             "lst_read_tc_hits_batch_host")
+
+    def lst_measure_fp32(self, fused, stream=None):
+        """Sustained fp32 Tflop/s of this GPU: separately rounded multiply + add (fused=False) or FMA (fused=True)."""
+        v = C.c_float(0.0)
+        _chk(self.lib.lst_measure_fp32(self.ctx, int(bool(fused)), C.byref(v), self._st(stream)), "lst_measure_fp32")
+        return float(v.value)
 
     def lst_run_batch_profile(self, first_slot, n, stream=None):
         """Per-launch device times in ms: dict name -> ms (memset + every kernel of one pass)."""

@@ -92,7 +92,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   L.run_c1 = cv.take<int>(nnz > 0 ? nnz : 1);
   L.batch_in_stride = blob_event_bytes(k.max_hits, k.max_pls) + 16;
   L.batch_in = cv.take<char>(L.batch_in_stride * n_slots + 1024);
-  L.batch_out_stride = LST_N_CNT + 3 * (size_t)k.max_tc;
+  L.batch_out_stride = LST_N_CNT + 13 * (size_t)k.max_tc;
   L.batch_out = cv.take<int>(L.batch_out_stride * n_slots);
   if (out) out->assign(n_slots, Slot{});
   // zero region (contiguous over slots so one memset covers a batch)
@@ -460,16 +460,50 @@ int lst_load_batch_host(lst_ctx* c, int32_t first, int32_t n, const void* h_blob
   return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
 }
 
-int lst_read_tc_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out, int32_t max_rows, void* cuda_stream) {
+static int read_tc_batch(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out, int32_t max_rows, void* cuda_stream, bool hits) {
   if (!c || !h_out || first < 0 || n <= 0 || first + n > c->n_slots || max_rows < 0) return LST_EINVAL;
   if (c->sticky_cuda_error) return LST_ECUDA;
   if (max_rows > c->caps.max_tc) return LST_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   int* dst = c->batch_out + c->batch_out_stride * first;
-  k_pack_tc<<<dim3(8, n), 256, 0, st>>>(c->d_slots + first, max_rows, dst);
+  if (hits) k_pack_tc<true><<<dim3(8, n), 256, 0, st>>>(c->d_slots + first, max_rows, dst);
+  else k_pack_tc<false><<<dim3(8, n), 256, 0, st>>>(c->d_slots + first, max_rows, dst);
   if (bad(c, cudaGetLastError())) return LST_ECUDA;
-  const size_t bytes = sizeof(int32_t) * (LST_N_CNT + 3 * (size_t)max_rows) * n;
+  const size_t bytes = sizeof(int32_t) * (LST_N_CNT + (hits ? 13 : 3) * (size_t)max_rows) * n;
   return bad(c, cudaMemcpyAsync(h_out, dst, bytes, cudaMemcpyDeviceToHost, st)) ? LST_ECUDA : LST_OK;
+}
+
+int lst_read_tc_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out, int32_t max_rows, void* cuda_stream) {
+  return read_tc_batch(c, first, n, h_out, max_rows, cuda_stream, false);
+}
+
+int lst_read_tc_hits_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out, int32_t max_rows, void* cuda_stream) {
+  return read_tc_batch(c, first, n, h_out, max_rows, cuda_stream, true);
+}
+
+int lst_measure_fp32(lst_ctx* c, int32_t fused, float* h_tflops, void* cuda_stream) {
+  if (!c || !h_tflops) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  float* scratch = reinterpret_cast<float*>(c->batch_out);
+  cudaEvent_t a, b;
+  if (bad(c, cudaEventCreate(&a)) || bad(c, cudaEventCreate(&b))) return LST_ECUDA;
+  const int blocks = 148 * 8, iters = 8192;
+  float best = 0.f;
+  for (int rep = 0; rep < 4; ++rep) {             // first repetition warms up
+    cudaEventRecord(a, st);
+    if (fused) k_fp32_probe<true><<<blocks, 256, 0, st>>>(scratch, iters);
+    else k_fp32_probe<false><<<blocks, 256, 0, st>>>(scratch, iters);
+    cudaEventRecord(b, st);
+    if (bad(c, cudaEventSynchronize(b))) { cudaEventDestroy(a); cudaEventDestroy(b); return LST_ECUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    const double flop = 2.0 * 8.0 * iters * 256.0 * blocks;      // one multiply + one add per chain step, fused or not
+    if (rep && ms > 0.f) best = fmaxf(best, (float)(flop / (ms * 1e-3) / 1e12));
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  *h_tflops = best;
+  return LST_OK;
 }
 
 void lst_destroy(lst_ctx* c) {

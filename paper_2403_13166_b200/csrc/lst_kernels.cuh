@@ -686,13 +686,57 @@ __global__ void k_bind_batch(Slot* slots, int first, int n, const char* blob) {
   s.in_px = g; s.in_py = g + np; s.in_pz = g + 2 * (size_t)np; s.in_z0 = g + 3 * (size_t)np;
   s.in_q = reinterpret_cast<const int8_t*>(g + 4 * (size_t)np); s.n_pls = np;
 }
-// packs counters + the first `rows` TC rows of n slots into one contiguous buffer [n][LST_N_CNT + 3 rows]
+// packs counters + the first `rows` TC rows of n slots into one contiguous buffer [n][LST_N_CNT + W rows].
+// W = 3: (type, pLS, object index).  W = 13: the same followed by the candidate's ORIGINAL hit indices -- the ten hits of a
+// T5 (pT5 / T5), the six hits of a T3 (pT3), -1 padded -- so that the host-side result is self-contained.
+template <bool HITS>
 __global__ void k_pack_tc(const Slot* __restrict__ slots, int rows, int* __restrict__ out) {
   const Slot& s = slots[blockIdx.y];
-  const int w = LST_N_CNT + 3 * rows;
-  int* o = out + (size_t)blockIdx.y * w;
-  const int n = LST_N_CNT + 3 * min(rows, s.tc_hdr[LST_CNT_TC]);
-  LST_FOR_ITEMS(i, n) o[i] = s.tc_hdr[i];
+  constexpr int RW = HITS ? 13 : 3;
+  int* o = out + (size_t)blockIdx.y * (LST_N_CNT + RW * rows);
+  const int n_rows = min(rows, s.tc_hdr[LST_CNT_TC]);
+  if (!HITS) {
+    LST_FOR_ITEMS(i, LST_N_CNT + 3 * n_rows) o[i] = s.tc_hdr[i];
+    return;
+  }
+  LST_FOR_ITEMS(i, LST_N_CNT) o[i] = s.tc_hdr[i];
+  LST_FOR_ITEMS(i, n_rows) {
+    const int type = s.tc[3 * i], obj = s.tc[3 * i + 2];
+    int* r = o + LST_N_CNT + 13 * i;
+    r[0] = type; r[1] = s.tc[3 * i + 1]; r[2] = obj;
+    int md[5] = {-1, -1, -1, -1, -1};
+    if (type <= 1) {
+      const int* m5 = s.t5c_md + 5 * s.t5_list[obj];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) md[q] = m5[q];
+    } else if (type == 2) {
+      const int4 abc = s.t3_abc[obj];
+      md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      const int2 h = md[q] >= 0 ? s.md_hits[md[q]] : make_int2(-1, -1);
+      r[3 + 2 * q] = h.x; r[4 + 2 * q] = h.y;
+    }
+  }
+}
+
+// FP32 throughput probes for the roofline denominators (measurement only): eight independent dependent chains per thread of
+// either un-fused multiply + add pairs (the cut arithmetic may not contract, BASELINE.json north_star) or fused multiply-adds.
+template <bool FUSED>
+__global__ void __launch_bounds__(256) k_fp32_probe(float* __restrict__ out, int iters) {
+  float x[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = 1.0f + 1.0e-3f * (threadIdx.x + k);
+  const float a = 0.999999f, b = 1.0e-6f;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) x[k] = FUSED ? fmaf(x[k], a, b) : __fadd_rn(__fmul_rn(x[k], a), b);
+  }
+  float acc = 0.f;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc += x[k];
+  if (acc == 123.456f) out[0] = acc;        // never true: keeps the chains alive
 }
 
 }  // namespace lst
