@@ -143,7 +143,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.t5c_score = cv.take<float>(k.max_t5c); t.t5c_pass = cv.take<int>(k.max_t5c); t.t5_scan = cv.take<int>(k.max_t5c + 8);
     t.t5_list = cv.take<int>(k.max_t5);
     t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.pls_key = cv.take<int>(k.max_pls);
-    t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls);
+    t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls); t.pls_pos = cv.take<int>(k.max_pls); t.pls_taken = cv.take<int>(k.max_pls);
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
@@ -231,6 +231,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   }
   if (e == cudaSuccess) e = cudaDeviceSynchronize();       // the memsets above are asynchronous on device memory
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
+  if (cudaFuncSetAttribute(k_pls_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, PLS_BIN_SMEM) != cudaSuccess) { delete c; return LST_ECUDA; }
   if (const char* g = std::getenv("LST_GRAPHS")) c->use_graphs = !(g[0] == '0');
   if (c->use_graphs) {            // host-side objects only; without them the binning simply stays in line
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess) c->side = nullptr;
@@ -307,7 +308,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   const bool fork = c->capturing && c->side;
   if (fork) {
     if (bad(c, cudaEventRecord(c->ev_fork, st)) || bad(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0))) return LST_ECUDA;
-    k_pls_bin<<<G1, 1024, 0, c->side>>>(sl);
+    k_pls_bin<<<G1, 1024, PLS_BIN_SMEM, c->side>>>(sl);
     if (bad(c, cudaEventRecord(c->ev_join, c->side))) return LST_ECUDA;
   }
   k_hist<<<G, 256, 0, st>>>(sl, g); LST_MARK();
@@ -325,7 +326,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
   k_scan_lb<SCAN_T5><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
   if (fork) { if (bad(c, cudaStreamWaitEvent(st, c->ev_join, 0))) return LST_ECUDA; }
-  else k_pls_bin<<<G1, 1024, 0, st>>>(sl);
+  else k_pls_bin<<<G1, 1024, PLS_BIN_SMEM, st>>>(sl);
   LST_MARK();
   k_match<5, false><<<G, MATCH_WARPS * 32, 0, st>>>(sl); LST_MARK();
   k_pt5_lists<<<G, 128, 0, st>>>(sl); LST_MARK();

@@ -63,7 +63,7 @@ struct Slot {
   int* t5_off; int* t5c_md; int2* t5c_t3; float* t5c_curv; float* t5c_feat; float* t5c_score; int* t5c_pass;
   int* t5_scan; int* t5_list;
   // a6
-  float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_bin_start;
+  float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
   // host-load staging
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
@@ -318,27 +318,40 @@ __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, 
 // ------------------------------------------------------------------------------------------------
 // a6: track candidates (SPEC.md 4.6)
 // ------------------------------------------------------------------------------------------------
-// pLS binning.  The matching of SPEC.md 4.6 is defined over all (pLS, object) pairs; to avoid the
-// all-pairs sweep the pLS are bucketed by (half-curvature h = 1/(2R), azimuth psi of the helix centre).
-// For an anchor at (r, phi) the transverse test |e| <= dT is, in exact arithmetic,
-//   |u - cos(phi - psi)| <= tau(u),  u = r*h,  tau(u) = 0.003 + 0.03*u + 0.02/r,
-// so for one h-bucket only two psi windows can hold a passing pLS.  The windows are widened by margins
-// (2e-3 in cos, 1e-3 rad) that exceed the fp32 rounding of every quantity involved by > 100x, so the
-// bucket walk is a conservative prefilter: every pair that passes the exact test is visited, and the
-// decisions themselves are still taken by the exact SPEC.md arithmetic.  pLS whose h is outside the
-// bucketed range (pT < ~0.76 GeV, NaN) or whose q is not +-1 go to an overflow bucket every object visits.
-constexpr int PLS_NB = 512, PLS_K = 8, PLS_NBINS = (PLS_K + 1) * PLS_NB;
+// pLS binning.  The matching of SPEC.md 4.6 is defined over all (pLS, object) pairs; to avoid the all-pairs sweep the pLS
+// are bucketed by (half-curvature h = 1/(2R), zeta = z the helix reaches at r = 40 cm, azimuth psi of the helix centre).
+// For an anchor at (r, phi, z):
+//  * the transverse test |e| <= dT is, in exact arithmetic, |u - cos(phi - psi)| <= tau(u), u = r*h,
+//    tau(u) = 0.003 + 0.03*u + 0.02/r, so for one h-bucket only two psi windows can hold a passing pLS;
+//  * the longitudinal test |z - z0 - s*cot| <= dZ gives zeta = z0 + s40*cot = rho*z + (1 - rho)*z0 - rho*zres with
+//    rho = s40(h)/s(h) (monotone in h: both arc lengths are the same positive-coefficient polynomial), |z0| <= 20 cm and
+//    |zres| <= dZ, so only a short zeta interval can hold a passing pLS.
+// The windows are widened by margins (2e-3 in cos, 1e-3 rad, 2 % in rho and 1 cm in zeta) that exceed the fp32 rounding of
+// every quantity involved by > 100x, so the bucket walk is a conservative prefilter: every pair that passes the exact test is
+// visited, and the decisions themselves are still taken by the exact SPEC.md arithmetic.  pLS outside the bucketed range
+// (pT < ~0.76 GeV, |z0| > 20 cm, |cot| > 8, q not +-1, NaN) go to an overflow bucket that every object visits.
+constexpr int PLS_NB = 256, PLS_NZ = 16, PLS_K = 2;
+constexpr int PLS_NREG = PLS_K * PLS_NZ * PLS_NB;          // regular bins: ((kb * NZ + zb) * NB + pb); bin PLS_NREG = overflow
+constexpr int PLS_NBINS = PLS_NREG + 1;
 #define LST_PLS_HMAX 0.0075f
+#define LST_PLS_Z0B 20.0f
+#define LST_PLS_COTCAP 8.0f
+#define LST_PLS_RREF 40.0f
+#define LST_PLS_ZR 256.0f
 #define LST_PI_F 3.14159265358979f
 
 __device__ __forceinline__ int psi_bin_raw(float ang) {   // unbounded bin index of an angle in radians
   return (int)floorf((ang + LST_PI_F) * (PLS_NB / (2.0f * LST_PI_F)));
 }
+__device__ __forceinline__ int zeta_bin(float zeta) {     // clamped bin index of a z at the reference radius
+  return min(PLS_NZ - 1, max(0, (int)floorf((zeta + LST_PLS_ZR) * (PLS_NZ / (2.0f * LST_PLS_ZR)))));
+}
 
-// one block per event: derive, histogram, scan, scatter (all in shared memory; ~2.6k pLS per event).  Depends only on
+// one block per event: derive, histogram, scan, scatter (histogram in shared memory; ~2.6k pLS per event).  Depends only on
 // the event's inputs, so lst_run puts it on a side branch of the launch graph, off the critical path.
+constexpr int PLS_BIN_SMEM = (PLS_NBINS + 1) * (int)sizeof(int);
 __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots) {
-  __shared__ int hist[PLS_NBINS + 1];
+  extern __shared__ int hist[];          // [PLS_NBINS + 1]
   __shared__ int sm[34];
   const Slot& s = slots[blockIdx.y];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -350,21 +363,22 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
     const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
     s.pls_a[p] = make_float4(d.cx, d.cy, d.h, d.cot);
     s.pls_b[p] = make_float2(d.sec, d.z0);
-    int kb = PLS_K, pb = 0;
-    if (d.h < LST_PLS_HMAX && (q == 1 || q == -1)) {
-      kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
-      pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
+    int key = PLS_NREG;
+    if (d.h < LST_PLS_HMAX && (q == 1 || q == -1) && fabsf(d.z0) <= LST_PLS_Z0B && fabsf(d.cot) <= LST_PLS_COTCAP) {
+      const int kb = min(PLS_K - 1, (int)(d.h * (PLS_K / LST_PLS_HMAX)));
+      const int pb = min(PLS_NB - 1, max(0, psi_bin_raw(atan2f(d.cy, d.cx))));
+      const float t = LST_PLS_RREF * d.h;
+      const int zb = zeta_bin(d.z0 + LST_PLS_RREF * arcfac(t * t) * d.cot);
+      key = (kb * PLS_NZ + zb) * PLS_NB + pb;
     }
-    const int key = kb * PLS_NB + pb;
     s.pls_key[p] = key;
     atomicAdd(&hist[key], 1);
   }
   __syncthreads();
-  // exclusive scan of hist[0..PLS_NBINS] (5 items per thread)
+  // exclusive scan of hist[0..PLS_NBINS]
   constexpr int IT = (PLS_NBINS + 1 + 1023) / 1024;
-  int v[IT], tsum = 0;
-#pragma unroll
-  for (int k = 0; k < IT; ++k) { const int i = tid * IT + k; v[k] = (i <= PLS_NBINS) ? hist[i] : 0; tsum += v[k]; }
+  int tsum = 0;
+  for (int k = 0; k < IT; ++k) { const int i = tid * IT + k; tsum += (i <= PLS_NBINS) ? hist[i] : 0; }
   int inc = tsum;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
@@ -378,11 +392,9 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
   }
   __syncthreads();
   int run = sm[wid] + inc - tsum;
-#pragma unroll
   for (int k = 0; k < IT; ++k) {
     const int i = tid * IT + k;
-    if (i <= PLS_NBINS) { hist[i] = run; s.pls_bin_start[i] = run; }
-    run += v[k];
+    if (i <= PLS_NBINS) { const int v = hist[i]; hist[i] = run; s.pls_bin_start[i] = run; run += v; }
   }
   __syncthreads();
   for (int p = tid; p < n; p += 1024) {
@@ -390,6 +402,7 @@ __global__ void __launch_bounds__(1024) k_pls_bin(const Slot* __restrict__ slots
     s.pls_sa[pos] = s.pls_a[p];
     s.pls_sb[pos] = s.pls_b[p];
     s.pls_sidx[pos] = p;
+    s.pls_pos[p] = pos;
   }
 }
 
@@ -398,15 +411,18 @@ __device__ __forceinline__ unsigned long long win_key(float chi2, int idx) {
 }
 
 // Match objects with NA anchors against the pLS buckets their first anchor can reach, and reduce to the winners.
-// One thread per object (T5 of the T5 list / T3); it visits the nine h-buckets in turn (so all lanes of a warp are in the
-// same h-bucket: uniform window arithmetic, similar loop lengths) and applies the cheap transverse test of the first
-// anchor to every pLS of its windows.  Survivors are queued per warp, and whenever 32 are queued the warp evaluates them
-// densely: first the full test of the first anchor, then -- queued again -- the remaining anchors.  The object's best
-// match is argmin over (chi2, p), kept as a 64-bit key in shared memory (independent of the visiting order); when the
-// object is done its thread folds it into the pLS's winner with a 64-bit atomicMin on (chi2, object): argmin over
-// (chi2, object) among the objects whose best pLS it is (SPEC.md 4.6).  T3 pass: T3s contained in a pT5 are skipped
-// (walk of the pT5 entries that hold the T3's first MD), and so are pLS that own a pT5.
+// One thread per object (T5 of the T5 list / T3).  It visits the h-buckets in turn (all lanes of a warp are in the same
+// bucket: uniform window arithmetic) and, per bucket, looks up the few (zeta bin, psi window) ranges of sorted pLS its first
+// anchor can reach -- all look-ups issued together, the non-empty ranges compacted into four register slots -- and applies the
+// cheap transverse test of the first anchor to every pLS in them.  Survivors are queued per warp, and whenever 32 are queued
+// the warp evaluates them densely: first the full test of the first anchor, then -- queued again -- the remaining anchors
+// (loaded together).  The object's best match is argmin over (chi2, p), kept as a 64-bit key in shared memory (independent of
+// the visiting order); when the object is done its thread folds it into the pLS's winner with a 64-bit atomicMin on
+// (chi2, object): argmin over (chi2, object) among the objects whose best pLS it is (SPEC.md 4.6).  No block-level barrier.
+// T3 pass: T3s contained in a pT5 are skipped (walk of the pT5 entries that hold the T3's first MD), and so are pLS that own
+// a pT5.
 constexpr int MATCH_WARPS = 4, MQ_CAP = 64;
+constexpr int MATCH_ZB = 3;           // zeta bins whose ranges are looked up in one go (wider windows take the slow walk)
 struct MatchWarp {
   unsigned long long key[32];                    // best (chi2, p) per lane's object
   int o_md[32][5];                               // the objects' MDs
@@ -415,43 +431,45 @@ struct MatchWarp {
 };
 
 template <int NA, bool IS_T3>
-__device__ __forceinline__ void match_drain2(const Slot& s, MatchWarp& W, int n, int lane) {
+__device__ __forceinline__ void match_drain2(const Slot& s, unsigned long long* key, MatchWarp& W, int n, int lane) {
   if (lane < n) {
     const int o = W.q2_o[lane], j = W.q2_j[lane];
     float chi = W.q2_c[lane];
     const float4 pa = s.pls_sa[j];
     const float2 pb = s.pls_sb[j];
     Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w; P.sec = pb.x; P.z0 = pb.y;
+    float4 an[NA]; int mt[NA];
+#pragma unroll
+    for (int q = 1; q < NA; ++q) { const int m = W.o_md[o][q]; an[q] = s.md_pos[m]; mt[q] = s.md_modt[m] & 3; }      // independent loads
     bool ok = true;
 #pragma unroll
     for (int q = 1; q < NA; ++q)
-      if (ok) { const int m = W.o_md[o][q]; ok = pls_anchor(P, s.md_pos[m], s.md_modt[m] & 3, chi); }
-    if (ok) atomicMin(&W.key[o], ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j]);   // chi2 >= 0: bit order = value order
+      if (ok) ok = pls_anchor(P, an[q], mt[q], chi);
+    if (ok) atomicMin(&key[o], ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j]);   // chi2 >= 0: bit order = value order
   }
 }
 template <int NA, bool IS_T3>
-__device__ __forceinline__ void match_drain1(const Slot& s, MatchWarp& W, int n, int& q2n, int lane, unsigned lt, int& n_cand) {
+__device__ __forceinline__ void match_drain1(const Slot& s, unsigned long long* key, MatchWarp& W, int n, int& q2n, int lane, unsigned lt) {
   bool ok = false;
   int o = 0, j = 0;
   float chi = 0.0f;
   if (lane < n) {
     o = W.q1_o[lane]; j = W.q1_j[lane];
-    ok = !IS_T3 || s.win5[s.pls_sidx[j]] == WIN_EMPTY;             // T3 pass: only pLS without a pT5
-    if (ok) {
-      const float4 pa = s.pls_sa[j];
-      const float2 pb = s.pls_sb[j];
-      Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w; P.sec = pb.x; P.z0 = pb.y;
-      const int m = W.o_md[o][0];
-      ok = pls_anchor(P, s.md_pos[m], s.md_modt[m] & 3, chi);
-    }
+    const int m = W.o_md[o][0];
+    const float4 pa = s.pls_sa[j];
+    const float2 pb = s.pls_sb[j];
+    const float4 a0 = s.md_pos[m];
+    const int mt0 = s.md_modt[m] & 3;
+    ok = !IS_T3 || !s.pls_taken[j];                              // T3 pass: only pLS without a pT5
+    Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w; P.sec = pb.x; P.z0 = pb.y;
+    if (ok) ok = pls_anchor(P, a0, mt0, chi);
   }
-  n_cand += n;
   const unsigned mask = __ballot_sync(0xffffffffu, ok);
   if (ok) { const int i = q2n + __popc(mask & lt); W.q2_o[i] = o; W.q2_j[i] = j; W.q2_c[i] = chi; }
   q2n += __popc(mask);
   __syncwarp();
   if (q2n >= 32) {
-    match_drain2<NA, IS_T3>(s, W, 32, lane);
+    match_drain2<NA, IS_T3>(s, key, W, 32, lane);
     __syncwarp();
     const int rest = q2n - 32;
     int a = 0, b = 0; float c = 0.f;
@@ -470,6 +488,7 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
   const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
   const int lane = threadIdx.x & 31;
   MatchWarp& W = Wall[threadIdx.x >> 5];
+  unsigned long long* key = W.key;
   const unsigned lt = (1u << lane) - 1u;
   const int* __restrict__ bstart = s.pls_bin_start;
   const float4* __restrict__ psa = s.pls_sa;
@@ -477,10 +496,11 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
   const int n_warps = gridDim.x * MATCH_WARPS;
   for (int t0 = (blockIdx.x * MATCH_WARPS + (threadIdx.x >> 5)) * 32; t0 < n; t0 += n_warps * 32) {
     const int t = t0 + lane;
+    // every warp loads the tile's objects for itself (no barrier before the walk)
     bool act = t < n;
     int md0 = 0;
     __syncwarp();
-    W.key[lane] = WIN_EMPTY;
+    key[lane] = WIN_EMPTY;
     if (act) {
       if (IS_T3) {
         const int4 abc = s.t3_abc[t];
@@ -503,74 +523,136 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
         md0 = m5[0];
       }
     }
+    __syncwarp();
     float4 a0 = make_float4(1.f, 0.f, 0.f, 1.f);
-    if (act) a0 = s.md_pos[md0];
+    int mt0 = 0;
+    if (act) { a0 = s.md_pos[md0]; mt0 = s.md_modt[md0] & 3; }
     const float r = a0.w;
     const float phi = atan2f(a0.y, a0.x);
     const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
     int q1n = 0, q2n = 0;
-    __syncwarp();
     for (int kb = 0; kb <= PLS_K; ++kb) {
-      const int base = kb * PLS_NB;
-      if (bstart[base + PLS_NB] == bstart[base]) continue;               // empty h-bucket (uniform)
-      // up to four index ranges [js, je) of sorted pLS for this object in this h-bucket
-      int js[4] = {0, 0, 0, 0}, len[4] = {0, 0, 0, 0};
-      if (act) {
-        if (kb == PLS_K) { js[0] = bstart[base]; len[0] = bstart[base + PLS_NB] - js[0]; }
-        else {
-          const float ulo = r * (kb * (LST_PLS_HMAX / PLS_K)), uhi = r * ((kb + 1) * (LST_PLS_HMAX / PLS_K));
-          const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
-          if (clo <= 1.0f) {                                             // else no circle of this curvature reaches r
-            const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
+    if (kb == PLS_K && bstart[PLS_NREG + 1] == bstart[PLS_NREG]) break;      // empty overflow bucket (uniform)
+    // ranges of sorted pLS this object must visit in this h-bucket: per zeta bin up to two psi windows, each possibly
+    // wrapping around -> up to MATCH_ZB x 4 slots.  All slot look-ups are independent loads issued together; the non-empty
+    // ranges (rarely more than one or two) are compacted into four register slots, the rest is walked afterwards.
+    int zb_lo = 0, n_zb = 0, pb0[2] = {0, 0}, pnb[2] = {0, 0};
+    if (kb == PLS_K) { n_zb = act ? 1 : 0; }
+    else if (act) {
+      const float h_lo = kb * (LST_PLS_HMAX / PLS_K), h_hi = (kb + 1) * (LST_PLS_HMAX / PLS_K);
+      const float ulo = r * h_lo, uhi = r * h_hi;
+      const float clo = 0.97f * ulo - tconst, chi_ = 1.03f * uhi + tconst;
+      if (clo <= 1.0f) {                                             // else no circle of this curvature reaches r
+        // psi windows
+        const float dmin = acosf(fminf(chi_, 1.0f)) - 1.0e-3f, dmax = acosf(fmaxf(clo, -1.0f)) + 1.0e-3f;
 #pragma unroll
-            for (int sgn = 0; sgn < 2; ++sgn) {
-              const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
-              const int blo = psi_bin_raw(lo);
-              const int nb = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
-              const int b0 = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
-              const int e0 = min(b0 + nb, PLS_NB);
-              js[2 * sgn] = bstart[base + b0]; len[2 * sgn] = bstart[base + e0] - js[2 * sgn];
-              if (b0 + nb > PLS_NB) { js[2 * sgn + 1] = bstart[base]; len[2 * sgn + 1] = bstart[base + b0 + nb - PLS_NB] - js[2 * sgn + 1]; }
-            }
-          }
+        for (int sgn = 0; sgn < 2; ++sgn) {
+          const float lo = sgn ? phi + dmin : phi - dmax, hi = sgn ? phi + dmax : phi - dmin;
+          const int blo = psi_bin_raw(lo);
+          pnb[sgn] = min(psi_bin_raw(hi) - blo + 1, PLS_NB);
+          pb0[sgn] = ((blo % PLS_NB) + PLS_NB) % PLS_NB;
         }
-      }
-      const int c1 = len[0], c2 = c1 + len[1], c3 = c2 + len[2], total = c3 + len[3];
-      for (int q = 0; __any_sync(0xffffffffu, q < total); ++q) {
-        bool pass = false;
-        int j = 0;
-        if (q < total) {
-          j = q < c1 ? js[0] + q : q < c2 ? js[1] + (q - c1) : q < c3 ? js[2] + (q - c2) : js[3] + (q - c3);
-          const float4 pa = __ldg(psa + j);
-          Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
-          float e, dT;
-          pass = pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT);                 // transverse test of the first anchor
-          ++n_tests;
-        }
-        const unsigned mask = __ballot_sync(0xffffffffu, pass);
-        if (mask) {
-          if (pass) { const int i = q1n + __popc(mask & lt); W.q1_o[i] = lane; W.q1_j[i] = j; }
-          q1n += __popc(mask);
-          __syncwarp();
-          if (q1n >= 32) {
-            match_drain1<NA, IS_T3>(s, W, 32, q2n, lane, lt, n_cand);
-            const int rest = q1n - 32;
-            int a = 0, b = 0;
-            if (lane < rest) { a = W.q1_o[32 + lane]; b = W.q1_j[32 + lane]; }
-            __syncwarp();
-            if (lane < rest) { W.q1_o[lane] = a; W.q1_j[lane] = b; }
-            q1n = rest;
-            __syncwarp();
-          }
-        }
+        // zeta window
+        const float ta = r * (0.97f * h_lo), tb = r * (1.03f * h_hi);
+        const float s_lo = 0.99f * r * arcfac(ta * ta), s_hi = 1.01f * r * arcfac(tb * tb);
+        const float ra = LST_PLS_RREF * (0.97f * h_lo), rb = LST_PLS_RREF * (1.03f * h_hi);
+        const float rho_a = LST_PLS_RREF * arcfac(ra * ra) / (r * arcfac(ta * ta)), rho_b = LST_PLS_RREF * arcfac(rb * rb) / (r * arcfac(tb * tb));
+        const float rho_lo = 0.98f * fminf(rho_a, rho_b), rho_hi = 1.02f * fmaxf(rho_a, rho_b);
+        const float dz = anchor_dz(mt0), dr = anchor_dr(mt0);
+        const float den = s_lo - dr - 0.003f * s_hi;
+        float cb = LST_PLS_COTCAP;
+        if (den > 0.5f * s_lo) cb = fminf(cb, 1.02f * (fabsf(a0.z) + LST_PLS_Z0B + dz + 0.003f * s_hi + 0.05f) / den);
+        const float dZmax = dz + dr * cb + 0.003f * s_hi * (1.0f + cb) + 0.05f;
+        const float spread = fmaxf(fabsf(1.0f - rho_lo), fabsf(1.0f - rho_hi)) * LST_PLS_Z0B + rho_hi * dZmax + 1.0f;
+        const float zmin = fminf(rho_lo * a0.z, rho_hi * a0.z) - spread, zmax = fmaxf(rho_lo * a0.z, rho_hi * a0.z) + spread;
+        zb_lo = zeta_bin(zmin);
+        n_zb = zeta_bin(zmax) - zb_lo + 1;
       }
     }
-    if (q1n) match_drain1<NA, IS_T3>(s, W, q1n, q2n, lane, lt, n_cand);
+    int rjs[4] = {0, 0, 0, 0}, rlen[4] = {0, 0, 0, 0}, nr = 0;
+    auto add_range = [&](int js, int len) {
+      if (len > 0) {
+        if (nr == 0) { rjs[0] = js; rlen[0] = len; } else if (nr == 1) { rjs[1] = js; rlen[1] = len; }
+        else if (nr == 2) { rjs[2] = js; rlen[2] = len; } else if (nr == 3) { rjs[3] = js; rlen[3] = len; }
+        ++nr;
+      }
+    };
+    auto slot_range = [&](int sl, int& js, int& len) {
+      js = 0; len = 0;
+      if (kb == PLS_K) { if (sl == 0) { js = bstart[PLS_NREG]; len = bstart[PLS_NREG + 1] - js; } return; }
+      const int zb = zb_lo + (sl >> 2), sgn = (sl >> 1) & 1, part = sl & 1;
+      const int base = (kb * PLS_NZ + zb) * PLS_NB;
+      const int b0 = sgn ? pb0[1] : pb0[0], nb = sgn ? pnb[1] : pnb[0];
+      if (part == 0) { const int e0 = min(b0 + nb, PLS_NB); js = bstart[base + b0]; len = bstart[base + e0] - js; }
+      else if (b0 + nb > PLS_NB) { js = bstart[base]; len = bstart[base + b0 + nb - PLS_NB] - js; }
+    };
+    const int n_slots = n_zb * 4;
+    {
+      int js[MATCH_ZB * 4], len[MATCH_ZB * 4];
+#pragma unroll
+      for (int sl = 0; sl < MATCH_ZB * 4; ++sl) { js[sl] = 0; len[sl] = 0; if (sl < n_slots) slot_range(sl, js[sl], len[sl]); }
+#pragma unroll
+      for (int sl = 0; sl < MATCH_ZB * 4; ++sl) add_range(js[sl], len[sl]);
+    }
+    // walk: first the (up to four) compacted ranges as one flat index space ...
+    auto test_one = [&](bool has, int j) {
+      bool pass = false;
+      if (has) {
+        const float4 pa = __ldg(psa + j);
+        Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
+        float e, dT;
+        pass = pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT);                 // transverse test of the first anchor
+        ++n_tests;
+      }
+      const unsigned mask = __ballot_sync(0xffffffffu, pass);
+      if (mask) {
+        if (pass) { const int i = q1n + __popc(mask & lt); W.q1_o[i] = lane; W.q1_j[i] = j; }
+        q1n += __popc(mask);
+        __syncwarp();
+        if (q1n >= 32) {
+          n_cand += 32;
+          match_drain1<NA, IS_T3>(s, key, W, 32, q2n, lane, lt);
+          const int rest = q1n - 32;
+          int a = 0, b = 0;
+          if (lane < rest) { a = W.q1_o[32 + lane]; b = W.q1_j[32 + lane]; }
+          __syncwarp();
+          if (lane < rest) { W.q1_o[lane] = a; W.q1_j[lane] = b; }
+          q1n = rest;
+          __syncwarp();
+        }
+      }
+    };
+    {
+      const int c1 = rlen[0], c2 = c1 + rlen[1], c3 = c2 + rlen[2], total = c3 + rlen[3];
+      for (int q = 0; __any_sync(0xffffffffu, q < total); ++q) {
+        const int j = q < c1 ? rjs[0] + q : q < c2 ? rjs[1] + (q - c1) : q < c3 ? rjs[2] + (q - c2) : rjs[3] + (q - c3);
+        test_one(q < total, j);
+      }
+    }
+    // ... then whatever did not fit: more than four non-empty ranges, or a zeta window wider than MATCH_ZB bins (rare)
+    if (__any_sync(0xffffffffu, nr > 4 || n_zb > MATCH_ZB)) {
+      for (int sl = 0; __any_sync(0xffffffffu, sl < n_slots); ++sl) {
+        int js = 0, len = 0;
+        if (sl < n_slots && (nr > 4 || n_zb > MATCH_ZB)) {
+          slot_range(sl, js, len);
+          // skip the ranges the flat walk already covered: the first four non-empty ones among the first MATCH_ZB * 4 slots
+          if (sl < MATCH_ZB * 4 && len > 0) {
+            bool covered = false;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) covered |= (k < min(nr, 4)) && rjs[k] == js && rlen[k] == len;
+            if (covered) len = 0;
+          }
+        }
+        for (int q = 0; __any_sync(0xffffffffu, q < len); ++q) test_one(q < len, js + q);
+      }
+    }
+    }     // h-buckets
+    if (q1n) { n_cand += q1n; match_drain1<NA, IS_T3>(s, key, W, q1n, q2n, lane, lt); }
     __syncwarp();
-    if (q2n) match_drain2<NA, IS_T3>(s, W, q2n, lane);
+    if (q2n) match_drain2<NA, IS_T3>(s, key, W, q2n, lane);
     __syncwarp();
     if (act) {
-      const unsigned long long k = W.key[lane];
+      const unsigned long long k = key[lane];
       const int best = (k == WIN_EMPTY) ? -1 : (int)(k & 0xFFFFFFFFull);
       const float chi = (k == WIN_EMPTY) ? 0.0f : __uint_as_float((unsigned)(k >> 32));
       if (IS_T3) { s.best3[t] = best; s.chi3[t] = chi; if (best >= 0) atomicMin(s.win3 + best, win_key(chi, t)); }
@@ -591,6 +673,7 @@ __global__ void k_pt5_lists(const Slot* __restrict__ slots) {
   const Slot& s = slots[blockIdx.y];
   LST_FOR_ITEMS(p, s.n_pls) {
     const unsigned long long w = s.win5[p];
+    s.pls_taken[s.pls_pos[p]] = (w != WIN_EMPTY);        // by sorted position: one load in the T3 pass
     if (w == WIN_EMPTY) continue;
     const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(w & 0xFFFFFFFFull)];
     for (int q = 0; q < 5; ++q) {
