@@ -43,7 +43,7 @@ extern "C" {
 
 /* object types for lst_get */
 enum { LST_OBJ_HIT = 0, LST_OBJ_MD = 1, LST_OBJ_LS = 2, LST_OBJ_T3 = 3, LST_OBJ_T5C = 4, LST_OBJ_T5 = 5,
-       LST_OBJ_TC = 6, LST_OBJ_MATCH5 = 7, LST_N_OBJ = 8 };
+       LST_OBJ_TC = 6, LST_OBJ_MATCH5 = 7, LST_OBJ_TCC = 8, LST_OBJ_TCX = 9, LST_N_OBJ = 10 };
 
 /* indices into counts[] of lst_status: number of objects per type after clamping to capacity,
  * then the UNCLAMPED totals (what the stage would have produced), then pair-test counts. */
@@ -54,7 +54,9 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        LST_CNT_M5_TESTS, LST_CNT_M5_CAND, LST_CNT_M3_TESTS, LST_CNT_M3_CAND,
        /* internal: fill of the MD / LS record buffers; tile tickets of the row scans and of the T3 / T5 tiles */
        LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TK_SENSOR, LST_CNT_TK_MD, LST_CNT_TK_LS, LST_CNT_TK_T5,
-       LST_CNT_DYN_T3, LST_CNT_DYN_T5, LST_N_CNT = 32 };
+       LST_CNT_DYN_T3, LST_CNT_DYN_T5,
+       /* f1: number of track candidates kept by the duplicate cleaning; tile ticket of that step */
+       LST_CNT_TCC, LST_CNT_TK_TCC, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */
 
@@ -91,6 +93,9 @@ typedef struct {
  *  TC    : i0 = tc[n][3] int32 (type 0 pT5 / 1 T5 / 2 pT3 / 3 pLS, pLS index or -1, T5-list or T3
  *          index or -1)
  *  MATCH5: i0 = best5_pls[n_t5] int32 (-1 = unmatched), f0 = chi2[n_t5]
+ *  TCC   : i0 = tcc[n][3] int32: the TC rows kept by the duplicate cleaning (SPEC.md 4.7), in TC order
+ *  TCX   : per row of the TC list (count = the TC count): i0 = keep[n] int32 (1 = kept), i1 = hits[n][12] int32 (the ten ORIGINAL hit
+ *          indices of the candidate's MDs, lower then upper, -1 padded, then two -1 to make rows 48 bytes), i2 = q[n] (bit pattern of the chi2 in its rank key)
  */
 typedef struct {
   int32_t capacity;

@@ -261,6 +261,39 @@ inline bool pls_anchor(const PLS<R>& p, const MD<R>& m, R loosen, R* chi2) {
   return true;
 }
 
+// ---------------------------------------------------------------- f1: duplicate cleaning (SPEC.md 4.7)
+// rank key (type, q, row), smaller = better; X is a duplicate iff a better-ranked Y holds more than half of X's hits
+inline bool better_rank(const TC& y, uint32_t qy, int32_t iy, const TC& x, uint32_t qx, int32_t ix) {
+  if (y.type != x.type) return y.type < x.type;
+  if (qy != qx) return qy < qx;
+  return iy < ix;
+}
+inline void clean_duplicates(int32_t n, const TC* tc, const uint32_t* q, const int32_t* hits /*[n][10]*/, const int32_t* nh,
+                             std::vector<int32_t>& keep) {
+  keep.assign(n, 1);
+  // Y can only hold more than half of X's hits if it holds at least one of them: list, per hit, the candidates that
+  // contain it, and test X only against the candidates found under X's own hits (otherwise the plain all-pairs loop)
+  int32_t max_hit = -1;
+  for (int32_t i = 0; i < n; ++i) for (int a = 0; a < nh[i]; ++a) max_hit = std::max(max_hit, hits[10 * i + a]);
+  std::vector<std::vector<int32_t>> holders(size_t(max_hit + 1));
+  for (int32_t i = 0; i < n; ++i) if (tc[i].type <= 2) for (int a = 0; a < nh[i]; ++a) holders[hits[10 * i + a]].push_back(i);
+  for (int32_t x = 0; x < n; ++x) {
+    if (tc[x].type > 2) continue;                       // pLS candidates carry no outer-tracker hits
+    for (int a0 = 0; a0 < nh[x] && keep[x]; ++a0) {
+      for (int32_t y : holders[hits[10 * x + a0]]) {
+        if (y == x || !better_rank(tc[y], q[y], y, tc[x], q[x], x)) continue;
+        int shared = 0;
+        for (int a = 0; a < nh[x]; ++a) {               // slots of X whose hit occurs anywhere in Y
+          bool in_y = false;
+          for (int b = 0; b < nh[y]; ++b) in_y = in_y || hits[10 * y + b] == hits[10 * x + a];
+          shared += in_y;
+        }
+        if (2 * shared > nh[x]) keep[x] = 0;
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------- the chain
 template <typename R> struct Result {
   uint32_t flags = 0;                 // bit 0: a hit key was out of range (hit dropped)
@@ -277,6 +310,11 @@ template <typename R> struct Result {
   std::vector<TC> tc;
   std::vector<int32_t> best5_pls;     // per T5: best matching pLS or -1
   std::vector<float> chi5;            // per T5: chi2 of that match
+  std::vector<float> chi3;            // per T3: chi2 of its best free-seed match (0 if none)
+  std::vector<int32_t> tc_keep;       // per TC row: 1 = kept by the duplicate cleaning (SPEC.md 4.7)
+  std::vector<int32_t> tc_hits;       // per TC row: its 10 ORIGINAL hit indices (-1 padded), the tuple the cleaning compares
+  std::vector<int32_t> tc_q;          // per TC row: chi2 bit pattern that enters its rank key
+  std::vector<TC> tcc;                // cleaned TC list
   int64_t n_md_pairs = 0, n_ls_pairs = 0, n_t3_pairs = 0, n_t5_pairs = 0, n_match5 = 0, n_match3 = 0;
 };
 
@@ -463,11 +501,37 @@ Result<R>* run_chain(int32_t M, const uint8_t* subdet, const uint8_t* mtype, con
     if (p < 0) continue;
     if (win3[p] < 0 || chi3[x] < chi3[win3[p]]) win3[p] = x;
   }
+  res->chi3.assign(n_t3, 0.0f);
+  for (int32_t x = 0; x < n_t3; ++x) res->chi3[x] = float(chi3[x]);
   // emit: pT5 (by p), T5 (by t), pT3 (by p), pLS (by p) -- mutually exclusive
   for (int32_t p = 0; p < n_pls; ++p) if (win5[p] >= 0) res->tc.push_back(TC{0, p, win5[p]});
   for (int32_t t = 0; t < n_t5; ++t) if (res->best5_pls[t] < 0) res->tc.push_back(TC{1, -1, t});
   for (int32_t p = 0; p < n_pls; ++p) if (win5[p] < 0 && win3[p] >= 0) res->tc.push_back(TC{2, p, win3[p]});
   for (int32_t p = 0; p < n_pls; ++p) if (win5[p] < 0 && win3[p] < 0) res->tc.push_back(TC{3, p, -1});
+  if (last_stage < 6) return res;
+
+  // ---- f1: duplicate cleaning (SPEC.md 4.7)
+  {
+    const int32_t n_tc = int32_t(res->tc.size());
+    std::vector<int32_t> hits(size_t(n_tc) * 10, -1), nh(n_tc, 0);
+    std::vector<uint32_t> q(n_tc, 0u);
+    for (int32_t i = 0; i < n_tc; ++i) {
+      const TC& c = res->tc[i];
+      int32_t mds[5], nm = 0;
+      if (c.type <= 1) { const int32_t* m5 = res->t5c[res->t5[c.obj]].md; for (int k = 0; k < 5; ++k) mds[k] = m5[k]; nm = 5; }
+      else if (c.type == 2) { const T3<R>& u = res->t3[c.obj]; mds[0] = u.a; mds[1] = u.b; mds[2] = u.c; nm = 3; }
+      for (int k = 0; k < nm; ++k) { hits[10 * i + 2 * k] = ho[res->md[mds[k]].hit_lo]; hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_up]; }
+      nh[i] = 2 * nm;
+      float chi = 0.0f;
+      if (c.type == 0) chi = res->chi5[c.obj];
+      if (c.type == 2) chi = res->chi3[c.obj];
+      std::memcpy(&q[i], &chi, 4);
+    }
+    clean_duplicates(n_tc, res->tc.data(), q.data(), hits.data(), nh.data(), res->tc_keep);
+    res->tc_hits = hits;
+    res->tc_q.assign(q.begin(), q.end());
+    for (int32_t i = 0; i < n_tc; ++i) if (res->tc_keep[i]) res->tcc.push_back(res->tc[i]);
+  }
   return res;
 }
 
@@ -482,6 +546,7 @@ template <typename R> int64_t count_of(const Result<R>* r, int what) {
     case 4: return int64_t(r->t5c.size());
     case 5: return int64_t(r->t5.size());
     case 6: return int64_t(r->tc.size());
+    case 8: return int64_t(r->tcc.size());
     case 10: return r->n_md_pairs;
     case 11: return r->n_ls_pairs;
     case 12: return r->n_t3_pairs;
@@ -510,6 +575,10 @@ template <typename R> void copy_int(const Result<R>* r, int what, int32_t* o) {
     case 5: for (size_t i = 0; i < r->t5.size(); ++i) o[i] = r->t5[i]; break;
     case 6: for (size_t i = 0; i < r->tc.size(); ++i) { o[3 * i] = r->tc[i].type; o[3 * i + 1] = r->tc[i].pls; o[3 * i + 2] = r->tc[i].obj; } break;
     case 7: for (size_t i = 0; i < r->best5_pls.size(); ++i) o[i] = r->best5_pls[i]; break;
+    case 8: for (size_t i = 0; i < r->tcc.size(); ++i) { o[3 * i] = r->tcc[i].type; o[3 * i + 1] = r->tcc[i].pls; o[3 * i + 2] = r->tcc[i].obj; } break;
+    case 9: for (size_t i = 0; i < r->tc_keep.size(); ++i) o[i] = r->tc_keep[i]; break;
+    case 10: for (size_t i = 0; i < r->tc_hits.size(); ++i) o[i] = r->tc_hits[i]; break;
+    case 11: for (size_t i = 0; i < r->tc_q.size(); ++i) o[i] = r->tc_q[i]; break;
     case 21: for (size_t i = 0; i < r->sensor_start.size(); ++i) o[i] = r->sensor_start[i]; break;
   }
 }
@@ -525,6 +594,7 @@ template <typename R> void copy_real(const Result<R>* r, int what, double* o) {
         q[0] = double(t.cin); q[1] = double(t.cbr); q[2] = double(t.cout); q[3] = double(t.score);
         for (int f = 0; f < N_FEAT; ++f) q[4 + f] = double(t.feat[f]); } break;
     case 7: for (size_t i = 0; i < r->chi5.size(); ++i) o[i] = double(r->chi5[i]); break;
+    case 9: for (size_t i = 0; i < r->chi3.size(); ++i) o[i] = double(r->chi3[i]); break;
   }
 }
 
@@ -610,6 +680,14 @@ void lst_oracle_pls_residual(const double* pls5, int32_t q, const double* xyz, d
   const double t = r * p.h;
   const double s = r * arcfac<double>(t * t);
   out[0] = e; out[1] = xyz[2] - (p.z0 + s * p.cot); out[2] = s;
+}
+// duplicate cleaning on hand-made candidates: types[n], q[n] (chi2 bit patterns), hits[n][10] (-1 padded), nh[n] -> keep[n]
+void lst_oracle_tc_clean(int32_t n, const int32_t* types, const uint32_t* q, const int32_t* hits, const int32_t* nh, int32_t* keep_out) {
+  std::vector<TC> tc(n);
+  for (int i = 0; i < n; ++i) tc[i] = TC{types[i], -1, -1};
+  std::vector<int32_t> keep;
+  clean_duplicates(n, tc.data(), q, hits, nh, keep);
+  for (int i = 0; i < n; ++i) keep_out[i] = keep[i];
 }
 float lst_oracle_arcfac(float u) { return arcfac<float>(u); }
 double lst_oracle_arcfac_f64(double u) { return arcfac<double>(u); }

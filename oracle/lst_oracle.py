@@ -14,7 +14,7 @@ _LIB = os.path.join(_HERE, "liblst_oracle.so")
 CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
 
 CUTS = ["M2", "M3", "L1", "L2", "L3", "T1", "T2", "T3", "Q1", "Q2", "P5", "P3"]
-STAGE = {"sort": 0, "md": 1, "ls": 2, "t3": 3, "t5": 4, "tc": 5}
+STAGE = {"sort": 0, "md": 1, "ls": 2, "t3": 3, "t5": 4, "tc": 5, "clean": 6}
 
 
 def build(force: bool = False) -> str:
@@ -48,6 +48,7 @@ def _bind(path):
     L.lst_oracle_pls_match.restype = C.c_int32
     L.lst_oracle_pls_match.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
     L.lst_oracle_pls_residual.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    L.lst_oracle_tc_clean.argtypes = [C.c_int32] + [C.c_void_p] * 5
     L.lst_oracle_arcfac.restype = C.c_float
     L.lst_oracle_arcfac.argtypes = [C.c_float]
     L.lst_oracle_arcfac_f64.restype = C.c_double
@@ -96,8 +97,8 @@ class OracleResult:
     def __init__(self, h, L):
         cnt = lambda w: int(L.lst_oracle_count(h, w))
 
-        def ints(w, k):
-            n = cnt(w if w < 7 else 5)
+        def ints(w, k, nw=None):
+            n = cnt((w if w < 7 else 5) if nw is None else nw)
             o = np.zeros((n, k), dtype=np.int32)
             if n:
                 L.lst_oracle_copy_int(h, w, _p(o))
@@ -129,12 +130,18 @@ class OracleResult:
         self.tc = ints(6, 3)
         self.best5_pls = ints(7, 1)[:, 0]
         self.chi5 = reals(7, 1, nw=5)[:, 0]
+        self.chi3 = reals(9, 1, nw=3)[:, 0]
+        self.tcc = ints(8, 3, nw=8)                 # cleaned TC list (SPEC.md 4.7)
+        self.tc_keep = ints(9, 1, nw=6)[:, 0]
+        has_clean = len(self.tc_keep) == len(self.tc)
+        self.tc_hits = ints(10, 10, nw=6) if has_clean else np.zeros((0, 10), np.int32)     # hit tuple of every TC row
+        self.tc_q = ints(11, 1, nw=6)[:, 0].view(np.uint32) if has_clean else np.zeros(0, np.uint32)
         self.counts = dict(hits=cnt(0), md=cnt(1), ls=cnt(2), t3=cnt(3), t5c=cnt(4), t5=cnt(5), tc=cnt(6),
                            md_pairs=cnt(10), ls_pairs=cnt(11), t3_pairs=cnt(12), t5_pairs=cnt(13),
                            match5=cnt(14), match3=cnt(15))
 
 
-def run(geo, weights, ev, *, t5_override=None, loosen=None, use_double=False, last_stage="tc",
+def run(geo, weights, ev, *, t5_override=None, loosen=None, use_double=False, last_stage="clean",
         counts_only=False):
     """Run the whole chain on one event.  `geo` needs n_modules, subdet, mtype, conn_rowptr, conn_col."""
     L = lib()
@@ -197,6 +204,16 @@ def pls_residual(pls5, q, xyz):
     out = np.zeros(3, dtype=np.float64)
     lib().lst_oracle_pls_residual(_p(p), int(q), _p(a), _p(out))
     return out
+
+
+def tc_clean(types, chi2, hits, nh):
+    """SPEC.md 4.7 on hand-made candidates: types[n], chi2[n] (fp32), hits[n][10] (-1 padded), nh[n] -> keep[n]"""
+    t = np.ascontiguousarray(types, dtype=np.int32); n = t.size
+    q = np.ascontiguousarray(chi2, dtype=np.float32).view(np.uint32)
+    h = np.ascontiguousarray(hits, dtype=np.int32).reshape(n, 10); k = np.ascontiguousarray(nh, dtype=np.int32)
+    keep = np.zeros(n, dtype=np.int32)
+    lib().lst_oracle_tc_clean(n, _p(t), _p(q), _p(h), _p(k), _p(keep))
+    return keep
 
 
 def arcfac(u, f64=False):

@@ -10,9 +10,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = os.path.join(_HERE, "liblst_b200.so")
 
 LST_N_CNT = 32
-OBJ = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, match5=7)
+OBJ = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, match5=7, tcc=8, tcx=9)
 CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t3=9, raw_t5c=10,
-           raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20)
+           raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20, tcc=29)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
            "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_measure_fp32", "lst_launches_per_run",
@@ -119,7 +119,10 @@ _FIELDS = {
     "t5": dict(i0=("cand", "i32", 1)),
     "tc": dict(i0=("tc", "i32", 3)),
     "match5": dict(i0=("best5_pls", "i32", 1), f0=("chi2", "f32", 1)),
+    "tcc": dict(i0=("tc", "i32", 3)),
+    "tcx": dict(i0=("keep", "i32", 1), i1=("hits", "i32", 12), i2=("q", "i32", 1)),
 }
+_ROWS = {"match5": "t5", "tcx": "tc"}      # views whose row count is another list's count
 
 
 class LST:
@@ -198,7 +201,7 @@ class LST:
         _chk(self.lib.lst_get(self.ctx, slot, OBJ[name], C.byref(v)), "lst_get")
         if n is None:
             _, cnt = self.lst_status(slot)
-            n = cnt["t5" if name == "match5" else name]
+            n = cnt[_ROWS.get(name, name)]
         out = {}
         t = self.torch
         for fld, (label, dt, cols) in _FIELDS[name].items():
@@ -292,7 +295,7 @@ class LST:
         bits, cnt = self.lst_status(slot)
         res = dict(status=bits, counts=cnt)
         for name in _FIELDS:
-            n = cnt["t5" if name == "match5" else name]
+            n = cnt[_ROWS.get(name, name)]
             res[name] = {k: v.cpu().numpy() for k, v in self.lst_get(slot, name, n).items()}
         return res
 

@@ -113,7 +113,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   // 0xFF region
   {
     Carver z{nullptr};
-    z.take<unsigned long long>(k.max_pls); z.take<unsigned long long>(k.max_pls); z.take<int>(k.max_md);
+    z.take<unsigned long long>(k.max_pls); z.take<unsigned long long>(k.max_pls); z.take<int>(k.max_md); z.take<int>(k.max_hits);
     L.ones_stride = z.off;
     L.ones_base = base ? base + cv.off : nullptr;
     for (int s = 0; s < n_slots; ++s) {
@@ -121,7 +121,8 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
       auto* w5 = c2.take<unsigned long long>(k.max_pls);
       auto* w3 = c2.take<unsigned long long>(k.max_pls);
       int* head = c2.take<int>(k.max_md);
-      if (out) { (*out)[s].win5 = w5; (*out)[s].win3 = w3; (*out)[s].md_head = head; }
+      int* hhead = c2.take<int>(k.max_hits);
+      if (out) { (*out)[s].win5 = w5; (*out)[s].win3 = w3; (*out)[s].md_head = head; (*out)[s].hit_head = hhead; }
     }
     cv.off += L.ones_stride * n_slots;
   }
@@ -147,10 +148,12 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
+    t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc);
+    t.tcc = cv.take<int>(3 * (size_t)k.max_tc); t.chain_tcc = cv.take<unsigned long long>(k.max_tc / TCC_ROWS + 4);
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
-      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head;
+      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
       d = t;
     }
   }
@@ -163,7 +166,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 19;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 21;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -226,6 +229,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (M / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (c->caps.max_md / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5s, 0, sizeof(unsigned long long) * (c->caps.max_t5c / SCAN_TILE + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_tcc, 0, sizeof(unsigned long long) * (c->caps.max_tc / TCC_ROWS + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t3, 0, sizeof(unsigned long long) * (c->caps.max_ls / TUPLE_TPB + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
   }
@@ -332,6 +336,8 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_pt5_lists<<<G, 128, 0, st>>>(sl); LST_MARK();
   k_match<3, true><<<G, MATCH_WARPS * 32, 0, st>>>(sl); LST_MARK();
   k_tc_emit<<<G1, 1024, 0, st>>>(sl, k); LST_MARK();
+  k_tc_tuples<<<G, 128, 0, st>>>(sl); LST_MARK();
+  k_tc_clean<<<GL, TCC_TPB, 0, st>>>(sl, k); LST_MARK();
 #undef LST_MARK
   if (li != N_LAUNCHES + 2) return LST_EINVAL;
   return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
@@ -388,7 +394,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
       "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_sweep", "a1.scan", "a1.md_finish", "a2.ls_sweep", "a2.scan", "a2.ls_finish",
-      "a3.t3", "a4.t5", "a5.dnn", "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit"};
+      "a3.t3", "a4.t5", "a5.dnn", "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit", "f1.tc_tuples", "f1.tc_clean"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 
@@ -412,6 +418,8 @@ int lst_get(lst_ctx* c, int32_t slot, int32_t objtype, lst_view* v) {
     case LST_OBJ_T5: v->capacity = c->caps.max_t5; v->count = s.cnt + LST_CNT_T5; v->i0 = s.t5_list; break;
     case LST_OBJ_TC: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TC; v->i0 = s.tc; break;
     case LST_OBJ_MATCH5: v->capacity = c->caps.max_t5; v->count = s.cnt + LST_CNT_T5; v->i0 = s.best5; v->f0 = s.chi5; break;
+    case LST_OBJ_TCC: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TCC; v->i0 = s.tcc; break;
+    case LST_OBJ_TCX: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TC; v->i0 = s.tc_keep; v->i1 = s.tc_hits; v->i2 = s.tc_q; break;
   }
   return LST_OK;
 }

@@ -15,6 +15,7 @@ namespace lst {
 constexpr int N_FEAT = 23, N_HID = 32, N_W = 1857;
 constexpr int CNT_STATUS = LST_N_CNT - 1;
 constexpr unsigned long long WIN_EMPTY = 0xFFFFFFFFFFFFFFFFull;
+constexpr int TC_HSTRIDE = 12;         // ints per row of the candidates' hit tuples (10 hits, padded for 16-byte loads)
 
 struct Geo {   // device copies, shared by all slots
   int n_modules;
@@ -48,6 +49,7 @@ struct Slot {
   unsigned long long* win5; // [max_pls]  (chi2 bits << 32 | T5 index)
   unsigned long long* win3; // [max_pls]
   int* md_head;             // [max_md]  head of the list of pT5 entries containing this MD
+  int* hit_head;            // [max_hits] head of the list of (TC row, slot) entries holding this ORIGINAL hit (f1)
   // a0
   int2* tmp_ok; float4* hit; int* hit_orig;
   // a1
@@ -65,6 +67,7 @@ struct Slot {
   // a6
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
+  int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc;     // f1 duplicate cleaning
   // host-load staging
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
   int* tc_hdr;                       // copy of cnt[] in front of the TC rows, so one D2H copy reads both
@@ -736,8 +739,120 @@ __global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots
     s.cnt[LST_CNT_TC] = min(base_out, caps.max_tc);
     if (base_out > caps.max_tc) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_TC);
   }
-  __syncthreads();
-  if (tid < LST_N_CNT) s.tc_hdr[tid] = s.cnt[tid];      // every counter is final here: last kernel of the chain
+}
+
+// f1 (SPEC.md 4.7), step 1: the hit tuple of every candidate (ORIGINAL indices: lower, upper hit of each of its MDs), the chi2
+// of its rank key, and its entry in the list of every hit it holds.  One thread per TC row.
+__global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  LST_FOR_ITEMS(o, s.cnt[LST_CNT_TC]) {
+    const int type = s.tc[3 * o], obj = s.tc[3 * o + 2];
+    int md[5] = {-1, -1, -1, -1, -1};
+    float chi = 0.0f;
+    if (type <= 1) {
+      const int* m5 = s.t5c_md + 5 * s.t5_list[obj];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) md[q] = m5[q];
+      if (type == 0) chi = s.chi5[obj];
+    } else if (type == 2) {
+      const int4 abc = s.t3_abc[obj];
+      md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
+      chi = s.chi3[obj];
+    }
+    s.tc_q[o] = __float_as_int(chi);
+    int2 h[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) h[q] = md[q] >= 0 ? s.md_hits[md[q]] : make_int2(-1, -1);
+    int* row = s.tc_hits + TC_HSTRIDE * o;
+    *reinterpret_cast<int4*>(row) = make_int4(h[0].x, h[0].y, h[1].x, h[1].y);
+    *reinterpret_cast<int4*>(row + 4) = make_int4(h[2].x, h[2].y, h[3].x, h[3].y);
+    *reinterpret_cast<int4*>(row + 8) = make_int4(h[4].x, h[4].y, -1, -1);
+#pragma unroll
+    for (int q = 0; q < 5; ++q)
+      if (md[q] >= 0) {
+        s.tc_next[10 * o + 2 * q] = atomicExch(s.hit_head + h[q].x, 10 * o + 2 * q);
+        s.tc_next[10 * o + 2 * q + 1] = atomicExch(s.hit_head + h[q].y, 10 * o + 2 * q + 1);
+      }
+  }
+}
+
+// f1, step 2: X is dropped iff some candidate Y with a better rank key (type, chi2 bits, row) holds more than half of X's
+// hits.  Y must then hold at least one of them: one thread per (row X, hit slot) walks the list of that hit.  A tile is
+// TCC_ROWS rows x 10 slots; the kept rows are compacted in order with a block scan + look-back across tiles (by ticket).
+constexpr int TCC_TPB = 128, TCC_ROWS = 12;
+__global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ slots, Caps caps) {
+  __shared__ int s_keep[TCC_ROWS];
+  __shared__ int s_tile, s_base;
+  const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
+  const int n = s.cnt[LST_CNT_TC];
+  const int n_tiles = (n + TCC_ROWS - 1) / TCC_ROWS + (n == 0);
+  const int lane = threadIdx.x & 31;
+  const int rl = threadIdx.x / 10, slot = threadIdx.x - 10 * rl;       // row of the tile, hit slot
+  while (true) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(s.cnt + LST_CNT_TK_TCC, 1);
+    if (threadIdx.x < TCC_ROWS) s_keep[threadIdx.x] = 1;
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int x = tile * TCC_ROWS + rl;
+    if (rl < TCC_ROWS && x < n) {
+      const int type = s.tc[3 * x];
+      const int nh = type == 2 ? 6 : type <= 1 ? 10 : 0;
+      if (slot < nh) {
+        const unsigned qx = (unsigned)s.tc_q[x];
+        const int* rx = s.tc_hits + TC_HSTRIDE * x;
+        const int4 x0 = *reinterpret_cast<const int4*>(rx), x1 = *reinterpret_cast<const int4*>(rx + 4), x2 = *reinterpret_cast<const int4*>(rx + 8);
+        const int hx[10] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w, x2.x, x2.y};
+        int mine = hx[0];
+#pragma unroll
+        for (int a = 1; a < 10; ++a) mine = (slot == a) ? hx[a] : mine;
+        for (int e = s.hit_head[mine]; e >= 0; e = s.tc_next[e]) {
+          const int y = e / 10;
+          if (y == x) continue;
+          const int ty = s.tc[3 * y];
+          const unsigned qy = (unsigned)s.tc_q[y];
+          const bool better = ty != type ? ty < type : qy != qx ? qy < qx : y < x;
+          if (!better) continue;
+          const int* ry = s.tc_hits + TC_HSTRIDE * y;
+          const int4 y0 = *reinterpret_cast<const int4*>(ry), y1 = *reinterpret_cast<const int4*>(ry + 4), y2 = *reinterpret_cast<const int4*>(ry + 8);
+          const int hy[10] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w, y2.x, y2.y};     // -1 padded: never equals a hit of X
+          int shared = 0;
+#pragma unroll
+          for (int a = 0; a < 10; ++a) {
+            bool in_y = false;
+#pragma unroll
+            for (int b = 0; b < 10; ++b) in_y |= hy[b] == hx[a];
+            shared += (a < nh) && in_y;
+          }
+          if (2 * shared > nh) { s_keep[rl] = 0; break; }
+        }
+      }
+    }
+    __syncthreads();
+    // ordered compaction of the kept rows (the tile's rows are handled by its first TCC_ROWS threads: one warp)
+    int keep = 0;
+    const int xr = tile * TCC_ROWS + threadIdx.x;
+    if (threadIdx.x < TCC_ROWS && xr < n) keep = s_keep[threadIdx.x];
+    if (threadIdx.x < 32) {
+      const unsigned bal = __ballot_sync(0xffffffffu, keep);
+      const int btot = __popc(bal);
+      const int base = chain_exclusive(s.chain_tcc, tile, btot, lane, epoch);
+      if (threadIdx.x < TCC_ROWS && xr < n) {
+        s.tc_keep[xr] = keep;
+        if (keep) {
+          const int o = base + __popc(bal & ((1u << lane) - 1u));
+          s.tcc[3 * o] = s.tc[3 * xr]; s.tcc[3 * o + 1] = s.tc[3 * xr + 1]; s.tcc[3 * o + 2] = s.tc[3 * xr + 2];
+        }
+      }
+      if (tile == n_tiles - 1) {       // last kernel of the chain: every counter is final once this tile knows its base
+        if (lane == 0) s.cnt[LST_CNT_TCC] = base + btot;
+        __syncwarp();
+        if (lane < LST_N_CNT) s.tc_hdr[lane] = s.cnt[lane];      // header copy in front of the TC rows (one D2H copy reads both)
+      }
+    }
+    __syncthreads();
+  }
 }
 
 // binds an event to a slot (stream-ordered, so a later lst_run on the same stream sees it)
@@ -784,23 +899,10 @@ __global__ void k_pack_tc(const Slot* __restrict__ slots, int rows, int* __restr
   }
   LST_FOR_ITEMS(i, LST_N_CNT) o[i] = s.tc_hdr[i];
   LST_FOR_ITEMS(i, n_rows) {
-    const int type = s.tc[3 * i], obj = s.tc[3 * i + 2];
     int* r = o + LST_N_CNT + 13 * i;
-    r[0] = type; r[1] = s.tc[3 * i + 1]; r[2] = obj;
-    int md[5] = {-1, -1, -1, -1, -1};
-    if (type <= 1) {
-      const int* m5 = s.t5c_md + 5 * s.t5_list[obj];
+    r[0] = s.tc[3 * i]; r[1] = s.tc[3 * i + 1]; r[2] = s.tc[3 * i + 2];
 #pragma unroll
-      for (int q = 0; q < 5; ++q) md[q] = m5[q];
-    } else if (type == 2) {
-      const int4 abc = s.t3_abc[obj];
-      md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
-    }
-#pragma unroll
-    for (int q = 0; q < 5; ++q) {
-      const int2 h = md[q] >= 0 ? s.md_hits[md[q]] : make_int2(-1, -1);
-      r[3 + 2 * q] = h.x; r[4 + 2 * q] = h.y;
-    }
+    for (int q = 0; q < 10; ++q) r[3 + q] = s.tc_hits[TC_HSTRIDE * i + q];
   }
 }
 

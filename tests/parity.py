@@ -68,10 +68,16 @@ def compare(geo, weights, ev, gpu, check_order=True):
     ta = canon.tc_tuples(g["md"]["hits"], g["t3"]["abc"][:, :3], g["t5c"]["md"][g["t5"]["cand"]], g["tc"]["tc"].reshape(-1, 3))
     tb = canon.tc_tuples(r.md_hits, r.t3[:, :3], r.t5c[r.t5][:, :5], r.tc)
     assert canon.same_set(ta, tb)
+    # f1: hit tuples and rank chi2 of every candidate, keep flags, cleaned list (SPEC.md 4.7)
+    assert np.array_equal(g["tcx"]["hits"].reshape(-1, 12)[:, :10], r.tc_hits), "TC hit tuples differ"
+    assert np.array_equal(g["tcx"]["q"].view(np.uint32), r.tc_q), "rank chi2 not bit-exact"
+    assert np.array_equal(g["tcx"]["keep"], r.tc_keep), "duplicate-cleaning flags differ"
+    assert np.array_equal(g["tcc"]["tc"].reshape(-1, 3), r.tcc), "cleaned TC lists differ"
+    assert g["counts"]["tcc"] == len(r.tcc)
     c = g["counts"]
     for k in ("md", "ls", "t3", "t5c", "t5", "tc"):
         assert c[k] == r.counts[k], (k, c[k], r.counts[k])
     tcb = np.bincount(r.tc[:, 0], minlength=4) if len(r.tc) else np.zeros(4, int)
     assert [c["pt5"], c["t5tc"], c["pt3"], c["plstc"]] == tcb.tolist()
-    out = dict(r.counts); out.update(border=n_border, flips=n_flip)
+    out = dict(r.counts); out.update(border=n_border, flips=n_flip, tcc=len(r.tcc))
     return out

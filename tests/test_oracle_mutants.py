@@ -77,6 +77,17 @@ MUTANTS = [
     ("a6: T3 used with 2 of 3 MDs", "if (found == 3) t3_used[x] = 1;", "if (found >= 2) t3_used[x] = 1;", [("pin_tc_used_and_free_rules", "barrel")]),
     ("a6: pT3 pass not skipping pLS that own a pT5", "      if (win5[p] >= 0) continue;\n      R chi = R(0.0f);", "      R chi = R(0.0f);", [("pin_tc_used_and_free_rules", "barrel")]),
     ("a6: T3-used test never fires", "if (found == 3) t3_used[x] = 1;", "", [("pin_tc_used_and_free_rules", "barrel")]),
+    # ---- f1 duplicate cleaning
+    ("f1: more than half -> at least half", "if (2 * shared > nh[x]) keep[x] = 0;", "if (2 * shared >= nh[x]) keep[x] = 0;", [("pin_clean_rule_by_hand", None)]),
+    ("f1: fraction of Y's hits instead of X's", "if (2 * shared > nh[x]) keep[x] = 0;", "if (2 * shared > nh[y]) keep[x] = 0;", [("pin_clean_rule_by_hand", None)]),
+    ("f1: rank ignores the type", "  if (y.type != x.type) return y.type < x.type;\n", "", [("pin_clean_rule_by_hand", None)]),
+    ("f1: rank ignores chi2", "  if (qy != qx) return qy < qx;\n", "", [("pin_clean_rule_by_hand", None)]),
+    ("f1: chi2 order reversed", "  if (qy != qx) return qy < qx;", "  if (qy != qx) return qy > qx;", [("pin_clean_rule_by_hand", None)]),
+    ("f1: ties to the later row", "  return iy < ix;", "  return iy > ix;", [("pin_clean_rule_by_hand", None)]),
+    ("f1: greedy (dropped candidates no longer drop others)", "        if (y == x || !better_rank(tc[y], q[y], y, tc[x], q[x], x)) continue;",
+     "        if (y == x || !keep[y] || !better_rank(tc[y], q[y], y, tc[x], q[x], x)) continue;", [("pin_clean_rule_by_hand", None)]),
+    ("f1: pT3 ranked with the T5's chi2", "      if (c.type == 2) chi = res->chi3[c.obj];", "      if (c.type == 2) chi = res->chi5[0];", [("pin_clean_all_pairs", "geo")]),
+    ("f1: upper hits left out of the tuples", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_up];", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_lo];", [("pin_clean_all_pairs", "geo")]),
 ]
 
 

@@ -554,7 +554,93 @@ def pin_smeared_endcap_efficiency(geo):
     return found["ls"] / tot["ls"], found["t3"] / tot["t3"]
 
 
+# ====================================================================== f1: duplicate cleaning (SPEC.md 4.7)
+def _tup(*h):
+    return list(h) + [-1] * (10 - len(h))
+
+
+def pin_clean_rule_by_hand():
+    """SPEC.md 4.7 on hand-made candidates.  X is dropped iff a better-ranked Y (type, chi2 bits, row) holds MORE than half of
+    X's hits; pLS candidates (type 3) neither drop nor are dropped; the rule is not greedy."""
+    T5A = _tup(*range(100, 110))
+    # a pT3 with 3 of its 6 hits in a T5: exactly half -> kept; with 4 of 6 -> dropped
+    assert O.tc_clean([1, 2], [0, 1.0], [T5A, _tup(100, 101, 102, 1, 2, 3)], [10, 6]).tolist() == [1, 1]
+    assert O.tc_clean([1, 2], [0, 1.0], [T5A, _tup(100, 101, 102, 103, 2, 3)], [10, 6]).tolist() == [1, 0]
+    # the fraction is of X's OWN hits: the T5 has 6 of its 10 hits in a better-ranked pT5 -> dropped; 5 of 10 -> kept
+    assert O.tc_clean([0, 1], [3.0, 0], [_tup(100, 101, 102, 103, 104, 105, 1, 2, 3, 4), T5A], [10, 10]).tolist() == [1, 0]
+    assert O.tc_clean([0, 1], [3.0, 0], [_tup(100, 101, 102, 103, 104, 1, 2, 3, 4, 5), T5A], [10, 10]).tolist() == [1, 1]
+    # type outranks chi2: a pT3 never drops a T5, however good its chi2
+    assert O.tc_clean([1, 2], [0, 0.0], [T5A, _tup(100, 101, 102, 103, 104, 105)], [10, 6]).tolist() == [1, 0]
+    assert O.tc_clean([2, 1], [0.0, 0], [_tup(100, 101, 102, 103, 104, 105), T5A], [6, 10]).tolist() == [0, 1]
+    # same type: smaller chi2 wins (bit pattern of a non-negative float orders like the value); ties go to the earlier row
+    assert O.tc_clean([0, 0], [2.0, 1.0], [T5A, T5A], [10, 10]).tolist() == [0, 1]
+    assert O.tc_clean([0, 0], [0.5, 1.0], [T5A, T5A], [10, 10]).tolist() == [1, 0]
+    assert O.tc_clean([0, 0], [1.0, 1.0], [T5A, T5A], [10, 10]).tolist() == [1, 0]
+    assert O.tc_clean([1, 1, 1], [0, 0, 0], [T5A, T5A, T5A], [10, 10, 10]).tolist() == [1, 0, 0]       # T5s: build order
+    # not greedy: A > B > C in rank, B overlaps both, A and C are disjoint: B is dropped by A, C by B all the same
+    A, B, C = _tup(*range(0, 10)), _tup(*range(4, 14)), _tup(*range(8, 18))
+    assert O.tc_clean([1, 1, 1], [0, 0, 0], [A, B, C], [10, 10, 10]).tolist() == [1, 0, 0]
+    # pLS candidates take no part
+    assert O.tc_clean([3, 1, 3], [0, 0, 0], [_tup(), T5A, _tup()], [0, 10, 0]).tolist() == [1, 1, 1]
+    # disjoint candidates are all kept
+    assert O.tc_clean([0, 1, 2], [1.0, 0, 1.0], [T5A, _tup(*range(10)), _tup(*range(20, 26))], [10, 10, 6]).tolist() == [1, 1, 1]
+
+
+def pin_clean_chain(geo_barrel):
+    """Through the chain.  One clean six-layer muon WITHOUT a seed: the two T5s (layers 1-5 and 2-6) share 8 of 10 hits,
+    the later one in build order is the duplicate.  With seeds [exact, pT * 1.01]: TC = [pT5, pT3]; the pT3's T3 shares two
+    MDs = 4 of its 6 hits with the pT5 (> half) and is dropped."""
+    ev = _muon_with_seeds(geo_barrel, ["exact"])
+    for name in ("pls_px", "pls_py", "pls_pz", "pls_z0", "pls_q", "pls_particle"):
+        setattr(ev, name, getattr(ev, name)[:0])
+    r = O.run(geo_barrel, xavier_weights(1), ev)
+    assert [tuple(t) for t in r.tc.tolist()] == [(1, -1, 0), (1, -1, 1)]
+    assert r.tc_keep.tolist() == [1, 0] and [tuple(t) for t in r.tcc.tolist()] == [(1, -1, 0)]
+    ev = _muon_with_seeds(geo_barrel, ["exact", ("pt", 1.01)])
+    r = O.run(geo_barrel, xavier_weights(1), ev)
+    assert [t[0] for t in r.tc.tolist()] == [0, 2] and r.tc_keep.tolist() == [1, 0]
+    assert [tuple(t) for t in r.tcc.tolist()] == [tuple(r.tc[0].tolist())]
+    # the chi2 in the rank keys is the chi2 of the candidate's own seed match (single-anchor predicate, summed)
+    chi_pt3 = _chi_of(geo_barrel, r, ev, 1, r.t3[r.tc[1][2], :3].tolist())
+    chi_pt5 = _chi_of(geo_barrel, r, ev, 0, r.t5c[r.t5[r.tc[0][2]], :5].tolist())
+    assert r.tc_q.tolist() == [int(chi_pt5.view(np.uint32)), int(chi_pt3.view(np.uint32))] and chi_pt3 > chi_pt5
+
+
+def pin_clean_all_pairs(geo):
+    """The cleaned list of the PU50 event against the definition written with Python sets over ALL pairs of candidates."""
+    ev = config_event(geo, 1)
+    r = O.run(geo, xavier_weights(2), ev)
+    hits, key = [], []
+    for i, (ty, p, o) in enumerate(r.tc.tolist()):
+        mds = r.t5c[r.t5[o], :5] if ty <= 1 else r.t3[o, :3] if ty == 2 else []
+        hits.append([int(h) for m in mds for h in r.md_hits[m]])
+        chi = np.float32(r.chi5[o]) if ty == 0 else np.float32(r.chi3[o]) if ty == 2 else np.float32(0)
+        key.append((ty, int(chi.view(np.uint32)), i))
+    keep = []
+    for x in range(len(hits)):
+        dup = False
+        if key[x][0] <= 2:
+            for y in range(len(hits)):
+                if y != x and key[y][0] <= 2 and key[y] < key[x]:
+                    sy = set(hits[y])
+                    dup |= 2 * sum(h in sy for h in hits[x]) > len(hits[x])
+        keep.append(0 if dup else 1)
+    assert keep == r.tc_keep.tolist()
+    assert 0 < sum(keep) < len(keep)
+    assert [tuple(t) for t in r.tcc.tolist()] == [tuple(t) for t, k in zip(r.tc.tolist(), keep) if k]
+    # what the cleaning compared: the hit tuple (lower, upper hit of every MD, in MD order) and the chi2 of the rank key
+    for i, (ty, p, o) in enumerate(r.tc.tolist()):
+        assert r.tc_hits[i].tolist() == hits[i] + [-1] * (10 - len(hits[i]))
+        assert int(r.tc_q[i]) == key[i][1]
+    n_up_only = sum(len(set(h)) for h in hits if h) - sum(len(set(h[0::2])) for h in hits if h)
+    assert n_up_only > 1000                  # the upper hits are really in the tuples
+    assert len({key[i][1] for i in range(len(key)) if key[i][0] == 2}) > 50      # pT3 ranks are their own chi2
+
+
 # ---------------------------------------------------------------------- pytest entry points
+def test_clean_rule_by_hand(): pin_clean_rule_by_hand()
+def test_clean_chain(geo_barrel): pin_clean_chain(geo_barrel)
+def test_clean_all_pairs(geo_full): pin_clean_all_pairs(geo_full)
 def test_ls_L2_terms(): pin_ls_L2_terms()
 def test_ls_curvature_L1_L3(): pin_ls_curvature_L1_L3()
 def test_ls_L2_uses_arc_length(): pin_ls_L2_uses_arc_length()
