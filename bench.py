@@ -361,6 +361,18 @@ def run_ours(args):
     prof = profile(0, n_prof)
     tot, stages = algorithmic_work(lst, geo, range(n_prof))
 
+    # ---- f4: MD / LS graph export of one stream's batch (PAPER.md:127 quotes "1 to 2 ms" for graph building per event)
+    torch.cuda.synchronize()
+    ga, gb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):
+        lst.lst_export_graph(0, n_prof, main)
+    ga.record(main)
+    for _ in range(20):
+        lst.lst_export_graph(0, n_prof, main)
+    gb.record(main)
+    torch.cuda.synchronize()
+    graph_ms = ga.elapsed_time(gb) / 20
+
     # ---- single event: configs[2] exactly (seed 3), one event, one stream ---------------------------------------------
     lst.load_numpy_event(0, ev_c2)
     torch.cuda.synchronize()
@@ -468,6 +480,9 @@ def run_ours(args):
                         host_link_gbs=round((h2d + d2h) / (e2e_ms * 1e-3) / 1e9, 1)),
                gpu_launches=args.steps * S * lst.launches_per_run(), launch_floor_us=round(launch_floor_us, 2),
                clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows, single_event=single,
+               graph_export=dict(us_per_event=round(graph_ms * 1e3 / n_prof, 3), us_per_launch=round(graph_ms * 1e3, 2), events_per_launch=n_prof,
+                                 nodes_per_event=round(tot["md"] / n_prof, 1), edges_per_event=round(tot["ls"] / n_prof, 1),
+                                 note="lst_export_graph after lst_run: packs node features + CSR columns (SPEC.md 4.8); the paper quotes 1 to 2 ms per event for graph building (PAPER.md:127, other hardware)"),
                kernels_ms={k: round(v, 4) for k, v in prof.items()},
                per_event=dict(us=round(ms * 1e3 / E, 2), objects={k: round(v / n_prof, 1) for k, v in tot.items()}),
                wall_ms_per_step_incl_flush=round(t_wall * 1e3 / args.steps, 3))

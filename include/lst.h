@@ -43,7 +43,7 @@ extern "C" {
 
 /* object types for lst_get */
 enum { LST_OBJ_HIT = 0, LST_OBJ_MD = 1, LST_OBJ_LS = 2, LST_OBJ_T3 = 3, LST_OBJ_T5C = 4, LST_OBJ_T5 = 5,
-       LST_OBJ_TC = 6, LST_OBJ_MATCH5 = 7, LST_OBJ_TCC = 8, LST_OBJ_TCX = 9, LST_N_OBJ = 10 };
+       LST_OBJ_TC = 6, LST_OBJ_MATCH5 = 7, LST_OBJ_TCC = 8, LST_OBJ_TCX = 9, LST_OBJ_GRAPH = 10, LST_N_OBJ = 11 };
 
 /* indices into counts[] of lst_status: number of objects per type after clamping to capacity,
  * then the UNCLAMPED totals (what the stage would have produced), then pair-test counts. */
@@ -94,6 +94,10 @@ typedef struct {
  *          index or -1)
  *  MATCH5: i0 = best5_pls[n_t5] int32 (-1 = unmatched), f0 = chi2[n_t5]
  *  TCC   : i0 = tcc[n][3] int32: the TC rows kept by the duplicate cleaning (SPEC.md 4.7), in TC order
+ *  GRAPH : the MD / LS graph of PAPER.md:127 (SPEC.md 4.8), valid after lst_export_graph: count = number of nodes (MDs);
+ *          i0 = rowptr[n_md+1] (CSR over the inner MD; = ls_start), i1 = col[n_ls] (outer MD of every LS), i2 = node hits
+ *          [n_md][2] (ORIGINAL lower, upper hit index), f0 = node features [n_md][8] (x, y, z, r, phi, eta, c_md, w_md),
+ *          f1 = edge feature c_ls[n_ls]
  *  TCX   : per row of the TC list (count = the TC count): i0 = keep[n] int32 (1 = kept), i1 = hits[n][12] int32 (the ten ORIGINAL hit
  *          indices of the candidate's MDs, lower then upper, -1 padded, then two -1 to make rows 48 bytes), i2 = q[n] (bit pattern of the chi2 in its rank key)
  */
@@ -182,6 +186,12 @@ int lst_launches_per_run(void);
  * the lst_launches_per_run() kernels to h_ms[0 .. lst_launches_per_run()] (HOST).  Not a bench
  * path: the events serialise nothing but add launch gaps. */
 int lst_run_batch_profile(lst_ctx* ctx, int32_t first_slot, int32_t n, void* cuda_stream, float* h_ms);
+
+/* f4: pack the MD / LS graph (nodes = MDs, edges = LSs, SPEC.md 4.8) of slots [first_slot, first_slot + n)
+ * after their lst_run: ONE launch that writes the node-feature table and the CSR column array into the workspace; the row
+ * pointer, the node -> original-hit table and the edge feature are the chain's own MD / LS outputs.  Read the result through
+ * lst_get(LST_OBJ_GRAPH).  Enqueues only. */
+int lst_export_graph(lst_ctx* ctx, int32_t first_slot, int32_t n, void* cuda_stream);
 
 /* Measurement only: sustained fp32 throughput of this GPU in Tflop/s (HOST *h_tflops), counted as one multiply + one add
  * per chain step, with separately rounded multiply and add (fused = 0: the form the cut arithmetic must use) or with fused

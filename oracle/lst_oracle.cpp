@@ -555,6 +555,7 @@ template <typename R> int64_t count_of(const Result<R>* r, int what) {
     case 15: return r->n_match3;
     case 20: return int64_t(r->flags);
     case 21: return int64_t(r->sensor_start.size());
+    case 22: return int64_t(r->ls_start.size());
   }
   return -1;
 }
@@ -579,6 +580,7 @@ template <typename R> void copy_int(const Result<R>* r, int what, int32_t* o) {
     case 9: for (size_t i = 0; i < r->tc_keep.size(); ++i) o[i] = r->tc_keep[i]; break;
     case 10: for (size_t i = 0; i < r->tc_hits.size(); ++i) o[i] = r->tc_hits[i]; break;
     case 11: for (size_t i = 0; i < r->tc_q.size(); ++i) o[i] = r->tc_q[i]; break;
+    case 12: for (size_t i = 0; i < r->ls_start.size(); ++i) o[i] = r->ls_start[i]; break;       // f4: CSR rowptr of the MD/LS graph
     case 21: for (size_t i = 0; i < r->sensor_start.size(); ++i) o[i] = r->sensor_start[i]; break;
   }
 }
@@ -595,6 +597,10 @@ template <typename R> void copy_real(const Result<R>* r, int what, double* o) {
         for (int f = 0; f < N_FEAT; ++f) q[4 + f] = double(t.feat[f]); } break;
     case 7: for (size_t i = 0; i < r->chi5.size(); ++i) o[i] = double(r->chi5[i]); break;
     case 9: for (size_t i = 0; i < r->chi3.size(); ++i) o[i] = double(r->chi3[i]); break;
+    case 12: for (size_t i = 0; i < r->md.size(); ++i) {                    // f4 (SPEC.md 4.8): node features [n][8], fp32 arithmetic
+        const MD<R>& d = r->md[i]; double* q = o + 8 * i;
+        const float x = float(d.x), y = float(d.y), z = float(d.z), rr = float(d.r);
+        q[0] = x; q[1] = y; q[2] = z; q[3] = rr; q[4] = std::atan2(y, x); q[5] = std::asinh(z / rr); q[6] = double(float(d.c)); q[7] = double(float(d.w)); } break;
   }
 }
 

@@ -136,6 +136,9 @@ class OracleResult:
         has_clean = len(self.tc_keep) == len(self.tc)
         self.tc_hits = ints(10, 10, nw=6) if has_clean else np.zeros((0, 10), np.int32)     # hit tuple of every TC row
         self.tc_q = ints(11, 1, nw=6)[:, 0].view(np.uint32) if has_clean else np.zeros(0, np.uint32)
+        # f4 (SPEC.md 4.8): the MD / LS graph -- nodes = MDs, CSR edges = LSs by inner MD
+        self.graph = dict(rowptr=ints(12, 1, nw=22)[:, 0], col=self.ls[:, 1].copy(), node_hits=self.md_hits, node_feat=reals(12, 8, nw=1),
+                          edge_c=self.ls_c)
         self.counts = dict(hits=cnt(0), md=cnt(1), ls=cnt(2), t3=cnt(3), t5c=cnt(4), t5=cnt(5), tc=cnt(6),
                            md_pairs=cnt(10), ls_pairs=cnt(11), t3_pairs=cnt(12), t5_pairs=cnt(13),
                            match5=cnt(14), match3=cnt(15))

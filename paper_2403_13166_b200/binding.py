@@ -10,12 +10,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = os.path.join(_HERE, "liblst_b200.so")
 
 LST_N_CNT = 32
-OBJ = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, match5=7, tcc=8, tcx=9)
+OBJ = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, match5=7, tcc=8, tcx=9, graph=10)
 CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t3=9, raw_t5c=10,
            raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20, tcc=29)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
-           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_measure_fp32", "lst_launches_per_run",
+           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_export_graph", "lst_measure_fp32", "lst_launches_per_run",
            "lst_destroy"]
 
 
@@ -85,6 +85,7 @@ def load_library():
     L.lst_read_tc_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
     L.lst_read_tc_hits_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
     L.lst_measure_fp32.argtypes = [vp, i32, C.POINTER(C.c_float), vp]
+    L.lst_export_graph.argtypes = [vp, i32, i32, vp]
     L.lst_launches_per_run.argtypes = []
     L.lst_run_batch_profile.argtypes = [vp, i32, i32, vp, vp]
     L.lst_launch_name.argtypes = [i32]
@@ -248,6 +249,22 @@ class LST:
         rows = (int(h_out.shape[1]) - LST_N_CNT) // 13
         _chk(self.lib.lst_read_tc_hits_batch_host(self.ctx, first_slot, n, C.c_void_p(h_out.data_ptr()), rows, self._st(stream)),
              "lst_read_tc_hits_batch_host")
+
+    def lst_export_graph(self, first_slot, n, stream=None):
+        _chk(self.lib.lst_export_graph(self.ctx, first_slot, n, self._st(stream)), "lst_export_graph")
+
+    def fetch_graph(self, slot):
+        """MD / LS graph of a slot as numpy arrays (after lst_export_graph): rowptr, col, node_hits, node_feat, edge_c."""
+        _, cnt = self.lst_status(slot)
+        v = _View()
+        _chk(self.lib.lst_get(self.ctx, slot, OBJ["graph"], C.byref(v)), "lst_get")
+        t = self.torch
+        def view(ptr, n, dt):
+            off = ptr - self.workspace.data_ptr()
+            return self.workspace[off:off + 4 * n].view(dt).cpu().numpy()
+        n_md, n_ls = cnt["md"], cnt["ls"]
+        return dict(rowptr=view(v.i0, n_md + 1, t.int32), col=view(v.i1, n_ls, t.int32), node_hits=view(v.i2, 2 * n_md, t.int32).reshape(n_md, 2),
+                    node_feat=view(v.f0, 8 * n_md, t.float32).reshape(n_md, 8), edge_c=view(v.f1, n_ls, t.float32))
 
     def lst_measure_fp32(self, fused, stream=None):
         """Sustained fp32 Tflop/s of this GPU: separately rounded multiply + add (fused=False) or FMA (fused=True)."""

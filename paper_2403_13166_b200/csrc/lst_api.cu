@@ -150,6 +150,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
     t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc);
     t.tcc = cv.take<int>(3 * (size_t)k.max_tc); t.chain_tcc = cv.take<unsigned long long>(k.max_tc / TCC_ROWS + 4);
+    t.g_node = cv.take<float>(8 * (size_t)k.max_md); t.g_col = cv.take<int>(k.max_ls);
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
@@ -418,6 +419,8 @@ int lst_get(lst_ctx* c, int32_t slot, int32_t objtype, lst_view* v) {
     case LST_OBJ_T5: v->capacity = c->caps.max_t5; v->count = s.cnt + LST_CNT_T5; v->i0 = s.t5_list; break;
     case LST_OBJ_TC: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TC; v->i0 = s.tc; break;
     case LST_OBJ_MATCH5: v->capacity = c->caps.max_t5; v->count = s.cnt + LST_CNT_T5; v->i0 = s.best5; v->f0 = s.chi5; break;
+    case LST_OBJ_GRAPH: v->capacity = c->caps.max_md; v->count = s.cnt + LST_CNT_MD; v->i0 = s.ls_start; v->i1 = s.g_col; v->i2 = I(s.md_hits);
+      v->f0 = s.g_node; v->f1 = s.ls_c; break;
     case LST_OBJ_TCC: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TCC; v->i0 = s.tcc; break;
     case LST_OBJ_TCX: v->capacity = c->caps.max_tc; v->count = s.cnt + LST_CNT_TC; v->i0 = s.tc_keep; v->i1 = s.tc_hits; v->i2 = s.tc_q; break;
   }
@@ -488,6 +491,15 @@ int lst_read_tc_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out,
 
 int lst_read_tc_hits_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h_out, int32_t max_rows, void* cuda_stream) {
   return read_tc_batch(c, first, n, h_out, max_rows, cuda_stream, true);
+}
+
+int lst_export_graph(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
+  if (!c || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
+  if (c->sticky_cuda_error) return LST_ECUDA;
+  int gx = (148 * 4 + n - 1) / n;
+  if (gx < 4) gx = 4;
+  k_graph_export<<<dim3(gx, n), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->d_slots + first);
+  return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
 }
 
 int lst_measure_fp32(lst_ctx* c, int32_t fused, float* h_tflops, void* cuda_stream) {

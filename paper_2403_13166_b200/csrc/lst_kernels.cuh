@@ -68,6 +68,7 @@ struct Slot {
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
   int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc;     // f1 duplicate cleaning
+  float* g_node; int* g_col;         // f4 graph export: node features [n_md][8], CSR column (outer MD) per LS
   // host-load staging
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
   int* tc_hdr;                       // copy of cnt[] in front of the TC rows, so one D2H copy reads both
@@ -853,6 +854,20 @@ __global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ s
     }
     __syncthreads();
   }
+}
+
+// f4 (SPEC.md 4.8): pack the MD / LS graph -- eight node features per MD and the CSR column (outer MD) of every LS.  The
+// row pointer (ls_start), the node -> original hits table (md_hits) and the edge feature (ls_c) are the chain's own outputs.
+__global__ void __launch_bounds__(256) k_graph_export(const Slot* __restrict__ slots) {
+  const Slot& s = slots[blockIdx.y];
+  LST_FOR_ITEMS(a, s.cnt[LST_CNT_MD]) {
+    const float4 p = s.md_pos[a];
+    const float2 cw = s.md_cw[a];
+    float4* o = reinterpret_cast<float4*>(s.g_node + 8 * (size_t)a);
+    o[0] = p;
+    o[1] = make_float4(atan2f(p.y, p.x), asinhf(__fdiv_rn(p.z, p.w)), cw.x, cw.y);
+  }
+  LST_FOR_ITEMS(l, s.cnt[LST_CNT_LS]) s.g_col[l] = s.ls_ab[l].y;
 }
 
 // binds an event to a slot (stream-ordered, so a later lst_run on the same stream sees it)

@@ -81,3 +81,15 @@ def compare(geo, weights, ev, gpu, check_order=True):
     assert [c["pt5"], c["t5tc"], c["pt3"], c["plstc"]] == tcb.tolist()
     out = dict(r.counts); out.update(border=n_border, flips=n_flip, tcc=len(r.tcc))
     return out
+
+
+def compare_graph(geo, weights, ev, g):
+    """`g` = LST.fetch_graph(slot): the exported MD / LS graph against the oracle's (SPEC.md 4.8)."""
+    r = O.run(geo, weights, ev, last_stage="ls")
+    o = r.graph
+    assert np.array_equal(g["rowptr"], o["rowptr"]) and np.array_equal(g["col"], o["col"]) and np.array_equal(g["node_hits"], o["node_hits"])
+    assert bits_equal(g["edge_c"], o["edge_c"])
+    assert bits_equal(g["node_feat"][:, :4], o["node_feat"][:, :4]) and bits_equal(g["node_feat"][:, 6:], o["node_feat"][:, 6:])
+    a, b = g["node_feat"][:, 4:6].astype(np.float64), o["node_feat"][:, 4:6]
+    assert np.all(np.abs(a - b) <= FEAT_RTOL * np.maximum(np.abs(a), np.abs(b)) + FEAT_ATOL)
+    return len(o["col"])

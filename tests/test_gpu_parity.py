@@ -256,3 +256,17 @@ def test_batched_host_load_and_read(P, geo_full):
     with pytest.raises(P.LstError):
         lst.lst_load_batch_host(0, 3, bad)
     lst.close()
+
+
+def test_graph_export(P, geo_full):
+    """f4 (SPEC.md 4.8): nodes = MDs, CSR edges = LSs, original hit numbering, for a batch of events."""
+    w = xavier_weights(3)
+    evs = [config_event(geo_full, 2, seed=100), config_event(geo_full, 1), make_event(geo_full, 9)]
+    lst = P.LST(geo_full, w, P.default_caps(len(evs)))
+    for i, ev in enumerate(evs):
+        lst.load_numpy_event(i, ev)
+    lst.lst_run_batch(0, len(evs))
+    lst.lst_export_graph(0, len(evs))
+    n_edges = [parity.compare_graph(geo_full, w, ev, lst.fetch_graph(i)) for i, ev in enumerate(evs)]
+    assert n_edges[0] > 10000 and n_edges[2] == 0
+    lst.close()

@@ -637,7 +637,31 @@ def pin_clean_all_pairs(geo):
     assert len({key[i][1] for i in range(len(key)) if key[i][0] == 2}) > 50      # pT3 ranks are their own chi2
 
 
+# ====================================================================== f4: MD / LS graph (SPEC.md 4.8)
+def pin_graph_export(geo):
+    """The graph is a view of the MD and LS lists: row a of the CSR lists exactly the LSs whose inner MD is a, in LS order,
+    every (a, col) is an LS, and the node features are the anchor's coordinates with phi / eta from their definitions."""
+    ev = config_event(geo, 1)
+    r = O.run(geo, xavier_weights(2), ev, last_stage="ls")
+    g = r.graph
+    n_md, n_ls = len(r.md_hits), len(r.ls)
+    assert g["rowptr"].shape == (n_md + 1,) and g["rowptr"][0] == 0 and g["rowptr"][-1] == n_ls and np.all(np.diff(g["rowptr"]) >= 0)
+    edges = [(a, int(g["col"][l])) for a in range(n_md) for l in range(g["rowptr"][a], g["rowptr"][a + 1])]
+    assert edges == [tuple(t) for t in r.ls.tolist()]
+    assert np.array_equal(g["node_hits"], r.md_hits) and np.array_equal(g["edge_c"], r.ls_c)
+    x, y, z, rr = (r.md_real[:, k] for k in (2, 3, 4, 5))
+    f = g["node_feat"]
+    assert np.array_equal(f[:, 0], x) and np.array_equal(f[:, 1], y) and np.array_equal(f[:, 2], z) and np.array_equal(f[:, 3], rr)
+    assert np.allclose(f[:, 4], np.arctan2(y, x), rtol=2e-6, atol=1e-7) and np.allclose(f[:, 5], np.arcsinh(z / rr), rtol=2e-6, atol=1e-7)
+    assert np.array_equal(f[:, 6], r.md_real[:, 0]) and np.array_equal(f[:, 7], r.md_real[:, 1])
+    # the edge's hits: the two MDs of the LS, in original numbering
+    l = n_ls // 2
+    a = int(np.searchsorted(g["rowptr"], l, side="right") - 1)
+    assert g["node_hits"][a].tolist() == r.md_hits[r.ls[l, 0]].tolist() and g["node_hits"][g["col"][l]].tolist() == r.md_hits[r.ls[l, 1]].tolist()
+
+
 # ---------------------------------------------------------------------- pytest entry points
+def test_graph_export(geo_full): pin_graph_export(geo_full)
 def test_clean_rule_by_hand(): pin_clean_rule_by_hand()
 def test_clean_chain(geo_barrel): pin_clean_chain(geo_barrel)
 def test_clean_all_pairs(geo_full): pin_clean_all_pairs(geo_full)
