@@ -67,8 +67,17 @@ typedef struct {
   const uint8_t* mtype;       /* [n_modules] 0 PS, 1 2S                                           */
   const int32_t* conn_rowptr; /* [n_modules+1] CSR of module -> connected modules, rowptr[0] = 0  */
   const int32_t* conn_col;    /* [rowptr[n_modules]] ascending and unique within a row, no self   */
-  const float* dnn_weights;   /* [1857] W1[32][23], b1[32], W2[32][32], b2[32], w3[32], b3        */
+  const float* dnn_weights;   /* [1857] W1[32][23], b1[32], W2[32][32], b2[32], w3[32], b3 for the default network;
+                               * in general lst_dnn_n_weights(n_feat, n_hidden) floats: W1[32][n_feat], b1[32],
+                               * (n_hidden - 1) x (W[32][32], b[32]), w_out[32], b_out (SPEC.md 4.9)              */
+  const uint8_t* layer;       /* optional [n_modules]: detector layer of each module (1..6 barrel, 7..11 disks); only an
+                               * input feature of the 38-input DNN.  NULL = 0 everywhere                          */
+  int32_t dnn_n_feat;         /* 0 or 23: the 23 inputs of configs[0] (SPEC.md 4.5); 38: the paper's input list (4.9) */
+  int32_t dnn_n_hidden;       /* 0 or 2: two hidden layers of 32; 1, 3, 4: the depth scan of PAPER.md:78 */
 } lst_geometry;
+
+/* Number of floats of `dnn_weights` for a DNN variant. */
+int lst_dnn_n_weights(int32_t n_feat, int32_t n_hidden);
 
 /* Per-slot capacities (objects).  max_tc is forced to >= max_pls + max_t5 internally. */
 typedef struct {
@@ -88,7 +97,7 @@ typedef struct {
  *  T3    : i0 = abc[n][4] int32 (MD a, b, c, first LS), i1 = second LS [n], f0 = k[n],
  *          i2 = t3_start[n_md+1]
  *  T5C   : i0 = md[n][5] int32, i1 = t3[n][2] int32, f0 = curv[n][3] (c_in, c_br, c_out),
- *          f1 = feat[n][23], f2 = score[n], i2 = pass[n] int32 (0/1)
+ *          f1 = feat[n][n_feat] (23 or 38), f2 = score[n], i2 = pass[n] int32 (0/1)
  *  T5    : i0 = cand[n] int32 (index into T5C)
  *  TC    : i0 = tc[n][3] int32 (type 0 pT5 / 1 T5 / 2 pT3 / 3 pLS, pLS index or -1, T5-list or T3
  *          index or -1)

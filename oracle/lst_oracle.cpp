@@ -40,7 +40,7 @@ constexpr float Z0_MAX_F = 15.0f;
 constexpr float DT_F[2] = {0.01225f, 0.01102f};   // 3 sqrt2 sigma_t  (PS, 2S)
 constexpr float DL_F[2] = {0.1299f, 4.330f};      // 3 sigma_l
 constexpr float DL2_F[2] = {0.1837f, 6.124f};     // 3 sqrt2 sigma_l
-constexpr int N_FEAT = 23, N_HID = 32;
+constexpr int N_FEAT = 23, N_HID = 32, N_FEAT_MAX = 38;
 
 // cut identifiers for the loosening factors (tests only; all 1.0 in normal use, and x*1.0 is exact)
 enum { CUT_M2, CUT_M3, CUT_L1, CUT_L2, CUT_L3, CUT_T1, CUT_T2, CUT_T3, CUT_Q1, CUT_Q2, CUT_P5, CUT_P3, N_CUTS };
@@ -72,7 +72,7 @@ template <typename R> struct MD {
 template <typename R> struct LS { int32_t a, b; R c; };
 template <typename R> struct T3 { int32_t ls0, ls1; int32_t a, b, c; R k; };
 template <typename R> struct T5C {
-  int32_t t3in, t3out; int32_t md[5]; R cin, cbr, cout; float feat[N_FEAT]; float score; int8_t pass;
+  int32_t t3in, t3out; int32_t md[5]; R cin, cbr, cout; float feat[N_FEAT_MAX]; float score; int8_t pass;
 };
 struct TC { int32_t type, pls, obj; };
 
@@ -195,28 +195,58 @@ inline void t5_features(const float* ax, const float* ay, const float* az, const
   x[21] = radius_feature(cbr);
   x[22] = radius_feature(cout);
 }
+// f3 (SPEC.md 4.9): the paper's 38 inputs -- 2 T3 x (pT, radius), 6 anchors (a, b, c, c, d, e) x (r, phi, z, eta, layer),
+// T5 (pT, eta, phi), bridge radius
+inline float pt_feature(float c) {
+  const float ac = std::fabs(c);
+  const float rad = std::fmin(1.0f / ac, 1.0e5f);
+  return std::log10(KAPPA_F * rad);
+}
+inline void t5_features38(const float* ax, const float* ay, const float* az, const float* ar, const int* layer,
+                          float cin, float cbr, float cout, float* x) {
+  x[0] = pt_feature(cin); x[1] = radius_feature(cin); x[2] = pt_feature(cout); x[3] = radius_feature(cout);
+  const int order[6] = {0, 1, 2, 2, 3, 4};
+  for (int i = 0; i < 6; ++i) {
+    const int q = order[i];
+    x[4 + 5 * i + 0] = ar[q] * 0.01f;
+    x[4 + 5 * i + 1] = std::atan2(ay[q], ax[q]);
+    x[4 + 5 * i + 2] = az[q] * 0.01f;
+    x[4 + 5 * i + 3] = std::asinh(az[q] / ar[q]);
+    x[4 + 5 * i + 4] = float(layer[q]) * 0.1f;
+  }
+  const float c5 = 0.5f * (cin + cout);
+  x[34] = pt_feature(c5);
+  x[35] = std::asinh(az[0] / ar[0]);
+  x[36] = std::atan2(ay[0], ax[0]);
+  x[37] = radius_feature(cbr);
+}
 // "the DNN matrix multiplication is done through nested for-loops": acc = b[j];
-// for i ascending: acc = acc + W[j][i] * x[i].  ReLU on both hidden layers, sigmoid output.
-inline float mlp_forward(const float* w, const float* x) {
-  const float* W1 = w;
-  const float* b1 = W1 + N_HID * N_FEAT;
-  const float* W2 = b1 + N_HID;
-  const float* b2 = W2 + N_HID * N_HID;
-  const float* w3 = b2 + N_HID;
-  const float* b3 = w3 + N_HID;
-  float h1[N_HID], h2[N_HID];
+// for i ascending: acc = acc + W[j][i] * x[i].  ReLU on every hidden layer, sigmoid output.  n_in inputs, n_hidden hidden
+// layers of 32 (PAPER.md:68 has two; :78 scans one to four).
+inline float mlp_forward(const float* w, const float* x, int n_in = N_FEAT, int n_hidden = 2) {
+  float h[N_HID], g[N_HID];
+  const float* W = w;
+  const float* b = W + N_HID * n_in;
   for (int j = 0; j < N_HID; ++j) {
-    float acc = b1[j];
-    for (int i = 0; i < N_FEAT; ++i) acc = acc + W1[j * N_FEAT + i] * x[i];
-    h1[j] = acc > 0.0f ? acc : 0.0f;
+    float acc = b[j];
+    for (int i = 0; i < n_in; ++i) acc = acc + W[j * n_in + i] * x[i];
+    h[j] = acc > 0.0f ? acc : 0.0f;
   }
-  for (int j = 0; j < N_HID; ++j) {
-    float acc = b2[j];
-    for (int i = 0; i < N_HID; ++i) acc = acc + W2[j * N_HID + i] * h1[i];
-    h2[j] = acc > 0.0f ? acc : 0.0f;
+  const float* p = b + N_HID;
+  for (int l = 1; l < n_hidden; ++l) {
+    const float* Wl = p;
+    const float* bl = Wl + N_HID * N_HID;
+    for (int j = 0; j < N_HID; ++j) {
+      float acc = bl[j];
+      for (int i = 0; i < N_HID; ++i) acc = acc + Wl[j * N_HID + i] * h[i];
+      g[j] = acc > 0.0f ? acc : 0.0f;
+    }
+    for (int j = 0; j < N_HID; ++j) h[j] = g[j];
+    p = bl + N_HID;
   }
-  float y = b3[0];
-  for (int i = 0; i < N_HID; ++i) y = y + w3[i] * h2[i];
+  const float* w3 = p;
+  float y = w3[N_HID];
+  for (int i = 0; i < N_HID; ++i) y = y + w3[i] * h[i];
   return 1.0f / (1.0f + std::exp(-y));
 }
 
@@ -324,7 +354,8 @@ Result<R>* run_chain(int32_t M, const uint8_t* subdet, const uint8_t* mtype, con
                      const float* hy, const float* hz, const uint32_t* key, int32_t n_pls,
                      const float* ppx, const float* ppy, const float* ppz, const float* pz0,
                      const int8_t* pq, const int8_t* t5_override, int32_t n_override,
-                     const float* loosen, int32_t last_stage) {
+                     const float* loosen, int32_t last_stage, int32_t n_feat = N_FEAT, int32_t n_hidden = 2,
+                     const uint8_t* layer = nullptr) {
   Result<R>* res = new Result<R>();
   Loosen<R> lo;
   for (int i = 0; i < N_CUTS; ++i) lo.f[i] = loosen ? R(loosen[i]) : R(1.0f);
@@ -429,8 +460,15 @@ Result<R>* run_chain(int32_t M, const uint8_t* subdet, const uint8_t* mtype, con
         const MD<R>& d = res->md[t.md[q]];
         ax[q] = float(d.x); ay[q] = float(d.y); az[q] = float(d.z); ar[q] = float(d.r);
       }
-      t5_features(ax, ay, az, ar, float(t.cin), float(t.cbr), float(t.cout), t.feat);
-      t.score = mlp_forward(weights, t.feat);
+      for (int q = 0; q < N_FEAT_MAX; ++q) t.feat[q] = 0.0f;
+      if (n_feat == N_FEAT_MAX) {
+        int lay[5];
+        for (int q = 0; q < 5; ++q) lay[q] = layer ? int(layer[res->md[t.md[q]].mod]) : 0;
+        t5_features38(ax, ay, az, ar, lay, float(t.cin), float(t.cbr), float(t.cout), t.feat);
+      } else {
+        t5_features(ax, ay, az, ar, float(t.cin), float(t.cbr), float(t.cout), t.feat);
+      }
+      t.score = mlp_forward(weights, t.feat, n_feat, n_hidden);
       t.pass = t.score > 0.5f ? 1 : 0;
       const int32_t ci = int32_t(res->t5c.size());
       if (t5_override && ci < n_override && t5_override[ci] >= 0) t.pass = t5_override[ci];
@@ -591,10 +629,10 @@ template <typename R> void copy_real(const Result<R>* r, int what, double* o) {
         q[0] = double(d.c); q[1] = double(d.w); q[2] = double(d.x); q[3] = double(d.y); q[4] = double(d.z); q[5] = double(d.r); } break;
     case 2: for (size_t i = 0; i < r->ls.size(); ++i) o[i] = double(r->ls[i].c); break;
     case 3: for (size_t i = 0; i < r->t3.size(); ++i) o[i] = double(r->t3[i].k); break;
-    case 4: for (size_t i = 0; i < r->t5c.size(); ++i) {                    // [n][27] cin, cbr, cout, score, feat[23]
-        const T5C<R>& t = r->t5c[i]; double* q = o + 27 * i;
+    case 4: for (size_t i = 0; i < r->t5c.size(); ++i) {                    // [n][42] cin, cbr, cout, score, feat[38] (unused = 0)
+        const T5C<R>& t = r->t5c[i]; double* q = o + 42 * i;
         q[0] = double(t.cin); q[1] = double(t.cbr); q[2] = double(t.cout); q[3] = double(t.score);
-        for (int f = 0; f < N_FEAT; ++f) q[4 + f] = double(t.feat[f]); } break;
+        for (int f = 0; f < N_FEAT_MAX; ++f) q[4 + f] = double(t.feat[f]); } break;
     case 7: for (size_t i = 0; i < r->chi5.size(); ++i) o[i] = double(r->chi5[i]); break;
     case 9: for (size_t i = 0; i < r->chi3.size(); ++i) o[i] = double(r->chi3[i]); break;
     case 12: for (size_t i = 0; i < r->md.size(); ++i) {                    // f4 (SPEC.md 4.8): node features [n][8], fp32 arithmetic
@@ -612,15 +650,16 @@ void* lst_oracle_run(int32_t n_modules, const uint8_t* subdet, const uint8_t* mt
                      const int32_t* col, const float* weights, int32_t n_hits, const float* x, const float* y,
                      const float* z, const uint32_t* key, int32_t n_pls, const float* px, const float* py,
                      const float* pz, const float* z0, const int8_t* q, const int8_t* t5_override,
-                     int32_t n_override, const float* loosen, int32_t use_double, int32_t last_stage) {
+                     int32_t n_override, const float* loosen, int32_t use_double, int32_t last_stage,
+                     int32_t n_feat, int32_t n_hidden, const uint8_t* layer) {
   Handle* h = new Handle();
   h->is_double = use_double;
   if (use_double)
     h->p = run_chain<double>(n_modules, subdet, mtype, rowptr, col, weights, n_hits, x, y, z, key, n_pls, px, py,
-                             pz, z0, q, t5_override, n_override, loosen, last_stage);
+                             pz, z0, q, t5_override, n_override, loosen, last_stage, n_feat, n_hidden, layer);
   else
     h->p = run_chain<float>(n_modules, subdet, mtype, rowptr, col, weights, n_hits, x, y, z, key, n_pls, px, py,
-                            pz, z0, q, t5_override, n_override, loosen, last_stage);
+                            pz, z0, q, t5_override, n_override, loosen, last_stage, n_feat, n_hidden, layer);
   return h;
 }
 int64_t lst_oracle_count(void* hv, int32_t what) {
@@ -700,5 +739,8 @@ double lst_oracle_arcfac_f64(double u) { return arcfac<double>(u); }
 void lst_oracle_features(const float* ax, const float* ay, const float* az, const float* ar, float cin, float cbr,
                          float cout, float* x23) { t5_features(ax, ay, az, ar, cin, cbr, cout, x23); }
 float lst_oracle_mlp(const float* weights, const float* x23) { return mlp_forward(weights, x23); }
+float lst_oracle_mlp_n(const float* weights, const float* x, int32_t n_in, int32_t n_hidden) { return mlp_forward(weights, x, n_in, n_hidden); }
+void lst_oracle_features38(const float* ax, const float* ay, const float* az, const float* ar, const int32_t* layer, float cin,
+                           float cbr, float cout, float* x38) { t5_features38(ax, ay, az, ar, layer, cin, cbr, cout, x38); }
 
 }  // extern "C"

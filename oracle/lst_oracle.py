@@ -31,7 +31,7 @@ def _bind(path):
     L = C.CDLL(path)
     L.lst_oracle_run.restype = C.c_void_p
     L.lst_oracle_run.argtypes = [C.c_int32] + [C.c_void_p] * 5 + [C.c_int32] + [C.c_void_p] * 4 + \
-        [C.c_int32] + [C.c_void_p] * 5 + [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32]
+        [C.c_int32] + [C.c_void_p] * 5 + [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32] + [C.c_int32, C.c_int32, C.c_void_p]
     L.lst_oracle_count.restype = C.c_int64
     L.lst_oracle_count.argtypes = [C.c_void_p, C.c_int32]
     L.lst_oracle_copy_int.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
@@ -56,6 +56,9 @@ def _bind(path):
     L.lst_oracle_features.argtypes = [C.c_void_p] * 4 + [C.c_float] * 3 + [C.c_void_p]
     L.lst_oracle_mlp.restype = C.c_float
     L.lst_oracle_mlp.argtypes = [C.c_void_p, C.c_void_p]
+    L.lst_oracle_mlp_n.restype = C.c_float
+    L.lst_oracle_mlp_n.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32]
+    L.lst_oracle_features38.argtypes = [C.c_void_p] * 5 + [C.c_float] * 3 + [C.c_void_p]
     return L
 
 
@@ -94,7 +97,7 @@ class OracleResult:
     md_hits[n,2] original hit indices (lower, upper); ls[n,2] MD indices; t3[n,5] = MD a,b,c + LS i,j;
     t5c[n,8] = MD[5], T3 in, T3 out, pass; t5[n] candidate indices; tc[n,3] = type, pLS, object."""
 
-    def __init__(self, h, L):
+    def __init__(self, h, L, n_feat=23):
         cnt = lambda w: int(L.lst_oracle_count(h, w))
 
         def ints(w, k, nw=None):
@@ -124,8 +127,8 @@ class OracleResult:
         self.t3 = ints(3, 5)
         self.t3_k = reals(3, 1)[:, 0]
         self.t5c = ints(4, 8)
-        r5 = reals(4, 27)
-        self.t5c_curv, self.t5c_score, self.t5c_feat = r5[:, :3].copy(), r5[:, 3].copy(), r5[:, 4:].copy()
+        r5 = reals(4, 42)
+        self.t5c_curv, self.t5c_score, self.t5c_feat = r5[:, :3].copy(), r5[:, 3].copy(), r5[:, 4:4 + n_feat].copy()
         self.t5 = ints(5, 1)[:, 0]
         self.tc = ints(6, 3)
         self.best5_pls = ints(7, 1)[:, 0]
@@ -145,8 +148,9 @@ class OracleResult:
 
 
 def run(geo, weights, ev, *, t5_override=None, loosen=None, use_double=False, last_stage="clean",
-        counts_only=False):
-    """Run the whole chain on one event.  `geo` needs n_modules, subdet, mtype, conn_rowptr, conn_col."""
+        counts_only=False, dnn=(23, 2)):
+    """Run the whole chain on one event.  `geo` needs n_modules, subdet, mtype, conn_rowptr, conn_col (and `layer` for the
+    38-input DNN variant).  `dnn` = (n_feat, n_hidden) of SPEC.md 4.9."""
     L = lib()
     w = np.ascontiguousarray(weights, dtype=np.float32)
     ov = None if t5_override is None else np.ascontiguousarray(t5_override, dtype=np.int8)
@@ -158,13 +162,14 @@ def run(geo, weights, ev, *, t5_override=None, loosen=None, use_double=False, la
     h = L.lst_oracle_run(int(geo.n_modules), _p(geo.subdet), _p(geo.mtype), _p(geo.conn_rowptr), _p(geo.conn_col),
                          _p(w), ev.n_hits, _p(ev.x), _p(ev.y), _p(ev.z), _p(ev.key), ev.n_pls, _p(ev.pls_px),
                          _p(ev.pls_py), _p(ev.pls_pz), _p(ev.pls_z0), _p(ev.pls_q), _p(ov),
-                         0 if ov is None else int(ov.size), _p(lo), int(bool(use_double)), STAGE[last_stage])
+                         0 if ov is None else int(ov.size), _p(lo), int(bool(use_double)), STAGE[last_stage],
+                         int(dnn[0]), int(dnn[1]), _p(np.ascontiguousarray(geo.layer, dtype=np.uint8)) if dnn[0] == 38 else None)
     try:
         if counts_only:
             names = dict(hits=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, md_pairs=10, ls_pairs=11, t3_pairs=12,
                          t5_pairs=13, match5=14, match3=15)
             return {k: int(L.lst_oracle_count(h, v)) for k, v in names.items()}
-        return OracleResult(h, L)
+        return OracleResult(h, L, int(dnn[0]))
     finally:
         L.lst_oracle_free(h)
 
@@ -233,3 +238,16 @@ def features(ax, ay, az, ar, cin, cbr, cout):
 def mlp(weights, x23):
     w = np.ascontiguousarray(weights, dtype=np.float32); x = np.ascontiguousarray(x23, dtype=np.float32)
     return float(lib().lst_oracle_mlp(_p(w), _p(x)))
+
+
+def mlp_n(weights, x, n_hidden):
+    w = np.ascontiguousarray(weights, dtype=np.float32); x = np.ascontiguousarray(x, dtype=np.float32)
+    return float(lib().lst_oracle_mlp_n(_p(w), _p(x), int(x.size), int(n_hidden)))
+
+
+def features38(ax, ay, az, ar, layer, cin, cbr, cout):
+    a = [np.ascontiguousarray(v, dtype=np.float32) for v in (ax, ay, az, ar)]
+    lay = np.ascontiguousarray(layer, dtype=np.int32)
+    out = np.zeros(38, dtype=np.float32)
+    lib().lst_oracle_features38(_p(a[0]), _p(a[1]), _p(a[2]), _p(a[3]), _p(lay), float(cin), float(cbr), float(cout), _p(out))
+    return out

@@ -15,7 +15,7 @@ CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t
            raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20, tcc=29)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
-           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_export_graph", "lst_measure_fp32", "lst_launches_per_run",
+           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_export_graph", "lst_dnn_n_weights", "lst_measure_fp32", "lst_launches_per_run",
            "lst_destroy"]
 
 
@@ -25,7 +25,8 @@ class LstError(RuntimeError):
 
 class _Geometry(C.Structure):
     _fields_ = [("n_modules", C.c_int32), ("subdet", C.c_void_p), ("mtype", C.c_void_p),
-                ("conn_rowptr", C.c_void_p), ("conn_col", C.c_void_p), ("dnn_weights", C.c_void_p)]
+                ("conn_rowptr", C.c_void_p), ("conn_col", C.c_void_p), ("dnn_weights", C.c_void_p),
+                ("layer", C.c_void_p), ("dnn_n_feat", C.c_int32), ("dnn_n_hidden", C.c_int32)]
 
 
 class _Caps(C.Structure):
@@ -86,6 +87,7 @@ def load_library():
     L.lst_read_tc_hits_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
     L.lst_measure_fp32.argtypes = [vp, i32, C.POINTER(C.c_float), vp]
     L.lst_export_graph.argtypes = [vp, i32, i32, vp]
+    L.lst_dnn_n_weights.argtypes = [i32, i32]
     L.lst_launches_per_run.argtypes = []
     L.lst_run_batch_profile.argtypes = [vp, i32, i32, vp, vp]
     L.lst_launch_name.argtypes = [i32]
@@ -129,7 +131,7 @@ _ROWS = {"match5": "t5", "tcx": "tc"}      # views whose row count is another li
 class LST:
     """One context = one uploaded geometry + `caps.n_slots` event slots in a torch-owned workspace."""
 
-    def __init__(self, geo, weights, caps: Caps = None, device="cuda:0"):
+    def __init__(self, geo, weights, caps: Caps = None, device="cuda:0", dnn=(23, 2)):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -139,10 +141,13 @@ class LST:
         self._keep = dict(subdet=np.ascontiguousarray(geo.subdet, np.uint8), mtype=np.ascontiguousarray(geo.mtype, np.uint8),
                           rowptr=np.ascontiguousarray(geo.conn_rowptr, np.int32), col=np.ascontiguousarray(geo.conn_col, np.int32),
                           w=np.ascontiguousarray(weights, np.float32))
-        if self._keep["w"].size != 1857:
-            raise LstError("dnn_weights must hold 1857 floats")
+        self.n_feat, self.n_hidden = int(dnn[0]), int(dnn[1])
+        if self._keep["w"].size != self.lib.lst_dnn_n_weights(self.n_feat, self.n_hidden):
+            raise LstError(f"dnn_weights must hold {self.lib.lst_dnn_n_weights(self.n_feat, self.n_hidden)} floats for this DNN variant")
         k = self._keep
-        self._g = _Geometry(self.n_modules, _hp(k["subdet"]), _hp(k["mtype"]), _hp(k["rowptr"]), _hp(k["col"]), _hp(k["w"]))
+        k["layer"] = np.ascontiguousarray(geo.layer, np.uint8) if getattr(geo, "layer", None) is not None else None
+        self._g = _Geometry(self.n_modules, _hp(k["subdet"]), _hp(k["mtype"]), _hp(k["rowptr"]), _hp(k["col"]), _hp(k["w"]),
+                            _hp(k["layer"]), self.n_feat, self.n_hidden)
         self._c = _Caps(**asdict(self.caps))
         nbytes = C.c_size_t(0)
         _chk(self.lib.lst_workspace_bytes(C.byref(self._g), C.byref(self._c), C.byref(nbytes)), "lst_workspace_bytes")
@@ -206,6 +211,8 @@ class LST:
         out = {}
         t = self.torch
         for fld, (label, dt, cols) in _FIELDS[name].items():
+            if label == "feat":
+                cols = self.n_feat
             ptr = getattr(v, fld)
             off = ptr - self.workspace.data_ptr()
             raw = self.workspace[off:off + 4 * n * cols]

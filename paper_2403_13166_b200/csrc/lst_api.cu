@@ -49,6 +49,8 @@ int validate(const lst_geometry* g, const lst_caps* c) {
       c->max_t5 <= 0 || c->max_pls <= 0)
     return LST_EINVAL;
   if (c->max_pls > (1 << 28) / 5) return LST_EINVAL;
+  if (g->dnn_n_feat != 0 && g->dnn_n_feat != N_FEAT && g->dnn_n_feat != N_FEAT_MAX) return LST_EINVAL;
+  if (g->dnn_n_hidden < 0 || g->dnn_n_hidden > 4) return LST_EINVAL;
   const int M = g->n_modules;
   if (g->conn_rowptr[0] != 0) return LST_EINVAL;
   for (int m = 0; m < M; ++m) {
@@ -74,7 +76,7 @@ Caps make_caps(const lst_caps* c) {
 // One pass lays out the whole workspace; used both to measure and to carve.
 struct Layout {
   char* batch_in; size_t batch_in_stride; int* batch_out; size_t batch_out_stride;
-  Slot* slots; uint8_t* modt; int* rowptr; int* col; float* weights; int* run_ptr; int* run_c0; int* run_c1;
+  Slot* slots; uint8_t* modt; uint8_t* layer; int* rowptr; int* col; float* weights; int* run_ptr; int* run_c0; int* run_c1;
   char* zero_base; size_t zero_stride; char* ones_base; size_t ones_stride;
   size_t total;
 };
@@ -84,9 +86,10 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   Layout L{};
   L.slots = cv.take<Slot>(n_slots);
   L.modt = cv.take<uint8_t>(M);
+  L.layer = cv.take<uint8_t>(M);
   L.rowptr = cv.take<int>(M + 1);
   L.col = cv.take<int>(nnz > 0 ? nnz : 1);
-  L.weights = cv.take<float>(N_W);
+  L.weights = cv.take<float>(dnn_n_weights(N_FEAT_MAX, 4));
   L.run_ptr = cv.take<int>(M + 1);
   L.run_c0 = cv.take<int>(nnz > 0 ? nnz : 1);      // a row has at most as many runs as entries
   L.run_c1 = cv.take<int>(nnz > 0 ? nnz : 1);
@@ -140,7 +143,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
     t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
     t.t5_off = cv.take<int>(k.max_t3 + 8); t.t5c_md = cv.take<int>(5 * (size_t)k.max_t5c); t.t5c_t3 = cv.take<int2>(k.max_t5c);
-    t.t5c_curv = cv.take<float>(3 * (size_t)k.max_t5c); t.t5c_feat = cv.take<float>((size_t)N_FEAT * k.max_t5c);
+    t.t5c_curv = cv.take<float>(3 * (size_t)k.max_t5c); t.t5c_feat = cv.take<float>((size_t)N_FEAT_MAX * k.max_t5c);
     t.t5c_score = cv.take<float>(k.max_t5c); t.t5c_pass = cv.take<int>(k.max_t5c); t.t5_scan = cv.take<int>(k.max_t5c + 8);
     t.t5_list = cv.take<int>(k.max_t5);
     t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.pls_key = cv.take<int>(k.max_pls);
@@ -175,6 +178,11 @@ extern "C" {
 
 int lst_launches_per_run(void) { return N_LAUNCHES; }
 
+int lst_dnn_n_weights(int32_t n_feat, int32_t n_hidden) {
+  if ((n_feat != N_FEAT && n_feat != N_FEAT_MAX) || n_hidden < 1 || n_hidden > 4) return LST_EINVAL;
+  return dnn_n_weights(n_feat, n_hidden);
+}
+
 int lst_workspace_bytes(const lst_geometry* geo, const lst_caps* caps, size_t* out_bytes) {
   if (!out_bytes) return LST_EINVAL;
   const int rc = validate(geo, caps);
@@ -207,7 +215,13 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   cudaError_t e = cudaMemcpy(L.modt, modt.data(), M, cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemcpy(L.rowptr, geo->conn_rowptr, sizeof(int) * (M + 1), cudaMemcpyHostToDevice);
   if (e == cudaSuccess && nnz > 0) e = cudaMemcpy(L.col, geo->conn_col, sizeof(int) * nnz, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy(L.weights, geo->dnn_weights, sizeof(float) * N_W, cudaMemcpyHostToDevice);
+  const int n_feat = geo->dnn_n_feat ? geo->dnn_n_feat : N_FEAT, n_hidden = geo->dnn_n_hidden ? geo->dnn_n_hidden : 2;
+  if (e == cudaSuccess) e = cudaMemcpy(L.weights, geo->dnn_weights, sizeof(float) * dnn_n_weights(n_feat, n_hidden), cudaMemcpyHostToDevice);
+  {
+    std::vector<uint8_t> lay(M, 0);
+    if (geo->layer) for (int m = 0; m < M; ++m) lay[m] = geo->layer[m];
+    if (e == cudaSuccess) e = cudaMemcpy(L.layer, lay.data(), M, cudaMemcpyHostToDevice);
+  }
   {   // CSR rows -> runs of consecutive module ids (one run = one contiguous MD range, lst_pairs.cuh)
     std::vector<int> run_ptr(M + 1, 0), c0, c1;
     for (int m = 0; m < M; ++m) {
@@ -246,7 +260,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     }
     (void)cudaGetLastError();
   }
-  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights;
+  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
   c->geo.run_ptr = L.run_ptr; c->geo.run_c0 = L.run_c0; c->geo.run_c1 = L.run_c1;
   *out = c;
   return LST_OK;
@@ -328,7 +342,14 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   k_ls_finish<<<GL, PAIR_WARPS * 32, 0, st>>>(sl, g, k); LST_MARK();
   k_t3_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
   k_t5_one<<<GL, TUPLE_TPB, 0, st>>>(sl, k); LST_MARK();
-  k_dnn<<<G, 128, 0, st>>>(sl, g); LST_MARK();
+  {
+#define LST_DNN(NI, NH_) k_dnn<NI, NH_><<<G, 128, 0, st>>>(sl, g)
+    const int nh = g.n_hidden;
+    if (g.n_feat == N_FEAT) { if (nh == 1) LST_DNN(N_FEAT, 1); else if (nh == 2) LST_DNN(N_FEAT, 2); else if (nh == 3) LST_DNN(N_FEAT, 3); else LST_DNN(N_FEAT, 4); }
+    else { if (nh == 1) LST_DNN(N_FEAT_MAX, 1); else if (nh == 2) LST_DNN(N_FEAT_MAX, 2); else if (nh == 3) LST_DNN(N_FEAT_MAX, 3); else LST_DNN(N_FEAT_MAX, 4); }
+#undef LST_DNN
+  }
+  LST_MARK();
   k_scan_lb<SCAN_T5><<<GS, SCAN_TPB, 0, st>>>(sl, g, k); LST_MARK();
   if (fork) { if (bad(c, cudaStreamWaitEvent(st, c->ev_join, 0))) return LST_ECUDA; }
   else k_pls_bin<<<G1, 1024, PLS_BIN_SMEM, st>>>(sl);

@@ -12,7 +12,7 @@
 
 namespace lst {
 
-constexpr int N_FEAT = 23, N_HID = 32, N_W = 1857;
+constexpr int N_FEAT = 23, N_FEAT_MAX = 38, N_HID = 32, N_W = 1857;
 constexpr int CNT_STATUS = LST_N_CNT - 1;
 constexpr unsigned long long WIN_EMPTY = 0xFFFFFFFFFFFFFFFFull;
 constexpr int TC_HSTRIDE = 12;         // ints per row of the candidates' hit tuples (10 hits, padded for 16-byte loads)
@@ -22,7 +22,9 @@ struct Geo {   // device copies, shared by all slots
   const uint8_t* modt;      // [M] subdet<<1 | mtype
   const int* rowptr;        // [M+1]
   const int* col;           // [nnz]
-  const float* weights;     // [1857]
+  const float* weights;     // [dnn_n_weights(n_feat, n_hidden)]
+  const uint8_t* layer;     // [M] detector layer of the module (0 if the caller gave none): a 38-feature DNN input only
+  int n_feat, n_hidden;     // DNN variant (SPEC.md 4.9): 23 or 38 inputs, 1..4 hidden layers of 32
   // CSR rows compressed into runs of consecutive module ids (built by lst_create): row m = runs [run_ptr[m], run_ptr[m+1]),
   // run e = modules [run_c0[e], run_c1[e]).  MDs are stored in module order, so a run is one contiguous MD range.
   const int* run_ptr;       // [M+1]
@@ -251,66 +253,109 @@ __global__ void k_rank(const Slot* __restrict__ slots) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// a5: T5-DNN (SPEC.md 4.5).  One thread per candidate; features, hidden activations and the
-// running sums stay in registers, the 1857 weights sit in shared memory and are read as
-// warp-uniform (broadcast) float4s.  FMA is allowed here (scores agree with the oracle to 1e-5).
+// a5: T5-DNN (SPEC.md 4.5; variants 4.9).  One thread per candidate; features, hidden activations and the
+// running sums stay in registers, the weights sit in shared memory and are read as warp-uniform
+// (broadcast) float4s.  FMA is allowed here (scores agree with the oracle to 1e-5).  NIN = 23 (configs[0]) or 38 (the
+// paper's input list), NH = 1..4 hidden layers of 32.
 // ------------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int dnn_n_weights(int n_feat, int n_hidden) {
+  return N_HID * n_feat + N_HID + (n_hidden - 1) * (N_HID * N_HID + N_HID) + N_HID + 1;
+}
+__device__ __forceinline__ float feat_radius(float c) { return log10f(fminf(__fdiv_rn(1.0f, fabsf(c)), 1.0e5f)); }
+__device__ __forceinline__ float feat_pt(float c) { return log10f(__fmul_rn(LST_KAPPA, fminf(__fdiv_rn(1.0f, fabsf(c)), 1.0e5f))); }
+
+template <int NIN, int NH>
 __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, Geo geo) {
-  __shared__ __align__(16) float W1[N_HID * 24];   // rows padded 23 -> 24 for float4 reads
-  __shared__ __align__(16) float W2[N_HID * N_HID];
-  __shared__ float B1[N_HID], B2[N_HID], W3[N_HID + 1];
-  for (int i = threadIdx.x; i < N_HID * 24; i += blockDim.x) {
-    const int j = i / 24, k = i - 24 * j;
-    W1[i] = (k < N_FEAT) ? geo.weights[j * N_FEAT + k] : 0.0f;
+  constexpr int PIN = (NIN + 3) & ~3;             // rows of W1 padded for float4 reads
+  __shared__ __align__(16) float W1[N_HID * PIN];
+  __shared__ __align__(16) float WH[(NH > 1 ? NH - 1 : 1) * N_HID * N_HID];
+  __shared__ float BS[NH * N_HID], W3[N_HID + 1];
+  const float* gw = geo.weights;
+  for (int i = threadIdx.x; i < N_HID * PIN; i += blockDim.x) {
+    const int j = i / PIN, k = i - PIN * j;
+    W1[i] = (k < NIN) ? gw[j * NIN + k] : 0.0f;
   }
-  for (int i = threadIdx.x; i < N_HID * N_HID; i += blockDim.x) W2[i] = geo.weights[N_HID * N_FEAT + N_HID + i];
-  if (threadIdx.x < N_HID) {
-    B1[threadIdx.x] = geo.weights[N_HID * N_FEAT + threadIdx.x];
-    B2[threadIdx.x] = geo.weights[N_HID * N_FEAT + N_HID + N_HID * N_HID + threadIdx.x];
-    W3[threadIdx.x] = geo.weights[N_HID * N_FEAT + 2 * N_HID + N_HID * N_HID + threadIdx.x];
+  for (int i = threadIdx.x; i < N_HID; i += blockDim.x) BS[i] = gw[N_HID * NIN + i];
+  {
+    const float* p = gw + N_HID * NIN + N_HID;
+    for (int l = 1; l < NH; ++l) {
+      for (int i = threadIdx.x; i < N_HID * N_HID; i += blockDim.x) WH[(l - 1) * N_HID * N_HID + i] = p[i];
+      for (int i = threadIdx.x; i < N_HID; i += blockDim.x) BS[l * N_HID + i] = p[N_HID * N_HID + i];
+      p += N_HID * N_HID + N_HID;
+    }
+    for (int i = threadIdx.x; i <= N_HID; i += blockDim.x) W3[i] = p[i];
   }
-  if (threadIdx.x == 0) W3[N_HID] = geo.weights[N_W - 1];
   __syncthreads();
   const Slot& s = slots[blockIdx.y];
   const int n = s.cnt[LST_CNT_T5C];
   LST_FOR_ITEMS(i, n) {
-    float x[24];
+    float x[PIN];
+    if (NIN == N_FEAT) {
 #pragma unroll
-    for (int q = 0; q < 5; ++q) {
-      const float4 p = s.md_pos[s.t5c_md[5 * i + q]];
-      x[4 * q + 0] = p.w * 0.01f;
-      x[4 * q + 1] = p.z * 0.01f;
-      x[4 * q + 2] = asinhf(__fdiv_rn(p.z, p.w));
-      x[4 * q + 3] = atan2f(p.y, p.x);
+      for (int q = 0; q < 5; ++q) {
+        const float4 p = s.md_pos[s.t5c_md[5 * i + q]];
+        x[4 * q + 0] = p.w * 0.01f;
+        x[4 * q + 1] = p.z * 0.01f;
+        x[4 * q + 2] = asinhf(__fdiv_rn(p.z, p.w));
+        x[4 * q + 3] = atan2f(p.y, p.x);
+      }
+#pragma unroll
+      for (int q = 0; q < 3; ++q) x[20 + q] = feat_radius(s.t5c_curv[3 * i + q]);
+    } else {      // SPEC.md 4.9: 2 T3 x (pT, radius), anchors a, b, c, c, d, e x (r, phi, z, eta, layer), T5 (pT, eta, phi), bridge radius
+      const float cin = s.t5c_curv[3 * i], cbr = s.t5c_curv[3 * i + 1], cout = s.t5c_curv[3 * i + 2];
+      x[0] = feat_pt(cin); x[1] = feat_radius(cin); x[2] = feat_pt(cout); x[3] = feat_radius(cout);
+      float a5[5][5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) {
+        const int m = s.t5c_md[5 * i + q];
+        const float4 p = s.md_pos[m];
+        a5[q][0] = p.w * 0.01f; a5[q][1] = atan2f(p.y, p.x); a5[q][2] = p.z * 0.01f; a5[q][3] = asinhf(__fdiv_rn(p.z, p.w));
+        a5[q][4] = (float)geo.layer[s.md_modt[m] >> 2] * 0.1f;
+      }
+#pragma unroll
+      for (int k = 0; k < 6; ++k) {
+        const int q = k < 3 ? k : k - 1;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) x[4 + 5 * k + f] = a5[q][f];
+      }
+      x[34] = feat_pt(__fmul_rn(0.5f, __fadd_rn(cin, cout)));
+      x[35] = a5[0][3]; x[36] = a5[0][1]; x[37] = feat_radius(cbr);
     }
 #pragma unroll
-    for (int q = 0; q < 3; ++q) x[20 + q] = log10f(fminf(__fdiv_rn(1.0f, fabsf(s.t5c_curv[3 * i + q])), 1.0e5f));
-    x[23] = 0.0f;
-    float* fo = s.t5c_feat + (size_t)N_FEAT * i;
+    for (int k = NIN; k < PIN; ++k) x[k] = 0.0f;
+    float* fo = s.t5c_feat + (size_t)NIN * i;
 #pragma unroll
-    for (int k = 0; k < N_FEAT; ++k) fo[k] = x[k];
-    float h1[N_HID];
+    for (int k = 0; k < NIN; ++k) fo[k] = x[k];
+    float h[N_HID];
 #pragma unroll
     for (int j = 0; j < N_HID; ++j) {
-      float acc = B1[j];
+      float acc = BS[j];
 #pragma unroll
-      for (int k = 0; k < 24; k += 4) {
-        const float4 w = *reinterpret_cast<const float4*>(&W1[j * 24 + k]);
+      for (int k = 0; k < PIN; k += 4) {
+        const float4 w = *reinterpret_cast<const float4*>(&W1[j * PIN + k]);
         acc = fmaf(w.x, x[k], acc); acc = fmaf(w.y, x[k + 1], acc); acc = fmaf(w.z, x[k + 2], acc); acc = fmaf(w.w, x[k + 3], acc);
       }
-      h1[j] = fmaxf(acc, 0.0f);
+      h[j] = fmaxf(acc, 0.0f);
+    }
+#pragma unroll
+    for (int l = 1; l < NH; ++l) {
+      float g[N_HID];
+#pragma unroll
+      for (int j = 0; j < N_HID; ++j) {
+        float acc = BS[l * N_HID + j];
+#pragma unroll
+        for (int k = 0; k < N_HID; k += 4) {
+          const float4 w = *reinterpret_cast<const float4*>(&WH[((l - 1) * N_HID + j) * N_HID + k]);
+          acc = fmaf(w.x, h[k], acc); acc = fmaf(w.y, h[k + 1], acc); acc = fmaf(w.z, h[k + 2], acc); acc = fmaf(w.w, h[k + 3], acc);
+        }
+        g[j] = fmaxf(acc, 0.0f);
+      }
+#pragma unroll
+      for (int j = 0; j < N_HID; ++j) h[j] = g[j];
     }
     float y = W3[N_HID];
 #pragma unroll
-    for (int j = 0; j < N_HID; ++j) {
-      float acc = B2[j];
-#pragma unroll
-      for (int k = 0; k < N_HID; k += 4) {
-        const float4 w = *reinterpret_cast<const float4*>(&W2[j * N_HID + k]);
-        acc = fmaf(w.x, h1[k], acc); acc = fmaf(w.y, h1[k + 1], acc); acc = fmaf(w.z, h1[k + 2], acc); acc = fmaf(w.w, h1[k + 3], acc);
-      }
-      y = fmaf(W3[j], fmaxf(acc, 0.0f), y);
-    }
+    for (int j = 0; j < N_HID; ++j) y = fmaf(W3[j], h[j], y);
     const float score = __fdiv_rn(1.0f, 1.0f + expf(-y));
     const int pass = score > 0.5f;
     s.t5c_score[i] = score;

@@ -17,9 +17,9 @@ def bits_equal(a, b):
     return a.shape == b.shape and bool(np.array_equal(a.view(np.uint32), b.view(np.uint32)))
 
 
-def compare(geo, weights, ev, gpu, check_order=True):
+def compare(geo, weights, ev, gpu, check_order=True, dnn=(23, 2)):
     """`gpu` = LST.fetch(slot) dict.  Returns a dict of counts; raises AssertionError on any mismatch."""
-    r = O.run(geo, weights, ev)
+    r = O.run(geo, weights, ev, dnn=dnn)
     g = gpu
     assert g["status"] == r.flags, (g["status"], r.flags)
     # a0
@@ -58,7 +58,7 @@ def compare(geo, weights, ev, gpu, check_order=True):
         n_flip = int(flip.sum())
         if n_flip:   # replay the oracle with the GPU's decision on the borderline candidates only
             ov = -np.ones(n5c, np.int8); ov[flip] = gp[flip]
-            r = O.run(geo, weights, ev, t5_override=ov)
+            r = O.run(geo, weights, ev, t5_override=ov, dnn=dnn)
     # T5 list, matching, TC
     assert np.array_equal(g["t5"]["cand"], r.t5)
     assert np.array_equal(g["match5"]["best5_pls"], r.best5_pls)

@@ -270,3 +270,18 @@ def test_graph_export(P, geo_full):
     n_edges = [parity.compare_graph(geo_full, w, ev, lst.fetch_graph(i)) for i, ev in enumerate(evs)]
     assert n_edges[0] > 10000 and n_edges[2] == 0
     lst.close()
+
+
+@pytest.mark.parametrize("n_feat,n_hidden", [(23, 1), (23, 3), (23, 4), (38, 1), (38, 2), (38, 3), (38, 4)])
+def test_dnn_variants(P, geo_full, n_feat, n_hidden):
+    """f3 (SPEC.md 4.9): the paper's 38 inputs and the 1 / 3 / 4 hidden-layer networks of its depth scan, end to end."""
+    w = xavier_weights(11, bias_scale=0.3, n_feat=n_feat, n_hidden=n_hidden)
+    ev = config_event(geo_full, 1, seed=31)
+    lst = P.LST(geo_full, w, P.default_caps(1), dnn=(n_feat, n_hidden))
+    lst.load_numpy_event(0, ev)
+    lst.lst_run(0)
+    out = lst.fetch(0)
+    lst.close()
+    assert out["t5c"]["feat"].shape[1] == n_feat
+    c = parity.compare(geo_full, w, ev, out, dnn=(n_feat, n_hidden))
+    assert c["t5c"] > 500

@@ -31,7 +31,7 @@ def _geo_struct(P, geo, w):
     keep = [np.ascontiguousarray(geo.subdet, np.uint8), np.ascontiguousarray(geo.mtype, np.uint8),
             np.ascontiguousarray(geo.conn_rowptr, np.int32), np.ascontiguousarray(geo.conn_col, np.int32),
             np.ascontiguousarray(w, np.float32)]
-    return _Geometry(int(geo.n_modules), *[_hp(a) for a in keep]), keep
+    return _Geometry(int(geo.n_modules), *[_hp(a) for a in keep], None, 0, 0), keep
 
 
 def test_workspace_bytes_and_validation(lib, geo_full):

@@ -87,6 +87,10 @@ MUTANTS = [
     ("f1: greedy (dropped candidates no longer drop others)", "        if (y == x || !better_rank(tc[y], q[y], y, tc[x], q[x], x)) continue;",
      "        if (y == x || !keep[y] || !better_rank(tc[y], q[y], y, tc[x], q[x], x)) continue;", [("pin_clean_rule_by_hand", None)]),
     ("f1: pT3 ranked with the T5's chi2", "      if (c.type == 2) chi = res->chi3[c.obj];", "      if (c.type == 2) chi = res->chi5[0];", [("pin_clean_all_pairs", "geo")]),
+    ("f3: hidden layers beyond the first skipped", "  for (int l = 1; l < n_hidden; ++l) {", "  for (int l = 1; l < 1; ++l) {", [("pin_dnn_variants", "geo")]),
+    ("f3: 38 features: anchor order a,b,c,d,e,e", "const int order[6] = {0, 1, 2, 2, 3, 4};", "const int order[6] = {0, 1, 2, 3, 4, 4};", [("pin_dnn_variants", "geo")]),
+    ("f3: 38 features: layer not fed", "x[4 + 5 * i + 4] = float(layer[q]) * 0.1f;", "x[4 + 5 * i + 4] = 0.0f;", [("pin_dnn_variants", "geo")]),
+    ("f3: 38 features: T5 pT from c_in only", "const float c5 = 0.5f * (cin + cout);", "const float c5 = cin;", [("pin_dnn_variants", "geo")]),
     ("f1: upper hits left out of the tuples", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_up];", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_lo];", [("pin_clean_all_pairs", "geo")]),
 ]
 

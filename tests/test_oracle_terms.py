@@ -660,7 +660,60 @@ def pin_graph_export(geo):
     assert g["node_hits"][a].tolist() == r.md_hits[r.ls[l, 0]].tolist() and g["node_hits"][g["col"][l]].tolist() == r.md_hits[r.ls[l, 1]].tolist()
 
 
+# ====================================================================== f3: DNN variants (SPEC.md 4.9)
+def _mlp64_n(w, x, n_hidden):
+    """independent float64 restatement: W1[32][n_in], b1, (n_hidden - 1) x (W[32][32], b), w_out[32], b_out"""
+    w = w.astype(np.float64); n_in = x.size
+    o = 32 * n_in
+    h = np.maximum(w[:o].reshape(32, n_in) @ x + w[o:o + 32], 0.0); o += 32
+    for _ in range(n_hidden - 1):
+        h = np.maximum(w[o:o + 1024].reshape(32, 32) @ h + w[o + 1024:o + 1056], 0.0); o += 1056
+    assert o + 33 == w.size
+    return 1.0 / (1.0 + np.exp(-(w[o:o + 32] @ h + w[o + 32])))
+
+
+def pin_dnn_variants(geo):
+    """Every (n_feat, n_hidden) against an independent float64 MLP on the oracle's own features, the 38 features against their
+    float64 definitions, and one-hot weights through every layer of the 4-deep network (a transposed or skipped layer fails)."""
+    ev = config_event(geo, 1)
+    lay = geo.layer.astype(np.int64)
+    for nf in (23, 38):
+        for nh in (1, 2, 3, 4):
+            w = xavier_weights(7, bias_scale=0.3, n_feat=nf, n_hidden=nh)
+            r = O.run(geo, w, ev, last_stage="t5", dnn=(nf, nh))
+            assert r.t5c_feat.shape[1] == nf and len(r.t5c) > 500
+            ref = np.array([_mlp64_n(w, f, nh) for f in r.t5c_feat[:300]])
+            assert np.abs(ref - r.t5c_score[:300]).max() < 2e-6, (nf, nh)
+            assert np.array_equal(r.t5c[:, 7] == 1, r.t5c_score > 0.5)
+    r = O.run(geo, xavier_weights(7, n_feat=38), ev, last_stage="t5", dnn=(38, 2))
+    K = np.float32(0.0114)
+    rad = lambda c: min(1.0 / abs(c), 1e5) if c != 0 else 1e5
+    for t, f, cv in list(zip(r.t5c, r.t5c_feat, r.t5c_curv))[:200]:
+        exp = [np.log10(K * rad(cv[0])), np.log10(rad(cv[0])), np.log10(K * rad(cv[2])), np.log10(rad(cv[2]))]
+        for m in (t[0], t[1], t[2], t[2], t[3], t[4]):
+            c, w_, x, y, z, rr = r.md_real[m]
+            exp += [rr / 100.0, np.arctan2(y, x), z / 100.0, np.arcsinh(z / rr), lay[r.md_mod[m]] * 0.1]
+        c5 = np.float32(0.5) * (np.float32(cv[0]) + np.float32(cv[2]))
+        c, w_, x, y, z, rr = r.md_real[t[0]]
+        exp += [np.log10(K * rad(float(c5))), np.arcsinh(z / rr), np.arctan2(y, x), np.log10(rad(cv[1]))]
+        assert np.allclose(f, exp, rtol=3e-6, atol=2e-6), np.abs(f - np.array(exp)).max()
+    assert len(set(np.round(r.t5c_feat[:, 8], 3).tolist())) >= 2          # the layer feature is really fed
+    # one-hot path through four hidden layers: x[5] -> h1[3] -> h2[7] -> h3[11] -> h4[2] -> out
+    nf, nh = 38, 4
+    w = np.zeros(32 * nf + 32 + 3 * 1056 + 33, np.float32)
+    w[:32 * nf].reshape(32, nf)[3, 5] = 2.0
+    o = 32 * nf + 32
+    for src, dst in ((3, 7), (7, 11), (11, 2)):
+        w[o:o + 1024].reshape(32, 32)[dst, src] = 1.5; o += 1056
+    w[o + 2] = 0.5
+    x = np.zeros(nf, np.float32); x[5] = 1.0
+    assert abs(O.mlp_n(w, x, nh) - 1 / (1 + np.exp(-2.0 * 1.5 ** 3 * 0.5))) < 1e-6
+    x[5] = -1.0
+    assert O.mlp_n(w, x, nh) == 0.5
+
+
 # ---------------------------------------------------------------------- pytest entry points
+def test_dnn_variants(geo_full): pin_dnn_variants(geo_full)
 def test_graph_export(geo_full): pin_graph_export(geo_full)
 def test_clean_rule_by_hand(): pin_clean_rule_by_hand()
 def test_clean_chain(geo_barrel): pin_clean_chain(geo_barrel)
