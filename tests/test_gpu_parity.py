@@ -48,7 +48,7 @@ def test_config2_pu200_headline(P, geo_full):
     assert c["md"] > 10000 and c["tc"] > 2000
 
 
-@pytest.mark.parametrize("pileup", [0, 100, 300])
+@pytest.mark.parametrize("pileup", [0, 100, 200, 300])
 def test_config4_displaced_stress(P, geo_full, pileup):
     w = xavier_weights(3)
     ev = config_event(geo_full, 4, seed=200 + pileup // 100, pileup=pileup)
@@ -112,6 +112,14 @@ def test_every_overflow_flag(P, geo_full):
             assert np.array_equal(out["md"]["hits"], ref.md_hits[:kw[name]])
         if name == "max_ls":
             assert np.array_equal(out["ls"]["ab"], ref.ls[:kw[name]])
+        if name == "max_t3":          # the first cap objects in build order, as include/lst.h promises
+            assert np.array_equal(out["t3"]["abc"][:, :3], ref.t3[:kw[name], :3]) and np.array_equal(out["t3"]["l1"], ref.t3[:kw[name], 4])
+        if name == "max_t5c":
+            assert np.array_equal(out["t5c"]["md"], ref.t5c[:kw[name], :5])
+        if name == "max_t5":
+            assert np.array_equal(out["t5"]["cand"], ref.t5[:kw[name]])
+        # LST_ST_OVF_TC cannot occur: the TC capacity is max_pls + max_t5 and the list holds at most one row per pLS and T5
+        assert not out["status"] & P.STATUS_BITS["ovf_tc"]
     # exact fit: no flag
     kw = dict(n_slots=1, max_hits=ev.n_hits, max_pls=ev.n_pls, **full)
     out = _run_one(P, geo_full, w, ev, P.Caps(**kw))
@@ -204,7 +212,7 @@ def test_packed_host_buffers_single_copies(P, geo_full):
 
 def test_bench_launch_configuration_sampled(P, geo_full):
     """The configuration bench.py times (configs[3]): 64 PU200 events, seeds 100-163, 4 streams x 16-event batched
-    launches, bench capacities.  Sampled events are compared with the oracle in full; every event must be
+    launches, bench capacities.  ALL 64 events are compared with the oracle in full; every event must be
     overflow-free and satisfy the TC partition identity n_pLS = pT5 + pT3 + pLS-TC."""
     import torch
     w = xavier_weights(3)
@@ -224,7 +232,7 @@ def test_bench_launch_configuration_sampled(P, geo_full):
         bits, c = lst.lst_status(i)
         assert bits == 0, (i, bits)
         assert c["pt5"] + c["pt3"] + c["plstc"] == ev.n_pls and c["pt5"] + c["t5tc"] + c["pt3"] + c["plstc"] == c["tc"], (i, c)
-    for i in (0, 21, 42, 63):
+    for i in range(E):                                    # every event of the timed configuration, in full
         parity.compare(geo_full, w, evs[i], lst.fetch(i))
     lst.close()
 
@@ -285,3 +293,126 @@ def test_dnn_variants(P, geo_full, n_feat, n_hidden):
     assert out["t5c"]["feat"].shape[1] == n_feat
     c = parity.compare(geo_full, w, ev, out, dnn=(n_feat, n_hidden))
     assert c["t5c"] > 500
+
+
+def _dup_hits(ev, sel, times):
+    """append `times` copies of the hits `sel` (same sensor, same position): every object built on them multiplies"""
+    for name in ("x", "y", "z", "key", "hit_particle"):
+        a = getattr(ev, name)
+        setattr(ev, name, np.concatenate([a] + [a[sel]] * times))
+
+
+def test_rows_with_many_partners(P, geo_barrel):
+    """a3 / a4 keep the first TUPLE_STASH = 3 passing partners of a row in registers and evaluate the row again when there
+    are more.  Hits of layers 3-5 of clean muons duplicated twice -> 9 MDs per layer and muon -> LS rows with 9 passing
+    partners, T3 rows with 9: the re-evaluation path is what produces these lists."""
+    w = xavier_weights(1)
+    ev = make_event(geo_barrel, 81, origin_muons=3, smear=False)
+    r = np.hypot(ev.x, ev.y)
+    _dup_hits(ev, np.flatnonzero((r > 50) & (r < 90)), 2)
+    out = _run_one(P, geo_barrel, w, ev)
+    c = parity.compare(geo_barrel, w, ev, out)
+    t3_per_row = np.bincount(out["t3"]["abc"][:, 3])
+    t5_per_row = np.bincount(out["t5c"]["t3"][:, 0])
+    assert t3_per_row.max() > 3 and t5_per_row.max() > 3, (t3_per_row.max(), t5_per_row.max())
+
+
+def test_csr_row_with_many_runs(P, geo_barrel):
+    """a2 caches the non-empty runs of a CSR row 32 at a time; a row with more runs than that takes the chunked path.  The
+    rows of the occupied layer-1 modules get 40 extra, non-consecutive columns (every second module of layer 2)."""
+    import dataclasses
+    w = xavier_weights(1)
+    ev = make_event(geo_barrel, 82, origin_muons=10)
+    l2 = int(geo_barrel.barrel_base[1])
+    occupied = set(int(k) >> 1 for k in ev.key if (int(k) >> 1) < l2)
+    # every second module of a stretch of layer 2 (mostly empty: runs that hold no MD) plus every occupied module beyond layer 1
+    extra = set(range(l2, l2 + 160, 2)) | set(range(l2 + 401, l2 + 481, 2)) | set(int(k) >> 1 for k in ev.key if (int(k) >> 1) >= l2)
+    rows = []
+    for m in range(geo_barrel.n_modules):
+        cols = set(geo_barrel.conn_col[geo_barrel.conn_rowptr[m]:geo_barrel.conn_rowptr[m + 1]].tolist())
+        if m in occupied:
+            cols |= extra
+        rows.append(sorted(cols))
+    rowptr = np.zeros(geo_barrel.n_modules + 1, np.int32)
+    rowptr[1:] = np.cumsum([len(c) for c in rows])
+    g2 = dataclasses.replace(geo_barrel, conn_rowptr=rowptr, conn_col=np.array([c for r in rows for c in r], np.int32))
+    n_runs = max(sum(1 for i, c in enumerate(r) if i == 0 or r[i - 1] != c - 1) for r in rows)
+    assert n_runs > 64
+    out = _run_one(P, g2, w, ev)
+    c = parity.compare(g2, w, ev, out)
+    assert c["ls_pairs"] > 400 and c["ls"] > 40
+
+
+def test_dense_module_takes_the_big_path(P, geo_barrel):
+    """a1 packs the cells of 32 modules into one flat index space unless a module alone has more than 2^20 cells; such a
+    module (1100 x 1100 hits here) is swept on its own with a 64-bit sweep counter.  Expect plain parity, no flag."""
+    w = xavier_weights(1)
+    ev = make_event(geo_barrel, 83, origin_muons=4)
+    rng = np.random.default_rng(9)
+    m = 5 * 24 + 12                                   # a layer-1 module: phi sector 5, central z tile
+    nphi = int(geo_barrel.barrel_nphi[0])
+    n = 1100
+    for up, rr in ((0, 23.0), (1, 23.26)):
+        ph = (5 + rng.uniform(0.05, 0.95, n)) * 2 * np.pi / nphi
+        ev.x = np.concatenate([ev.x, (rr * np.cos(ph)).astype(np.float32)]); ev.y = np.concatenate([ev.y, (rr * np.sin(ph)).astype(np.float32)])
+        ev.z = np.concatenate([ev.z, rng.uniform(0.5, 9.5, n).astype(np.float32)])
+        ev.key = np.concatenate([ev.key, np.full(n, 2 * m + up, np.uint32)])
+        ev.hit_particle = np.concatenate([ev.hit_particle, np.full(n, -1, np.int32)])
+    out = _run_one(P, geo_barrel, w, ev, P.Caps(n_slots=1, max_hits=8192, max_md=65536, max_ls=65536, max_t3=65536, max_t5c=65536, max_t5=65536, max_pls=64))
+    assert out["status"] == 0
+    c = parity.compare(geo_barrel, w, ev, out)
+    assert c["md_pairs"] > (1 << 20) and c["md"] > 1000
+
+
+def test_graphs_on_off_and_determinism(P, geo_full):
+    """The CUDA-graph replay (default on a non-default stream) and direct launches (LST_GRAPHS=0) give identical bytes, and
+    one PU200 event run 100 times gives the same bytes every time."""
+    import os, torch
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 2)
+    names = ("md", "ls", "t3", "t5c", "t5", "tc", "match5", "tcc", "tcx")
+
+    def snap(lst):
+        o = lst.fetch(0)
+        return {(n, k): v.copy().view(np.uint8) for n in names for k, v in o[n].items()}
+
+    st = torch.cuda.Stream()
+    lst = P.LST(geo_full, w, P.default_caps(1))
+    lst.load_numpy_event(0, ev)
+    torch.cuda.synchronize()
+    lst.lst_run(0, st)
+    torch.cuda.synchronize()
+    ref = snap(lst)
+    for _ in range(100):
+        lst.lst_run(0, st)
+    torch.cuda.synchronize()
+    again = snap(lst)
+    assert all(np.array_equal(ref[k], again[k]) for k in ref)
+    for rep in range(4):                 # a few full comparisons along the way as well
+        lst.lst_run(0, st)
+        torch.cuda.synchronize()
+        again = snap(lst)
+        assert all(np.array_equal(ref[k], again[k]) for k in ref), rep
+    lst.close()
+    os.environ["LST_GRAPHS"] = "0"
+    try:
+        lst = P.LST(geo_full, w, P.default_caps(1))
+        lst.load_numpy_event(0, ev)
+        torch.cuda.synchronize()
+        lst.lst_run(0, st)
+        torch.cuda.synchronize()
+        direct = snap(lst)
+        lst.close()
+    finally:
+        del os.environ["LST_GRAPHS"]
+    assert all(np.array_equal(ref[k], direct[k]) for k in ref)
+    # and the bytes that never changed are the right ones
+    lst = P.LST(geo_full, w, P.default_caps(1))
+    lst.load_numpy_event(0, ev)
+    torch.cuda.synchronize()
+    lst.lst_run(0, st)
+    torch.cuda.synchronize()
+    out = lst.fetch(0)
+    lst.close()
+    assert all(np.array_equal(ref[(n, k)], v.view(np.uint8)) for n in names for k, v in out[n].items())
+    parity.compare(geo_full, w, ev, out)
