@@ -7,7 +7,7 @@ Contract (one JSON line on stdout from rank 0):
 
 A "step" = one pass of the whole hot path over one batch of `--events` synthetic PU200 events
 (BASELINE.json configs[2] recipe, the seeds of configs[3]); `value` = events/s with the inputs resident
-in HBM; `e2e` = the same through lst_load_batch_host / lst_read_tc_hits_batch_host with pinned HOST buffers, copies
+in HBM; `e2e` = the same through lst_load_batch_host16 / lst_read_tc_hits_batch_host with pinned HOST buffers, copies
 inside the timed region; `single_event` = configs[2] exactly (one event, seed 3); `--config 4` = the occupancy sweep.  Events are independent, so N GPUs run N replicas on different seeds (weak
 scaling, no collective on the data path -- DESIGN.md "Multi-GPU").
 """
@@ -314,14 +314,14 @@ def run_ours(args):
     # rows WITH their original hit indices, lst_read_tc_hits_batch_host): 1 H2D + 1 D2H copy per 16-event batch, every step
     e2e_streams = streams if S > 1 else [main]
     nb = E // len(e2e_streams)
-    blobs = [P.pack_batch(events[si * nb:(si + 1) * nb]) for si in range(len(e2e_streams))]
+    blobs = [P.pack_batch(events[si * nb:(si + 1) * nb], key16=True) for si in range(len(e2e_streams))]      # 14 bytes per hit
     h_outs = [torch.zeros((nb, 32 + 13 * TC_ROWS), dtype=torch.int32).pin_memory() for _ in e2e_streams]
     h2d = sum(int(b.numel()) for b in blobs)
     d2h = E * (32 * 4 + TC_ROWS * 13 * 4)
 
     def e2e_step():
         for si, st in enumerate(e2e_streams):
-            lst.lst_load_batch_host(si * nb, nb, blobs[si], stream=st)
+            lst.lst_load_batch_host16(si * nb, nb, blobs[si], stream=st)
             lst.lst_run_batch(si * nb, nb, st)
             lst.lst_read_tc_hits_batch_host(si * nb, nb, h_outs[si], stream=st)
 

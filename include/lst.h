@@ -155,6 +155,12 @@ int lst_load_event_host(lst_ctx* ctx, int32_t slot, int32_t n_hits, const float*
 int lst_load_batch_host(lst_ctx* ctx, int32_t first_slot, int32_t n, const void* h_blob, size_t blob_bytes,
                         void* cuda_stream);
 
+/* The same with 16-bit sensor keys (14 instead of 16 bytes per hit over the host link): per event x[n_hits] y[n_hits] z[n_hits]
+ * (f32), key[n_hits] (u16, the array padded to a multiple of 4 bytes), then the pLS arrays as above; the event block padded to a
+ * multiple of 16 bytes.  Needs 2 * n_modules <= 65535 (LST_EINVAL otherwise). */
+int lst_load_batch_host16(lst_ctx* ctx, int32_t first_slot, int32_t n, const void* h_blob, size_t blob_bytes,
+                          void* cuda_stream);
+
 /* Batched read-back: h_out (HOST int32[n][LST_N_CNT + 3*max_rows]) receives, per slot, the counters (status word in
  * entry LST_N_CNT-1) and the first min(max_rows, count) TC rows (the rest of a slot's rows is left untouched on
  * the device side, i.e. undefined).  One pack launch + ONE device->host copy.  max_rows <= max_pls + max_t5. */

@@ -15,7 +15,7 @@ CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t
            raw_t5=11, raw_tc=12, pt5=13, t5tc=14, pt3=15, plstc=16, m5_tests=17, m5_cand=18, m3_tests=19, m3_cand=20, tcc=29)
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
-           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_export_graph", "lst_dnn_n_weights", "lst_measure_fp32", "lst_launches_per_run",
+           "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_load_batch_host16", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_export_graph", "lst_dnn_n_weights", "lst_measure_fp32", "lst_launches_per_run",
            "lst_destroy"]
 
 
@@ -83,6 +83,7 @@ def load_library():
     L.lst_status.argtypes = [vp, i32, C.POINTER(C.c_uint32), vp, vp]
     L.lst_read_tc_host.argtypes = [vp, i32, vp, vp, i32, vp]
     L.lst_load_batch_host.argtypes = [vp, i32, i32, vp, C.c_size_t, vp]
+    L.lst_load_batch_host16.argtypes = [vp, i32, i32, vp, C.c_size_t, vp]
     L.lst_read_tc_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
     L.lst_read_tc_hits_batch_host.argtypes = [vp, i32, i32, vp, i32, vp]
     L.lst_measure_fp32.argtypes = [vp, i32, C.POINTER(C.c_float), vp]
@@ -245,6 +246,11 @@ class LST:
         _chk(self.lib.lst_load_batch_host(self.ctx, first_slot, n, C.c_void_p(h_blob.data_ptr()), C.c_size_t(h_blob.numel()),
                                           self._st(stream)), "lst_load_batch_host")
 
+    def lst_load_batch_host16(self, first_slot, n, h_blob, stream=None):
+        """h_blob: HOST (pinned) uint8 tensor packed with 16-bit sensor keys (see pack_batch(..., key16=True))."""
+        _chk(self.lib.lst_load_batch_host16(self.ctx, first_slot, n, C.c_void_p(h_blob.data_ptr()), C.c_size_t(h_blob.numel()),
+                                            self._st(stream)), "lst_load_batch_host16")
+
     def lst_read_tc_batch_host(self, first_slot, n, h_out, stream=None):
         """h_out: HOST (pinned) int32 tensor [n, 32 + 3*max_rows]."""
         rows = (int(h_out.shape[1]) - LST_N_CNT) // 3
@@ -324,13 +330,14 @@ class LST:
         return res
 
 
-def pack_batch(events, pin=True):
+def pack_batch(events, pin=True, key16=False):
     """Pack events (objects with x, y, z, key, pls_px, pls_py, pls_pz, pls_z0, pls_q numpy arrays) into the blob
-    layout of lst_load_batch_host: argument marshalling only."""
+    layout of lst_load_batch_host (key16=False) or lst_load_batch_host16 (key16=True): argument marshalling only."""
     import torch
     n = len(events)
     hdr = (8 * n + 15) // 16 * 16
-    sizes = [((16 * ev.x.size + 17 * ev.pls_px.size + 15) // 16) * 16 for ev in events]
+    kb = lambda nh: (2 * nh + 3) // 4 * 4 if key16 else 4 * nh
+    sizes = [((12 * ev.x.size + kb(ev.x.size) + 17 * ev.pls_px.size + 15) // 16) * 16 for ev in events]
     blob = torch.zeros(hdr + sum(sizes), dtype=torch.uint8)
     if pin:
         blob = blob.pin_memory()
@@ -340,11 +347,15 @@ def pack_batch(events, pin=True):
     for i, ev in enumerate(events):
         nh, npl = int(ev.x.size), int(ev.pls_px.size)
         desc[2 * i], desc[2 * i + 1] = nh, npl
-        f = b[off:off + 16 * nh].view(np.float32)
+        f = b[off:off + 12 * nh].view(np.float32)
         f[0:nh], f[nh:2 * nh], f[2 * nh:3 * nh] = ev.x, ev.y, ev.z
-        f[3 * nh:4 * nh] = ev.key.view(np.float32)
-        g = b[off + 16 * nh:off + 16 * nh + 16 * npl].view(np.float32)
+        if key16:
+            b[off + 12 * nh:off + 14 * nh].view(np.uint16)[:] = ev.key.astype(np.uint16)
+        else:
+            b[off + 12 * nh:off + 16 * nh].view(np.uint32)[:] = ev.key
+        o2 = off + 12 * nh + kb(nh)
+        g = b[o2:o2 + 16 * npl].view(np.float32)
         g[0:npl], g[npl:2 * npl], g[2 * npl:3 * npl], g[3 * npl:4 * npl] = ev.pls_px, ev.pls_py, ev.pls_pz, ev.pls_z0
-        b[off + 16 * nh + 16 * npl:off + 16 * nh + 17 * npl] = ev.pls_q.view(np.uint8)
+        b[o2 + 16 * npl:o2 + 17 * npl] = ev.pls_q.view(np.uint8)
         off += sizes[i]
     return blob

@@ -41,6 +41,7 @@ struct __align__(16) LsRec { int a, b, seq; float c; };
 struct Slot {
   // bound inputs
   const float *in_x, *in_y, *in_z; const uint32_t* in_key; int n_hits;
+  int key16;                // 1: in_key points at 16-bit keys (lst_load_batch_host16)
   const float *in_px, *in_py, *in_pz, *in_z0; const int8_t* in_q; int n_pls;
   // zero-initialised per run
   unsigned* epoch_dev;      // run counter of the slot (not cleared): validates the look-back status words of a run
@@ -75,6 +76,18 @@ struct Slot {
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
   int* tc_hdr;                       // copy of cnt[] in front of the TC rows, so one D2H copy reads both
 };
+
+// Programmatic dependent launch (sm_90+): the kernels of the chain are launched with programmatic stream serialization, so the
+// next kernel's blocks are scheduled while this one drains; `launch_dependents` lets that happen as early as possible and
+// `wait` blocks until the preceding kernel has completed and its writes are visible.  Both are no-ops for a plain launch.
+__device__ __forceinline__ void pdl_begin() {
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+__device__ __forceinline__ unsigned hit_key(const Slot& s, int i) {
+  return s.key16 ? (unsigned)reinterpret_cast<const unsigned short*>(s.in_key)[i] : s.in_key[i];
+}
 
 #define LST_FOR_ITEMS(i, n) \
   for (int i = blockIdx.x * blockDim.x + threadIdx.x, _st = gridDim.x * blockDim.x; i < (n); i += _st)
@@ -140,6 +153,7 @@ enum { SCAN_SENSOR = 0, SCAN_MDROW, SCAN_LSROW, SCAN_T5 };
 
 template <int MODE>
 __global__ void __launch_bounds__(SCAN_TPB) k_scan_lb(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  pdl_begin();
   __shared__ int sm[SCAN_TPB / 32];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
@@ -216,26 +230,29 @@ __global__ void __launch_bounds__(SCAN_TPB) k_scan_lb(const Slot* __restrict__ s
 // a0: hit ingest (SPEC.md 4.0) -- histogram, scan (k_scan<SCAN_SENSOR>), scatter, in-sensor rank
 // ------------------------------------------------------------------------------------------------
 __global__ void k_hist(const Slot* __restrict__ slots, Geo geo) {
+  pdl_begin();
   const Slot& s = slots[blockIdx.y];
   if (blockIdx.x == 0 && threadIdx.x == 0) *s.epoch_dev = (*s.epoch_dev % 0x3FFFFFFFu) + 1u;   // first kernel of a run
   const unsigned S = 2u * geo.n_modules;
   LST_FOR_ITEMS(i, s.n_hits) {
-    const unsigned key = s.in_key[i];
+    const unsigned key = hit_key(s, i);
     if (key >= S) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_BAD_KEY);
     else atomicAdd(s.sensor_start + key, 1);
   }
 }
 __global__ void k_scatter(const Slot* __restrict__ slots, Geo geo) {
+  pdl_begin();
   const Slot& s = slots[blockIdx.y];
   const unsigned S = 2u * geo.n_modules;
   LST_FOR_ITEMS(i, s.n_hits) {
-    const unsigned key = s.in_key[i];
+    const unsigned key = hit_key(s, i);
     if (key < S) s.tmp_ok[s.sensor_start[key] + atomicAdd(s.cursor + key, 1)] = make_int2(i, (int)key);
   }
 }
 // stable order inside a sensor: rank of a hit = number of hits of the same sensor with a smaller
 // original index (sensors hold a handful of hits, so the quadratic count is cheap and exact)
 __global__ void k_rank(const Slot* __restrict__ slots) {
+  pdl_begin();
   const Slot& s = slots[blockIdx.y];
   const int n = s.cnt[LST_CNT_HIT];
   const int2* __restrict__ ok = s.tmp_ok;
@@ -266,6 +283,7 @@ __device__ __forceinline__ float feat_pt(float c) { return log10f(__fmul_rn(LST_
 
 template <int NIN, int NH>
 __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, Geo geo) {
+  pdl_begin();
   constexpr int PIN = (NIN + 3) & ~3;             // rows of W1 padded for float4 reads
   __shared__ __align__(16) float W1[N_HID * PIN];
   __shared__ __align__(16) float WH[(NH > 1 ? NH - 1 : 1) * N_HID * N_HID];
@@ -532,6 +550,7 @@ __device__ __forceinline__ void match_drain1(const Slot& s, unsigned long long* 
 
 template <int NA, bool IS_T3>
 __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restrict__ slots) {
+  pdl_begin();
   __shared__ MatchWarp Wall[MATCH_WARPS];
   const Slot& s = slots[blockIdx.y];
   const int n = IS_T3 ? s.cnt[LST_CNT_T3] : s.cnt[LST_CNT_T5];
@@ -719,6 +738,7 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
 
 // per-MD lists of the pT5 entries (p, q) that contain the MD, for the "T3 already in a pT5" test
 __global__ void k_pt5_lists(const Slot* __restrict__ slots) {
+  pdl_begin();
   const Slot& s = slots[blockIdx.y];
   LST_FOR_ITEMS(p, s.n_pls) {
     const unsigned long long w = s.win5[p];
@@ -734,6 +754,7 @@ __global__ void k_pt5_lists(const Slot* __restrict__ slots) {
 
 // ordered emission of the four candidate types: one block per event, four flag-scan-write sweeps
 __global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots, Caps caps) {
+  pdl_begin();
   __shared__ int sm[34];
   const Slot& s = slots[blockIdx.y];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -790,6 +811,7 @@ __global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots
 // f1 (SPEC.md 4.7), step 1: the hit tuple of every candidate (ORIGINAL indices: lower, upper hit of each of its MDs), the chi2
 // of its rank key, and its entry in the list of every hit it holds.  One thread per TC row.
 __global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slots) {
+  pdl_begin();
   const Slot& s = slots[blockIdx.y];
   LST_FOR_ITEMS(o, s.cnt[LST_CNT_TC]) {
     const int type = s.tc[3 * o], obj = s.tc[3 * o + 2];
@@ -827,6 +849,7 @@ __global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slot
 // TCC_ROWS rows x 10 slots; the kept rows are compacted in order with a block scan + look-back across tiles (by ticket).
 constexpr int TCC_TPB = 128, TCC_ROWS = 12;
 __global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ slots, Caps caps) {
+  pdl_begin();
   __shared__ int s_keep[TCC_ROWS];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
@@ -920,7 +943,7 @@ __global__ void k_bind(Slot* slots, int slot, const float* x, const float* y, co
                        int n_hits, const float* px, const float* py, const float* pz, const float* z0,
                        const int8_t* q, int n_pls) {
   Slot& s = slots[slot];
-  s.in_x = x; s.in_y = y; s.in_z = z; s.in_key = key; s.n_hits = n_hits;
+  s.in_x = x; s.in_y = y; s.in_z = z; s.in_key = key; s.n_hits = n_hits; s.key16 = 0;
   s.in_px = px; s.in_py = py; s.in_pz = pz; s.in_z0 = z0; s.in_q = q; s.n_pls = n_pls;
 }
 
@@ -940,10 +963,29 @@ __global__ void k_bind_batch(Slot* slots, int first, int n, const char* blob) {
   const float* f = reinterpret_cast<const float*>(blob + off);
   const float* g = f + 4 * (size_t)nh;
   Slot& s = slots[first + e];
-  s.in_x = f; s.in_y = f + nh; s.in_z = f + 2 * (size_t)nh; s.in_key = reinterpret_cast<const uint32_t*>(f + 3 * (size_t)nh); s.n_hits = nh;
+  s.in_x = f; s.in_y = f + nh; s.in_z = f + 2 * (size_t)nh; s.in_key = reinterpret_cast<const uint32_t*>(f + 3 * (size_t)nh); s.n_hits = nh; s.key16 = 0;
   s.in_px = g; s.in_py = g + np; s.in_pz = g + 2 * (size_t)np; s.in_z0 = g + 3 * (size_t)np;
   s.in_q = reinterpret_cast<const int8_t*>(g + 4 * (size_t)np); s.n_pls = np;
 }
+// the same with 16-bit sensor keys: per event x[n_hits] y z (f32), key[n_hits] (u16, padded to 4 bytes), then the pLS block
+__host__ __device__ inline size_t blob16_event_bytes(int n_hits, int n_pls) {
+  return ((size_t)12 * n_hits + ((size_t)2 * n_hits + 3) / 4 * 4 + (size_t)17 * n_pls + 15) / 16 * 16;
+}
+__global__ void k_bind_batch16(Slot* slots, int first, int n, const char* blob) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n) return;
+  const int* desc = reinterpret_cast<const int*>(blob);
+  size_t off = blob_header_bytes(n);
+  for (int i = 0; i < e; ++i) off += blob16_event_bytes(desc[2 * i], desc[2 * i + 1]);
+  const int nh = desc[2 * e], np = desc[2 * e + 1];
+  const float* f = reinterpret_cast<const float*>(blob + off);
+  const float* g = reinterpret_cast<const float*>(blob + off + (size_t)12 * nh + ((size_t)2 * nh + 3) / 4 * 4);
+  Slot& s = slots[first + e];
+  s.in_x = f; s.in_y = f + nh; s.in_z = f + 2 * (size_t)nh; s.in_key = reinterpret_cast<const uint32_t*>(f + 3 * (size_t)nh); s.n_hits = nh; s.key16 = 1;
+  s.in_px = g; s.in_py = g + np; s.in_pz = g + 2 * (size_t)np; s.in_z0 = g + 3 * (size_t)np;
+  s.in_q = reinterpret_cast<const int8_t*>(g + 4 * (size_t)np); s.n_pls = np;
+}
+
 // packs counters + the first `rows` TC rows of n slots into one contiguous buffer [n][LST_N_CNT + W rows].
 // W = 3: (type, pLS, object index).  W = 13: the same followed by the candidate's ORIGINAL hit indices -- the ten hits of a
 // T5 (pT5 / T5), the six hits of a T3 (pT3), -1 padded -- so that the host-side result is self-contained.

@@ -240,6 +240,7 @@ __device__ __forceinline__ void md_sweep_body(const Slot& s, const Geo& geo, con
 }
 
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  pdl_begin();
   __shared__ MdWarp Wall[PAIR_WARPS];
   md_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
 }
@@ -247,6 +248,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __rest
 // a1 finish (md_start holds the exclusive scan of the per-module counts by now): record -> md_start[module] + seq.
 // If the stage overflowed its capacity the record buffer is incomplete: run the sweep again, writing in place.
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  pdl_begin();
   __shared__ MdWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
   if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) { md_sweep_body<true>(s, geo, caps, Wall); return; }
@@ -434,6 +436,7 @@ __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, con
 }
 
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  pdl_begin();
   __shared__ LsWarp Wall[PAIR_WARPS];
   ls_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
 }
@@ -441,6 +444,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __rest
 // a2 finish (ls_start holds the exclusive scan of the per-row counts by now): record -> ls_start[a] + seq; on capacity
 // overflow the sweep runs again, in place
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_finish(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+  pdl_begin();
   __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
   if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) { ls_sweep_body<true>(s, geo, caps, Wall); return; }

@@ -31,6 +31,7 @@ __device__ __forceinline__ int block_excl(int v, int* sm /*[TUPLE_TPB/32 + 1]*/,
 
 // a3 (SPEC.md 4.3): rows = LS l0 = (a,b); partners = LSs whose inner MD is b
 __global__ void __launch_bounds__(TUPLE_TPB) k_t3_one(const Slot* __restrict__ slots, Caps caps) {
+  pdl_begin();
   __shared__ int sm[TUPLE_TPB / 32 + 1];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
@@ -113,6 +114,7 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t3_one(const Slot* __restrict__ s
 
 // a4 (SPEC.md 4.4): rows = T3 u = (a,b,c); partners = T3s whose inner MD is c; the bridge (b,c,d) must pass
 __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ slots, Caps caps) {
+  pdl_begin();
   __shared__ int sm[TUPLE_TPB / 32 + 1];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];

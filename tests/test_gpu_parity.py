@@ -257,6 +257,18 @@ def test_batched_host_load_and_read(P, geo_full):
         ntc = out["counts"]["tc"]
         assert int(h[i, 31]) == 0 and int(h[i, P.CNT["tc"]]) == ntc
         assert np.array_equal(h[i, 32:32 + 3 * ntc].numpy().reshape(ntc, 3), out["tc"]["tc"].reshape(ntc, 3))
+    # the 16-bit-key wire format gives the same events
+    lst.lst_load_batch_host16(1, 3, P.pack_batch(evs, key16=True))
+    lst.lst_run_batch(1, 3)
+    h2 = torch.zeros((3, 32 + 13 * rows), dtype=torch.int32).pin_memory()
+    lst.lst_read_tc_hits_batch_host(1, 3, h2)
+    torch.cuda.synchronize()
+    for i, ev in enumerate(evs):
+        out = lst.fetch(1 + i)
+        parity.compare(geo_full, w, ev, out)
+        ntc = out["counts"]["tc"]
+        got = h2[i, 32:32 + 13 * ntc].numpy().reshape(ntc, 13)
+        assert np.array_equal(got[:, :3], out["tc"]["tc"].reshape(ntc, 3)) and np.array_equal(got[:, 3:], out["tcx"]["hits"].reshape(ntc, 12)[:, :10])
     with pytest.raises(P.LstError):                      # short buffer
         lst.lst_load_batch_host(0, 3, blob[:1000])
     bad = blob.clone()
