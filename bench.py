@@ -144,6 +144,8 @@ def algorithmic_work(lst, geo, slots):
         # method; the bucket walk's failed first-anchor tests are overhead, reported as per_event.match_tests
         "a6": dict(bytes=tot["pls"] * (17 + 28) + tot["t5"] * (20 + 80 + 8) + tot["t3"] * (12 + 48 + 8) + tot["tc"] * 12,
                    flops=FLOPS["match_full"] * (tot["match5"] + tot["match3"]) + FLOPS["match_pair"] * (tot["t5"] + tot["t3"])),
+        # f1 duplicate cleaning: per TC row the row itself, its hit tuple (written and read), its list links, keep flag, cleaned row
+        "f1": dict(bytes=tot["tc"] * (12 + 2 * 40 + 40 + 4 + 4 + 12), flops=0),
     }
     return tot, stages
 
