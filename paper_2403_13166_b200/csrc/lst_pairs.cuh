@@ -29,7 +29,6 @@ constexpr int PAIR_WARPS = 4;        // warps per block
 constexpr int Q_CAP = 64;            // survivor queue / record staging per warp (drained / flushed at >= 32)
 constexpr int RUN_CAP = 32;          // runs of a CSR row cached per warp at a time
 constexpr int LS_ROWS = 8;           // consecutive MD rows a warp takes at a time
-constexpr int LS_BC = 4;             // sweeps of a module whose column -> MD mapping a lane keeps in registers
 constexpr int MD_BIG = 1 << 20;      // modules with more cells than this are swept alone (64-bit sweep counter)
 
 __device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
@@ -261,6 +260,8 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
 // ------------------------------------------------------------------------------------------------
 struct LsWarp {
   int r_off[RUN_CAP + 1], r_b0[RUN_CAP];      // non-empty runs of the current module: first column, first MD
+  float4 a_pos[LS_ROWS], a_aux[LS_ROWS];      // the rows of the current chunk: anchor, prefilter record
+  int cnt[LS_ROWS];                           // LSs found so far in each row of the chunk
   int q_a[Q_CAP], q_b[Q_CAP];
   LsRec st[Q_CAP];
 };
@@ -288,8 +289,10 @@ __device__ __forceinline__ void ls_flush(const Slot& s, LsWarp& W, int n, int la
   if (lane < n && base + lane < cap) s.ls_rec[base + lane] = W.st[lane];
 }
 
+// exact evaluation of the first `n` (<= 32) queued cells.  The queue holds cells of the current chunk only, and the cells of
+// one row arrive in ascending column order, so seq = (LSs of the row so far) + (rank among the row's passing cells of this batch).
 template <bool DIRECT>
-__device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int sn, int lane, unsigned lt, int& carry_row, int& carry_n) {
+__device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int sn, int lane, unsigned lt) {
   bool pass = false;
   int a = -1 - lane, b = 0;
   float c = 0.f;
@@ -299,14 +302,30 @@ __device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int sn,
     pass = ls_eval(A, B, c);
   }
   const unsigned mask = __ballot_sync(0xffffffffu, pass);
-  bool last;
-  const int seq = row_sequence(a, pass, mask, lt, lane, carry_row, carry_n, last);
+  if (!mask) return sn;
+  const unsigned peers = __match_any_sync(0xffffffffu, a) & mask;
   if (pass) {
-    LsRec r; r.a = a; r.b = b; r.seq = seq; r.c = c;
+    const int before = __popc(peers & lt);
+    LsRec r; r.a = a; r.b = b; r.seq = W.cnt[a & (LS_ROWS - 1)] + before; r.c = c;
     W.st[sn + __popc(mask & lt)] = r;
-    if (!DIRECT && last) s.ls_start[a] = seq + 1;              // LSs of this row so far
   }
+  __syncwarp();
+  if (pass && (peers >> lane) >> 1 == 0u) W.cnt[a & (LS_ROWS - 1)] += __popc(peers);      // last passing cell of its row in this batch
   return sn + __popc(mask);
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ void ls_flush_full(const Slot& s, LsWarp& W, int& sn, int lane, int cap) {
+  if (sn < 32) return;
+  __syncwarp();
+  ls_flush<DIRECT>(s, W, 32, lane, cap);
+  __syncwarp();
+  LsRec tr{};
+  if (lane < sn - 32) tr = W.st[32 + lane];
+  __syncwarp();
+  if (lane < sn - 32) W.st[lane] = tr;
+  sn -= 32;
+  __syncwarp();
 }
 
 // non-empty runs [e, e + 32) of CSR row m -> the warp's run table; returns the number of columns they hold
@@ -336,15 +355,14 @@ __device__ __forceinline__ int ls_column(const LsWarp& W, int t) {
 }
 
 template <bool DIRECT>
-__device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int a, int b, int& qn, int& sn, int lane, unsigned lt,
-                                        int& carry_row, int& carry_n, int cap) {
+__device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int a, int b, int& qn, int& sn, int lane, unsigned lt, int cap) {
   const unsigned mask = __ballot_sync(0xffffffffu, pre);
   if (!mask) return;
   if (pre) { const int q = qn + __popc(mask & lt); W.q_a[q] = a; W.q_b[q] = b; }
   qn += __popc(mask);
-  __syncwarp();
   if (qn < 32) return;
-  sn = ls_drain<DIRECT>(s, W, 32, sn, lane, lt, carry_row, carry_n);
+  __syncwarp();
+  sn = ls_drain<DIRECT>(s, W, 32, sn, lane, lt);
   __syncwarp();
   const int rest = qn - 32;
   int x = 0, y = 0;
@@ -352,18 +370,15 @@ __device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int 
   __syncwarp();
   if (lane < rest) { W.q_a[lane] = x; W.q_b[lane] = y; }
   qn = rest;
-  if (sn >= 32) {
-    ls_flush<DIRECT>(s, W, 32, lane, cap);
-    __syncwarp();
-    LsRec tr{};
-    if (lane < sn - 32) tr = W.st[32 + lane];
-    __syncwarp();
-    if (lane < sn - 32) W.st[lane] = tr;
-    sn -= 32;
-  }
+  ls_flush_full<DIRECT>(s, W, sn, lane, cap);
   __syncwarp();
 }
 
+// A warp takes LS_ROWS consecutive MDs (rows) at a time.  Rows of the same module share their columns, so the chunk is cut
+// into module segments and every segment is swept columns-outer / rows-inner: the 32 column MDs of a step are loaded once
+// into registers (next step's loads already in flight) and tested against each row of the segment, whose anchors sit in
+// shared memory (broadcast reads).  The survivor queue is emptied at the end of every chunk, so the per-row LS counts live in
+// shared memory for the duration of a chunk and the row table is written once, coalesced.
 template <bool DIRECT>
 __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, const Caps& caps, LsWarp* Wall) {
   const int lane = threadIdx.x & 31;
@@ -375,63 +390,54 @@ __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, con
   const int n_md = s.cnt[LST_CNT_MD];
   const int cap = caps.max_ls;
   const int n_warps = gridDim.x * PAIR_WARPS;
-  int qn = 0, sn = 0, carry_row = -1, carry_n = 0;
+  int qn = 0, sn = 0;
   for (int a0 = (blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5)) * LS_ROWS; a0 < n_md; a0 += n_warps * LS_ROWS) {
-    const int a1 = min(a0 + LS_ROWS, n_md);
-    if (!DIRECT && a0 + lane < a1) s.ls_start[a0 + lane] = 0;
+    const int n_rows = min(LS_ROWS, n_md - a0);
+    int my_m = -1;
     __syncwarp();
-    int cur_m = -1, L = 0, e0 = 0, e1 = 0;
-    int bc[LS_BC];                              // the lane's columns of the first LS_BC sweeps of the current module
-    float4 Ap = __ldg(mpos + a0), Aa = __ldg(maux + a0);
-    int m = s.md_modt[a0] >> 2;
-    for (int a = a0; a < a1; ++a) {
-      if (m != cur_m) {
-        cur_m = m;
-        e0 = geo.run_ptr[m]; e1 = geo.run_ptr[m + 1];
-        if (e1 - e0 <= RUN_CAP) {
-          L = ls_load_runs(geo, mds, W, e0, e1, lane, lt);
-#pragma unroll
-          for (int j = 0; j < LS_BC; ++j) bc[j] = (32 * j < L) ? ls_column(W, min(32 * j + lane, L - 1)) : 0;
-        }
-      }
-      const float4 Apc = Ap, Aac = Aa;
-      if (a + 1 < a1) { Ap = __ldg(mpos + a + 1); Aa = __ldg(maux + a + 1); m = s.md_modt[a + 1] >> 2; }     // next row, ahead of use
-      const float kinvA = -2.0f * Aac.w;
+    if (lane < n_rows) {
+      W.a_pos[lane] = __ldg(mpos + a0 + lane); W.a_aux[lane] = __ldg(maux + a0 + lane);
+      my_m = s.md_modt[a0 + lane] >> 2;
+    }
+    if (lane < LS_ROWS) W.cnt[lane] = 0;
+    __syncwarp();
+    for (int i0 = 0; i0 < n_rows;) {
+      const int m = __shfl_sync(0xffffffffu, my_m, i0);
+      const int i1 = i0 + __popc(__ballot_sync(0xffffffffu, my_m == m));      // MDs are stored in module order: rows [i0, i1) are module m's
+      const int e0 = geo.run_ptr[m], e1 = geo.run_ptr[m + 1];
       for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
-        const bool one_pass = e1 - e0 <= RUN_CAP;
-        if (!one_pass) L = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
-#pragma unroll
-        for (int j = 0; j < LS_BC; j += 2) {       // two sweeps in flight: their loads and prefilter chains are independent
-          if (32 * j < L) {
-            const bool two = 32 * (j + 1) < L;
-            const int b0 = one_pass ? bc[j] : ls_column(W, min(32 * j + lane, L - 1));
-            const int b1 = two ? (one_pass ? bc[j + 1] : ls_column(W, min(32 * (j + 1) + lane, L - 1))) : b0;
-            const float4 Bp0 = __ldg(mpos + b0), Ba0 = __ldg(maux + b0), Bp1 = __ldg(mpos + b1), Ba1 = __ldg(maux + b1);
-            const bool pre0 = ls_prefilter(Apc, Aac, kinvA, Bp0, Ba0) && (32 * j + lane < L);
-            const bool pre1 = ls_prefilter(Apc, Aac, kinvA, Bp1, Ba1) && (32 * (j + 1) + lane < L);
-            ls_push<DIRECT>(s, W, pre0, a, b0, qn, sn, lane, lt, carry_row, carry_n, cap);
-            ls_push<DIRECT>(s, W, pre1, a, b1, qn, sn, lane, lt, carry_row, carry_n, cap);
+        const int L = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
+        if (L == 0) continue;
+        int b = ls_column(W, min(lane, L - 1));
+        float4 Bp = __ldg(mpos + b), Ba = __ldg(maux + b);
+        for (int t0 = 0; t0 < L; t0 += 32) {
+          const int bc = b;
+          const float4 Bpc = Bp, Bac = Ba;
+          const bool valid = t0 + lane < L;
+          if (t0 + 32 < L) { b = ls_column(W, min(t0 + 32 + lane, L - 1)); Bp = __ldg(mpos + b); Ba = __ldg(maux + b); }     // next step, ahead of use
+          int i = i0;
+          for (; i + 1 < i1; i += 2) {             // two rows in flight: independent prefilter chains
+            const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i], Ap1 = W.a_pos[i + 1], Aa1 = W.a_aux[i + 1];
+            const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
+            const bool pre1 = ls_prefilter(Ap1, Aa1, -2.0f * Aa1.w, Bpc, Bac) && valid;
+            ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
+            ls_push<DIRECT>(s, W, pre1, a0 + i + 1, bc, qn, sn, lane, lt, cap);
+          }
+          if (i < i1) {
+            const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i];
+            const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
+            ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
           }
         }
-        for (int t0 = 32 * LS_BC; t0 < L; t0 += 32) {
-          const int b = ls_column(W, min(t0 + lane, L - 1));
-          const bool pre = ls_prefilter(Apc, Aac, kinvA, __ldg(mpos + b), __ldg(maux + b)) && (t0 + lane < L);
-          ls_push<DIRECT>(s, W, pre, a, b, qn, sn, lane, lt, carry_row, carry_n, cap);
-        }
       }
+      i0 = i1;
     }
+    // end of the chunk: empty the queue, then the chunk's row counts are final
+    if (qn) { __syncwarp(); sn = ls_drain<DIRECT>(s, W, qn, sn, lane, lt); qn = 0; ls_flush_full<DIRECT>(s, W, sn, lane, cap); }
+    __syncwarp();
+    if (!DIRECT && lane < n_rows) s.ls_start[a0 + lane] = W.cnt[lane];
   }
-  if (qn) { sn = ls_drain<DIRECT>(s, W, qn, sn, lane, lt, carry_row, carry_n); __syncwarp(); }
-  if (sn >= 32) {
-    ls_flush<DIRECT>(s, W, 32, lane, cap);
-    __syncwarp();
-    LsRec tr{};
-    if (lane < sn - 32) tr = W.st[32 + lane];
-    __syncwarp();
-    if (lane < sn - 32) W.st[lane] = tr;
-    sn -= 32;
-    __syncwarp();
-  }
+  __syncwarp();
   if (sn) ls_flush<DIRECT>(s, W, sn, lane, cap);
 }
 
