@@ -102,7 +102,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   // zero region (contiguous over slots so one memset covers a batch)
   {
     Carver z{nullptr};
-    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(2 * M);
+    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(2 * M); z.take<int>(N_TK);
     L.zero_stride = z.off;
     L.zero_base = base ? base + cv.off : nullptr;
     for (int s = 0; s < n_slots; ++s) {
@@ -110,7 +110,8 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
       int* cnt = c2.take<int>(LST_N_CNT);
       int* ss = c2.take<int>(2 * M + 2);
       int* cur = c2.take<int>(2 * M);
-      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].cursor = cur; }
+      int* tk = c2.take<int>(N_TK);
+      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].cursor = cur; (*out)[s].tk = tk; }
     }
     cv.off += L.zero_stride * n_slots;
   }
@@ -137,7 +138,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
     t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_aux = cv.take<float4>(k.max_md); t.md_start = cv.take<int>(M + 8);
     t.ls_rec = cv.take<LsRec>(k.max_ls);
-    t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
+    t.ls_tab = cv.take<int>(16 * (size_t)M); t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
     t.chain_sensor = cv.take<unsigned long long>(2 * (size_t)M / SCAN_TILE + 4); t.chain_md = cv.take<unsigned long long>(M / SCAN_TILE + 4);
     t.chain_ls = cv.take<unsigned long long>(k.max_md / SCAN_TILE + 4); t.chain_t5s = cv.take<unsigned long long>(k.max_t5c / SCAN_TILE + 4);
     t.chain_t3 = cv.take<unsigned long long>(k.max_ls / TUPLE_TPB + 4); t.chain_t5 = cv.take<unsigned long long>(k.max_t3 / TUPLE_TPB + 4);
@@ -158,7 +159,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
-      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
+      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.tk = d.tk; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
       d = t;
     }
   }

@@ -32,6 +32,8 @@ struct Geo {   // device copies, shared by all slots
   const int* run_c1;        // [n_runs]
 };
 
+enum { TK_LS_SWEEP = 0, TK_LS_DIRECT, TK_MD_SWEEP, TK_MD_DIRECT, N_TK = 16 };
+
 struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
 
 // records of the MD / LS sweeps (lst_pairs.cuh): seq = rank of the object among the objects of its row
@@ -48,6 +50,7 @@ struct Slot {
   int* cnt;                 // [LST_N_CNT]
   int* sensor_start;        // [2M+1] histogram, then exclusive scan in place
   int* cursor;              // [2M]
+  int* tk;                  // [N_TK] internal work tickets
   // 0xFF-initialised per run
   unsigned long long* win5; // [max_pls]  (chi2 bits << 32 | T5 index)
   unsigned long long* win3; // [max_pls]
@@ -58,7 +61,7 @@ struct Slot {
   // a1
   MdRec* md_rec; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; float4* md_aux; int* md_start;
   // a2
-  LsRec* ls_rec; int* ls_start; int2* ls_ab; float* ls_c;
+  LsRec* ls_rec; int* ls_start; int2* ls_ab; float* ls_c; int* ls_tab;
   // look-back status words of the row scans (sensor counts, MDs per module, LSs per MD, T5 pass flags)
   unsigned long long *chain_sensor, *chain_md, *chain_ls, *chain_t5s;
   // a3

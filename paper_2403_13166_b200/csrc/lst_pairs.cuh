@@ -29,6 +29,7 @@ constexpr int PAIR_WARPS = 4;        // warps per block
 constexpr int Q_CAP = 64;            // survivor queue / record staging per warp (drained / flushed at >= 32)
 constexpr int RUN_CAP = 32;          // runs of a CSR row cached per warp at a time
 constexpr int LS_ROWS = 8;           // consecutive MD rows a warp takes at a time
+constexpr int LS_TAB = 8;            // non-empty runs per module held by the precomputed column table
 constexpr int MD_BIG = 1 << 20;      // modules with more cells than this are swept alone (64-bit sweep counter)
 
 __device__ __forceinline__ unsigned lanemask_lt() { unsigned m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
@@ -244,22 +245,85 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __rest
   md_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
 }
 
+__device__ __forceinline__ void ls_write_tables(const Slot& s, const Geo& geo);      // a2's per-module column tables (below)
+
 // a1 finish (md_start holds the exclusive scan of the per-module counts by now): record -> md_start[module] + seq.
 // If the stage overflowed its capacity the record buffer is incomplete: run the sweep again, writing in place.
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   pdl_begin();
   __shared__ MdWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) { md_sweep_body<true>(s, geo, caps, Wall); return; }
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_MD) { ls_write_tables(s, geo); md_sweep_body<true>(s, geo, caps, Wall); return; }
+  // One pass over max(records, modules): item j places record j and writes the LS column table of module j.  Both are
+  // chains of dependent loads; all loads of a level are issued together (loads first, stores last), so an item costs
+  // three memory round trips in all.
   const int n_rec = min(s.cnt[LST_CNT_FILL_MD], caps.max_md);
-  LST_FOR_ITEMS(j, n_rec) md_emit<false>(s, s.md_rec[j], caps.max_md);
+  const int M = geo.n_modules;
+  const int* __restrict__ mds = s.md_start;
+  LST_FOR_ITEMS(j, max(n_rec, M)) {
+    const bool has_r = j < n_rec, has_m = j < M;
+    // level 1
+    MdRec r{};
+    int e0 = 0, e1 = 0, m0 = 0, m1 = 0;
+    if (has_r) r = s.md_rec[j];
+    if (has_m) { e0 = __ldg(geo.run_ptr + j); e1 = __ldg(geo.run_ptr + j + 1); m0 = mds[j]; m1 = mds[j + 1]; }
+    const bool tab_on = has_m && m1 > m0;               // modules without rows are never looked up
+    // level 2
+    int pos = 0, o_lo = 0, o_up = 0;
+    float4 h = make_float4(0.f, 0.f, 0.f, 1.f);
+    if (has_r) { pos = mds[r.mtm >> 2] + r.seq; h = s.hit[r.p_lo]; o_lo = s.hit_orig[r.p_lo]; o_up = s.hit_orig[r.p_up]; }
+    int c0[LS_TAB], c1[LS_TAB], b0[LS_TAB], b1[LS_TAB];
+#pragma unroll
+    for (int q = 0; q < LS_TAB; ++q) { const bool in = tab_on && e0 + q < e1; c0[q] = in ? __ldg(geo.run_c0 + e0 + q) : 0; c1[q] = in ? __ldg(geo.run_c1 + e0 + q) : 0; }
+    // level 3
+#pragma unroll
+    for (int q = 0; q < LS_TAB; ++q) { b0[q] = mds[c0[q]]; b1[q] = mds[c1[q]]; }
+    // stores
+    if (has_r && pos < caps.max_md) {
+      const int mt = r.mtm & 3;
+      s.md_hits[pos] = make_int2(o_lo, o_up);
+      s.md_modt[pos] = r.mtm;
+      s.md_pos[pos] = h;
+      s.md_cw[pos] = make_float2(r.c, r.w);
+      const float fm_ = __int_as_float(__float_as_int(md_relf(mt) * 1.0001f) | mt);
+      s.md_aux[pos] = make_float4(r.c, fmaf(r.w, 1.0001f, 3.0e-7f), fm_, 1.0f / h.w);
+    }
+    if (tab_on) {
+      int ends[LS_TAB], dl[LS_TAB];
+      int k = 0, L = 0;
+#pragma unroll
+      for (int q = 0; q < LS_TAB; ++q) {
+        const int n = b1[q] - b0[q];
+        if (n > 0) {
+#pragma unroll
+          for (int t = 0; t < LS_TAB; ++t) if (t == k) { dl[t] = b0[q] - L; ends[t] = L + n; }
+          L += n; ++k;
+        }
+      }
+      for (int e = e0 + LS_TAB; e < e1; ++e) {             // more than LS_TAB runs in the CSR row (rare)
+        const int bb = mds[geo.run_c0[e]], n = mds[geo.run_c1[e]] - bb;
+        if (n > 0) {
+#pragma unroll
+          for (int t = 0; t < LS_TAB; ++t) if (t == k) { dl[t] = bb - L; ends[t] = L + n; }
+          L += n; ++k;
+        }
+      }
+#pragma unroll
+      for (int t = 0; t < LS_TAB; ++t) if (t >= k) { ends[t] = L; dl[t] = 0; }
+      if (k > LS_TAB) ends[LS_TAB - 1] = -1;
+      int4* tab = reinterpret_cast<int4*>(s.ls_tab + 2 * LS_TAB * (size_t)j);
+      static_assert(LS_TAB == 8, "table layout");
+      tab[0] = make_int4(ends[0], ends[1], ends[2], ends[3]); tab[1] = make_int4(ends[4], ends[5], ends[6], ends[7]);
+      tab[2] = make_int4(dl[0], dl[1], dl[2], dl[3]); tab[3] = make_int4(dl[4], dl[5], dl[6], dl[7]);
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
 // a2: row = MD a of module m; columns = the MDs of the runs of CSR row m, ascending
 // ------------------------------------------------------------------------------------------------
 struct LsWarp {
-  int r_off[RUN_CAP + 1], r_b0[RUN_CAP];      // non-empty runs of the current module: first column, first MD
+  int r_off[RUN_CAP + 1], r_b0[RUN_CAP];      // non-empty runs of the current module: first column, (first MD) - (first column)
   float4 a_pos[LS_ROWS], a_aux[LS_ROWS];      // the rows of the current chunk: anchor, prefilter record
   int cnt[LS_ROWS];                           // LSs found so far in each row of the chunk
   int q_a[Q_CAP], q_b[Q_CAP];
@@ -341,17 +405,57 @@ __device__ __forceinline__ int ls_load_runs(const Geo& geo, const int* __restric
   __syncwarp();
   W.r_off[lane + 1] = total;                    // padding for the search
   __syncwarp();
-  if (n > 0) { const int i = __popc(nz & lt); W.r_off[i] = inc - n; W.r_b0[i] = b0; }
+  if (n > 0) { const int i = __popc(nz & lt); W.r_off[i] = inc - n; W.r_b0[i] = b0 - (inc - n); }
   __syncwarp();
   return total;
 }
-// column t of the run table -> MD index
+// the same from the per-module column table written by k_md_finish (modules with at most LS_TAB non-empty runs)
+__device__ __forceinline__ void ls_table_runs(const int* __restrict__ tab, LsWarp& W, int lane) {
+  __syncwarp();
+  if (lane < 2 * LS_TAB) {
+    const int v = __ldg(tab + lane);
+    if (lane < LS_TAB) W.r_off[lane + 1] = v; else W.r_b0[lane - LS_TAB] = v;
+  }
+  if (lane == 0) W.r_off[0] = 0;
+  __syncwarp();
+}
+// column t of the run table -> MD index; SMALL: at most LS_TAB runs
+template <bool SMALL>
 __device__ __forceinline__ int ls_column(const LsWarp& W, int t) {
   int r = 0;
 #pragma unroll
-  for (int step = RUN_CAP / 2; step > 0; step >>= 1)
+  for (int step = (SMALL ? LS_TAB : RUN_CAP) / 2; step > 0; step >>= 1)
     if (W.r_off[r + step] <= t) r += step;
-  return W.r_b0[r] + (t - W.r_off[r]);
+  return W.r_b0[r] + t;
+}
+
+// per-module column table for the LS sweep: [0, LS_TAB) = last column + 1 of each non-empty run (padded with the module's
+// column count L, so entry LS_TAB - 1 is L), [LS_TAB, 2 LS_TAB) = (first MD) - (first column) of each run.  More than LS_TAB
+// non-empty runs: entry LS_TAB - 1 = -1 and the sweep builds its run table itself.
+__device__ __forceinline__ void ls_write_tables(const Slot& s, const Geo& geo) {
+  const int* __restrict__ mds = s.md_start;
+  LST_FOR_ITEMS(m, geo.n_modules) {
+    int* tab = s.ls_tab + 2 * LS_TAB * (size_t)m;
+    if (mds[m] == mds[m + 1]) continue;                 // no rows: never read
+    int k = 0, L = 0;
+    for (int e = geo.run_ptr[m], e1 = geo.run_ptr[m + 1]; e < e1; e += 8) {      // 8 runs at a time: their loads are independent
+      int c0[8], c1[8], b0[8], b1[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { const bool in = e + j < e1; c0[j] = in ? __ldg(geo.run_c0 + e + j) : 0; c1[j] = in ? __ldg(geo.run_c1 + e + j) : 0; }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { b0[j] = mds[c0[j]]; b1[j] = mds[c1[j]]; }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int n = b1[j] - b0[j];
+        if (n > 0) {
+          if (k < LS_TAB) { tab[LS_TAB + k] = b0[j] - L; tab[k] = L + n; }
+          L += n; ++k;
+        }
+      }
+    }
+    for (int j = k; j < LS_TAB; ++j) { tab[j] = L; tab[LS_TAB + j] = 0; }
+    if (k > LS_TAB) tab[LS_TAB - 1] = -1;
+  }
 }
 
 template <bool DIRECT>
@@ -379,6 +483,40 @@ __device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int 
 // into registers (next step's loads already in flight) and tested against each row of the segment, whose anchors sit in
 // shared memory (broadcast reads).  The survivor queue is emptied at the end of every chunk, so the per-row LS counts live in
 // shared memory for the duration of a chunk and the row table is written once, coalesced.
+template <bool SMALL, bool DIRECT>
+__device__ __forceinline__ void ls_sweep_columns(const Slot& s, LsWarp& W, int L, int a0, int i0, int i1, int& qn, int& sn, int lane, unsigned lt, int cap) {
+  const float4* __restrict__ mpos = s.md_pos;
+  const float4* __restrict__ maux = s.md_aux;
+  int b = ls_column<SMALL>(W, min(lane, L - 1));
+  float4 Bp = __ldg(mpos + b), Ba = __ldg(maux + b);
+  for (int t0 = 0; t0 < L; t0 += 32) {
+    const int bc = b;
+    const float4 Bpc = Bp, Bac = Ba;
+    const bool valid = t0 + lane < L;
+    if (t0 + 32 < L) { b = ls_column<SMALL>(W, min(t0 + 32 + lane, L - 1)); Bp = __ldg(mpos + b); Ba = __ldg(maux + b); }     // next step, ahead of use
+    int i = i0;
+    for (; i + 1 < i1; i += 2) {             // two rows in flight: independent prefilter chains
+      const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i], Ap1 = W.a_pos[i + 1], Aa1 = W.a_aux[i + 1];
+      const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
+      const bool pre1 = ls_prefilter(Ap1, Aa1, -2.0f * Aa1.w, Bpc, Bac) && valid;
+      ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
+      ls_push<DIRECT>(s, W, pre1, a0 + i + 1, bc, qn, sn, lane, lt, cap);
+    }
+    if (i < i1) {
+      const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i];
+      const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
+      ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
+    }
+  }
+}
+
+// A warp takes LS_ROWS consecutive MDs (rows) at a time, handed out by an atomic ticket (the next ticket is fetched while the
+// current chunk is swept).  Rows of the same module share their columns, so the chunk is cut into module segments and every
+// segment is swept columns-outer / rows-inner: the 32 column MDs of a step are loaded once into registers (next step's loads
+// already in flight) and tested against each row of the segment, whose anchors sit in shared memory (broadcast reads).  The
+// survivor queue is emptied at the end of every chunk, so the per-row LS counts live in shared memory for the duration of a
+// chunk and the row table is written once, coalesced.  Which warp sweeps which chunk does not matter: a record carries its
+// row and its rank in the row.
 template <bool DIRECT>
 __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, const Caps& caps, LsWarp* Wall) {
   const int lane = threadIdx.x & 31;
@@ -389,9 +527,14 @@ __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, con
   const float4* __restrict__ maux = s.md_aux;
   const int n_md = s.cnt[LST_CNT_MD];
   const int cap = caps.max_ls;
-  const int n_warps = gridDim.x * PAIR_WARPS;
+  int* ticket = s.tk + (DIRECT ? TK_LS_DIRECT : TK_LS_SWEEP);
   int qn = 0, sn = 0;
-  for (int a0 = (blockIdx.x * PAIR_WARPS + (threadIdx.x >> 5)) * LS_ROWS; a0 < n_md; a0 += n_warps * LS_ROWS) {
+  int next = 0;
+  if (lane == 0) next = atomicAdd(ticket, 1);
+  while (true) {
+    const int a0 = __shfl_sync(0xffffffffu, next, 0) * LS_ROWS;
+    if (a0 >= n_md) break;
+    if (lane == 0) next = atomicAdd(ticket, 1);
     const int n_rows = min(LS_ROWS, n_md - a0);
     int my_m = -1;
     __syncwarp();
@@ -404,30 +547,16 @@ __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, con
     for (int i0 = 0; i0 < n_rows;) {
       const int m = __shfl_sync(0xffffffffu, my_m, i0);
       const int i1 = i0 + __popc(__ballot_sync(0xffffffffu, my_m == m));      // MDs are stored in module order: rows [i0, i1) are module m's
-      const int e0 = geo.run_ptr[m], e1 = geo.run_ptr[m + 1];
-      for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
-        const int L = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
-        if (L == 0) continue;
-        int b = ls_column(W, min(lane, L - 1));
-        float4 Bp = __ldg(mpos + b), Ba = __ldg(maux + b);
-        for (int t0 = 0; t0 < L; t0 += 32) {
-          const int bc = b;
-          const float4 Bpc = Bp, Bac = Ba;
-          const bool valid = t0 + lane < L;
-          if (t0 + 32 < L) { b = ls_column(W, min(t0 + 32 + lane, L - 1)); Bp = __ldg(mpos + b); Ba = __ldg(maux + b); }     // next step, ahead of use
-          int i = i0;
-          for (; i + 1 < i1; i += 2) {             // two rows in flight: independent prefilter chains
-            const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i], Ap1 = W.a_pos[i + 1], Aa1 = W.a_aux[i + 1];
-            const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
-            const bool pre1 = ls_prefilter(Ap1, Aa1, -2.0f * Aa1.w, Bpc, Bac) && valid;
-            ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
-            ls_push<DIRECT>(s, W, pre1, a0 + i + 1, bc, qn, sn, lane, lt, cap);
-          }
-          if (i < i1) {
-            const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i];
-            const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
-            ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
-          }
+      const int* tab = s.ls_tab + 2 * LS_TAB * (size_t)m;
+      const int L = __ldg(tab + LS_TAB - 1);
+      if (L > 0) {
+        ls_table_runs(tab, W, lane);
+        ls_sweep_columns<true, DIRECT>(s, W, L, a0, i0, i1, qn, sn, lane, lt, cap);
+      } else if (L < 0) {                                          // more than LS_TAB non-empty runs
+        const int e0 = geo.run_ptr[m], e1 = geo.run_ptr[m + 1];
+        for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
+          const int L2 = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
+          if (L2 > 0) ls_sweep_columns<false, DIRECT>(s, W, L2, a0, i0, i1, qn, sn, lane, lt, cap);
         }
       }
       i0 = i1;
