@@ -29,6 +29,9 @@ struct lst_ctx {
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
+#ifndef LS_GRID_PER_SM
+#define LS_GRID_PER_SM 7
+#endif
 namespace {
 
 constexpr size_t ALIGN = 256;
@@ -356,7 +359,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   launch(pdl, k_md_sweep, GL, BP, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_scan_lb<SCAN_MDROW>, GS, BS, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_md_finish, GL, BP, 0, st, sl, g, k); LST_MARK();
-  launch(pdl, k_ls_sweep, GL, BP, 0, st, sl, g, k); LST_MARK();
+  launch(pdl, k_ls_sweep, dim3(n < 8 ? 148 * 4 : 148 * LS_GRID_PER_SM, (n + 31) / 32), BP, 0, st, sl, (int)n, g, k); LST_MARK();      // persistent grid: the resident blocks
   launch(pdl, k_scan_lb<SCAN_LSROW>, GS, BS, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_ls_finish, GL, BP, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_t3_one, GL, BT, 0, st, sl, k); LST_MARK();

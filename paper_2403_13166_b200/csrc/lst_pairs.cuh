@@ -324,7 +324,8 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
 // ------------------------------------------------------------------------------------------------
 struct LsWarp {
   int r_off[RUN_CAP + 1], r_b0[RUN_CAP];      // non-empty runs of the current module: first column, (first MD) - (first column)
-  float4 a_pos[LS_ROWS], a_aux[LS_ROWS];      // the rows of the current chunk: anchor, prefilter record
+  float4 a_pos[LS_ROWS], a_aux[LS_ROWS];      // the rows of the current chunk: anchor, prefilter record (.w = -2 / r)
+  __align__(16) int tab[LS_ROWS][2 * LS_TAB]; // ... and the column table of each row's module
   int cnt[LS_ROWS];                           // LSs found so far in each row of the chunk
   int q_a[Q_CAP], q_b[Q_CAP];
   LsRec st[Q_CAP];
@@ -409,22 +410,11 @@ __device__ __forceinline__ int ls_load_runs(const Geo& geo, const int* __restric
   __syncwarp();
   return total;
 }
-// the same from the per-module column table written by k_md_finish (modules with at most LS_TAB non-empty runs)
-__device__ __forceinline__ void ls_table_runs(const int* __restrict__ tab, LsWarp& W, int lane) {
-  __syncwarp();
-  if (lane < 2 * LS_TAB) {
-    const int v = __ldg(tab + lane);
-    if (lane < LS_TAB) W.r_off[lane + 1] = v; else W.r_b0[lane - LS_TAB] = v;
-  }
-  if (lane == 0) W.r_off[0] = 0;
-  __syncwarp();
-}
-// column t of the run table -> MD index; SMALL: at most LS_TAB runs
-template <bool SMALL>
+// column t of the run table -> MD index
 __device__ __forceinline__ int ls_column(const LsWarp& W, int t) {
   int r = 0;
 #pragma unroll
-  for (int step = (SMALL ? LS_TAB : RUN_CAP) / 2; step > 0; step >>= 1)
+  for (int step = RUN_CAP / 2; step > 0; step >>= 1)
     if (W.r_off[r + step] <= t) r += step;
   return W.r_b0[r] + t;
 }
@@ -483,83 +473,133 @@ __device__ __forceinline__ void ls_push(const Slot& s, LsWarp& W, bool pre, int 
 // into registers (next step's loads already in flight) and tested against each row of the segment, whose anchors sit in
 // shared memory (broadcast reads).  The survivor queue is emptied at the end of every chunk, so the per-row LS counts live in
 // shared memory for the duration of a chunk and the row table is written once, coalesced.
-template <bool SMALL, bool DIRECT>
-__device__ __forceinline__ void ls_sweep_columns(const Slot& s, LsWarp& W, int L, int a0, int i0, int i1, int& qn, int& sn, int lane, unsigned lt, int cap) {
-  const float4* __restrict__ mpos = s.md_pos;
-  const float4* __restrict__ maux = s.md_aux;
-  int b = ls_column<SMALL>(W, min(lane, L - 1));
-  float4 Bp = __ldg(mpos + b), Ba = __ldg(maux + b);
-  for (int t0 = 0; t0 < L; t0 += 32) {
-    const int bc = b;
-    const float4 Bpc = Bp, Bac = Ba;
-    const bool valid = t0 + lane < L;
-    if (t0 + 32 < L) { b = ls_column<SMALL>(W, min(t0 + 32 + lane, L - 1)); Bp = __ldg(mpos + b); Ba = __ldg(maux + b); }     // next step, ahead of use
-    int i = i0;
-    for (; i + 1 < i1; i += 2) {             // two rows in flight: independent prefilter chains
-      const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i], Ap1 = W.a_pos[i + 1], Aa1 = W.a_aux[i + 1];
-      const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
-      const bool pre1 = ls_prefilter(Ap1, Aa1, -2.0f * Aa1.w, Bpc, Bac) && valid;
-      ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
-      ls_push<DIRECT>(s, W, pre1, a0 + i + 1, bc, qn, sn, lane, lt, cap);
-    }
-    if (i < i1) {
-      const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i];
-      const bool pre0 = ls_prefilter(Ap0, Aa0, -2.0f * Aa0.w, Bpc, Bac) && valid;
-      ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
-    }
+// one step: the 32 column MDs (bc, Bpc, Bac) against rows [i0, i1) of the chunk
+template <bool DIRECT>
+__device__ __forceinline__ void ls_rows(const Slot& s, LsWarp& W, int a0, int i0, int i1, bool valid, int bc, float4 Bpc, float4 Bac, int& qn, int& sn,
+                                        int lane, unsigned lt, int cap) {
+  int i = i0;
+  for (; i + 1 < i1; i += 2) {             // two rows in flight: independent prefilter chains
+    const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i], Ap1 = W.a_pos[i + 1], Aa1 = W.a_aux[i + 1];
+    const bool pre0 = ls_prefilter(Ap0, Aa0, Aa0.w, Bpc, Bac) && valid;
+    const bool pre1 = ls_prefilter(Ap1, Aa1, Aa1.w, Bpc, Bac) && valid;
+    ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
+    ls_push<DIRECT>(s, W, pre1, a0 + i + 1, bc, qn, sn, lane, lt, cap);
+  }
+  if (i < i1) {
+    const float4 Ap0 = W.a_pos[i], Aa0 = W.a_aux[i];
+    const bool pre0 = ls_prefilter(Ap0, Aa0, Aa0.w, Bpc, Bac) && valid;
+    ls_push<DIRECT>(s, W, pre0, a0 + i, bc, qn, sn, lane, lt, cap);
   }
 }
 
-// A warp takes LS_ROWS consecutive MDs (rows) at a time, handed out by an atomic ticket (the next ticket is fetched while the
-// current chunk is swept).  Rows of the same module share their columns, so the chunk is cut into module segments and every
-// segment is swept columns-outer / rows-inner: the 32 column MDs of a step are loaded once into registers (next step's loads
-// already in flight) and tested against each row of the segment, whose anchors sit in shared memory (broadcast reads).  The
-// survivor queue is emptied at the end of every chunk, so the per-row LS counts live in shared memory for the duration of a
-// chunk and the row table is written once, coalesced.  Which warp sweeps which chunk does not matter: a record carries its
-// row and its rank in the row.
+// slow path (module with more than LS_TAB non-empty runs): run table built here, one column step after the other
 template <bool DIRECT>
-__device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, const Caps& caps, LsWarp* Wall) {
+__device__ __forceinline__ void ls_sweep_columns(const Slot& s, LsWarp& W, int L, int a0, int i0, int i1, int& qn, int& sn, int lane, unsigned lt, int cap) {
+  for (int t0 = 0; t0 < L; t0 += 32) {
+    const int b = ls_column(W, min(t0 + lane, L - 1));
+    ls_rows<DIRECT>(s, W, a0, i0, i1, t0 + lane < L, b, __ldg(s.md_pos + b), __ldg(s.md_aux + b), qn, sn, lane, lt, cap);
+  }
+}
+
+// column t of a module's column table (k_md_finish) -> MD index
+__device__ __forceinline__ int ls_tab_column(const int* tab, int t) {
+  int r = (tab[3] <= t) ? 4 : 0;
+  if (tab[r + 1] <= t) r += 2;
+  if (tab[r] <= t) r += 1;                    // r = number of runs that end at or before t (entry LS_TAB - 1 = L > t)
+  return t + tab[LS_TAB + r];
+}
+
+// The chunks (LS_ROWS consecutive MDs = rows) of ALL the events of a launch are handed out by one atomic ticket (kept in the
+// first slot; the next ticket is fetched while the current chunk is swept), so every warp of the persistent grid works until
+// the whole launch is done.  Rows of the same module share their columns, so a chunk is cut into module segments and every
+// segment is swept columns-outer / rows-inner: the 32 column MDs of a step are loaded once into registers and tested against
+// each row of the segment, whose anchors sit in shared memory (broadcast reads).  The (segment, step) pairs of a chunk form
+// one sequence and the column loads of the next pair -- possibly of the next segment -- are in flight while the current one
+// is tested; the column tables of all the chunk's modules are fetched together at the start of the chunk, so a chunk costs
+// three dependent memory round trips (rows, tables, first columns) however many modules it spans.  The survivor queue is
+// emptied at the end of every chunk, so the per-row LS counts live in shared memory for the duration of a chunk and the
+// row table is written once, coalesced.  Which warp sweeps which chunk does not matter: a record carries its row and its
+// rank in the row.
+template <bool DIRECT>
+__device__ __forceinline__ void ls_sweep_body(const Slot* __restrict__ slots, int n_ev, const Geo& geo, const Caps& caps, LsWarp* Wall) {
   const int lane = threadIdx.x & 31;
   LsWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
-  const int* __restrict__ mds = s.md_start;
-  const float4* __restrict__ mpos = s.md_pos;
-  const float4* __restrict__ maux = s.md_aux;
-  const int n_md = s.cnt[LST_CNT_MD];
   const int cap = caps.max_ls;
-  int* ticket = s.tk + (DIRECT ? TK_LS_DIRECT : TK_LS_SWEEP);
+  // chunks of events [0, lane] (inclusive scan over the events of the launch; at most 32 events per ticket)
+  int cum = 0;
+  if (lane < n_ev) cum = (slots[lane].cnt[LST_CNT_MD] + LS_ROWS - 1) / LS_ROWS;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, cum, d); if (lane >= d) cum += t; }
+  int* ticket = slots[0].tk + (DIRECT ? TK_LS_DIRECT : TK_LS_SWEEP);
   int qn = 0, sn = 0;
   int next = 0;
   if (lane == 0) next = atomicAdd(ticket, 1);
+  int ev_prev = -1;
   while (true) {
-    const int a0 = __shfl_sync(0xffffffffu, next, 0) * LS_ROWS;
-    if (a0 >= n_md) break;
+    const int T = __shfl_sync(0xffffffffu, next, 0);
+    const int ev = __popc(__ballot_sync(0xffffffffu, lane < n_ev && cum <= T));
+    if (ev >= n_ev) break;
     if (lane == 0) next = atomicAdd(ticket, 1);
-    const int n_rows = min(LS_ROWS, n_md - a0);
+    const int first = __shfl_sync(0xffffffffu, cum, max(ev - 1, 0));
+    const int a0 = (T - (ev ? first : 0)) * LS_ROWS;
+    if (ev != ev_prev && sn) { __syncwarp(); ls_flush<DIRECT>(slots[ev_prev], W, sn, lane, cap); sn = 0; __syncwarp(); }      // records go to their own event
+    ev_prev = ev;
+    const Slot& s = slots[ev];
+    const float4* __restrict__ mpos = s.md_pos;
+    const float4* __restrict__ maux = s.md_aux;
+    const int n_rows = min(LS_ROWS, s.cnt[LST_CNT_MD] - a0);
     int my_m = -1;
     __syncwarp();
     if (lane < n_rows) {
-      W.a_pos[lane] = __ldg(mpos + a0 + lane); W.a_aux[lane] = __ldg(maux + a0 + lane);
+      const float4 aux = __ldg(maux + a0 + lane);
+      W.a_pos[lane] = __ldg(mpos + a0 + lane); W.a_aux[lane] = make_float4(aux.x, aux.y, aux.z, -2.0f * aux.w);      // .w = -2 / r
       my_m = s.md_modt[a0 + lane] >> 2;
     }
     if (lane < LS_ROWS) W.cnt[lane] = 0;
+    {
+      static_assert(LS_ROWS * 4 <= 32 && LS_TAB == 8, "one int4 of the tables per lane");
+      const int row = lane >> 2, m_r = __shfl_sync(0xffffffffu, my_m, row);
+      if (m_r >= 0) reinterpret_cast<int4*>(W.tab[row])[lane & 3] = __ldg(reinterpret_cast<const int4*>(s.ls_tab + 2 * LS_TAB * (size_t)m_r) + (lane & 3));
+    }
+    const int prev_m = __shfl_up_sync(0xffffffffu, my_m, 1);
+    const unsigned segs = __ballot_sync(0xffffffffu, lane < n_rows && (lane == 0 || my_m != prev_m));    // first rows of the module segments
     __syncwarp();
-    for (int i0 = 0; i0 < n_rows;) {
-      const int m = __shfl_sync(0xffffffffu, my_m, i0);
-      const int i1 = i0 + __popc(__ballot_sync(0xffffffffu, my_m == m));      // MDs are stored in module order: rows [i0, i1) are module m's
-      const int* tab = s.ls_tab + 2 * LS_TAB * (size_t)m;
-      const int L = __ldg(tab + LS_TAB - 1);
-      if (L > 0) {
-        ls_table_runs(tab, W, lane);
-        ls_sweep_columns<true, DIRECT>(s, W, L, a0, i0, i1, qn, sn, lane, lt, cap);
-      } else if (L < 0) {                                          // more than LS_TAB non-empty runs
-        const int e0 = geo.run_ptr[m], e1 = geo.run_ptr[m + 1];
-        for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
-          const int L2 = ls_load_runs(geo, mds, W, eb, min(eb + RUN_CAP, e1), lane, lt);
-          if (L2 > 0) ls_sweep_columns<false, DIRECT>(s, W, L2, a0, i0, i1, qn, sn, lane, lt, cap);
-        }
+    unsigned todo = segs, slow = 0;
+    int ni0 = 0, ni1 = 0, nL = 0, nt0 = 0;
+    auto pop = [&]() -> bool {                // next segment with columns; segments that need the slow path are set aside
+      while (todo) {
+        ni0 = __ffs(todo) - 1; todo &= todo - 1;
+        ni1 = todo ? __ffs(todo) - 1 : n_rows;
+        nL = W.tab[ni0][LS_TAB - 1];
+        if (nL > 0) return true;
+        if (nL < 0) slow |= 1u << ni0;
       }
-      i0 = i1;
+      return false;
+    };
+    bool have = pop();
+    int b = 0;
+    float4 Bp = make_float4(0.f, 0.f, 0.f, 1.f), Ba = Bp;
+    if (have) { b = ls_tab_column(W.tab[ni0], min(lane, nL - 1)); Bp = __ldg(mpos + b); Ba = __ldg(maux + b); }
+    while (have) {
+      const int i0 = ni0, i1 = ni1, bc = b;
+      const float4 Bpc = Bp, Bac = Ba;
+      const bool valid = nt0 + lane < nL;
+      if (nt0 + 32 < nL) nt0 += 32; else { have = pop(); nt0 = 0; }
+      if (have) { b = ls_tab_column(W.tab[ni0], min(nt0 + lane, nL - 1)); Bp = __ldg(mpos + b); Ba = __ldg(maux + b); }      // next pair, ahead of use
+      ls_rows<DIRECT>(s, W, a0, i0, i1, valid, bc, Bpc, Bac, qn, sn, lane, lt, cap);
+    }
+    while (slow) {                            // modules with more than LS_TAB non-empty runs
+      const int i0 = __ffs(slow) - 1;
+      slow &= slow - 1;
+      const unsigned rest = segs & ~((2u << i0) - 1u);
+      const int i1 = rest ? __ffs(rest) - 1 : n_rows;
+      const int m = __shfl_sync(0xffffffffu, my_m, i0);
+      const int e0 = geo.run_ptr[m], e1 = geo.run_ptr[m + 1];
+      for (int eb = e0; eb < e1; eb += RUN_CAP) {                // one pass unless the CSR row has more than RUN_CAP runs
+        const int L2 = ls_load_runs(geo, s.md_start, W, eb, min(eb + RUN_CAP, e1), lane, lt);
+        if (L2 > 0) ls_sweep_columns<DIRECT>(s, W, L2, a0, i0, i1, qn, sn, lane, lt, cap);
+      }
     }
     // end of the chunk: empty the queue, then the chunk's row counts are final
     if (qn) { __syncwarp(); sn = ls_drain<DIRECT>(s, W, qn, sn, lane, lt); qn = 0; ls_flush_full<DIRECT>(s, W, sn, lane, cap); }
@@ -567,13 +607,17 @@ __device__ __forceinline__ void ls_sweep_body(const Slot& s, const Geo& geo, con
     if (!DIRECT && lane < n_rows) s.ls_start[a0 + lane] = W.cnt[lane];
   }
   __syncwarp();
-  if (sn) ls_flush<DIRECT>(s, W, sn, lane, cap);
+  if (sn) ls_flush<DIRECT>(slots[ev_prev], W, sn, lane, cap);
 }
 
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+// grid (persistent blocks, groups of up to 32 events)
+#ifndef LS_MIN_BLOCKS
+#define LS_MIN_BLOCKS 7            // 72 registers: 28 warps per SM measured best (64 / 56 registers spill, 84 leave 20 warps)
+#endif
+__global__ void __launch_bounds__(PAIR_WARPS * 32, LS_MIN_BLOCKS) k_ls_sweep(const Slot* __restrict__ slots, int n_ev, Geo geo, Caps caps) {
   pdl_begin();
   __shared__ LsWarp Wall[PAIR_WARPS];
-  ls_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
+  ls_sweep_body<false>(slots + 32 * blockIdx.y, min(32, n_ev - 32 * (int)blockIdx.y), geo, caps, Wall);
 }
 
 // a2 finish (ls_start holds the exclusive scan of the per-row counts by now): record -> ls_start[a] + seq; on capacity
@@ -582,7 +626,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_finish(const Slot* __res
   pdl_begin();
   __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) { ls_sweep_body<true>(s, geo, caps, Wall); return; }
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) { ls_sweep_body<true>(slots + blockIdx.y, 1, geo, caps, Wall); return; }
   const int n_rec = min(s.cnt[LST_CNT_FILL_LS], caps.max_ls);
   LST_FOR_ITEMS(j, n_rec) {
     const LsRec r = s.ls_rec[j];
