@@ -22,6 +22,7 @@ struct lst_ctx {
   char* ones_base = nullptr; size_t ones_stride = 0;
   bool sticky_cuda_error = false;
   bool capturing = false;         // run_sequence is being recorded into a graph
+  bool use_xs = true;             // a6 with per-surface crossing keys when the geometry carries layers (LST_XS=0: the generic (h, zeta, psi) buckets)
   bool use_pdl = false;           // programmatic dependent launch between the kernels of the chain (LST_PDL=1 enables; measured: no gain under graph replay)
   bool use_graphs = true;         // replay lst_run_batch as a CUDA graph on capturable streams (LST_GRAPHS=0 disables)
   std::map<long long, cudaGraphExec_t> graphs;   // (first_slot, n) -> instantiated launch sequence
@@ -105,7 +106,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   // zero region (contiguous over slots so one memset covers a batch)
   {
     Carver z{nullptr};
-    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(2 * M); z.take<int>(N_TK);
+    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(2 * M); z.take<int>(N_TK); z.take<unsigned>(XS_NS); z.take<unsigned>(XS_NS);
     L.zero_stride = z.off;
     L.zero_base = base ? base + cv.off : nullptr;
     for (int s = 0; s < n_slots; ++s) {
@@ -114,14 +115,16 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
       int* ss = c2.take<int>(2 * M + 2);
       int* cur = c2.take<int>(2 * M);
       int* tk = c2.take<int>(N_TK);
-      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].cursor = cur; (*out)[s].tk = tk; }
+      unsigned* shi = c2.take<unsigned>(XS_NS);
+      unsigned* srh = c2.take<unsigned>(XS_NS);
+      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].cursor = cur; (*out)[s].tk = tk; (*out)[s].surf_hi = shi; (*out)[s].surf_rhi = srh; }
     }
     cv.off += L.zero_stride * n_slots;
   }
   // 0xFF region
   {
     Carver z{nullptr};
-    z.take<unsigned long long>(k.max_pls); z.take<unsigned long long>(k.max_pls); z.take<int>(k.max_md); z.take<int>(k.max_hits);
+    z.take<unsigned long long>(k.max_pls); z.take<unsigned long long>(k.max_pls); z.take<int>(k.max_md); z.take<int>(k.max_hits); z.take<unsigned>(XS_NS);
     L.ones_stride = z.off;
     L.ones_base = base ? base + cv.off : nullptr;
     for (int s = 0; s < n_slots; ++s) {
@@ -130,7 +133,8 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
       auto* w3 = c2.take<unsigned long long>(k.max_pls);
       int* head = c2.take<int>(k.max_md);
       int* hhead = c2.take<int>(k.max_hits);
-      if (out) { (*out)[s].win5 = w5; (*out)[s].win3 = w3; (*out)[s].md_head = head; (*out)[s].hit_head = hhead; }
+      unsigned* slo = c2.take<unsigned>(XS_NS);
+      if (out) { (*out)[s].win5 = w5; (*out)[s].win3 = w3; (*out)[s].md_head = head; (*out)[s].hit_head = hhead; (*out)[s].surf_lo = slo; }
     }
     cv.off += L.ones_stride * n_slots;
   }
@@ -153,7 +157,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.t5_list = cv.take<int>(k.max_t5);
     t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.pls_key = cv.take<int>(k.max_pls);
     t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls); t.pls_pos = cv.take<int>(k.max_pls); t.pls_taken = cv.take<int>(k.max_pls);
-    t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.best5 = cv.take<int>(k.max_t5);
+    t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.xs_start = cv.take<int>((size_t)XS_NS * (XS_BINS + 1)); t.xs_ent = cv.take<float4>((size_t)XS_NS * 2 * k.max_pls); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
     t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc);
@@ -162,7 +166,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
-      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.tk = d.tk; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
+      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.tk = d.tk; t.surf_hi = d.surf_hi; t.surf_rhi = d.surf_rhi; t.surf_lo = d.surf_lo; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
       d = t;
     }
   }
@@ -270,6 +274,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
   if (cudaFuncSetAttribute(k_pls_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, PLS_BIN_SMEM) != cudaSuccess) { delete c; return LST_ECUDA; }
   if (const char* g = std::getenv("LST_GRAPHS")) c->use_graphs = !(g[0] == '0');
   if (const char* g = std::getenv("LST_PDL")) c->use_pdl = !(g[0] == '0');
+  if (const char* g = std::getenv("LST_XS")) c->use_xs = !(g[0] == '0');
   if (c->use_graphs) {            // host-side objects only; without them the binning simply stays in line
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess) c->side = nullptr;
     if (c->side && (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -278,7 +283,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     }
     (void)cudaGetLastError();
   }
-  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
+  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.has_layer = geo->layer ? 1 : 0; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
   c->geo.run_ptr = L.run_ptr; c->geo.run_c0 = L.run_c0; c->geo.run_c1 = L.run_c1;
   *out = c;
   return LST_OK;
@@ -342,8 +347,11 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   const dim3 G(gx, n), G1(1, n), GL(2 * gx, n);   // GL: the 128-thread link kernels
   const dim3 GS(gx < 16 ? gx : 16, n);            // look-back scans: tiles of 2048 entries by ticket
   // the pLS binning depends on the inputs only: under stream capture it becomes a side branch of the graph
+  // (with a layer per module the binning uses the surfaces measured by k_md_finish: the branch forks after that kernel)
   const bool fork = c->capturing && c->side;
-  if (fork) {
+  const bool xs = g.has_layer && c->use_xs;
+  const dim3 GX(XS_NS, n);
+  if (fork && !xs) {
     if (bad(c, cudaEventRecord(c->ev_fork, st)) || bad(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0))) return LST_ECUDA;
     k_pls_bin<<<G1, 1024, PLS_BIN_SMEM, c->side>>>(sl);
     if (bad(c, cudaEventRecord(c->ev_join, c->side))) return LST_ECUDA;
@@ -359,6 +367,11 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   launch(pdl, k_md_sweep, GL, BP, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_scan_lb<SCAN_MDROW>, GS, BS, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_md_finish, GL, BP, 0, st, sl, g, k); LST_MARK();
+  if (fork && xs) {
+    if (bad(c, cudaEventRecord(c->ev_fork, st)) || bad(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0))) return LST_ECUDA;
+    k_pls_cross<<<GX, XS_TPB, XS_SMEM, c->side>>>(sl, k.max_pls);
+    if (bad(c, cudaEventRecord(c->ev_join, c->side))) return LST_ECUDA;
+  }
   launch(pdl, k_ls_sweep, dim3(n < 8 ? 148 * 4 : 148 * LS_GRID_PER_SM, (n + 31) / 32), BP, 0, st, sl, (int)n, g, k); LST_MARK();      // persistent grid: the resident blocks
   launch(pdl, k_scan_lb<SCAN_LSROW>, GS, BS, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_ls_finish, GL, BP, 0, st, sl, g, k); LST_MARK();
@@ -374,11 +387,14 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   LST_MARK();
   launch(pdl, k_scan_lb<SCAN_T5>, GS, BS, 0, st, sl, g, k); LST_MARK();
   if (fork) { if (bad(c, cudaStreamWaitEvent(st, c->ev_join, 0))) return LST_ECUDA; }
+  else if (xs) launch(false, k_pls_cross, GX, dim3(XS_TPB), XS_SMEM, st, sl, k.max_pls);
   else launch(false, k_pls_bin, G1, dim3(1024), PLS_BIN_SMEM, st, sl);
   LST_MARK();
-  launch(pdl && !fork, k_match<5, false>, G, BM, 0, st, sl); LST_MARK();
+  if (xs) launch(pdl && !fork, k_match<5, false, true>, G, BM, 0, st, sl, g, k.max_pls); else launch(pdl && !fork, k_match<5, false, false>, G, BM, 0, st, sl, g, k.max_pls);
+  LST_MARK();
   launch(pdl, k_pt5_lists, G, B128, 0, st, sl); LST_MARK();
-  launch(pdl, k_match<3, true>, G, BM, 0, st, sl); LST_MARK();
+  if (xs) launch(pdl, k_match<3, true, true>, G, BM, 0, st, sl, g, k.max_pls); else launch(pdl, k_match<3, true, false>, G, BM, 0, st, sl, g, k.max_pls);
+  LST_MARK();
   launch(pdl, k_tc_emit, G1, dim3(1024), 0, st, sl, k); LST_MARK();
   launch(pdl, k_tc_tuples, G, B128, 0, st, sl); LST_MARK();
   launch(pdl, k_tc_clean, GL, dim3(TCC_TPB), 0, st, sl, k); LST_MARK();

@@ -24,6 +24,7 @@ struct Geo {   // device copies, shared by all slots
   const int* col;           // [nnz]
   const float* weights;     // [dnn_n_weights(n_feat, n_hidden)]
   const uint8_t* layer;     // [M] detector layer of the module (0 if the caller gave none): a 38-feature DNN input only
+  int has_layer;            // the caller gave a layer per module: a6 uses the per-surface crossing keys
   int n_feat, n_hidden;     // DNN variant (SPEC.md 4.9): 23 or 38 inputs, 1..4 hidden layers of 32
   // CSR rows compressed into runs of consecutive module ids (built by lst_create): row m = runs [run_ptr[m], run_ptr[m+1]),
   // run e = modules [run_c0[e], run_c1[e]).  MDs are stored in module order, so a run is one contiguous MD range.
@@ -31,6 +32,9 @@ struct Geo {   // device copies, shared by all slots
   const int* run_c0;        // [n_runs]
   const int* run_c1;        // [n_runs]
 };
+
+// a6 surfaces: a barrel layer, or one side of an endcap disk (lst_kernels.cuh, "crossing keys")
+constexpr int XS_NS = 32, XS_NP = 256, XS_NZ = 16, XS_REG = XS_NP * XS_NZ, XS_BINS = XS_REG + 1;     // + the surface's overflow bin
 
 enum { TK_LS_SWEEP = 0, TK_LS_DIRECT, TK_MD_SWEEP, TK_MD_DIRECT, N_TK = 16 };
 
@@ -51,11 +55,14 @@ struct Slot {
   int* sensor_start;        // [2M+1] histogram, then exclusive scan in place
   int* cursor;              // [2M]
   int* tk;                  // [N_TK] internal work tickets
+  unsigned* surf_hi;        // [XS_NS] float bits: largest reference coordinate (r barrel, |z| endcap) of the MD anchors of a surface
+  unsigned* surf_rhi;       // [XS_NS] float bits: largest anchor r of a surface
   // 0xFF-initialised per run
   unsigned long long* win5; // [max_pls]  (chi2 bits << 32 | T5 index)
   unsigned long long* win3; // [max_pls]
   int* md_head;             // [max_md]  head of the list of pT5 entries containing this MD
   int* hit_head;            // [max_hits] head of the list of (TC row, slot) entries holding this ORIGINAL hit (f1)
+  unsigned* surf_lo;        // [XS_NS] float bits: smallest reference coordinate of the MD anchors of a surface
   // a0
   int2* tmp_ok; float4* hit; int* hit_orig;
   // a1
@@ -72,6 +79,7 @@ struct Slot {
   int* t5_scan; int* t5_list;
   // a6
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
+  int* xs_start; float4* xs_ent;     // pLS crossing-key bins per surface: [XS_NS][XS_BINS + 1] starts, [XS_NS][2 max_pls] entries (cx, cy, h, pLS)
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
   int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc;     // f1 duplicate cleaning
   float* g_node; int* g_col;         // f4 graph export: node features [n_md][8], CSR column (outer MD) per LS
@@ -480,6 +488,144 @@ __device__ __forceinline__ unsigned long long win_key(float chi2, int idx) {
   return ((unsigned long long)__float_as_uint(chi2) << 32) | (unsigned)idx;   // chi2 >= 0: bit order = value order
 }
 
+// ------------------------------------------------------------------------------------------------
+// Crossing keys (used when the caller gave a layer per module; the (h, zeta, psi) buckets above stay for geometries without).
+// A surface is a barrel layer or one side of an endcap disk.  k_md_finish measures, per event and surface, the range
+// [lo, hi] of the reference coordinate of its MD anchors (r for a barrel layer, |z| for a disk) and the largest anchor r;
+// ref = (lo + hi)/2, eps = (hi - lo)/2 (0 for the cylinders / planes of BASELINE.json's geometry, but nothing relies on it).
+// Per surface every pLS is keyed by WHERE its helix crosses the surface:
+//   barrel:  azimuth psi +- acos(ref h) (both intersections of the circle with the cylinder: the transverse test is algebraic
+//            and passes near either) and z_c = z0 + s(ref) cot;
+//   endcap:  arc length s_d = (z_d - z0)/cot, radius r_d = sin(s_d h)/h, azimuth psi +- (pi/2 - s_d h);
+// and binned in (z_c or r_d: XS_NZ bins, azimuth: XS_NP bins).  An object whose first anchor lies on the surface visits the
+// bins inside a window around its own (z or r, phi) that is wide enough for every pLS that can pass the exact first-anchor
+// test (derivation in DESIGN.md "a6"): the window is small because it does not depend on the curvature any more -- one
+// look-up instead of one per curvature bucket, 4x fewer first-anchor tests.  pLS for which a key cannot be bounded (h, z0,
+// cot out of range, helix nearly tangent to the surface, NaN) sit in the surface's overflow bin, visited by every object
+// of the surface; pLS that provably cannot pass on the surface are left out.  As before this only selects which pairs get
+// the exact test.
+// ------------------------------------------------------------------------------------------------
+#define XS_UMAX 0.88f           // keys are formed where r h < 0.88 (asin(0.88) = 1.0759)
+#define XS_VMAX 1.0759f
+#define XS_ZR 128.0f            // barrel z bins cover [-128, 128), clamped
+#define XS_R0 16.0f             // endcap r bins cover [16, 120), clamped
+#define XS_RW 6.5f
+__device__ __forceinline__ int xs_surface(int mt, int layer, float z) {
+  return (mt & 2) ? 16 + (((layer & 7) << 1) | (z > 0.0f ? 1 : 0)) : (layer & 15);
+}
+__device__ __forceinline__ int xs_pbin_raw(float ang) { return (int)floorf((ang + LST_PI_F) * (XS_NP / (2.0f * LST_PI_F))); }
+__device__ __forceinline__ int xs_pmod(int b) { b %= XS_NP; return b < 0 ? b + XS_NP : b; }
+__device__ __forceinline__ int xs_zbin(float z) { return min(XS_NZ - 1, max(0, (int)floorf((z + XS_ZR) * (XS_NZ / (2.0f * XS_ZR))))); }
+__device__ __forceinline__ int xs_rbin(float r) { return min(XS_NZ - 1, max(0, (int)floorf((r - XS_R0) * (1.0f / XS_RW)))); }
+__device__ __forceinline__ float arcfac_fast(float u) {      // same polynomial, fused (window arithmetic only)
+  float p = 0.017352764f;
+  p = fmaf(u, p, 0.022372159f); p = fmaf(u, p, 0.030381944f); p = fmaf(u, p, 0.044642857f);
+  p = fmaf(u, p, 0.075f); p = fmaf(u, p, 0.16666667f); p = fmaf(u, p, 1.0f);
+  return p;
+}
+
+// the (up to two) bins of pLS `d` on surface sg; -1 = none.  ref / eps / rhi: the surface's measured geometry.
+__device__ __forceinline__ void xs_keys(int sg, float ref, float eps, float rhi, const Pls& d, int q, int& k0, int& k1) {
+  k0 = XS_REG; k1 = -1;                                  // default: overflow bin
+  if (!(d.h < LST_PLS_HMAX) || !(q == 1 || q == -1) || !(fabsf(d.z0) <= LST_PLS_Z0B) || !(fabsf(d.cot) <= LST_PLS_COTCAP)) return;
+  const float psi = atan2f(d.cy, d.cx);
+  float a, c2;
+  if (sg < 16) {
+    const float u = ref * d.h;
+    if (!(u < XS_UMAX)) return;
+    a = acosf(u);
+    c2 = d.z0 + ref * arcfac_fast(u * u) * d.cot;
+    if (!(fabsf(c2) < 1.0e30f) || !(psi == psi)) return;
+    const int zb = xs_zbin(c2) * XS_NP;
+    k0 = zb + xs_pmod(xs_pbin_raw(psi + a)); k1 = zb + xs_pmod(xs_pbin_raw(psi - a));
+  } else {
+    const float zd = (sg & 1) ? ref : -ref;
+    const float th = rhi * d.h;
+    const float s_hi = 1.01f * rhi * arcfac_fast(fminf(th * th, 4.0f));              // longest arc to any anchor of the surface
+    const float dZb = 4.330f * fabsf(d.cot) + 0.003f * s_hi * d.sec + 0.05f;      // >= dZ of any anchor of the surface
+    if (!(d.cot * zd > 0.0f)) {                        // helix moves away from the disk: |zres| >= |z| - |z0|
+      if (ref - eps - fabsf(d.z0) > dZb + 0.5f) k0 = -1;
+      return;
+    }
+    const float sd = (zd - d.z0) / d.cot;
+    if (!(sd > 0.0f)) return;
+    if (sd > s_hi + (dZb + eps) / fabsf(d.cot) + 0.5f) { k0 = -1; return; }       // reaches the disk outside every anchor
+    const float v = sd * d.h;
+    if (!(v < XS_VMAX)) return;
+    c2 = (d.h > 1.0e-7f) ? sinf(v) / d.h : sd;
+    a = 0.5f * LST_PI_F - v;
+    if (!(fabsf(c2) < 1.0e30f) || !(psi == psi)) return;
+    const int rb = xs_rbin(c2) * XS_NP;
+    k0 = rb + xs_pmod(xs_pbin_raw(psi + a)); k1 = rb + xs_pmod(xs_pbin_raw(psi - a));
+  }
+}
+
+// one block per (surface, event): derive, histogram in shared memory, scan, scatter.  Runs after k_md_finish (the surfaces'
+// geometry is measured there) on a side branch of the launch graph.
+constexpr int XS_TPB = 256, XS_SMEM = (XS_BINS + 1) * (int)sizeof(int);
+__global__ void __launch_bounds__(XS_TPB) k_pls_cross(const Slot* __restrict__ slots, int max_pls) {
+  extern __shared__ int hist[];          // [XS_BINS + 1]
+  __shared__ int sm[XS_TPB / 32 + 1];
+  const Slot& s = slots[blockIdx.y];
+  const int sg = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int n = s.n_pls;
+  if (sg == 0) {                          // the derived quantities, in input order (the walk's drains read them by pLS index)
+    for (int p = tid; p < n; p += XS_TPB) {
+      const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], (int)s.in_q[p]);
+      s.pls_sa[p] = make_float4(d.cx, d.cy, d.h, d.cot);
+      s.pls_sb[p] = make_float2(d.sec, d.z0);
+      s.pls_sidx[p] = p; s.pls_pos[p] = p;
+    }
+  }
+  const unsigned ulo = s.surf_lo[sg], uhi = s.surf_hi[sg];
+  if (uhi == 0u || ulo > uhi) return;     // no MD on this surface: nobody will look
+  const float lo = __uint_as_float(ulo), hi = __uint_as_float(uhi), rhi = __uint_as_float(s.surf_rhi[sg]);
+  const float ref = 0.5f * (lo + hi), eps = 0.5f * (hi - lo);
+  for (int i = tid; i <= XS_BINS; i += XS_TPB) hist[i] = 0;
+  __syncthreads();
+  for (int p = tid; p < n; p += XS_TPB) {
+    const int q = (int)s.in_q[p];
+    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
+    int k0, k1;
+    xs_keys(sg, ref, eps, rhi, d, q, k0, k1);
+    if (k0 >= 0) atomicAdd(&hist[k0], 1);
+    if (k1 >= 0) atomicAdd(&hist[k1], 1);
+  }
+  __syncthreads();
+  constexpr int IT = (XS_BINS + 1 + XS_TPB - 1) / XS_TPB;
+  int tsum = 0;
+  for (int k = 0; k < IT; ++k) { const int i = tid * IT + k; tsum += (i <= XS_BINS) ? hist[i] : 0; }
+  int inc = tsum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+  if (lane == 31) sm[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    const int w = lane < XS_TPB / 32 ? sm[lane] : 0; int winc = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, d); if (lane >= d) winc += t; }
+    if (lane < XS_TPB / 32) sm[lane] = winc - w;
+  }
+  __syncthreads();
+  int* start = s.xs_start + sg * (XS_BINS + 1);
+  int run = sm[wid] + inc - tsum;
+  for (int k = 0; k < IT; ++k) {
+    const int i = tid * IT + k;
+    if (i <= XS_BINS) { const int v = hist[i]; hist[i] = run; start[i] = run; run += v; }
+  }
+  __syncthreads();
+  float4* ent = s.xs_ent + (size_t)sg * 2 * max_pls;
+  for (int p = tid; p < n; p += XS_TPB) {
+    const int q = (int)s.in_q[p];
+    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
+    int k0, k1;
+    xs_keys(sg, ref, eps, rhi, d, q, k0, k1);
+    const float4 e = make_float4(d.cx, d.cy, d.h, __int_as_float(p));
+    if (k0 >= 0) ent[atomicAdd(&hist[k0], 1)] = e;       // order inside a bin is free: argmin ties break on p
+    if (k1 >= 0) ent[atomicAdd(&hist[k1], 1)] = e;
+  }
+}
+
 // Match objects with NA anchors against the pLS buckets their first anchor can reach, and reduce to the winners.
 // One thread per object (T5 of the T5 list / T3).  It visits the h-buckets in turn (all lanes of a warp are in the same
 // bucket: uniform window arithmetic) and, per bucket, looks up the few (zeta bin, psi window) ranges of sorted pLS its first
@@ -551,8 +697,8 @@ __device__ __forceinline__ void match_drain1(const Slot& s, unsigned long long* 
   }
 }
 
-template <int NA, bool IS_T3>
-__global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restrict__ slots) {
+template <int NA, bool IS_T3, bool XS>
+__global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restrict__ slots, Geo geo, int max_pls) {
   pdl_begin();
   __shared__ MatchWarp Wall[MATCH_WARPS];
   const Slot& s = slots[blockIdx.y];
@@ -596,19 +742,70 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
     }
     __syncwarp();
     float4 a0 = make_float4(1.f, 0.f, 0.f, 1.f);
-    int mt0 = 0;
-    if (act) { a0 = s.md_pos[md0]; mt0 = s.md_modt[md0] & 3; }
+    int mt0 = 0, sg = 0;
+    if (act) {
+      a0 = s.md_pos[md0];
+      const int mm = s.md_modt[md0];
+      mt0 = mm & 3;
+      if (XS) sg = xs_surface(mt0, geo.layer[mm >> 2], a0.z);
+    }
     const float r = a0.w;
     const float phi = atan2f(a0.y, a0.x);
     const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
     int q1n = 0, q2n = 0;
-    for (int kb = 0; kb <= PLS_K; ++kb) {
-    if (kb == PLS_K && bstart[PLS_NREG + 1] == bstart[PLS_NREG]) break;      // empty overflow bucket (uniform)
+    for (int kb = 0; kb <= (XS ? 0 : PLS_K); ++kb) {
+    if (!XS && kb == PLS_K && bstart[PLS_NREG + 1] == bstart[PLS_NREG]) break;      // empty overflow bucket (uniform)
+    int xb0 = 0, xnb = 0;                     // XS: first azimuth bin and number of bins of the window
+    const int* bst = bstart;
+    const float4* ent = psa;
+    if (XS) { bst = s.xs_start + sg * (XS_BINS + 1); ent = s.xs_ent + (size_t)sg * 2 * max_pls; }
     // ranges of sorted pLS this object must visit in this h-bucket: per zeta bin up to two psi windows, each possibly
     // wrapping around -> up to MATCH_ZB x 4 slots.  All slot look-ups are independent loads issued together; the non-empty
     // ranges (rarely more than one or two) are compacted into four register slots, the rest is walked afterwards.
     int zb_lo = 0, n_zb = 0, pb0[2] = {0, 0}, pnb[2] = {0, 0};
-    if (kb == PLS_K) { n_zb = act ? 1 : 0; }
+    if (XS) {
+      if (act) {
+        // window of crossing keys (comment above k_pls_cross): every pLS that passes the exact first-anchor test
+        // has a key within `del` in azimuth and `zwin` / `wr` in z / r of the anchor, whatever its curvature below HMAX
+        const unsigned ulo = s.surf_lo[sg], uhi = s.surf_hi[sg];
+        const float eps = 0.5f * (__uint_as_float(uhi) - __uint_as_float(ulo));
+        const float hm = LST_PLS_HMAX * 1.0001f;
+        const float tau = tconst + 0.03f * r * hm;
+        const float dz = anchor_dz(mt0), dr = anchor_dr(mt0);
+        const float tb = 1.03f * r * hm;
+        const float s_hi = 1.01f * r * arcfac_fast(tb * tb);
+        bool slow = !(r * hm < XS_UMAX) || uhi == 0u || ulo > uhi;
+        float x, dnum;
+        if (sg < 16) {
+          const float s_lo = 0.99f * r;
+          const float den = s_lo - dr - 0.003f * s_hi;
+          float cb = LST_PLS_COTCAP;
+          if (den > 0.5f * s_lo) cb = fminf(cb, 1.02f * (fabsf(a0.z) + LST_PLS_Z0B + dz + 0.003f * s_hi + 0.05f) / den);
+          const float zwin = dz + dr * cb + 0.003f * s_hi * (1.0f + cb) + 0.05f + 2.5f * eps * cb + 0.5f;
+          zb_lo = xs_zbin(a0.z - zwin);
+          n_zb = xs_zbin(a0.z + zwin) - zb_lo + 1;
+          dnum = tau + eps * hm;
+          x = r * hm + dnum;
+        } else {
+          const float A = fabsf(a0.z) - LST_PLS_Z0B - 0.05f;
+          const float cmin = (A - 0.003f * s_hi) / (1.003f * s_hi + dr);
+          slow |= !(cmin > 0.2f);
+          const float ic = 1.0f / fmaxf(cmin, 0.2f);
+          const float wr = dr + 0.003f * s_hi * (1.0f + ic) + (0.05f + eps) * ic + 0.008f * s_hi + 0.1f;
+          zb_lo = xs_rbin(r - wr);
+          n_zb = xs_rbin(r + wr) - zb_lo + 1;
+          dnum = tau + wr * hm;
+          x = r * hm + dnum;
+        }
+        slow |= !(x < 0.97f);
+        const float del = dnum * rsqrtf(fmaxf(1.0f - x * x, 0.05f)) * 1.01f + 1.0e-3f;
+        const int blo = xs_pbin_raw(phi - del);
+        xnb = min(xs_pbin_raw(phi + del) - blo + 1, XS_NP);
+        xb0 = xs_pmod(blo);
+        if (slow || !(del == del)) { zb_lo = 0; n_zb = XS_NZ; xb0 = 0; xnb = XS_NP; }      // no bound: the whole surface
+      }
+    }
+    else if (kb == PLS_K) { n_zb = act ? 1 : 0; }
     else if (act) {
       const float h_lo = kb * (LST_PLS_HMAX / PLS_K), h_hi = (kb + 1) * (LST_PLS_HMAX / PLS_K);
       const float ulo = r * h_lo, uhi = r * h_hi;
@@ -650,6 +847,13 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
     };
     auto slot_range = [&](int sl, int& js, int& len) {
       js = 0; len = 0;
+      if (XS) {                               // per z / r bin: the azimuth window, possibly wrapping; last slot: the overflow bin
+        if (sl == 2 * n_zb) { js = bst[XS_REG]; len = bst[XS_REG + 1] - js; return; }
+        const int base = (zb_lo + (sl >> 1)) * XS_NP;
+        if ((sl & 1) == 0) { const int e0 = min(xb0 + xnb, XS_NP); js = bst[base + xb0]; len = bst[base + e0] - js; }
+        else if (xb0 + xnb > XS_NP) { js = bst[base]; len = bst[base + xb0 + xnb - XS_NP] - js; }
+        return;
+      }
       if (kb == PLS_K) { if (sl == 0) { js = bstart[PLS_NREG]; len = bstart[PLS_NREG + 1] - js; } return; }
       const int zb = zb_lo + (sl >> 2), sgn = (sl >> 1) & 1, part = sl & 1;
       const int base = (kb * PLS_NZ + zb) * PLS_NB;
@@ -657,7 +861,8 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
       if (part == 0) { const int e0 = min(b0 + nb, PLS_NB); js = bstart[base + b0]; len = bstart[base + e0] - js; }
       else if (b0 + nb > PLS_NB) { js = bstart[base]; len = bstart[base + b0 + nb - PLS_NB] - js; }
     };
-    const int n_slots = n_zb * 4;
+    const int n_slots = XS ? (act ? 2 * n_zb + 1 : 0) : n_zb * 4;
+    const bool wide = XS ? n_slots > MATCH_ZB * 4 : n_zb > MATCH_ZB;
     {
       int js[MATCH_ZB * 4], len[MATCH_ZB * 4];
 #pragma unroll
@@ -669,10 +874,11 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
     auto test_one = [&](bool has, int j) {
       bool pass = false;
       if (has) {
-        const float4 pa = __ldg(psa + j);
+        const float4 pa = __ldg(ent + j);
         Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
         float e, dT;
         pass = pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT);                 // transverse test of the first anchor
+        if (XS) j = __float_as_int(pa.w);                                // the entry carries the pLS index
         ++n_tests;
       }
       const unsigned mask = __ballot_sync(0xffffffffu, pass);
@@ -701,10 +907,10 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
       }
     }
     // ... then whatever did not fit: more than four non-empty ranges, or a zeta window wider than MATCH_ZB bins (rare)
-    if (__any_sync(0xffffffffu, nr > 4 || n_zb > MATCH_ZB)) {
+    if (__any_sync(0xffffffffu, nr > 4 || wide)) {
       for (int sl = 0; __any_sync(0xffffffffu, sl < n_slots); ++sl) {
         int js = 0, len = 0;
-        if (sl < n_slots && (nr > 4 || n_zb > MATCH_ZB)) {
+        if (sl < n_slots && (nr > 4 || wide)) {
           slot_range(sl, js, len);
           // skip the ranges the flat walk already covered: the first four non-empty ones among the first MATCH_ZB * 4 slots
           if (sl < MATCH_ZB * 4 && len > 0) {

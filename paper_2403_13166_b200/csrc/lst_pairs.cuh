@@ -62,10 +62,11 @@ struct MdWarp {   // per-warp shared memory
   int P[33]; int4 par[32]; float inv[32];     // non-empty modules of the warp's current group: first flat cell, (lb, ub, n_up, mtm), 1/n_up
   int q_lo[Q_CAP], q_up[Q_CAP], q_mt[Q_CAP];
   MdRec st[Q_CAP];
+  const uint8_t* layer;                        // the modules' layers if the caller gave them (a6 surface ranges), else null
 };
 
 template <bool DIRECT>
-__device__ __forceinline__ void md_emit(const Slot& s, const MdRec& r, int cap) {      // final arrays of one MD
+__device__ __forceinline__ void md_emit(const Slot& s, const MdRec& r, int cap, const uint8_t* layer = nullptr) {      // final arrays of one MD
   const int pos = s.md_start[r.mtm >> 2] + r.seq;
   if (pos >= cap) return;
   const float4 h = s.hit[r.p_lo];
@@ -78,12 +79,17 @@ __device__ __forceinline__ void md_emit(const Slot& s, const MdRec& r, int cap) 
   // carry the module type (they only widen the tolerance)
   const float fm_ = __int_as_float(__float_as_int(md_relf(mt) * 1.0001f) | mt);
   s.md_aux[pos] = make_float4(r.c, fmaf(r.w, 1.0001f, 3.0e-7f), fm_, 1.0f / h.w);
+  if (DIRECT && layer) {                                // surface ranges for a6 (the record path aggregates them per block)
+    const int sg = xs_surface(mt, layer[r.mtm >> 2], h.z);
+    const unsigned ref = __float_as_uint((mt & 2) ? fabsf(h.z) : h.w);
+    atomicMin(s.surf_lo + sg, ref); atomicMax(s.surf_hi + sg, ref); atomicMax(s.surf_rhi + sg, __float_as_uint(h.w));
+  }
 }
 
 template <bool DIRECT>
 __device__ __forceinline__ void md_flush(const Slot& s, MdWarp& W, int n, int lane, int cap) {
   if (DIRECT) {
-    if (lane < n) md_emit<true>(s, W.st[lane], cap);
+    if (lane < n) md_emit<true>(s, W.st[lane], cap, W.layer);
     return;
   }
   int base = 0;
@@ -156,6 +162,8 @@ __device__ __forceinline__ void md_sweep_body(const Slot& s, const Geo& geo, con
   const int cap = caps.max_md;
   const int n_warps = gridDim.x * PAIR_WARPS;
   int qn = 0, sn = 0, carry_row = -1, carry_n = 0;
+  if (lane == 0) W.layer = geo.has_layer ? geo.layer : nullptr;
+  __syncwarp();
   // modules are interleaved over the warps (heavy inner-layer modules have consecutive ids).  A warp takes 32 of its modules
   // at a time (one round of range loads) and sweeps their cells as ONE flat index space, 32 cells per step: most modules
   // hold fewer than 32 cells, so per-module sweeps would leave most lanes idle.
@@ -260,6 +268,10 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
   const int n_rec = min(s.cnt[LST_CNT_FILL_MD], caps.max_md);
   const int M = geo.n_modules;
   const int* __restrict__ mds = s.md_start;
+  // a6 surface ranges (reference coordinate of the anchors per barrel layer / disk side): per block in shared memory first
+  __shared__ unsigned b_lo[XS_NS], b_hi[XS_NS], b_rh[XS_NS];
+  if (threadIdx.x < XS_NS) { b_lo[threadIdx.x] = 0xFFFFFFFFu; b_hi[threadIdx.x] = 0u; b_rh[threadIdx.x] = 0u; }
+  __syncthreads();
   LST_FOR_ITEMS(j, max(n_rec, M)) {
     const bool has_r = j < n_rec, has_m = j < M;
     // level 1
@@ -271,7 +283,11 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
     // level 2
     int pos = 0, o_lo = 0, o_up = 0;
     float4 h = make_float4(0.f, 0.f, 0.f, 1.f);
-    if (has_r) { pos = mds[r.mtm >> 2] + r.seq; h = s.hit[r.p_lo]; o_lo = s.hit_orig[r.p_lo]; o_up = s.hit_orig[r.p_up]; }
+    int lay = 0;
+    if (has_r) {
+      pos = mds[r.mtm >> 2] + r.seq; h = s.hit[r.p_lo]; o_lo = s.hit_orig[r.p_lo]; o_up = s.hit_orig[r.p_up];
+      if (geo.has_layer) lay = geo.layer[r.mtm >> 2];
+    }
     int c0[LS_TAB], c1[LS_TAB], b0[LS_TAB], b1[LS_TAB];
 #pragma unroll
     for (int q = 0; q < LS_TAB; ++q) { const bool in = tab_on && e0 + q < e1; c0[q] = in ? __ldg(geo.run_c0 + e0 + q) : 0; c1[q] = in ? __ldg(geo.run_c1 + e0 + q) : 0; }
@@ -287,6 +303,11 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
       s.md_cw[pos] = make_float2(r.c, r.w);
       const float fm_ = __int_as_float(__float_as_int(md_relf(mt) * 1.0001f) | mt);
       s.md_aux[pos] = make_float4(r.c, fmaf(r.w, 1.0001f, 3.0e-7f), fm_, 1.0f / h.w);
+      if (geo.has_layer) {
+        const int sg = xs_surface(mt, lay, h.z);
+        const unsigned ref = __float_as_uint((mt & 2) ? fabsf(h.z) : h.w);      // positive floats: bit order = value order
+        atomicMin(&b_lo[sg], ref); atomicMax(&b_hi[sg], ref); atomicMax(&b_rh[sg], __float_as_uint(h.w));
+      }
     }
     if (tab_on) {
       int ends[LS_TAB], dl[LS_TAB];
@@ -315,6 +336,13 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
       static_assert(LS_TAB == 8, "table layout");
       tab[0] = make_int4(ends[0], ends[1], ends[2], ends[3]); tab[1] = make_int4(ends[4], ends[5], ends[6], ends[7]);
       tab[2] = make_int4(dl[0], dl[1], dl[2], dl[3]); tab[3] = make_int4(dl[4], dl[5], dl[6], dl[7]);
+    }
+  }
+  if (geo.has_layer) {
+    __syncthreads();
+    if (threadIdx.x < XS_NS && b_hi[threadIdx.x] != 0u) {
+      atomicMin(s.surf_lo + threadIdx.x, b_lo[threadIdx.x]); atomicMax(s.surf_hi + threadIdx.x, b_hi[threadIdx.x]);
+      atomicMax(s.surf_rhi + threadIdx.x, b_rh[threadIdx.x]);
     }
   }
 }
