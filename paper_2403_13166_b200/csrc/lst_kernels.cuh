@@ -715,17 +715,33 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
     const int t = t0 + lane;
     // every warp loads the tile's objects for itself (no barrier before the walk)
     bool act = t < n;
-    int md0 = 0;
     __syncwarp();
     key[lane] = WIN_EMPTY;
+    float4 a0 = make_float4(1.f, 0.f, 0.f, 1.f);
+    int mt0 = 0, sg = 0;
     if (act) {
+      int md0, head = -1;
+      int4 abc = make_int4(0, 0, 0, 0);
       if (IS_T3) {
-        const int4 abc = s.t3_abc[t];
+        abc = s.t3_abc[t];
         W.o_md[lane][0] = abc.x; W.o_md[lane][1] = abc.y; W.o_md[lane][2] = abc.z;
         md0 = abc.x;
+        head = s.md_head[md0];                 // issued together with the anchor loads below
+      } else {
+        const int* m5 = s.t5c_md + 5 * s.t5_list[t];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) W.o_md[lane][q] = m5[q];
+        md0 = m5[0];
+      }
+      a0 = s.md_pos[md0];
+      const int mm = s.md_modt[md0];
+      mt0 = mm & 3;
+      int lay = 0;
+      if (XS) lay = geo.layer[mm >> 2];
+      if (IS_T3) {
         // used iff {a,b,c} is contained in the five MDs of some pT5: walk the pT5 entries that contain a
         bool used = false;
-        for (int e = s.md_head[abc.x]; e >= 0 && !used; e = s.pt5_next[e]) {
+        for (int e = head; e >= 0 && !used; e = s.pt5_next[e]) {
           const int* m5 = s.t5c_md + 5 * s.t5_list[(int)(s.win5[e / 5] & 0xFFFFFFFFull)];
           int found = 0;
 #pragma unroll
@@ -733,22 +749,10 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
           used = (found == 2);
         }
         if (used) { act = false; s.best3[t] = -2; }
-      } else {
-        const int* m5 = s.t5c_md + 5 * s.t5_list[t];
-#pragma unroll
-        for (int q = 0; q < 5; ++q) W.o_md[lane][q] = m5[q];
-        md0 = m5[0];
       }
+      if (XS) sg = xs_surface(mt0, lay, a0.z);
     }
     __syncwarp();
-    float4 a0 = make_float4(1.f, 0.f, 0.f, 1.f);
-    int mt0 = 0, sg = 0;
-    if (act) {
-      a0 = s.md_pos[md0];
-      const int mm = s.md_modt[md0];
-      mt0 = mm & 3;
-      if (XS) sg = xs_surface(mt0, geo.layer[mm >> 2], a0.z);
-    }
     const float r = a0.w;
     const float phi = atan2f(a0.y, a0.x);
     const float tconst = 0.003f + 0.02f / r + 2.0e-3f;
@@ -871,10 +875,9 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
       for (int sl = 0; sl < MATCH_ZB * 4; ++sl) add_range(js[sl], len[sl]);
     }
     // walk: first the (up to four) compacted ranges as one flat index space ...
-    auto test_one = [&](bool has, int j) {
+    auto test_one = [&](bool has, int j, float4 pa) {
       bool pass = false;
       if (has) {
-        const float4 pa = __ldg(ent + j);
         Pls P; P.cx = pa.x; P.cy = pa.y; P.h = pa.z; P.cot = pa.w;
         float e, dT;
         pass = pls_anchor_t(P, a0.x, a0.y, a0.w, e, dT);                 // transverse test of the first anchor
@@ -901,9 +904,19 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
     };
     {
       const int c1 = rlen[0], c2 = c1 + rlen[1], c3 = c2 + rlen[2], total = c3 + rlen[3];
-      for (int q = 0; __any_sync(0xffffffffu, q < total); ++q) {
-        const int j = q < c1 ? rjs[0] + q : q < c2 ? rjs[1] + (q - c1) : q < c3 ? rjs[2] + (q - c2) : rjs[3] + (q - c3);
-        test_one(q < total, j);
+      for (int q0 = 0; __any_sync(0xffffffffu, q0 < total); q0 += 4) {      // four entries at a time: their loads are independent
+        int j[4];
+        float4 pa[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int q = q0 + u;
+          j[u] = q < c1 ? rjs[0] + q : q < c2 ? rjs[1] + (q - c1) : q < c3 ? rjs[2] + (q - c2) : rjs[3] + (q - c3);
+          pa[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (q < total) pa[u] = __ldg(ent + j[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+          if (__any_sync(0xffffffffu, q0 + u < total)) test_one(q0 + u < total, j[u], pa[u]);
       }
     }
     // ... then whatever did not fit: more than four non-empty ranges, or a zeta window wider than MATCH_ZB bins (rare)
@@ -920,7 +933,7 @@ __global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restri
             if (covered) len = 0;
           }
         }
-        for (int q = 0; __any_sync(0xffffffffu, q < len); ++q) test_one(q < len, js + q);
+        for (int q = 0; __any_sync(0xffffffffu, q < len); ++q) test_one(q < len, js + q, q < len ? __ldg(ent + js + q) : make_float4(0.f, 0.f, 0.f, 0.f));
       }
     }
     }     // h-buckets
