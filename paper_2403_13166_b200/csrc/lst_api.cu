@@ -157,7 +157,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.t5_list = cv.take<int>(k.max_t5);
     t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.pls_key = cv.take<int>(k.max_pls);
     t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls); t.pls_pos = cv.take<int>(k.max_pls); t.pls_taken = cv.take<int>(k.max_pls);
-    t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.xs_start = cv.take<int>((size_t)XS_NS * (XS_BINS + 1)); t.xs_ent = cv.take<float4>((size_t)XS_NS * 2 * k.max_pls); t.best5 = cv.take<int>(k.max_t5);
+    t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.xs_key = cv.take<int>((size_t)XS_NS * k.max_pls); t.xs_start = cv.take<int>((size_t)XS_NS * (XS_BINS + 1)); t.xs_ent = cv.take<float4>((size_t)XS_NS * 2 * k.max_pls); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
     t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc);
@@ -283,7 +283,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     }
     (void)cudaGetLastError();
   }
-  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.has_layer = geo->layer ? 1 : 0; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
+  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.has_layer = (geo->layer && c->use_xs) ? 1 : 0; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
   c->geo.run_ptr = L.run_ptr; c->geo.run_c0 = L.run_c0; c->geo.run_c1 = L.run_c1;
   *out = c;
   return LST_OK;
@@ -349,7 +349,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   // the pLS binning depends on the inputs only: under stream capture it becomes a side branch of the graph
   // (with a layer per module the binning uses the surfaces measured by k_md_finish: the branch forks after that kernel)
   const bool fork = c->capturing && c->side;
-  const bool xs = g.has_layer && c->use_xs;
+  const bool xs = g.has_layer != 0;
   const dim3 GX(XS_NS, n);
   if (fork && !xs) {
     if (bad(c, cudaEventRecord(c->ev_fork, st)) || bad(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0))) return LST_ECUDA;

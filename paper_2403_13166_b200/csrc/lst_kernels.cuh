@@ -17,6 +17,14 @@ constexpr int CNT_STATUS = LST_N_CNT - 1;
 constexpr unsigned long long WIN_EMPTY = 0xFFFFFFFFFFFFFFFFull;
 constexpr int TC_HSTRIDE = 12;         // ints per row of the candidates' hit tuples (10 hits, padded for 16-byte loads)
 
+// pLS that the a6 bins cannot hold (overflow bins): h >= HMAX, |z0| > Z0B, |cot| > COTCAP, q not +-1, NaN
+#define LST_PLS_HMAX 0.0075f
+#define LST_PLS_Z0B 20.0f
+#define LST_PLS_COTCAP 8.0f
+#define LST_PLS_RREF 40.0f
+#define LST_PLS_ZR 256.0f
+#define LST_PI_F 3.14159265358979f
+
 struct Geo {   // device copies, shared by all slots
   int n_modules;
   const uint8_t* modt;      // [M] subdet<<1 | mtype
@@ -79,7 +87,7 @@ struct Slot {
   int* t5_scan; int* t5_list;
   // a6
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
-  int* xs_start; float4* xs_ent;     // pLS crossing-key bins per surface: [XS_NS][XS_BINS + 1] starts, [XS_NS][2 max_pls] entries (cx, cy, h, pLS)
+  int* xs_key; int* xs_start; float4* xs_ent;     // pLS crossing-key bins per surface: [XS_NS][XS_BINS + 1] starts, [XS_NS][2 max_pls] entries (cx, cy, h, pLS)
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
   int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc;     // f1 duplicate cleaning
   float* g_node; int* g_col;         // f4 graph export: node features [n_md][8], CSR column (outer MD) per LS
@@ -250,6 +258,17 @@ __global__ void k_hist(const Slot* __restrict__ slots, Geo geo) {
     if (key >= S) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_BAD_KEY);
     else atomicAdd(s.sensor_start + key, 1);
   }
+  if (geo.has_layer) {      // a6 with crossing keys: the derived pLS quantities in input order, once (they depend on the inputs only)
+    LST_FOR_ITEMS(p, s.n_pls) {
+      const int q = (int)s.in_q[p];
+      const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
+      s.pls_sa[p] = make_float4(d.cx, d.cy, d.h, d.cot);
+      s.pls_sb[p] = make_float2(d.sec, d.z0);
+      s.pls_sidx[p] = p; s.pls_pos[p] = p;
+      const bool bad = !(d.h < LST_PLS_HMAX) || !(q == 1 || q == -1) || !(fabsf(d.z0) <= LST_PLS_Z0B) || !(fabsf(d.cot) <= LST_PLS_COTCAP);
+      s.pls_a[p] = make_float4(atan2f(d.cy, d.cx), bad ? 1.0f : 0.0f, 0.0f, 0.0f);      // (psi, no key can be formed)
+    }
+  }
 }
 __global__ void k_scatter(const Slot* __restrict__ slots, Geo geo) {
   pdl_begin();
@@ -411,12 +430,6 @@ __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, 
 constexpr int PLS_NB = 256, PLS_NZ = 16, PLS_K = 2;
 constexpr int PLS_NREG = PLS_K * PLS_NZ * PLS_NB;          // regular bins: ((kb * NZ + zb) * NB + pb); bin PLS_NREG = overflow
 constexpr int PLS_NBINS = PLS_NREG + 1;
-#define LST_PLS_HMAX 0.0075f
-#define LST_PLS_Z0B 20.0f
-#define LST_PLS_COTCAP 8.0f
-#define LST_PLS_RREF 40.0f
-#define LST_PLS_ZR 256.0f
-#define LST_PI_F 3.14159265358979f
 
 __device__ __forceinline__ int psi_bin_raw(float ang) {   // unbounded bin index of an angle in radians
   return (int)floorf((ang + LST_PI_F) * (PLS_NB / (2.0f * LST_PI_F)));
@@ -525,10 +538,9 @@ __device__ __forceinline__ float arcfac_fast(float u) {      // same polynomial,
 }
 
 // the (up to two) bins of pLS `d` on surface sg; -1 = none.  ref / eps / rhi: the surface's measured geometry.
-__device__ __forceinline__ void xs_keys(int sg, float ref, float eps, float rhi, const Pls& d, int q, int& k0, int& k1) {
+__device__ __forceinline__ void xs_keys(int sg, float ref, float eps, float rhi, const Pls& d, float psi, bool bad, int& k0, int& k1) {
   k0 = XS_REG; k1 = -1;                                  // default: overflow bin
-  if (!(d.h < LST_PLS_HMAX) || !(q == 1 || q == -1) || !(fabsf(d.z0) <= LST_PLS_Z0B) || !(fabsf(d.cot) <= LST_PLS_COTCAP)) return;
-  const float psi = atan2f(d.cy, d.cx);
+  if (bad) return;
   float a, c2;
   if (sg < 16) {
     const float u = ref * d.h;
@@ -562,32 +574,27 @@ __device__ __forceinline__ void xs_keys(int sg, float ref, float eps, float rhi,
 
 // one block per (surface, event): derive, histogram in shared memory, scan, scatter.  Runs after k_md_finish (the surfaces'
 // geometry is measured there) on a side branch of the launch graph.
-constexpr int XS_TPB = 256, XS_SMEM = (XS_BINS + 1) * (int)sizeof(int);
+constexpr int XS_TPB = 1024, XS_SMEM = (XS_BINS + 1) * (int)sizeof(int);
 __global__ void __launch_bounds__(XS_TPB) k_pls_cross(const Slot* __restrict__ slots, int max_pls) {
   extern __shared__ int hist[];          // [XS_BINS + 1]
   __shared__ int sm[XS_TPB / 32 + 1];
   const Slot& s = slots[blockIdx.y];
   const int sg = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int n = s.n_pls;
-  if (sg == 0) {                          // the derived quantities, in input order (the walk's drains read them by pLS index)
-    for (int p = tid; p < n; p += XS_TPB) {
-      const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], (int)s.in_q[p]);
-      s.pls_sa[p] = make_float4(d.cx, d.cy, d.h, d.cot);
-      s.pls_sb[p] = make_float2(d.sec, d.z0);
-      s.pls_sidx[p] = p; s.pls_pos[p] = p;
-    }
-  }
   const unsigned ulo = s.surf_lo[sg], uhi = s.surf_hi[sg];
   if (uhi == 0u || ulo > uhi) return;     // no MD on this surface: nobody will look
   const float lo = __uint_as_float(ulo), hi = __uint_as_float(uhi), rhi = __uint_as_float(s.surf_rhi[sg]);
   const float ref = 0.5f * (lo + hi), eps = 0.5f * (hi - lo);
   for (int i = tid; i <= XS_BINS; i += XS_TPB) hist[i] = 0;
   __syncthreads();
+  int* keys = s.xs_key + (size_t)sg * max_pls;           // (k0 | k1 << 16) per pLS, 0xFFFF = none
   for (int p = tid; p < n; p += XS_TPB) {
-    const int q = (int)s.in_q[p];
-    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
+    const float4 a = s.pls_sa[p], ps = s.pls_a[p];
+    const float2 b = s.pls_sb[p];
+    Pls d; d.cx = a.x; d.cy = a.y; d.h = a.z; d.cot = a.w; d.sec = b.x; d.z0 = b.y;
     int k0, k1;
-    xs_keys(sg, ref, eps, rhi, d, q, k0, k1);
+    xs_keys(sg, ref, eps, rhi, d, ps.x, ps.y != 0.0f, k0, k1);
+    keys[p] = (k0 & 0xFFFF) | (k1 << 16);
     if (k0 >= 0) atomicAdd(&hist[k0], 1);
     if (k1 >= 0) atomicAdd(&hist[k1], 1);
   }
@@ -616,11 +623,11 @@ __global__ void __launch_bounds__(XS_TPB) k_pls_cross(const Slot* __restrict__ s
   __syncthreads();
   float4* ent = s.xs_ent + (size_t)sg * 2 * max_pls;
   for (int p = tid; p < n; p += XS_TPB) {
-    const int q = (int)s.in_q[p];
-    const Pls d = pls_derive(s.in_px[p], s.in_py[p], s.in_pz[p], s.in_z0[p], q);
-    int k0, k1;
-    xs_keys(sg, ref, eps, rhi, d, q, k0, k1);
-    const float4 e = make_float4(d.cx, d.cy, d.h, __int_as_float(p));
+    const int kk = keys[p];
+    const int k0 = (kk & 0xFFFF) == 0xFFFF ? -1 : (kk & 0xFFFF), k1 = kk >> 16;       // k1: arithmetic shift keeps -1
+    if (k0 < 0 && k1 < 0) continue;
+    const float4 a = s.pls_sa[p];
+    const float4 e = make_float4(a.x, a.y, a.z, __int_as_float(p));
     if (k0 >= 0) ent[atomicAdd(&hist[k0], 1)] = e;       // order inside a bin is free: argmin ties break on p
     if (k1 >= 0) ent[atomicAdd(&hist[k1], 1)] = e;
   }
