@@ -160,7 +160,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.xs_key = cv.take<int>((size_t)XS_NS * k.max_pls); t.xs_start = cv.take<int>((size_t)XS_NS * (XS_BINS + 1)); t.xs_ent = cv.take<float4>((size_t)XS_NS * 2 * k.max_pls); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
-    t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc);
+    t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc); t.tc_sig = cv.take<unsigned long long>(k.max_tc);
     t.tcc = cv.take<int>(3 * (size_t)k.max_tc); t.chain_tcc = cv.take<unsigned long long>(k.max_tc / TCC_ROWS + 4);
     t.g_node = cv.take<float>(8 * (size_t)k.max_md); t.g_col = cv.take<int>(k.max_ls);
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);

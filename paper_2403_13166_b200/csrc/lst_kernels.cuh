@@ -89,7 +89,7 @@ struct Slot {
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
   int* xs_key; int* xs_start; float4* xs_ent;     // pLS crossing-key bins per surface: [XS_NS][XS_BINS + 1] starts, [XS_NS][2 max_pls] entries (cx, cy, h, pLS)
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
-  int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc;     // f1 duplicate cleaning
+  int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc; unsigned long long* tc_sig;     // f1 duplicate cleaning
   float* g_node; int* g_col;         // f4 graph export: node features [n_md][8], CSR column (outer MD) per LS
   // host-load staging
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
@@ -1039,6 +1039,7 @@ __global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots
 
 // f1 (SPEC.md 4.7), step 1: the hit tuple of every candidate (ORIGINAL indices: lower, upper hit of each of its MDs), the chi2
 // of its rank key, and its entry in the list of every hit it holds.  One thread per TC row.
+__device__ __forceinline__ int tc_hash(int hit) { return (int)(((unsigned)hit * 0x9E3779B1u) >> 26); }
 __global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slots) {
   pdl_begin();
   const Slot& s = slots[blockIdx.y];
@@ -1064,6 +1065,11 @@ __global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slot
     *reinterpret_cast<int4*>(row) = make_int4(h[0].x, h[0].y, h[1].x, h[1].y);
     *reinterpret_cast<int4*>(row + 4) = make_int4(h[2].x, h[2].y, h[3].x, h[3].y);
     *reinterpret_cast<int4*>(row + 8) = make_int4(h[4].x, h[4].y, -1, -1);
+    unsigned long long sig = 0ull;                     // 64-bit signature of the row's hits (k_tc_clean's quick bound)
+#pragma unroll
+    for (int q = 0; q < 5; ++q)
+      if (md[q] >= 0) sig |= (1ull << tc_hash(h[q].x)) | (1ull << tc_hash(h[q].y));
+    s.tc_sig[o] = sig;
 #pragma unroll
     for (int q = 0; q < 5; ++q)
       if (md[q] >= 0) {
@@ -1074,22 +1080,25 @@ __global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slot
 }
 
 // f1, step 2: X is dropped iff some candidate Y with a better rank key (type, chi2 bits, row) holds more than half of X's
-// hits.  Y must then hold at least one of them: one thread per (row X, hit slot) walks the list of that hit.  A tile is
-// TCC_ROWS rows x 10 slots; the kept rows are compacted in order with a block scan + look-back across tiles (by ticket).
-constexpr int TCC_TPB = 128, TCC_ROWS = 12;
+// hits.  Such a Y misses fewer than half of them, so it holds at least one of X's first nh/2 hits: one thread per (row X,
+// slot < nh/2) walks the list of that hit.  A candidate on the list is first bounded through the 64-bit hit signatures (the
+// number of X's hits whose bit is set in Y's signature is >= the shared hits) and compared hit by hit only if that bound
+// allows a majority.  A tile is TCC_ROWS rows x 5 slots; the kept rows are compacted in order with a block scan + look-back
+// across tiles (by ticket).
+constexpr int TCC_TPB = 128, TCC_ROWS = 25;
 __global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ slots, Caps caps) {
   pdl_begin();
-  __shared__ int s_keep[TCC_ROWS];
+  __shared__ int s_keep[32];
   __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
   const unsigned epoch = *s.epoch_dev;
   const int n = s.cnt[LST_CNT_TC];
   const int n_tiles = (n + TCC_ROWS - 1) / TCC_ROWS + (n == 0);
   const int lane = threadIdx.x & 31;
-  const int rl = threadIdx.x / 10, slot = threadIdx.x - 10 * rl;       // row of the tile, hit slot
+  const int rl = threadIdx.x / 5, slot = threadIdx.x - 5 * rl;       // row of the tile, hit slot
   while (true) {
     if (threadIdx.x == 0) s_tile = atomicAdd(s.cnt + LST_CNT_TK_TCC, 1);
-    if (threadIdx.x < TCC_ROWS) s_keep[threadIdx.x] = 1;
+    if (threadIdx.x < 32) s_keep[threadIdx.x] = 1;
     __syncthreads();
     const int tile = s_tile;
     if (tile >= n_tiles) break;
@@ -1097,21 +1106,29 @@ __global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ s
     if (rl < TCC_ROWS && x < n) {
       const int type = s.tc[3 * x];
       const int nh = type == 2 ? 6 : type <= 1 ? 10 : 0;
-      if (slot < nh) {
+      if (2 * slot < nh) {
         const unsigned qx = (unsigned)s.tc_q[x];
         const int* rx = s.tc_hits + TC_HSTRIDE * x;
         const int4 x0 = *reinterpret_cast<const int4*>(rx), x1 = *reinterpret_cast<const int4*>(rx + 4), x2 = *reinterpret_cast<const int4*>(rx + 8);
         const int hx[10] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w, x2.x, x2.y};
+        int bx[10];
+#pragma unroll
+        for (int a = 0; a < 10; ++a) bx[a] = (a < nh) ? tc_hash(hx[a]) : 64;     // 64: shifted out (never counts)
         int mine = hx[0];
 #pragma unroll
-        for (int a = 1; a < 10; ++a) mine = (slot == a) ? hx[a] : mine;
+        for (int a = 1; a < 5; ++a) mine = (slot == a) ? hx[a] : mine;
         for (int e = s.hit_head[mine]; e >= 0; e = s.tc_next[e]) {
           const int y = e / 10;
           if (y == x) continue;
           const int ty = s.tc[3 * y];
           const unsigned qy = (unsigned)s.tc_q[y];
+          const unsigned long long sg = s.tc_sig[y];
           const bool better = ty != type ? ty < type : qy != qx ? qy < qx : y < x;
           if (!better) continue;
+          int bound = 0;
+#pragma unroll
+          for (int a = 0; a < 10; ++a) bound += (bx[a] < 64) ? (int)((sg >> bx[a]) & 1ull) : 0;
+          if (2 * bound <= nh) continue;
           const int* ry = s.tc_hits + TC_HSTRIDE * y;
           const int4 y0 = *reinterpret_cast<const int4*>(ry), y1 = *reinterpret_cast<const int4*>(ry + 4), y2 = *reinterpret_cast<const int4*>(ry + 8);
           const int hy[10] = {y0.x, y0.y, y0.z, y0.w, y1.x, y1.y, y1.z, y1.w, y2.x, y2.y};     // -1 padded: never equals a hit of X
