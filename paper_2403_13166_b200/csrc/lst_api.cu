@@ -106,18 +106,17 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   // zero region (contiguous over slots so one memset covers a batch)
   {
     Carver z{nullptr};
-    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(2 * M); z.take<int>(N_TK); z.take<unsigned>(XS_NS); z.take<unsigned>(XS_NS);
+    z.take<int>(LST_N_CNT); z.take<int>(2 * M + 2); z.take<int>(N_TK); z.take<unsigned>(XS_NS); z.take<unsigned>(XS_NS);
     L.zero_stride = z.off;
     L.zero_base = base ? base + cv.off : nullptr;
     for (int s = 0; s < n_slots; ++s) {
       Carver c2{base ? base + cv.off + s * L.zero_stride : nullptr};
       int* cnt = c2.take<int>(LST_N_CNT);
       int* ss = c2.take<int>(2 * M + 2);
-      int* cur = c2.take<int>(2 * M);
       int* tk = c2.take<int>(N_TK);
       unsigned* shi = c2.take<unsigned>(XS_NS);
       unsigned* srh = c2.take<unsigned>(XS_NS);
-      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].cursor = cur; (*out)[s].tk = tk; (*out)[s].surf_hi = shi; (*out)[s].surf_rhi = srh; }
+      if (out) { (*out)[s].cnt = cnt; (*out)[s].sensor_start = ss; (*out)[s].tk = tk; (*out)[s].surf_hi = shi; (*out)[s].surf_rhi = srh; }
     }
     cv.off += L.zero_stride * n_slots;
   }
@@ -140,7 +139,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   }
   for (int s = 0; s < n_slots; ++s) {
     Slot t{};
-    t.epoch_dev = cv.take<unsigned>(4); t.tmp_ok = cv.take<int2>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
+    t.epoch_dev = cv.take<unsigned>(4); t.tmp_a = cv.take<float4>(k.max_hits); t.tmp_k = cv.take<int>(k.max_hits); t.hit = cv.take<float4>(k.max_hits); t.hit_orig = cv.take<int>(k.max_hits);
     t.md_rec = cv.take<MdRec>(k.max_md);
     t.md_hits = cv.take<int2>(k.max_md); t.md_modt = cv.take<int>(k.max_md);
     t.md_pos = cv.take<float4>(k.max_md); t.md_cw = cv.take<float2>(k.max_md); t.md_aux = cv.take<float4>(k.max_md); t.md_start = cv.take<int>(M + 8);
@@ -166,7 +165,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
     if (out) {
       Slot& d = (*out)[s];
-      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.cursor = d.cursor; t.tk = d.tk; t.surf_hi = d.surf_hi; t.surf_rhi = d.surf_rhi; t.surf_lo = d.surf_lo; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
+      t.cnt = d.cnt; t.sensor_start = d.sensor_start; t.tk = d.tk; t.surf_hi = d.surf_hi; t.surf_rhi = d.surf_rhi; t.surf_lo = d.surf_lo; t.win5 = d.win5; t.win3 = d.win3; t.md_head = d.md_head; t.hit_head = d.hit_head;
       d = t;
     }
   }

@@ -61,7 +61,6 @@ struct Slot {
   unsigned* epoch_dev;      // run counter of the slot (not cleared): validates the look-back status words of a run
   int* cnt;                 // [LST_N_CNT]
   int* sensor_start;        // [2M+1] histogram, then exclusive scan in place
-  int* cursor;              // [2M]
   int* tk;                  // [N_TK] internal work tickets
   unsigned* surf_hi;        // [XS_NS] float bits: largest reference coordinate (r barrel, |z| endcap) of the MD anchors of a surface
   unsigned* surf_rhi;       // [XS_NS] float bits: largest anchor r of a surface
@@ -72,7 +71,7 @@ struct Slot {
   int* hit_head;            // [max_hits] head of the list of (TC row, slot) entries holding this ORIGINAL hit (f1)
   unsigned* surf_lo;        // [XS_NS] float bits: smallest reference coordinate of the MD anchors of a surface
   // a0
-  int2* tmp_ok; float4* hit; int* hit_orig;
+  float4* tmp_a; int* tmp_k; float4* hit; int* hit_orig;     // tmp_a / tmp_k: (x, y, z, original index) and sensor key, sensor by sensor in arrival order
   // a1
   MdRec* md_rec; int2* md_hits; int* md_modt; float4* md_pos; float2* md_cw; float4* md_aux; int* md_start;
   // a2
@@ -253,10 +252,22 @@ __global__ void k_hist(const Slot* __restrict__ slots, Geo geo) {
   const Slot& s = slots[blockIdx.y];
   if (blockIdx.x == 0 && threadIdx.x == 0) *s.epoch_dev = (*s.epoch_dev % 0x3FFFFFFFu) + 1u;   // first kernel of a run
   const unsigned S = 2u * geo.n_modules;
-  LST_FOR_ITEMS(i, s.n_hits) {
-    const unsigned key = hit_key(s, i);
-    if (key >= S) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_BAD_KEY);
-    else atomicAdd(s.sensor_start + key, 1);
+  const int nh = s.n_hits, st = gridDim.x * blockDim.x;
+  for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < nh; i0 += 4 * st) {      // four hits per thread in flight
+    unsigned key[4];
+    int slot[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int i = i0 + u * st; key[u] = i < nh ? hit_key(s, i) : 0xFFFFFFFFu; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) slot[u] = key[u] < S ? atomicAdd(s.sensor_start + key[u], 1) : -1;      // arrival slot in the sensor
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * st;
+      if (i < nh) {
+        if (key[u] >= S) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_BAD_KEY);
+        else s.hit_orig[i] = slot[u];                                      // (hit_orig is free until k_rank)
+      }
+    }
   }
   if (geo.has_layer) {      // a6 with crossing keys: the derived pLS quantities in input order, once (they depend on the inputs only)
     LST_FOR_ITEMS(p, s.n_pls) {
@@ -274,9 +285,21 @@ __global__ void k_scatter(const Slot* __restrict__ slots, Geo geo) {
   pdl_begin();
   const Slot& s = slots[blockIdx.y];
   const unsigned S = 2u * geo.n_modules;
-  LST_FOR_ITEMS(i, s.n_hits) {
-    const unsigned key = hit_key(s, i);
-    if (key < S) s.tmp_ok[s.sensor_start[key] + atomicAdd(s.cursor + key, 1)] = make_int2(i, (int)key);
+  const int nh = s.n_hits, st = gridDim.x * blockDim.x;
+  for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < nh; i0 += 4 * st) {      // four hits per thread in flight
+    unsigned key[4];
+    int pos[4];
+    float4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * st;
+      key[u] = 0xFFFFFFFFu; pos[u] = 0; v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (i < nh) { key[u] = hit_key(s, i); pos[u] = s.hit_orig[i]; v[u] = make_float4(s.in_x[i], s.in_y[i], s.in_z[i], __int_as_float(i)); }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (key[u] < S) pos[u] += s.sensor_start[key[u]];            // hit_orig[i]: the hit's arrival slot in its sensor (k_hist)
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (key[u] < S) { s.tmp_a[pos[u]] = v[u]; s.tmp_k[pos[u]] = (int)key[u]; }
   }
 }
 // stable order inside a sensor: rank of a hit = number of hits of the same sensor with a smaller
@@ -285,16 +308,16 @@ __global__ void k_rank(const Slot* __restrict__ slots) {
   pdl_begin();
   const Slot& s = slots[blockIdx.y];
   const int n = s.cnt[LST_CNT_HIT];
-  const int2* __restrict__ ok = s.tmp_ok;
+  const float4* __restrict__ ta = s.tmp_a;
   LST_FOR_ITEMS(p, n) {
-    const int2 me = ok[p];
-    const int o = me.x, key = me.y;
-    const float x = s.in_x[o], y = s.in_y[o], z = s.in_z[o];        // independent of the rank: issued first
+    const float4 me = ta[p];
+    const int key = s.tmp_k[p];
+    const int o = __float_as_int(me.w);
     const int b = s.sensor_start[key], e = s.sensor_start[key + 1];
     int rank = 0;
-    for (int q = b; q < e; ++q) rank += (ok[q].x < o);
+    for (int q = b; q < e; ++q) rank += (__float_as_int(ta[q].w) < o);
     const int d = b + rank;
-    s.hit[d] = make_float4(x, y, z, fq(fa(fm(x, x), fm(y, y))));   // r as SPEC.md 4.1 computes it
+    s.hit[d] = make_float4(me.x, me.y, me.z, fq(fa(fm(me.x, me.x), fm(me.y, me.y))));   // r as SPEC.md 4.1 computes it
     s.hit_orig[d] = o;
   }
 }
