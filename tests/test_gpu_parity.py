@@ -428,3 +428,86 @@ def test_graphs_on_off_and_determinism(P, geo_full):
     lst.close()
     assert all(np.array_equal(ref[(n, k)], v.view(np.uint8)) for n in names for k, v in out[n].items())
     parity.compare(geo_full, w, ev, out)
+
+
+def _odd_pls(ev, rng):
+    """Overwrite a fifth of the seeds with values the a6 bins cannot hold (overflow bins): pT below the bucketed range, |z0| > 20 cm,
+    |cot| > 8, q = 0, and a few that curl up before the outer layers (r h > 0.88 there)."""
+    n = ev.n_pls
+    idx = rng.choice(n, max(5, n // 5), replace=False)
+    for k, p in enumerate(idx):
+        pt = float(np.hypot(ev.pls_px[p], ev.pls_py[p]))
+        mode = k % 5
+        if mode == 0: s = 0.5 / pt; ev.pls_px[p] *= s; ev.pls_py[p] *= s; ev.pls_pz[p] *= s      # pT = 0.5 GeV: h > HMAX
+        elif mode == 1: ev.pls_z0[p] = np.float32(25.0 if k % 2 else -31.0)
+        elif mode == 2: ev.pls_pz[p] = np.float32(9.5 * pt * (1 if k % 2 else -1))
+        elif mode == 3: ev.pls_q[p] = 0
+        else: s = 0.78 / pt; ev.pls_px[p] *= s; ev.pls_py[p] *= s; ev.pls_pz[p] *= s           # pT = 0.78 GeV: still bucketed, r h up to 0.8
+    return ev
+
+
+def test_a6_generic_buckets_relabelled_layers_and_odd_seeds(P, geo_full):
+    """a6 has two exact prefilters: per-surface crossing keys (geometry with a layer per module) and the generic (h, zeta, psi)
+    buckets (no layers, or LST_XS=0).  Both must give the oracle's lists: with the real layers, without layers, with every module
+    relabelled to ONE layer (surfaces 87 cm / 134 cm thick: windows open up, nothing may be lost), with a layer labelling that mixes
+    two barrel layers, and with seeds the bins cannot hold."""
+    import dataclasses, os
+    w = xavier_weights(3)
+    rng = np.random.default_rng(5)
+    ev = _odd_pls(config_event(geo_full, 2, seed=31), rng)
+    base = parity.compare(geo_full, w, ev, _run_one(P, geo_full, w, ev))
+    assert base["tc"] > 2000
+    g_none = dataclasses.replace(geo_full, layer=None)
+    parity.compare(g_none, w, ev, _run_one(P, g_none, w, ev))
+    g_one = dataclasses.replace(geo_full, layer=np.ones_like(geo_full.layer))
+    parity.compare(g_one, w, ev, _run_one(P, g_one, w, ev))
+    mixed = geo_full.layer.copy()
+    mixed[mixed == 3] = 2                      # layers 2 and 3 share a surface: 15 cm thick
+    mixed[mixed == 9] = 8                      # two disks share a surface: 29 cm thick
+    g_mix = dataclasses.replace(geo_full, layer=mixed)
+    parity.compare(g_mix, w, ev, _run_one(P, g_mix, w, ev))
+    os.environ["LST_XS"] = "0"
+    try:
+        parity.compare(geo_full, w, ev, _run_one(P, geo_full, w, ev))
+    finally:
+        del os.environ["LST_XS"]
+    ev4 = _odd_pls(config_event(geo_full, 4, seed=207, pileup=100), rng)          # displaced tracks as well
+    parity.compare(geo_full, w, ev4, _run_one(P, geo_full, w, ev4))
+    parity.compare(g_one, w, ev4, _run_one(P, g_one, w, ev4))
+
+
+def test_a2_module_with_more_than_eight_nonempty_runs(P, geo_barrel):
+    """a2 reads a per-module column table of up to 8 non-empty runs written by k_md_finish; a module whose CSR row holds more
+    non-empty runs builds its run table in the sweep.  Occupied layer-1 modules get every second OCCUPIED module beyond layer 1
+    as extra columns, so their rows hold 9 .. 32 non-empty runs (the 64+ case is test_csr_row_with_many_runs)."""
+    import dataclasses
+    w = xavier_weights(1)
+    ev = make_event(geo_barrel, 84, origin_muons=12)
+    l2 = int(geo_barrel.barrel_base[1])
+    occ = sorted(set(int(k) >> 1 for k in ev.key))
+    occupied_l1 = [m for m in occ if m < l2]
+    beyond = [m for m in occ if m >= l2]
+    extra = set(m for m in beyond if (m + 1) not in set(beyond) or m % 2 == 0)
+    rows = []
+    for m in range(geo_barrel.n_modules):
+        cols = set(geo_barrel.conn_col[geo_barrel.conn_rowptr[m]:geo_barrel.conn_rowptr[m + 1]].tolist())
+        if m in occupied_l1:
+            cols |= extra
+        rows.append(sorted(cols))
+    rowptr = np.zeros(geo_barrel.n_modules + 1, np.int32)
+    rowptr[1:] = np.cumsum([len(c) for c in rows])
+    g2 = dataclasses.replace(geo_barrel, conn_rowptr=rowptr, conn_col=np.array([c for r in rows for c in r], np.int32))
+    out = _run_one(P, g2, w, ev)
+    c = parity.compare(g2, w, ev, out)
+    # non-empty runs of the occupied layer-1 rows, from the oracle's own MD list
+    md_mod = set((out["md"]["modt"] >> 2).tolist())
+    n_ne = []
+    for m in occupied_l1:
+        r = rows[m]
+        runs = [[r[0]]]
+        for a, b in zip(r, r[1:]):
+            if b == a + 1: runs[-1].append(b)
+            else: runs.append([b])
+        n_ne.append(sum(1 for run in runs if any(x in md_mod for x in run)))
+    assert max(n_ne) > 8, max(n_ne)
+    assert c["ls"] > 40
