@@ -192,21 +192,36 @@ __device__ __forceinline__ void md_sweep_body(const Slot& s, const Geo& geo, con
       W.P[i] = inc - cells; W.par[i] = make_int4(lb, ub, n_up, (my_m << 2) | mt); W.inv[i] = rcp_fast((float)n_up);
     }
     __syncwarp();
-    for (int F = 0; F < total; F += 32) {
-      const int f = min(F + lane, total - 1);
+    if (total > 0) {
+      // lane's cell of sweep F: module k of the group (first sweep: binary search; later sweeps: k only moves forward), then
+      // (i, j) inside the module.  The hits of the next sweep are loaded while the current one is tested.
       int k = 0;
+      {
+        const int f = min(lane, total - 1);
 #pragma unroll
-      for (int step = 16; step > 0; step >>= 1)
-        if (W.P[k + step] <= f) k += step;
-      const int4 pr = W.par[k];
-      const int loc = f - W.P[k];
-      int i = (int)(((float)loc + 0.5f) * W.inv[k]);
-      int j = loc - i * pr.z;
-      if (j < 0) { --i; j += pr.z; } else if (j >= pr.z) { ++i; j -= pr.z; }
-      const int p_lo = pr.x + i, p_up = pr.y + j;
-      const float4 h1 = __ldg(hit + p_lo), h2 = __ldg(hit + p_up);
-      const bool pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, pr.w & 3) && (F + lane < total);
-      md_push<DIRECT>(s, W, pre, p_lo, p_up, pr.w, qn, sn, lane, lt, carry_row, carry_n, cap);
+        for (int step = 16; step > 0; step >>= 1)
+          if (W.P[k + step] <= f) k += step;
+      }
+      auto decode = [&](int F, int& p_lo, int& p_up, int& mtm) {
+        const int f = min(F + lane, total - 1);
+        while (W.P[k + 1] <= f) ++k;
+        const int4 pr = W.par[k];
+        const int loc = f - W.P[k];
+        int i = (int)(((float)loc + 0.5f) * W.inv[k]);
+        int j = loc - i * pr.z;
+        if (j < 0) { --i; j += pr.z; } else if (j >= pr.z) { ++i; j -= pr.z; }
+        p_lo = pr.x + i; p_up = pr.y + j; mtm = pr.w;
+      };
+      int n_lo_, n_up_, n_mt;
+      decode(0, n_lo_, n_up_, n_mt);
+      float4 n1 = __ldg(hit + n_lo_), n2 = __ldg(hit + n_up_);
+      for (int F = 0; F < total; F += 32) {
+        const int p_lo = n_lo_, p_up = n_up_, mtm = n_mt;
+        const float4 h1 = n1, h2 = n2;
+        if (F + 32 < total) { decode(F + 32, n_lo_, n_up_, n_mt); n1 = __ldg(hit + n_lo_); n2 = __ldg(hit + n_up_); }
+        const bool pre = md_prefilter(h1.x, h1.y, h1.z, h1.w, h2.x, h2.y, h2.z, h2.w, mtm & 3) && (F + lane < total);
+        md_push<DIRECT>(s, W, pre, p_lo, p_up, mtm, qn, sn, lane, lt, carry_row, carry_n, cap);
+      }
     }
     // modules too large for the flat space (only in pathological events): alone, (i, j) advanced incrementally
     unsigned todo = __ballot_sync(0xffffffffu, big);
