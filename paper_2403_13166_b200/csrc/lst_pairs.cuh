@@ -28,7 +28,8 @@ namespace lst {
 constexpr int PAIR_WARPS = 4;        // warps per block
 constexpr int Q_CAP = 64;            // survivor queue / record staging per warp (drained / flushed at >= 32)
 constexpr int RUN_CAP = 32;          // runs of a CSR row cached per warp at a time
-constexpr int LS_ROWS = 8;           // consecutive MD rows a warp takes at a time
+constexpr int LS_ROWS = 16;          // consecutive MD rows a warp takes at a time: 16 in batched launches (measured 4 / 8 / 16 / 32 rows: 119 / 90 / 83 / 86 us),
+                                     // 8 in launches of a few events, where more warps find work (single event: 27 vs 34 us)
 constexpr int LS_TAB = 8;            // non-empty runs per module held by the precomputed column table
 constexpr int MD_BIG = 1 << 20;      // modules with more cells than this are swept alone (64-bit sweep counter)
 
@@ -370,6 +371,7 @@ struct LsWarp {
   float4 a_pos[LS_ROWS], a_aux[LS_ROWS];      // the rows of the current chunk: anchor, prefilter record (.w = -2 / r)
   __align__(16) int tab[LS_ROWS][2 * LS_TAB]; // ... and the column table of each row's module
   int cnt[LS_ROWS];                           // LSs found so far in each row of the chunk
+  int rmask;                                  // rows per chunk - 1
   int q_a[Q_CAP], q_b[Q_CAP];
   LsRec st[Q_CAP];
 };
@@ -414,11 +416,11 @@ __device__ __forceinline__ int ls_drain(const Slot& s, LsWarp& W, int n, int sn,
   const unsigned peers = __match_any_sync(0xffffffffu, a) & mask;
   if (pass) {
     const int before = __popc(peers & lt);
-    LsRec r; r.a = a; r.b = b; r.seq = W.cnt[a & (LS_ROWS - 1)] + before; r.c = c;
+    LsRec r; r.a = a; r.b = b; r.seq = W.cnt[a & W.rmask] + before; r.c = c;
     W.st[sn + __popc(mask & lt)] = r;
   }
   __syncwarp();
-  if (pass && (peers >> lane) >> 1 == 0u) W.cnt[a & (LS_ROWS - 1)] += __popc(peers);      // last passing cell of its row in this batch
+  if (pass && (peers >> lane) >> 1 == 0u) W.cnt[a & W.rmask] += __popc(peers);      // last passing cell of its row in this batch
   return sn + __popc(mask);
 }
 
@@ -552,7 +554,7 @@ __device__ __forceinline__ int ls_tab_column(const int* tab, int t) {
   return t + tab[LS_TAB + r];
 }
 
-// The chunks (LS_ROWS consecutive MDs = rows) of ALL the events of a launch are handed out by one atomic ticket (kept in the
+// The chunks (`rows` consecutive MDs, 8 or 16) of ALL the events of a launch are handed out by one atomic ticket (kept in the
 // first slot; the next ticket is fetched while the current chunk is swept), so every warp of the persistent grid works until
 // the whole launch is done.  Rows of the same module share their columns, so a chunk is cut into module segments and every
 // segment is swept columns-outer / rows-inner: the 32 column MDs of a step are loaded once into registers and tested against
@@ -564,14 +566,15 @@ __device__ __forceinline__ int ls_tab_column(const int* tab, int t) {
 // row table is written once, coalesced.  Which warp sweeps which chunk does not matter: a record carries its row and its
 // rank in the row.
 template <bool DIRECT>
-__device__ __forceinline__ void ls_sweep_body(const Slot* __restrict__ slots, int n_ev, const Geo& geo, const Caps& caps, LsWarp* Wall) {
+__device__ __forceinline__ void ls_sweep_body(const Slot* __restrict__ slots, int n_ev, int rows, const Geo& geo, const Caps& caps, LsWarp* Wall) {
   const int lane = threadIdx.x & 31;
   LsWarp& W = Wall[threadIdx.x >> 5];
   const unsigned lt = lanemask_lt();
   const int cap = caps.max_ls;
   // chunks of events [0, lane] (inclusive scan over the events of the launch; at most 32 events per ticket)
   int cum = 0;
-  if (lane < n_ev) cum = (slots[lane].cnt[LST_CNT_MD] + LS_ROWS - 1) / LS_ROWS;
+  if (lane == 0) W.rmask = rows - 1;
+  if (lane < n_ev) cum = (slots[lane].cnt[LST_CNT_MD] + rows - 1) / rows;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, cum, d); if (lane >= d) cum += t; }
   int* ticket = slots[0].tk + (DIRECT ? TK_LS_DIRECT : TK_LS_SWEEP);
@@ -585,13 +588,13 @@ __device__ __forceinline__ void ls_sweep_body(const Slot* __restrict__ slots, in
     if (ev >= n_ev) break;
     if (lane == 0) next = atomicAdd(ticket, 1);
     const int first = __shfl_sync(0xffffffffu, cum, max(ev - 1, 0));
-    const int a0 = (T - (ev ? first : 0)) * LS_ROWS;
+    const int a0 = (T - (ev ? first : 0)) * rows;
     if (ev != ev_prev && sn) { __syncwarp(); ls_flush<DIRECT>(slots[ev_prev], W, sn, lane, cap); sn = 0; __syncwarp(); }      // records go to their own event
     ev_prev = ev;
     const Slot& s = slots[ev];
     const float4* __restrict__ mpos = s.md_pos;
     const float4* __restrict__ maux = s.md_aux;
-    const int n_rows = min(LS_ROWS, s.cnt[LST_CNT_MD] - a0);
+    const int n_rows = min(rows, s.cnt[LST_CNT_MD] - a0);
     int my_m = -1;
     __syncwarp();
     if (lane < n_rows) {
@@ -601,9 +604,12 @@ __device__ __forceinline__ void ls_sweep_body(const Slot* __restrict__ slots, in
     }
     if (lane < LS_ROWS) W.cnt[lane] = 0;
     {
-      static_assert(LS_ROWS * 4 <= 32 && LS_TAB == 8, "one int4 of the tables per lane");
-      const int row = lane >> 2, m_r = __shfl_sync(0xffffffffu, my_m, row);
-      if (m_r >= 0) reinterpret_cast<int4*>(W.tab[row])[lane & 3] = __ldg(reinterpret_cast<const int4*>(s.ls_tab + 2 * LS_TAB * (size_t)m_r) + (lane & 3));
+      static_assert(LS_TAB == 8, "four int4 per table");
+#pragma unroll
+      for (int r0 = 0; r0 < LS_ROWS; r0 += 8) if (r0 < rows) {           // one int4 of the tables per lane and round
+        const int row = r0 + (lane >> 2), m_r = __shfl_sync(0xffffffffu, my_m, row);
+        if (m_r >= 0) reinterpret_cast<int4*>(W.tab[row])[lane & 3] = __ldg(reinterpret_cast<const int4*>(s.ls_tab + 2 * LS_TAB * (size_t)m_r) + (lane & 3));
+      }
     }
     const int prev_m = __shfl_up_sync(0xffffffffu, my_m, 1);
     const unsigned segs = __ballot_sync(0xffffffffu, lane < n_rows && (lane == 0 || my_m != prev_m));    // first rows of the module segments
@@ -660,7 +666,7 @@ __device__ __forceinline__ void ls_sweep_body(const Slot* __restrict__ slots, in
 __global__ void __launch_bounds__(PAIR_WARPS * 32, LS_MIN_BLOCKS) k_ls_sweep(const Slot* __restrict__ slots, int n_ev, Geo geo, Caps caps) {
   pdl_begin();
   __shared__ LsWarp Wall[PAIR_WARPS];
-  ls_sweep_body<false>(slots + 32 * blockIdx.y, min(32, n_ev - 32 * (int)blockIdx.y), geo, caps, Wall);
+  ls_sweep_body<false>(slots + 32 * blockIdx.y, min(32, n_ev - 32 * (int)blockIdx.y), n_ev < 8 ? 8 : LS_ROWS, geo, caps, Wall);
 }
 
 // a2 finish (ls_start holds the exclusive scan of the per-row counts by now): record -> ls_start[a] + seq; on capacity
@@ -669,7 +675,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_ls_finish(const Slot* __res
   pdl_begin();
   __shared__ LsWarp Wall[PAIR_WARPS];
   const Slot& s = slots[blockIdx.y];
-  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) { ls_sweep_body<true>(slots + blockIdx.y, 1, geo, caps, Wall); return; }
+  if (s.cnt[CNT_STATUS] & LST_ST_OVF_LS) { ls_sweep_body<true>(slots + blockIdx.y, 1, 8, geo, caps, Wall); return; }
   const int n_rec = min(s.cnt[LST_CNT_FILL_LS], caps.max_ls);
   LST_FOR_ITEMS(j, n_rec) {
     const LsRec r = s.ls_rec[j];
