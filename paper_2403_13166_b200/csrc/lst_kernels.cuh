@@ -1140,7 +1140,8 @@ __global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ s
         int mine = hx[0];
 #pragma unroll
         for (int a = 1; a < 5; ++a) mine = (slot == a) ? hx[a] : mine;
-        for (int e = s.hit_head[mine]; e >= 0; e = s.tc_next[e]) {
+        for (int e = s.hit_head[mine], en; e >= 0; e = en) {
+          en = s.tc_next[e];                          // next link in flight while this candidate is looked at
           const int y = e / 10;
           if (y == x) continue;
           const int ty = s.tc[3 * y];

@@ -59,13 +59,23 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t3_one(const Slot* __restrict__ s
         A = make_pt(s.md_pos[ab.x], s.md_modt[ab.x] & 3);
         B = make_pt(s.md_pos[ab.y], s.md_modt[ab.y] & 3);
         c0 = s.ls_c[l0];
+        // partners one and two steps ahead are in flight while the current one is evaluated (index, then its MD)
+        int cn = s.ls_ab[j0].y, cnn = (j0 + 1 < j1) ? s.ls_ab[j0 + 1].y : 0;
+        float4 pn = s.md_pos[cn];
+        int mn = s.md_modt[cn];
+        float ln = s.ls_c[j0];
         for (int j = j0; j < j1; ++j) {
-          const int cidx = s.ls_ab[j].y;
-          const Pt C = make_pt(s.md_pos[cidx], s.md_modt[cidx] & 3);
+          const int cidx = cn;
+          const Pt C = make_pt(pn, mn & 3);
+          const float lcj = ln;
+          if (j + 1 < j1) {
+            cn = cnn; pn = s.md_pos[cn]; mn = s.md_modt[cn]; ln = s.ls_c[j + 1];
+            if (j + 2 < j1) cnn = s.ls_ab[j + 2].y;
+          }
           float k;
           if (!triplet_eval(A, B, C, k)) continue;
           if (!(fabsf(fs(c0, k)) <= LST_C_TOL3)) continue;                                  // T3
-          if (!(fabsf(fs(s.ls_c[j], k)) <= LST_C_TOL3)) continue;
+          if (!(fabsf(fs(lcj, k)) <= LST_C_TOL3)) continue;
 #pragma unroll
           for (int q = 0; q < TUPLE_STASH; ++q)
             if (np == q) { st_j[q] = j; st_c[q] = cidx; st_k[q] = k; }
@@ -124,7 +134,6 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ s
   const int cap = caps.max_t5c;
   // T3s whose inner MD is a = [t3_start[a], t3_start[a+1]) with t3_start[a] = t3_off[ls_start[a]]: the table is an output
   // (lst_get); this kernel itself goes through t3_off / ls_start so that it need not wait for it
-  LST_FOR_ITEMS(a, s.cnt[LST_CNT_MD] + 1) s.t3_start[a] = s.t3_off[s.ls_start[a]];
   while (true) {
     if (threadIdx.x == 0) s_tile = atomicAdd(s.cnt + LST_CNT_DYN_T5, 1);
     __syncthreads();
@@ -143,9 +152,15 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ s
       if (v0 < v1) {
         B = make_pt(s.md_pos[abc.y], s.md_modt[abc.y] & 3);
         C = make_pt(s.md_pos[abc.z], s.md_modt[abc.z] & 3);
+        int dn = s.t3_abc[v0].y, dnn = (v0 + 1 < v1) ? s.t3_abc[v0 + 1].y : 0;           // partners ahead in flight, as in a3
+        float4 pn = s.md_pos[dn];
+        int mn = s.md_modt[dn];
         for (int v = v0; v < v1; ++v) {
-          const int d = s.t3_abc[v].y;
-          const Pt D = make_pt(s.md_pos[d], s.md_modt[d] & 3);
+          const Pt D = make_pt(pn, mn & 3);
+          if (v + 1 < v1) {
+            dn = dnn; pn = s.md_pos[dn]; mn = s.md_modt[dn];
+            if (v + 2 < v1) dnn = s.t3_abc[v + 2].y;
+          }
           float kbr;
           if (!triplet_eval(B, C, D, kbr)) continue;                                        // Q1, Q2
 #pragma unroll
@@ -197,6 +212,7 @@ __global__ void __launch_bounds__(TUPLE_TPB) k_t5_one(const Slot* __restrict__ s
     }
     __syncthreads();
   }
+  LST_FOR_ITEMS(a, s.cnt[LST_CNT_MD] + 1) s.t3_start[a] = s.t3_off[s.ls_start[a]];      // (after the tiles: nobody here waits for it)
 }
 
 }  // namespace lst
