@@ -146,13 +146,13 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.ls_rec = cv.take<LsRec>(k.max_ls);
     t.ls_tab = cv.take<int>(16 * (size_t)M); t.ls_start = cv.take<int>(k.max_md + 8); t.ls_ab = cv.take<int2>(k.max_ls); t.ls_c = cv.take<float>(k.max_ls);
     t.chain_sensor = cv.take<unsigned long long>(2 * (size_t)M / SCAN_TILE + 4); t.chain_md = cv.take<unsigned long long>(M / SCAN_TILE + 4);
-    t.chain_ls = cv.take<unsigned long long>(k.max_md / SCAN_TILE + 4); t.chain_t5s = cv.take<unsigned long long>(k.max_t5c / SCAN_TILE + 4);
+    t.chain_ls = cv.take<unsigned long long>(k.max_md / SCAN_TILE + 4); t.chain_t5s = cv.take<unsigned long long>(k.max_t5c / 128 + 4);
     t.chain_t3 = cv.take<unsigned long long>(k.max_ls / TUPLE_TPB + 4); t.chain_t5 = cv.take<unsigned long long>(k.max_t3 / TUPLE_TPB + 4);
     t.t3_off = cv.take<int>(k.max_ls + 8); t.t3_abc = cv.take<int4>(k.max_t3); t.t3_l1 = cv.take<int>(k.max_t3);
     t.t3_k = cv.take<float>(k.max_t3); t.t3_start = cv.take<int>(k.max_md + 8);
     t.t5_off = cv.take<int>(k.max_t3 + 8); t.t5c_md = cv.take<int>(5 * (size_t)k.max_t5c); t.t5c_t3 = cv.take<int2>(k.max_t5c);
     t.t5c_curv = cv.take<float>(3 * (size_t)k.max_t5c); t.t5c_feat = cv.take<float>((size_t)N_FEAT_MAX * k.max_t5c);
-    t.t5c_score = cv.take<float>(k.max_t5c); t.t5c_pass = cv.take<int>(k.max_t5c); t.t5_scan = cv.take<int>(k.max_t5c + 8);
+    t.t5c_score = cv.take<float>(k.max_t5c); t.t5c_pass = cv.take<int>(k.max_t5c);
     t.t5_list = cv.take<int>(k.max_t5);
     t.pls_a = cv.take<float4>(k.max_pls); t.pls_b = cv.take<float2>(k.max_pls); t.pls_key = cv.take<int>(k.max_pls);
     t.pls_sa = cv.take<float4>(k.max_pls); t.pls_sb = cv.take<float2>(k.max_pls); t.pls_sidx = cv.take<int>(k.max_pls); t.pls_pos = cv.take<int>(k.max_pls); t.pls_taken = cv.take<int>(k.max_pls);
@@ -190,7 +190,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 21;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 20;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -263,7 +263,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_sensor, 0, sizeof(unsigned long long) * (2 * (size_t)M / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (M / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (c->caps.max_md / SCAN_TILE + 4));
-    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5s, 0, sizeof(unsigned long long) * (c->caps.max_t5c / SCAN_TILE + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5s, 0, sizeof(unsigned long long) * (c->caps.max_t5c / 128 + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_tcc, 0, sizeof(unsigned long long) * (c->caps.max_tc / TCC_ROWS + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t3, 0, sizeof(unsigned long long) * (c->caps.max_ls / TUPLE_TPB + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
@@ -377,14 +377,13 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   launch(pdl, k_t3_one, GL, BT, 0, st, sl, k); LST_MARK();
   launch(pdl, k_t5_one, GL, BT, 0, st, sl, k); LST_MARK();
   {
-#define LST_DNN(NI, NH_) launch(pdl, k_dnn<NI, NH_>, G, B128, 0, st, sl, g)
+#define LST_DNN(NI, NH_) launch(pdl, k_dnn<NI, NH_>, G, B128, 0, st, sl, g, k.max_t5)
     const int nh = g.n_hidden;
     if (g.n_feat == N_FEAT) { if (nh == 1) LST_DNN(N_FEAT, 1); else if (nh == 2) LST_DNN(N_FEAT, 2); else if (nh == 3) LST_DNN(N_FEAT, 3); else LST_DNN(N_FEAT, 4); }
     else { if (nh == 1) LST_DNN(N_FEAT_MAX, 1); else if (nh == 2) LST_DNN(N_FEAT_MAX, 2); else if (nh == 3) LST_DNN(N_FEAT_MAX, 3); else LST_DNN(N_FEAT_MAX, 4); }
 #undef LST_DNN
   }
   LST_MARK();
-  launch(pdl, k_scan_lb<SCAN_T5>, GS, BS, 0, st, sl, g, k); LST_MARK();
   if (fork) { if (bad(c, cudaStreamWaitEvent(st, c->ev_join, 0))) return LST_ECUDA; }
   else if (xs) launch(false, k_pls_cross, GX, dim3(XS_TPB), XS_SMEM, st, sl, k.max_pls);
   else launch(false, k_pls_bin, G1, dim3(1024), PLS_BIN_SMEM, st, sl);
@@ -453,7 +452,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
       "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_sweep", "a1.scan", "a1.md_finish", "a2.ls_sweep", "a2.scan", "a2.ls_finish",
-      "a3.t3", "a4.t5", "a5.dnn", "a5.scan", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit", "f1.tc_tuples", "f1.tc_clean"};
+      "a3.t3", "a4.t5", "a5.dnn", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit", "f1.tc_tuples", "f1.tc_clean"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 

@@ -44,7 +44,7 @@ struct Geo {   // device copies, shared by all slots
 // a6 surfaces: a barrel layer, or one side of an endcap disk (lst_kernels.cuh, "crossing keys")
 constexpr int XS_NS = 32, XS_NP = 256, XS_NZ = 16, XS_REG = XS_NP * XS_NZ, XS_BINS = XS_REG + 1;     // + the surface's overflow bin
 
-enum { TK_LS_SWEEP = 0, TK_LS_DIRECT, TK_MD_SWEEP, TK_MD_DIRECT, N_TK = 16 };
+enum { TK_LS_SWEEP = 0, TK_LS_DIRECT, TK_MD_SWEEP, TK_MD_DIRECT, TK_DNN, N_TK = 16 };
 
 struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
 
@@ -83,7 +83,7 @@ struct Slot {
   int* t3_off; int4* t3_abc; int* t3_l1; float* t3_k; int* t3_start;
   // a4 / a5
   int* t5_off; int* t5c_md; int2* t5c_t3; float* t5c_curv; float* t5c_feat; float* t5c_score; int* t5c_pass;
-  int* t5_scan; int* t5_list;
+  int* t5_list;
   // a6
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
   int* xs_key; int* xs_start; float4* xs_ent;     // pLS crossing-key bins per surface: [XS_NS][XS_BINS + 1] starts, [XS_NS][2 max_pls] entries (cx, cy, h, pLS)
@@ -164,10 +164,10 @@ __device__ __forceinline__ int chain_exclusive(unsigned long long* st, int tile,
 // as a multi-block single pass (tiles of SCAN_TILE entries, look-back across tiles).  The unclamped total and the
 // overflow bit go to the slot's counters.
 //   SENSOR: hits per sensor -> sensor_start            MDROW: MDs per module -> md_start
-//   LSROW : LSs per inner MD -> ls_start               T5   : pass flags -> positions in the T5 list (+ the list itself)
+//   LSROW : LSs per inner MD -> ls_start               (the T5 list is compacted inside k_dnn, by the same look-back)
 // ------------------------------------------------------------------------------------------------
 constexpr int SCAN_TPB = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_TPB * SCAN_ITEMS;
-enum { SCAN_SENSOR = 0, SCAN_MDROW, SCAN_LSROW, SCAN_T5 };
+enum { SCAN_SENSOR = 0, SCAN_MDROW, SCAN_LSROW };
 
 template <int MODE>
 __global__ void __launch_bounds__(SCAN_TPB) k_scan_lb(const Slot* __restrict__ slots, Geo geo, Caps caps) {
@@ -180,8 +180,7 @@ __global__ void __launch_bounds__(SCAN_TPB) k_scan_lb(const Slot* __restrict__ s
   int* a; int n, cap, icnt, iraw, itk; unsigned ovf; unsigned long long* chain;
   if (MODE == SCAN_SENSOR) { a = s.sensor_start; n = 2 * geo.n_modules; cap = caps.max_hits; icnt = LST_CNT_HIT; iraw = -1; ovf = 0; itk = LST_CNT_TK_SENSOR; chain = s.chain_sensor; }
   else if (MODE == SCAN_MDROW) { a = s.md_start; n = geo.n_modules; cap = caps.max_md; icnt = LST_CNT_MD; iraw = LST_CNT_RAW_MD; ovf = LST_ST_OVF_MD; itk = LST_CNT_TK_MD; chain = s.chain_md; }
-  else if (MODE == SCAN_LSROW) { a = s.ls_start; n = cnt[LST_CNT_MD]; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; itk = LST_CNT_TK_LS; chain = s.chain_ls; }
-  else { a = s.t5_scan; n = cnt[LST_CNT_T5C]; cap = caps.max_t5; icnt = LST_CNT_T5; iraw = LST_CNT_RAW_T5; ovf = LST_ST_OVF_T5; itk = LST_CNT_TK_T5; chain = s.chain_t5s; }
+  else { a = s.ls_start; n = cnt[LST_CNT_MD]; cap = caps.max_ls; icnt = LST_CNT_LS; iraw = LST_CNT_RAW_LS; ovf = LST_ST_OVF_LS; itk = LST_CNT_TK_LS; chain = s.chain_ls; }
   const int n_tiles = (n + SCAN_TILE - 1) / SCAN_TILE + (n == 0);
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   while (true) {
@@ -220,11 +219,6 @@ __global__ void __launch_bounds__(SCAN_TPB) k_scan_lb(const Slot* __restrict__ s
     int o[SCAN_ITEMS];
 #pragma unroll
     for (int k = 0; k < SCAN_ITEMS; ++k) { o[k] = min(run, cap); run += v[k]; }
-    if (MODE == SCAN_T5) {        // T5 list = passing candidates in candidate order
-#pragma unroll
-      for (int k = 0; k < SCAN_ITEMS; ++k)
-        if (v[k] && i0 + k < n && o[k] < cap) s.t5_list[o[k]] = i0 + k;
-    }
     if (i0 + SCAN_ITEMS <= n) {
       *reinterpret_cast<int4*>(a + i0) = make_int4(o[0], o[1], o[2], o[3]);
       *reinterpret_cast<int4*>(a + i0 + 4) = make_int4(o[4], o[5], o[6], o[7]);
@@ -335,7 +329,7 @@ __device__ __forceinline__ float feat_radius(float c) { return log10f(fminf(__fd
 __device__ __forceinline__ float feat_pt(float c) { return log10f(__fmul_rn(LST_KAPPA, fminf(__fdiv_rn(1.0f, fabsf(c)), 1.0e5f))); }
 
 template <int NIN, int NH>
-__global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, Geo geo) {
+__global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, Geo geo, int max_t5) {
   pdl_begin();
   constexpr int PIN = (NIN + 3) & ~3;             // rows of W1 padded for float4 reads
   __shared__ __align__(16) float W1[N_HID * PIN];
@@ -357,9 +351,21 @@ __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, 
     for (int i = threadIdx.x; i <= N_HID; i += blockDim.x) W3[i] = p[i];
   }
   __syncthreads();
+  // tiles of 128 candidates by ticket; the T5 list (passing candidates in candidate order) is written here as well: block scan of
+  // the pass flags + look-back across tiles
+  __shared__ int s_tile, s_base, s_w[4];
   const Slot& s = slots[blockIdx.y];
+  const unsigned epoch = *s.epoch_dev;
   const int n = s.cnt[LST_CNT_T5C];
-  LST_FOR_ITEMS(i, n) {
+  const int n_tiles = (n + 127) / 128 + (n == 0);
+  while (true) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(s.tk + TK_DNN, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int i = tile * 128 + threadIdx.x;
+    int pass = 0;
+    if (i < n) {
     float x[PIN];
     if (NIN == N_FEAT) {
 #pragma unroll
@@ -428,10 +434,35 @@ __global__ void __launch_bounds__(128, 4) k_dnn(const Slot* __restrict__ slots, 
 #pragma unroll
     for (int j = 0; j < N_HID; ++j) y = fmaf(W3[j], h[j], y);
     const float score = __fdiv_rn(1.0f, 1.0f + expf(-y));
-    const int pass = score > 0.5f;
+    pass = score > 0.5f;
     s.t5c_score[i] = score;
     s.t5c_pass[i] = pass;
-    s.t5_scan[i] = pass;
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, pass);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) s_w[wid] = __popc(bal);
+    __syncthreads();
+    const int btot = s_w[0] + s_w[1] + s_w[2] + s_w[3];
+    int wbase = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) wbase += (q < wid) ? s_w[q] : 0;
+    if (wid == 0) {
+      const int b = chain_exclusive(s.chain_t5s, tile, btot, lane, epoch);
+      if (lane == 0) s_base = b;
+    }
+    __syncthreads();
+    const int base = s_base;
+    if (pass) {
+      const int o = base + wbase + __popc(bal & ((1u << lane) - 1u));
+      if (o < max_t5) s.t5_list[o] = i;
+    }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) {
+      const int total = base + btot;
+      s.cnt[LST_CNT_T5] = min(total, max_t5);
+      s.cnt[LST_CNT_RAW_T5] = total;
+      if (total > max_t5) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_T5);
+    }
+    __syncthreads();
   }
 }
 
