@@ -159,7 +159,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
     t.pls_bin_start = cv.take<int>(PLS_NBINS + 1); t.xs_key = cv.take<int>((size_t)XS_NS * k.max_pls); t.xs_start = cv.take<int>((size_t)XS_NS * (XS_BINS + 1)); t.xs_ent = cv.take<float4>((size_t)XS_NS * 2 * k.max_pls); t.best5 = cv.take<int>(k.max_t5);
     t.chi5 = cv.take<float>(k.max_t5); t.pt5_next = cv.take<int>(5 * (size_t)k.max_pls); t.best3 = cv.take<int>(k.max_t3);
     t.chi3 = cv.take<float>(k.max_t3); t.tc_hdr = cv.take<int>(LST_N_CNT + 3 * (size_t)k.max_tc); t.tc = t.tc_hdr ? t.tc_hdr + LST_N_CNT : nullptr;
-    t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc); t.tc_sig = cv.take<unsigned long long>(k.max_tc);
+    t.tc_hits = cv.take<int>(TC_HSTRIDE * (size_t)k.max_tc); t.tc_q = cv.take<int>(k.max_tc); t.tc_next = cv.take<int>(10 * (size_t)k.max_tc); t.tc_keep = cv.take<int>(k.max_tc); t.tc_sig = cv.take<unsigned long long>(k.max_tc); t.chain_tce = cv.take<unsigned long long>((3 * (size_t)k.max_pls + k.max_t5) / TCE_TPB + 4);
     t.tcc = cv.take<int>(3 * (size_t)k.max_tc); t.chain_tcc = cv.take<unsigned long long>(k.max_tc / TCC_ROWS + 4);
     t.g_node = cv.take<float>(8 * (size_t)k.max_md); t.g_col = cv.take<int>(k.max_ls);
     t.st_hits = cv.take<float>(4 * (size_t)k.max_hits); t.st_pls = cv.take<float>(5 * (size_t)k.max_pls);
@@ -190,7 +190,7 @@ inline bool bad(lst_ctx* c, cudaError_t e) {
   return false;
 }
 
-constexpr int N_LAUNCHES = 20;   // kernels per lst_run / lst_run_batch (plus two memsets)
+constexpr int N_LAUNCHES = 19;   // kernels per lst_run / lst_run_batch (plus two memsets)
 
 }  // namespace
 
@@ -264,6 +264,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_md, 0, sizeof(unsigned long long) * (M / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_ls, 0, sizeof(unsigned long long) * (c->caps.max_md / SCAN_TILE + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5s, 0, sizeof(unsigned long long) * (c->caps.max_t5c / 128 + 4));
+    if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_tce, 0, sizeof(unsigned long long) * ((3 * (size_t)c->caps.max_pls + c->caps.max_t5) / TCE_TPB + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_tcc, 0, sizeof(unsigned long long) * (c->caps.max_tc / TCC_ROWS + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t3, 0, sizeof(unsigned long long) * (c->caps.max_ls / TUPLE_TPB + 4));
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
@@ -393,8 +394,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   launch(pdl, k_pt5_lists, G, B128, 0, st, sl); LST_MARK();
   if (xs) launch(pdl, k_match<3, true, true>, G, BM, 0, st, sl, g, k.max_pls); else launch(pdl, k_match<3, true, false>, G, BM, 0, st, sl, g, k.max_pls);
   LST_MARK();
-  launch(pdl, k_tc_emit, G1, dim3(1024), 0, st, sl, k); LST_MARK();
-  launch(pdl, k_tc_tuples, G, B128, 0, st, sl); LST_MARK();
+  launch(pdl, k_tc_emit, dim3(gx < 48 ? gx : 48, n), dim3(TCE_TPB), 0, st, sl, k); LST_MARK();
   launch(pdl, k_tc_clean, GL, dim3(TCC_TPB), 0, st, sl, k); LST_MARK();
 #undef LST_MARK
   if (li != N_LAUNCHES + 2) return LST_EINVAL;
@@ -452,7 +452,7 @@ int lst_run_batch_profile(lst_ctx* c, int32_t first, int32_t n, void* cuda_strea
 const char* lst_launch_name(int32_t i) {
   static const char* names[N_LAUNCHES + 1] = {
       "memset", "a0.hist", "a0.scan", "a0.scatter", "a0.rank", "a1.md_sweep", "a1.scan", "a1.md_finish", "a2.ls_sweep", "a2.scan", "a2.ls_finish",
-      "a3.t3", "a4.t5", "a5.dnn", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit", "f1.tc_tuples", "f1.tc_clean"};
+      "a3.t3", "a4.t5", "a5.dnn", "a6.pls_bin", "a6.match5", "a6.pt5_lists", "a6.match3", "a6.tc_emit", "f1.tc_clean"};
   return (i >= 0 && i <= N_LAUNCHES) ? names[i] : nullptr;
 }
 

@@ -44,7 +44,7 @@ struct Geo {   // device copies, shared by all slots
 // a6 surfaces: a barrel layer, or one side of an endcap disk (lst_kernels.cuh, "crossing keys")
 constexpr int XS_NS = 32, XS_NP = 256, XS_NZ = 16, XS_REG = XS_NP * XS_NZ, XS_BINS = XS_REG + 1;     // + the surface's overflow bin
 
-enum { TK_LS_SWEEP = 0, TK_LS_DIRECT, TK_MD_SWEEP, TK_MD_DIRECT, TK_DNN, N_TK = 16 };
+enum { TK_LS_SWEEP = 0, TK_LS_DIRECT, TK_MD_SWEEP, TK_MD_DIRECT, TK_DNN, TK_TCE, N_TK = 16 };
 
 struct Caps { int max_hits, max_md, max_ls, max_t3, max_t5c, max_t5, max_pls, max_tc; };
 
@@ -88,7 +88,7 @@ struct Slot {
   float4* pls_a; float2* pls_b; int* pls_key; float4* pls_sa; float2* pls_sb; int* pls_sidx; int* pls_pos; int* pls_taken; int* pls_bin_start;
   int* xs_key; int* xs_start; float4* xs_ent;     // pLS crossing-key bins per surface: [XS_NS][XS_BINS + 1] starts, [XS_NS][2 max_pls] entries (cx, cy, h, pLS)
   int* best5; float* chi5; int* pt5_next; int* best3; float* chi3; int* tc;
-  int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc; unsigned long long* tc_sig;     // f1 duplicate cleaning
+  int* tc_hits; int* tc_q; int* tc_next; int* tc_keep; int* tcc; unsigned long long* chain_tcc; unsigned long long* tc_sig; unsigned long long* chain_tce;     // f1 duplicate cleaning
   float* g_node; int* g_col;         // f4 graph export: node features [n_md][8], CSR column (outer MD) per LS
   // host-load staging
   float* st_hits; float* st_pls;     // packed [x|y|z|key] (4 n_hits words) and [px|py|pz|z0|q] (4 n_pls words + n_pls bytes)
@@ -1035,101 +1035,107 @@ __global__ void k_pt5_lists(const Slot* __restrict__ slots) {
   }
 }
 
-// ordered emission of the four candidate types: one block per event, four flag-scan-write sweeps
-__global__ void __launch_bounds__(1024) k_tc_emit(const Slot* __restrict__ slots, Caps caps) {
-  pdl_begin();
-  __shared__ int sm[34];
-  const Slot& s = slots[blockIdx.y];
-  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int n_pls = s.n_pls, n_t5 = s.cnt[LST_CNT_T5];
-  int base_out = 0;
-  int n_type[4];
-  for (int type = 0; type < 4; ++type) {
-    const int n = (type == 1) ? n_t5 : n_pls;
-    const int start_out = base_out;
-    for (int base = 0; base < n; base += 1024) {
-      const int i = base + tid;
-      int flag = 0, obj = -1;
-      if (i < n) {
-        if (type == 1) { flag = s.best5[i] < 0; obj = i; }
-        else {
-          const unsigned long long w5 = s.win5[i], w3 = s.win3[i];
-          if (type == 0) { flag = w5 != WIN_EMPTY; obj = (int)(w5 & 0xFFFFFFFFull); }
-          else if (type == 2) { flag = (w5 == WIN_EMPTY) && (w3 != WIN_EMPTY); obj = (int)(w3 & 0xFFFFFFFFull); }
-          else { flag = (w5 == WIN_EMPTY) && (w3 == WIN_EMPTY); obj = -1; }
-        }
-      }
-      const unsigned bal = __ballot_sync(0xffffffffu, flag);
-      if (lane == 0) sm[wid] = __popc(bal);
-      __syncthreads();
-      if (wid == 0) {
-        const int w = sm[lane];
-        int winc = w;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-          const int t = __shfl_up_sync(0xffffffffu, winc, d);
-          if (lane >= d) winc += t;
-        }
-        sm[lane] = winc - w;
-        if (lane == 31) sm[32] = winc;
-      }
-      __syncthreads();
-      if (flag) {
-        const int o = base_out + sm[wid] + __popc(bal & ((1u << lane) - 1u));
-        if (o < caps.max_tc) { s.tc[3 * o] = type; s.tc[3 * o + 1] = (type == 1) ? -1 : i; s.tc[3 * o + 2] = obj; }
-      }
-      base_out += sm[32];
-      __syncthreads();
-    }
-    n_type[type] = base_out - start_out;
-  }
-  if (tid == 0) {
-    s.cnt[LST_CNT_PT5] = n_type[0]; s.cnt[LST_CNT_T5TC] = n_type[1]; s.cnt[LST_CNT_PT3] = n_type[2]; s.cnt[LST_CNT_PLSTC] = n_type[3];
-    s.cnt[LST_CNT_RAW_TC] = base_out;
-    s.cnt[LST_CNT_TC] = min(base_out, caps.max_tc);
-    if (base_out > caps.max_tc) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_TC);
-  }
-}
-
-// f1 (SPEC.md 4.7), step 1: the hit tuple of every candidate (ORIGINAL indices: lower, upper hit of each of its MDs), the chi2
-// of its rank key, and its entry in the list of every hit it holds.  One thread per TC row.
+// Ordered emission of the four candidate types (SPEC.md 4.6) and, for every emitted row, f1's step 1 (SPEC.md 4.7): the hit tuple
+// of the candidate (ORIGINAL indices: lower, upper hit of each of its MDs), the chi2 of its rank key, a 64-bit signature of its
+// hits and its entry in the list of every hit it holds.  The TC list is the order-preserving compaction of one item sequence
+//   [pLS p as pT5 (owns a T5)] [T5 t of the T5 list not matched] [pLS p as pT3 (no T5, owns a T3)] [pLS p alone]
+// done in one pass: tiles of TCE_TPB items by ticket, block scan of the flags, look-back across tiles.
 __device__ __forceinline__ int tc_hash(int hit) { return (int)(((unsigned)hit * 0x9E3779B1u) >> 26); }
-__global__ void __launch_bounds__(128) k_tc_tuples(const Slot* __restrict__ slots) {
+constexpr int TCE_TPB = 256;
+__global__ void __launch_bounds__(TCE_TPB) k_tc_emit(const Slot* __restrict__ slots, Caps caps) {
   pdl_begin();
+  __shared__ int s_w[TCE_TPB / 32], s_type[4];
+  __shared__ int s_tile, s_base;
   const Slot& s = slots[blockIdx.y];
-  LST_FOR_ITEMS(o, s.cnt[LST_CNT_TC]) {
-    const int type = s.tc[3 * o], obj = s.tc[3 * o + 2];
+  const unsigned epoch = *s.epoch_dev;
+  const int n_pls = s.n_pls, n_t5 = s.cnt[LST_CNT_T5];
+  const int n = 3 * n_pls + n_t5;
+  const int n_tiles = (n + TCE_TPB - 1) / TCE_TPB + (n == 0);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  while (true) {
+    if (threadIdx.x == 0) s_tile = atomicAdd(s.tk + TK_TCE, 1);
+    if (threadIdx.x < 4) s_type[threadIdx.x] = 0;
+    __syncthreads();
+    const int tile = s_tile;
+    if (tile >= n_tiles) break;
+    const int u = tile * TCE_TPB + threadIdx.x;
+    int flag = 0, type = 0, pls = -1, obj = -1;
+    if (u < n) {
+      if (u >= n_pls && u < n_pls + n_t5) { type = 1; obj = u - n_pls; flag = s.best5[obj] < 0; }
+      else {
+        type = u < n_pls ? 0 : u < 2 * n_pls + n_t5 ? 2 : 3;
+        pls = u < n_pls ? u : u - (type == 2 ? n_pls : 2 * n_pls) - n_t5;
+        const unsigned long long w5 = s.win5[pls], w3 = s.win3[pls];
+        if (type == 0) { flag = w5 != WIN_EMPTY; obj = (int)(w5 & 0xFFFFFFFFull); }
+        else if (type == 2) { flag = (w5 == WIN_EMPTY) && (w3 != WIN_EMPTY); obj = (int)(w3 & 0xFFFFFFFFull); }
+        else { flag = (w5 == WIN_EMPTY) && (w3 == WIN_EMPTY); obj = -1; }
+      }
+    }
+    // what the row's tuple needs, loaded before the scan
     int md[5] = {-1, -1, -1, -1, -1};
     float chi = 0.0f;
-    if (type <= 1) {
-      const int* m5 = s.t5c_md + 5 * s.t5_list[obj];
+    if (flag) {
+      if (type <= 1) {
+        const int* m5 = s.t5c_md + 5 * s.t5_list[obj];
 #pragma unroll
-      for (int q = 0; q < 5; ++q) md[q] = m5[q];
-      if (type == 0) chi = s.chi5[obj];
-    } else if (type == 2) {
-      const int4 abc = s.t3_abc[obj];
-      md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
-      chi = s.chi3[obj];
+        for (int q = 0; q < 5; ++q) md[q] = m5[q];
+        if (type == 0) chi = s.chi5[obj];
+      } else if (type == 2) {
+        const int4 abc = s.t3_abc[obj];
+        md[0] = abc.x; md[1] = abc.y; md[2] = abc.z;
+        chi = s.chi3[obj];
+      }
     }
-    s.tc_q[o] = __float_as_int(chi);
     int2 h[5];
 #pragma unroll
     for (int q = 0; q < 5; ++q) h[q] = md[q] >= 0 ? s.md_hits[md[q]] : make_int2(-1, -1);
-    int* row = s.tc_hits + TC_HSTRIDE * o;
-    *reinterpret_cast<int4*>(row) = make_int4(h[0].x, h[0].y, h[1].x, h[1].y);
-    *reinterpret_cast<int4*>(row + 4) = make_int4(h[2].x, h[2].y, h[3].x, h[3].y);
-    *reinterpret_cast<int4*>(row + 8) = make_int4(h[4].x, h[4].y, -1, -1);
-    unsigned long long sig = 0ull;                     // 64-bit signature of the row's hits (k_tc_clean's quick bound)
+    const unsigned bal = __ballot_sync(0xffffffffu, flag);
+    if (lane == 0) s_w[wid] = __popc(bal);
 #pragma unroll
-    for (int q = 0; q < 5; ++q)
-      if (md[q] >= 0) sig |= (1ull << tc_hash(h[q].x)) | (1ull << tc_hash(h[q].y));
-    s.tc_sig[o] = sig;
+    for (int k = 0; k < 4; ++k) {                        // rows per type (counted whether or not they fit the capacity)
+      const unsigned bk = __ballot_sync(0xffffffffu, flag && type == k);
+      if (lane == 0 && bk) atomicAdd(&s_type[k], __popc(bk));
+    }
+    __syncthreads();
+    int btot = 0, wbase = 0;
 #pragma unroll
-    for (int q = 0; q < 5; ++q)
-      if (md[q] >= 0) {
-        s.tc_next[10 * o + 2 * q] = atomicExch(s.hit_head + h[q].x, 10 * o + 2 * q);
-        s.tc_next[10 * o + 2 * q + 1] = atomicExch(s.hit_head + h[q].y, 10 * o + 2 * q + 1);
+    for (int q = 0; q < TCE_TPB / 32; ++q) { const int c = s_w[q]; if (q < wid) wbase += c; btot += c; }
+    if (wid == 0) {
+      const int b = chain_exclusive(s.chain_tce, tile, btot, lane, epoch);
+      if (lane == 0) s_base = b;
+    }
+    if (threadIdx.x < 4 && s_type[threadIdx.x]) atomicAdd(s.cnt + LST_CNT_PT5 + threadIdx.x, s_type[threadIdx.x]);      // PT5, T5TC, PT3, PLSTC are consecutive
+    __syncthreads();
+    const int base = s_base;
+    if (flag) {
+      const int o = base + wbase + __popc(bal & ((1u << lane) - 1u));
+      if (o < caps.max_tc) {
+        s.tc[3 * o] = type; s.tc[3 * o + 1] = (type == 1) ? -1 : pls; s.tc[3 * o + 2] = obj;
+        s.tc_q[o] = __float_as_int(chi);
+        int* row = s.tc_hits + TC_HSTRIDE * o;
+        *reinterpret_cast<int4*>(row) = make_int4(h[0].x, h[0].y, h[1].x, h[1].y);
+        *reinterpret_cast<int4*>(row + 4) = make_int4(h[2].x, h[2].y, h[3].x, h[3].y);
+        *reinterpret_cast<int4*>(row + 8) = make_int4(h[4].x, h[4].y, -1, -1);
+        unsigned long long sig = 0ull;                     // 64-bit signature of the row's hits (k_tc_clean's quick bound)
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          if (md[q] >= 0) sig |= (1ull << tc_hash(h[q].x)) | (1ull << tc_hash(h[q].y));
+        s.tc_sig[o] = sig;
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          if (md[q] >= 0) {
+            s.tc_next[10 * o + 2 * q] = atomicExch(s.hit_head + h[q].x, 10 * o + 2 * q);
+            s.tc_next[10 * o + 2 * q + 1] = atomicExch(s.hit_head + h[q].y, 10 * o + 2 * q + 1);
+          }
       }
+    }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) {
+      const int total = base + btot;
+      s.cnt[LST_CNT_RAW_TC] = total;
+      s.cnt[LST_CNT_TC] = min(total, caps.max_tc);
+      if (total > caps.max_tc) atomicOr(reinterpret_cast<unsigned*>(s.cnt + CNT_STATUS), LST_ST_OVF_TC);
+    }
+    __syncthreads();
   }
 }
 
