@@ -263,7 +263,10 @@ __device__ __forceinline__ void md_sweep_body(const Slot& s, const Geo& geo, con
   if (sn) md_flush<DIRECT>(s, W, sn, lane, cap);
 }
 
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
+#ifndef MD_MIN_BLOCKS
+#define MD_MIN_BLOCKS 7
+#endif
+__global__ void __launch_bounds__(PAIR_WARPS * 32, MD_MIN_BLOCKS) k_md_sweep(const Slot* __restrict__ slots, Geo geo, Caps caps) {
   pdl_begin();
   __shared__ MdWarp Wall[PAIR_WARPS];
   md_sweep_body<false>(slots[blockIdx.y], geo, caps, Wall);
