@@ -406,7 +406,7 @@ int lst_run_batch(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
   if (c->sticky_cuda_error) return LST_ECUDA;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   // The launch sequence has no per-run arguments, so it is captured once per (first, n) and replayed as a CUDA graph
-  // (one submission instead of 26 launches + 2 memsets).  The legacy default stream cannot be captured: direct launches.
+  // (one submission instead of 19 launches + 2 memsets).  The legacy default stream cannot be captured: direct launches.
   if (c->use_graphs && st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread) {
     const long long key = ((long long)first << 32) | (unsigned)n;
     auto it = c->graphs.find(key);
