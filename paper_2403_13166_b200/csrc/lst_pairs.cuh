@@ -13,10 +13,14 @@
 //                  kernel writes record -> start[row] + seq.
 // A row is never split between warps and a warp visits its rows and columns in ascending order, so `seq`
 // depends only on the input (bit-reproducible output order), whatever the scheduling.
-// a1: row = module (cells = lower x upper hits of the module, both contiguous in the sorted hit store).
-// a2: row = MD a; its columns are the MDs of the modules connected to module(a), which are a few contiguous MD
-//     ranges: lst_create compresses every CSR row into runs of consecutive module ids (Geo::run_*), and MDs are
-//     stored in module order, so one run = one contiguous slice of md_pos / md_aux.
+// a1: row = module (cells = lower x upper hits of the module, both contiguous in the sorted hit store); a warp packs the cells of
+//     32 modules into one flat index space.
+// a2: row = MD a; its columns are the MDs of the modules connected to module(a), which are a few contiguous MD ranges:
+//     lst_create compresses every CSR row into runs of consecutive module ids (Geo::run_*), MDs are stored in module order, so
+//     one run = one contiguous slice of md_pos / md_aux, and k_md_finish writes a per-module column table (end column and MD
+//     offset of up to LS_TAB non-empty runs).  A warp takes a chunk of consecutive rows (launch-wide ticket), cuts it into
+//     module segments and sweeps every segment columns-outer / rows-inner: 32 column MDs in registers against each row of the
+//     segment (anchors in shared memory).  seq = the row's count so far (shared memory, per chunk) + rank within the batch.
 // Capacity overflow (more objects than the record buffer holds): the scan flags it, and the DIRECT instantiation
 // of the sweep runs the stage again (inside the finish kernel), writing start[row] + seq in place for positions below the
 // capacity ("first cap objects in build order").
