@@ -511,3 +511,23 @@ def test_a2_module_with_more_than_eight_nonempty_runs(P, geo_barrel):
         n_ne.append(sum(1 for run in runs if any(x in md_mod for x in run)))
     assert max(n_ne) > 8, max(n_ne)
     assert c["ls"] > 40
+
+
+def test_one_launch_over_more_than_32_events(P, geo_full):
+    """a2 hands out the chunks of up to 32 events by one ticket (one persistent grid per 32 events); a 45-event batch takes two
+    groups (32 + 13), mixed sizes incl. empty events, and offsets other than 0.  Every event against the oracle."""
+    w = xavier_weights(3)
+    evs = []
+    for i in range(45):
+        if i % 9 == 4: evs.append(make_event(geo_full, 300 + i))                     # empty
+        elif i % 3 == 0: evs.append(config_event(geo_full, 1, seed=300 + i))          # PU50
+        elif i % 3 == 1: evs.append(make_event(geo_full, 300 + i, origin_muons=5, n_noise=300))
+        else: evs.append(config_event(geo_full, 4, seed=300 + i, pileup=100 if i % 2 else 0))
+    caps = P.default_caps(48)
+    lst = P.LST(geo_full, w, caps)
+    for i, ev in enumerate(evs):
+        lst.load_numpy_event(i + 2, ev)          # slots 2 .. 46
+    lst.lst_run_batch(2, len(evs))
+    for i, ev in enumerate(evs):
+        parity.compare(geo_full, w, ev, lst.fetch(i + 2))
+    lst.close()
