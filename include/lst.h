@@ -73,8 +73,8 @@ typedef struct {
   const uint8_t* layer;       /* optional [n_modules]: detector layer of each module (1..6 barrel, 7..11 disks).  An input
                                * feature of the 38-input DNN (NULL = 0 everywhere).  When given it also selects the faster
                                * of the two exact pixel-seed prefilters of step a6 (pLS binned by where their helix
-                               * crosses each layer); results do not depend on
-                               * it: any labelling, or none, gives the same lists (only the run time changes)      */
+                               * crosses each layer); that choice never changes a
+                               * result: any labelling, or none, gives the same matches (only the run time changes)  */
   int32_t dnn_n_feat;         /* 0 or 23: the 23 inputs of configs[0] (SPEC.md 4.5); 38: the paper's input list (4.9) */
   int32_t dnn_n_hidden;       /* 0 or 2: two hidden layers of 32; 1, 3, 4: the depth scan of PAPER.md:78 */
 } lst_geometry;

@@ -759,7 +759,10 @@ __device__ __forceinline__ void match_drain1(const Slot& s, unsigned long long* 
 }
 
 template <int NA, bool IS_T3, bool XS>
-__global__ void __launch_bounds__(MATCH_WARPS * 32) k_match(const Slot* __restrict__ slots, Geo geo, int max_pls) {
+#ifndef MATCH_MIN_BLOCKS
+#define MATCH_MIN_BLOCKS 1
+#endif
+__global__ void __launch_bounds__(MATCH_WARPS * 32, MATCH_MIN_BLOCKS) k_match(const Slot* __restrict__ slots, Geo geo, int max_pls) {
   pdl_begin();
   __shared__ MatchWarp Wall[MATCH_WARPS];
   const Slot& s = slots[blockIdx.y];
