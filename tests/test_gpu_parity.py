@@ -531,3 +531,48 @@ def test_one_launch_over_more_than_32_events(P, geo_full):
     for i, ev in enumerate(evs):
         parity.compare(geo_full, w, ev, lst.fetch(i + 2))
     lst.close()
+
+
+def test_a6_prefilters_agree_on_many_events(P, geo_full):
+    """Both a6 prefilters only select which (pLS, object) pairs get the exact test, so they must produce identical bytes.  24 events
+    (PU200 / PU300 + displaced, a fifth of the seeds pushed to the edges of the binned range) through both, match tables and TC
+    lists compared byte by byte; four of the events also against the oracle."""
+    import os
+    w = xavier_weights(3)
+    rng = np.random.default_rng(11)
+    evs = []
+    for i in range(24):
+        ev = config_event(geo_full, 4, seed=400 + i, pileup=300 if i % 3 == 0 else 200)
+        n = ev.n_pls
+        idx = rng.choice(n, n // 5, replace=False)
+        for k, p in enumerate(idx):
+            pt = float(np.hypot(ev.pls_px[p], ev.pls_py[p]))
+            if k % 4 == 0: ev.pls_z0[p] = np.float32(rng.choice([-19.9, 19.9, -20.5, 20.5]))
+            elif k % 4 == 1: ev.pls_pz[p] = np.float32(rng.uniform(6.5, 8.5) * pt * rng.choice([-1, 1]))          # |cot| up to the cap
+            elif k % 4 == 2: s = rng.uniform(0.76, 0.85) / pt; ev.pls_px[p] *= s; ev.pls_py[p] *= s; ev.pls_pz[p] *= s      # around pT = 0.8
+            else: ev.pls_pz[p] = np.float32(rng.uniform(-0.05, 0.05) * pt)                                          # central: both circle intersections matter
+        evs.append(ev)
+    caps = P.Caps(n_slots=24, max_hits=196608, max_md=98304, max_ls=98304, max_t3=65536, max_t5c=32768, max_t5=32768, max_pls=8192)
+
+    def run():
+        lst = P.LST(geo_full, w, caps)
+        for i, ev in enumerate(evs):
+            lst.load_numpy_event(i, ev)
+        lst.lst_run_batch(0, len(evs))
+        out = [lst.fetch(i) for i in range(len(evs))]
+        lst.close()
+        return out
+
+    a = run()
+    os.environ["LST_XS"] = "0"
+    try:
+        b = run()
+    finally:
+        del os.environ["LST_XS"]
+    for i, (x, y) in enumerate(zip(a, b)):
+        assert x["status"] == 0 and y["status"] == 0, (i, x["status"], y["status"])
+        for obj in ("match5", "tc", "tcc", "tcx"):
+            for k in x[obj]:
+                assert np.array_equal(x[obj][k].view(np.uint8), y[obj][k].view(np.uint8)), (i, obj, k)
+    for i in (0, 7, 12, 23):
+        parity.compare(geo_full, w, evs[i], a[i])
