@@ -81,7 +81,7 @@ Caps make_caps(const lst_caps* c) {
 // One pass lays out the whole workspace; used both to measure and to carve.
 struct Layout {
   char* batch_in; size_t batch_in_stride; int* batch_out; size_t batch_out_stride;
-  Slot* slots; uint8_t* modt; uint8_t* layer; int* rowptr; int* col; float* weights; int* run_ptr; int* run_c0; int* run_c1;
+  Slot* slots; uint8_t* modt; uint8_t* layer; uint8_t* xs_layer; int* rowptr; int* col; float* weights; int* run_ptr; int* run_c0; int* run_c1;
   char* zero_base; size_t zero_stride; char* ones_base; size_t ones_stride;
   size_t total;
 };
@@ -92,6 +92,7 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   L.slots = cv.take<Slot>(n_slots);
   L.modt = cv.take<uint8_t>(M);
   L.layer = cv.take<uint8_t>(M);
+  L.xs_layer = cv.take<uint8_t>(M);
   L.rowptr = cv.take<int>(M + 1);
   L.col = cv.take<int>(nnz > 0 ? nnz : 1);
   L.weights = cv.take<float>(dnn_n_weights(N_FEAT_MAX, 4));
@@ -241,6 +242,14 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     std::vector<uint8_t> lay(M, 0);
     if (geo->layer) for (int m = 0; m < M; ++m) lay[m] = geo->layer[m];
     if (e == cudaSuccess) e = cudaMemcpy(L.layer, lay.data(), M, cudaMemcpyHostToDevice);
+    // a T3 / T5 starts on module m only if the CSR has a two-step path m -> m' -> m'': only those modules' MDs define the a6 surfaces
+    std::vector<uint8_t> xs(M, 255);
+    for (int m = 0; m < M; ++m)
+      for (int i = geo->conn_rowptr[m]; i < geo->conn_rowptr[m + 1] && xs[m] == 255; ++i) {
+        const int m1 = geo->conn_col[i];
+        if (geo->conn_rowptr[m1 + 1] > geo->conn_rowptr[m1]) xs[m] = lay[m];
+      }
+    if (e == cudaSuccess) e = cudaMemcpy(L.xs_layer, xs.data(), M, cudaMemcpyHostToDevice);
   }
   {   // CSR rows -> runs of consecutive module ids (one run = one contiguous MD range, lst_pairs.cuh)
     std::vector<int> run_ptr(M + 1, 0), c0, c1;
@@ -283,7 +292,7 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     }
     (void)cudaGetLastError();
   }
-  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.has_layer = (geo->layer && c->use_xs) ? 1 : 0; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
+  c->geo.n_modules = M; c->geo.modt = L.modt; c->geo.rowptr = L.rowptr; c->geo.col = L.col; c->geo.weights = L.weights; c->geo.layer = L.layer; c->geo.xs_layer = L.xs_layer; c->geo.has_layer = (geo->layer && c->use_xs) ? 1 : 0; c->geo.n_feat = n_feat; c->geo.n_hidden = n_hidden;
   c->geo.run_ptr = L.run_ptr; c->geo.run_c0 = L.run_c0; c->geo.run_c1 = L.run_c1;
   *out = c;
   return LST_OK;

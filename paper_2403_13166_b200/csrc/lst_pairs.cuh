@@ -84,7 +84,7 @@ __device__ __forceinline__ void md_emit(const Slot& s, const MdRec& r, int cap, 
   // carry the module type (they only widen the tolerance)
   const float fm_ = __int_as_float(__float_as_int(md_relf(mt) * 1.0001f) | mt);
   s.md_aux[pos] = make_float4(r.c, fmaf(r.w, 1.0001f, 3.0e-7f), fm_, 1.0f / h.w);
-  if (DIRECT && layer) {                                // surface ranges for a6 (the record path aggregates them per block)
+  if (DIRECT && layer && layer[r.mtm >> 2] != 255) {    // surface ranges for a6 (the record path aggregates them per block)
     const int sg = xs_surface(mt, layer[r.mtm >> 2], h.z);
     const unsigned ref = __float_as_uint((mt & 2) ? fabsf(h.z) : h.w);
     atomicMin(s.surf_lo + sg, ref); atomicMax(s.surf_hi + sg, ref); atomicMax(s.surf_rhi + sg, __float_as_uint(h.w));
@@ -167,7 +167,7 @@ __device__ __forceinline__ void md_sweep_body(const Slot& s, const Geo& geo, con
   const int cap = caps.max_md;
   const int n_warps = gridDim.x * PAIR_WARPS;
   int qn = 0, sn = 0, carry_row = -1, carry_n = 0;
-  if (lane == 0) W.layer = geo.has_layer ? geo.layer : nullptr;
+  if (lane == 0) W.layer = geo.has_layer ? geo.xs_layer : nullptr;
   __syncwarp();
   // modules are interleaved over the warps (heavy inner-layer modules have consecutive ids).  A warp takes 32 of its modules
   // at a time (one round of range loads) and sweeps their cells as ONE flat index space, 32 cells per step: most modules
@@ -309,7 +309,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
     int lay = 0;
     if (has_r) {
       pos = mds[r.mtm >> 2] + r.seq; h = s.hit[r.p_lo]; o_lo = s.hit_orig[r.p_lo]; o_up = s.hit_orig[r.p_up];
-      if (geo.has_layer) lay = geo.layer[r.mtm >> 2];
+      if (geo.has_layer) lay = geo.xs_layer[r.mtm >> 2];
     }
     int c0[LS_TAB], c1[LS_TAB], b0[LS_TAB], b1[LS_TAB];
 #pragma unroll
@@ -326,7 +326,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_md_finish(const Slot* __res
       s.md_cw[pos] = make_float2(r.c, r.w);
       const float fm_ = __int_as_float(__float_as_int(md_relf(mt) * 1.0001f) | mt);
       s.md_aux[pos] = make_float4(r.c, fmaf(r.w, 1.0001f, 3.0e-7f), fm_, 1.0f / h.w);
-      if (geo.has_layer) {
+      if (geo.has_layer && lay != 255) {
         const int sg = xs_surface(mt, lay, h.z);
         const unsigned ref = __float_as_uint((mt & 2) ? fabsf(h.z) : h.w);      // positive floats: bit order = value order
         atomicMin(&b_lo[sg], ref); atomicMax(&b_hi[sg], ref); atomicMax(&b_rh[sg], __float_as_uint(h.w));
