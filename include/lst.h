@@ -31,6 +31,7 @@ extern "C" {
 #define LST_EINVAL (-1)  /* null pointer, size above capacity, malformed CSR, bad slot / objtype   */
 #define LST_ECUDA (-2)   /* a CUDA runtime call failed (sticky)                                   */
 #define LST_ENOMEM (-3)  /* workspace smaller than lst_workspace_bytes()                          */
+#define LST_ETOOBIG (-4) /* lst_sort_hits_static only: input larger than its fixed built-in scratch   */
 
 /* status bits (lst_status) */
 #define LST_ST_BAD_KEY (1u << 0)   /* a hit key >= 2*n_modules was dropped (SPEC.md 4.0)          */
@@ -221,6 +222,37 @@ int lst_measure_fp32(lst_ctx* ctx, int32_t fused, float* h_tflops, void* cuda_st
 const char* lst_launch_name(int32_t i);
 
 void lst_destroy(lst_ctx* ctx);
+
+/* ---- a0 without a workspace: for callers that cannot allocate device memory ------------------------------------------
+ * Every call above works in a workspace the caller allocates and hands to lst_create.  Some callers cannot do even
+ * that: a plugin inside a trigger / event-processing job whose framework gave out all device memory at start-up and
+ * passes a module its input and output buffers and nothing more, or an event loop where cudaMalloc / cudaFree are
+ * forbidden because they synchronise the whole device and take an unbounded time.  For them this ONE entry point runs
+ * the hit ingest of step a0 (SPEC.md 4.0; hits grouped by pT-module sensor) with no context, no workspace
+ * and no allocation of any kind: its temporaries sit in a fixed array built into the library
+ * (LST_STATIC_SCRATCH_BYTES, about 1.3 MB, held by every GPU that loads the library until the process exits).
+ *
+ *  in  (DEVICE): d_x, d_y, d_z [n_hits] float; d_key [n_hits] uint32 = 2*module + isUpper
+ *  out (DEVICE): d_hit_xyzr [n_hits][4] float (16-byte aligned): hits in sensor order, stable in the original index,
+ *                as (x, y, z, r = sqrt(x*x + y*y)); d_hit_orig [n_hits] int32: sorted position -> original index;
+ *                d_sensor_start [2*n_modules + 1] int32: first sorted position of each sensor, last entry = hits kept;
+ *                d_count [2] int32: hits kept, status bits (LST_ST_BAD_KEY if a key >= 2*n_modules was dropped).
+ *                Rows past "hits kept" are left untouched.  Same values as lst_get(LST_OBJ_HIT) after lst_run.
+ *  Limits      : n_hits <= LST_STATIC_MAX_HITS and n_modules <= LST_STATIC_MAX_MODULES, else LST_ETOOBIG and nothing is
+ *                enqueued.  LST_EINVAL on null / misaligned pointers or negative sizes, LST_ECUDA if a CUDA call fails.
+ *  Device      : the device that owns `cuda_stream` and the buffers must be the current device.  The first call on each
+ *                device also looks up where the built-in array lives on that device (a one-time set-up that must not
+ *                happen inside a stream capture: make the first call on a device before any capture starts).
+ *  Sharing     : all calls on one GPU use the same array.  Each call clears the counters it needs, so a call never sees
+ *                the previous one's data, but two calls that run on the GPU at the same time (two streams, two host
+ *                threads) corrupt each other: keep them on one stream or order them with an event.
+ *  Enqueues only (one memset and four small kernels on `cuda_stream`); no host synchronisation. */
+#define LST_STATIC_MAX_HITS 131072
+#define LST_STATIC_MAX_MODULES 32768
+#define LST_STATIC_SCRATCH_BYTES (4 * (128 + 2 * LST_STATIC_MAX_MODULES + 2 * LST_STATIC_MAX_HITS))
+int lst_sort_hits_static(int32_t n_hits, int32_t n_modules, const float* d_x, const float* d_y, const float* d_z,
+                         const uint32_t* d_key, float* d_hit_xyzr, int32_t* d_hit_orig, int32_t* d_sensor_start,
+                         int32_t* d_count, void* cuda_stream);
 
 #ifdef __cplusplus
 }

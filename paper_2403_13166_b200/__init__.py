@@ -5,7 +5,7 @@ only: every step of the path runs in the CUDA kernels.  There is no CPU fallback
 binding fails loudly when the library is missing, and it never touches `oracle/`.
 """
 from .binding import (LST, Caps, load_library, library_path, OBJ, CNT, STATUS_BITS, LstError,
-                      default_caps, pack_batch)
+                      default_caps, pack_batch, lst_sort_hits_static)
 
 __all__ = ["LST", "Caps", "load_library", "library_path", "OBJ", "CNT", "STATUS_BITS", "LstError",
-           "default_caps", "pack_batch"]
+           "default_caps", "pack_batch", "lst_sort_hits_static"]

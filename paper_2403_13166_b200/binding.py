@@ -16,7 +16,8 @@ CNT = dict(hit=0, md=1, ls=2, t3=3, t5c=4, t5=5, tc=6, raw_md=7, raw_ls=8, raw_t
 STATUS_BITS = dict(bad_key=1, ovf_md=2, ovf_ls=4, ovf_t3=8, ovf_t5c=16, ovf_t5=32, ovf_tc=64)
 EXPORTS = ["lst_workspace_bytes", "lst_create", "lst_load_event", "lst_load_event_host", "lst_run",
            "lst_run_batch", "lst_run_batch_profile", "lst_launch_name", "lst_get", "lst_status", "lst_read_tc_host", "lst_load_batch_host", "lst_load_batch_host16", "lst_read_tc_batch_host", "lst_read_tc_hits_batch_host", "lst_export_graph", "lst_dnn_n_weights", "lst_measure_fp32", "lst_launches_per_run",
-           "lst_destroy"]
+           "lst_destroy", "lst_sort_hits_static"]
+STATIC_MAX_HITS, STATIC_MAX_MODULES = 131072, 32768      # include/lst.h LST_STATIC_MAX_*
 
 
 class LstError(RuntimeError):
@@ -93,6 +94,7 @@ def load_library():
     L.lst_run_batch_profile.argtypes = [vp, i32, i32, vp, vp]
     L.lst_launch_name.argtypes = [i32]
     L.lst_destroy.argtypes = [vp]
+    L.lst_sort_hits_static.argtypes = [i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.lst_destroy.restype = None
     for n in EXPORTS:
         if n not in ("lst_destroy", "lst_launch_name"):
@@ -105,7 +107,7 @@ def load_library():
 def _chk(rc, what):
     if rc != 0:
         raise LstError(f"{what} failed with code {rc} "
-                       f"({ {-1: 'LST_EINVAL', -2: 'LST_ECUDA', -3: 'LST_ENOMEM'}.get(rc, '?') })")
+                       f"({ {-1: 'LST_EINVAL', -2: 'LST_ECUDA', -3: 'LST_ENOMEM', -4: 'LST_ETOOBIG'}.get(rc, '?') })")
 
 
 def _hp(a):
@@ -328,6 +330,38 @@ class LST:
             n = cnt[_ROWS.get(name, name)]
             res[name] = {k: v.cpu().numpy() for k, v in self.lst_get(slot, name, n).items()}
         return res
+
+
+def lst_sort_hits_static(x, y, z, key, n_modules, hit_xyzr, hit_orig, sensor_start, count, stream=None):
+    """Step a0 (hits sorted by sensor, stable) for callers that cannot allocate device memory -- e.g. a module inside a
+    framework that owns all of it and only hands out input / output buffers, or an event loop where cudaMalloc is banned.
+    No context and no workspace: the temporaries live in a fixed array inside the library, so the call is limited to
+    STATIC_MAX_HITS hits and STATIC_MAX_MODULES modules (LstError naming the limits otherwise), and calls that overlap
+    on one GPU would corrupt each other -- keep them on one stream.  The device of the tensors must be current; make the
+    first call on a device outside any stream capture (include/lst.h has the details).
+
+    DEVICE tensors in: x, y, z float32 [n]; key int32/uint32 [n].  DEVICE tensors out (caller-provided): hit_xyzr float32
+    [n, 4], hit_orig int32 [n], sensor_start int32 [2 * n_modules + 1], count int32 [2] = (hits kept, status bits).
+    Enqueues on `stream` (default: torch's current stream); argument marshalling only."""
+    import torch as t
+    L = load_library()
+    n = int(x.numel())
+    for a in (x, y, z):
+        assert a.is_cuda and a.dtype == t.float32 and a.is_contiguous() and a.numel() == n
+    assert key.is_cuda and key.dtype in (t.int32, t.uint32) and key.is_contiguous() and key.numel() == n
+    assert hit_xyzr.is_cuda and hit_xyzr.dtype == t.float32 and hit_xyzr.is_contiguous() and hit_xyzr.numel() >= 4 * n
+    assert hit_orig.is_cuda and hit_orig.dtype == t.int32 and hit_orig.is_contiguous() and hit_orig.numel() >= n
+    assert sensor_start.is_cuda and sensor_start.dtype == t.int32 and sensor_start.is_contiguous() and sensor_start.numel() >= 2 * n_modules + 1
+    assert count.is_cuda and count.dtype == t.int32 and count.numel() >= 2
+    if stream is None:
+        stream = t.cuda.current_stream(x.device)
+    p = lambda a: C.c_void_p(a.data_ptr()) if a.numel() else C.c_void_p(0)
+    rc = L.lst_sort_hits_static(n, int(n_modules), p(x), p(y), p(z), p(key), p(hit_xyzr), p(hit_orig), p(sensor_start), p(count),
+                                C.c_void_p(stream.cuda_stream))
+    if rc == -4:
+        raise LstError(f"lst_sort_hits_static: {n} hits / {n_modules} modules exceed the built-in scratch "
+                       f"(at most {STATIC_MAX_HITS} hits and {STATIC_MAX_MODULES} modules); use LST with a workspace instead")
+    _chk(rc, "lst_sort_hits_static")
 
 
 def pack_batch(events, pin=True, key16=False):

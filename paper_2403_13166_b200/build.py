@@ -5,7 +5,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblst_b200.so")
-SOURCES = [os.path.join(CSRC, "lst_api.cu")]
+SOURCES = [os.path.join(CSRC, "lst_api.cu"), os.path.join(CSRC, "lst_static.cu")]
 HEADERS = [os.path.join(CSRC, "lst_kernels.cuh"), os.path.join(CSRC, "lst_math.cuh"), os.path.join(CSRC, "lst_pairs.cuh"), os.path.join(CSRC, "lst_tuples.cuh"),
            os.path.join(_HERE, "..", "include", "lst.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
