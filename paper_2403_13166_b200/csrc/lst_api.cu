@@ -242,12 +242,14 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     std::vector<uint8_t> lay(M, 0);
     if (geo->layer) for (int m = 0; m < M; ++m) lay[m] = geo->layer[m];
     if (e == cudaSuccess) e = cudaMemcpy(L.layer, lay.data(), M, cudaMemcpyHostToDevice);
-    // a T3 / T5 starts on module m only if the CSR has a two-step path m -> m' -> m'': only those modules' MDs define the a6 surfaces
+    // a T3 / T5 starts on module m only if the CSR has a two-step path m -> m' -> m'': only those modules' MDs define the a6 surfaces.
+    // The table holds the label reduced to the bits xs_surface() uses (<= 15), so the "not a start module" mark 255 can never
+    // collide with a caller's label (any uint8, 255 included, is a legal label).
     std::vector<uint8_t> xs(M, 255);
     for (int m = 0; m < M; ++m)
       for (int i = geo->conn_rowptr[m]; i < geo->conn_rowptr[m + 1] && xs[m] == 255; ++i) {
         const int m1 = geo->conn_col[i];
-        if (geo->conn_rowptr[m1 + 1] > geo->conn_rowptr[m1]) xs[m] = lay[m];
+        if (geo->conn_rowptr[m1 + 1] > geo->conn_rowptr[m1]) xs[m] = lay[m] & 15;
       }
     if (e == cudaSuccess) e = cudaMemcpy(L.xs_layer, xs.data(), M, cudaMemcpyHostToDevice);
   }

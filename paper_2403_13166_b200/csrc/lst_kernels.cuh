@@ -33,8 +33,8 @@ struct Geo {   // device copies, shared by all slots
   const float* weights;     // [dnn_n_weights(n_feat, n_hidden)]
   const uint8_t* layer;     // [M] detector layer of the module (0 if the caller gave none): a 38-feature DNN input only
   int has_layer;            // the caller gave a layer per module: a6 uses the per-surface crossing keys
-  const uint8_t* xs_layer;  // [M] = layer for modules that can hold the FIRST MD of a T3 / T5 (a two-step path in the CSR starts there),
-                            // 255 otherwise: only those MDs define the surfaces the pLS are binned on
+  const uint8_t* xs_layer;  // [M] = layer & 15 (all xs_surface() looks at) for modules that can hold the FIRST MD of a T3 / T5 (a two-step
+                            // path in the CSR starts there), 255 otherwise: only those MDs define the surfaces the pLS are binned on
   int n_feat, n_hidden;     // DNN variant (SPEC.md 4.9): 23 or 38 inputs, 1..4 hidden layers of 32
   // CSR rows compressed into runs of consecutive module ids (built by lst_create): row m = runs [run_ptr[m], run_ptr[m+1]),
   // run e = modules [run_c0[e], run_c1[e]).  MDs are stored in module order, so a run is one contiguous MD range.

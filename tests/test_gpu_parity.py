@@ -446,6 +446,23 @@ def _odd_pls(ev, rng):
     return ev
 
 
+def test_a6_layer_label_255(P, geo_full):
+    """Any uint8 is a legal layer label (include/lst.h: "any labelling, or none, gives the same matches").  255 used to double as the
+    library's internal "no T3 / T5 starts here" mark, so the surfaces of modules labelled 255 were never measured and their objects
+    were matched against stale bins.  Barrel layer 1 (where most T5s start) relabelled 255, then everything relabelled 255."""
+    import dataclasses
+    w = xavier_weights(3)
+    ev = config_event(geo_full, 2, seed=37)
+    base = parity.compare(geo_full, w, ev, _run_one(P, geo_full, w, ev))
+    assert base["tc"] > 2000
+    lab = geo_full.layer.copy()
+    lab[lab == 1] = 255
+    g1 = dataclasses.replace(geo_full, layer=lab)
+    parity.compare(g1, w, ev, _run_one(P, g1, w, ev))
+    g2 = dataclasses.replace(geo_full, layer=np.full_like(geo_full.layer, 255))
+    parity.compare(g2, w, ev, _run_one(P, g2, w, ev))
+
+
 def test_a6_generic_buckets_relabelled_layers_and_odd_seeds(P, geo_full):
     """a6 has two exact prefilters: per-surface crossing keys (geometry with a layer per module) and the generic (h, zeta, psi)
     buckets (no layers, or LST_XS=0).  Both must give the oracle's lists: with the real layers, without layers, with every module
