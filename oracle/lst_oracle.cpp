@@ -21,8 +21,10 @@
 // independent fp64 MLP, rotation / mirror / permutation invariance, cut-loosening monotonicity, and --
 // term by term -- hand-derived accept / reject boundaries for every tolerance term of M2/M3, L1-L3,
 // T1-T3, the anchor test and chi2, plus hand-built scenarios for run_chain's own assignments, the
-// bridge indices and the TC used / free / tie rules.  tests/test_oracle_mutants.py shows that 46
-// single-line mutations of this file each fail at least one pin.
+// bridge indices and the TC used / free / tie rules.  The BUILD ORDER of every list (stable a0 sort,
+// (m, i, j), CSR-row order, (l0, l1), (u, v)), the radius clamp and the sagitta cap of M3 are pinned by
+// tests/test_oracle_order.py with numpy only.  tests/test_oracle_mutants.py shows that every entry of
+// its MUTANTS table (single-line mutations of this file) fails at least one pin.
 #include <cmath>
 #include <cstdint>
 #include <cstring>

@@ -143,7 +143,7 @@ __device__ __forceinline__ bool ls_eval(const Anchor& A, const Anchor& B, float&
 // c is formed from the same quantities as in ls_eval but with fused / approximate operations: cr by one FMA
 // (|error| <= 2^-23 rA d, i.e. < 1e-8 in c), 1/sqrt by MUFU (2 ulp), 1/r precomputed per MD -- in all a few ulp of
 // |c| <= 0.015, i.e. < 1e-8 absolute.  Margins: L1 1e-4 relative; L3 1e-4 relative + 3e-7 absolute, folded into the
-// per-MD record by k_md_scatter: *a = (c_md, w*1.0001 + 3e-7, f*1.0001 | module-type bits, 1/r).  Rejections are positive
+// per-MD record by md_emit / k_md_finish: *a = (c_md, w*1.0001 + 3e-7, f*1.0001 | module-type bits, 1/r).  Rejections are positive
 // comparisons, so a NaN anywhere lets the pair through to the exact test.
 // kinvA = -2 / rA.
 __device__ __forceinline__ bool ls_prefilter(float4 Ap, float4 Aa, float kinvA, float4 Bp, float4 Ba) {

@@ -17,6 +17,7 @@ import pytest
 
 from oracle import lst_oracle as O
 import test_oracle_terms as T
+import test_oracle_order as TO
 
 SRC = open(os.path.join(os.path.dirname(O.__file__), "lst_oracle.cpp")).read()
 
@@ -91,6 +92,21 @@ MUTANTS = [
     ("f3: 38 features: anchor order a,b,c,d,e,e", "const int order[6] = {0, 1, 2, 2, 3, 4};", "const int order[6] = {0, 1, 2, 3, 4, 4};", [("pin_dnn_variants", "geo")]),
     ("f3: 38 features: layer not fed", "x[4 + 5 * i + 4] = float(layer[q]) * 0.1f;", "x[4 + 5 * i + 4] = 0.0f;", [("pin_dnn_variants", "geo")]),
     ("f3: 38 features: T5 pT from c_in only", "const float c5 = 0.5f * (cin + cout);", "const float c5 = cin;", [("pin_dnn_variants", "geo")]),
+    # ---- build order of the lists (SPEC.md 4.0-4.5 "Order" clauses) and the two branches no config event reaches
+    ("a0: hits of a sensor in reverse arrival order", "res->hit_orig[cur[key[i]]++] = i;",
+     "res->hit_orig[res->sensor_start[key[i] + 1] - 1 - (cur[key[i]]++ - res->sensor_start[key[i]])] = i;", [("pin_build_order", "geo")]),
+    ("a1: upper hit outer loop, lower hit inner", "    for (int32_t i = ss[2 * m]; i < ss[2 * m + 1]; ++i) {\n      for (int32_t j = ss[2 * m + 1]; j < ss[2 * m + 2]; ++j) {",
+     "    for (int32_t j = ss[2 * m + 1]; j < ss[2 * m + 2]; ++j) {\n      for (int32_t i = ss[2 * m]; i < ss[2 * m + 1]; ++i) {", [("pin_build_order", "geo")]),
+    ("a2: CSR row walked last column first", "for (int32_t e = rowptr[m]; e < rowptr[m + 1]; ++e) {", "for (int32_t e = rowptr[m + 1] - 1; e >= rowptr[m]; --e) {", [("pin_build_order", "geo")]),
+    ("a3: partner LS loop descending", "for (int32_t l1 = res->ls_start[s0.b]; l1 < res->ls_start[s0.b + 1]; ++l1) {",
+     "for (int32_t l1 = res->ls_start[s0.b + 1] - 1; l1 >= res->ls_start[s0.b]; --l1) {", [("pin_build_order", "geo")]),
+    ("a4: partner T3 loop descending", "for (int32_t i1 = res->t3_start[u.c]; i1 < res->t3_start[u.c + 1]; ++i1) {",
+     "for (int32_t i1 = res->t3_start[u.c + 1] - 1; i1 >= res->t3_start[u.c]; --i1) {", [("pin_build_order", "geo")]),
+    ("radius feature clamped at 1e4", "const float rad = std::fmin(1.0f / ac, 1.0e5f);   // c = 0 -> +inf -> clamped",
+     "const float rad = std::fmin(1.0f / ac, 1.0e4f);", [("pin_radius_clamp", None)]),
+    ("pT feature clamped at 1e4", "  const float rad = std::fmin(1.0f / ac, 1.0e5f);\n  return std::log10(KAPPA_F * rad);",
+     "  const float rad = std::fmin(1.0f / ac, 1.0e4f);\n  return std::log10(KAPPA_F * rad);", [("pin_radius_clamp", None)]),
+    ("md_eval: S without the cap at 1", "const R S = std::fmin(R(1.0f), r2 * R(C_HALF_F));", "const R S = r2 * R(C_HALF_F);", [("pin_md_sagitta_cap", None)]),
     ("f1: upper hits left out of the tuples", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_up];", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_lo];", [("pin_clean_all_pairs", "geo")]),
 ]
 
@@ -125,7 +141,7 @@ def test_every_mutant_is_noticed(mutant_libs, geo_full, geo_barrel):
         killed = False
         with O.use_library(lib):
             for pin, fixture in pins:
-                fn = getattr(T, pin)
+                fn = getattr(T, pin, None) or getattr(TO, pin)
                 try:
                     fn() if fixture is None else fn(geo_full if fixture == "geo" else geo_barrel)
                 except AssertionError:
