@@ -450,7 +450,7 @@ def run_ours(args):
         roof = dict(bound="alu", achieved=round(wk["flops"] / k_s / 1e12, 3), peak=round(peak_f, 2), unit="TFLOP/s",
                     peak_source="measured in this run by lst_measure_fp32 (separately rounded multiply + add)")
     traffic, tsrc = None, None       # DRAM bytes per launch of this kernel from the committed ncu --set full capture
-    for tname in ("r02_traffic.csv", "r01_traffic.csv"):
+    for tname in ("r03_traffic.csv", "r02_traffic.csv"):
         tpath = os.path.join(ROOT, "profiles", tname)
         if traffic is None and os.path.exists(tpath):
             for line in open(tpath).read().splitlines()[1:]:

@@ -15,6 +15,9 @@
  *    stream.  lst_load_event*, lst_run* and lst_read_* only ENQUEUE work; lst_status synchronises.
  *  - A context holds `n_slots` independent event slots that share one uploaded geometry
  *    (BASELINE.json configs[3]: "geometry and connectivity uploaded once").
+ *  - Threads: a context is NOT thread-safe.  lst_run_batch keeps a cache of captured launch graphs and shares one
+ *    capture side-stream per context, so all calls on one context must come from one host thread at a time (the paper's
+ *    own usage: one host thread per stream -- give each thread its own context, they share nothing).
  *  - Overflow of a stage capacity is NOT an error return: the stage keeps the first `cap` objects in
  *    build order and sets its bit in the slot's status word (SPEC.md 6) -- flagged, never silent.
  */
@@ -56,7 +59,8 @@ enum { LST_CNT_HIT = 0, LST_CNT_MD, LST_CNT_LS, LST_CNT_T3, LST_CNT_T5C, LST_CNT
        /* internal: fill of the MD / LS record buffers; tile tickets of the row scans and of the T3 / T5 tiles */
        LST_CNT_FILL_MD, LST_CNT_FILL_LS, LST_CNT_TK_SENSOR, LST_CNT_TK_MD, LST_CNT_TK_LS, LST_CNT_TK_T5,
        LST_CNT_DYN_T3, LST_CNT_DYN_T5,
-       /* f1: number of track candidates kept by the duplicate cleaning; tile ticket of that step */
+       /* f1: number of track candidates kept by the duplicate cleaning; tile ticket of that step (internal entries such as
+        * the tickets are bookkeeping, not results; the header copy read by lst_read_tc_* carries 0 in LST_CNT_TK_TCC) */
        LST_CNT_TCC, LST_CNT_TK_TCC, LST_N_CNT = 32 };
 
 typedef struct lst_ctx lst_ctx; /* opaque; owned by the library, freed by lst_destroy */

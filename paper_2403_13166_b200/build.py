@@ -35,10 +35,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             print(res.stderr)
         if res.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-        log_dir = os.path.join(_HERE, "..", "_work")          # ptxas -v output: a working file, not product
-        if os.path.isdir(log_dir):
-            with open(os.path.join(log_dir, "build_ptxas.log"), "w") as f:
-                f.write(" ".join(cmd) + "\n" + res.stderr)
+        with open(LIB + ".ptxas.log", "w") as f:              # ptxas -v output next to the library (git-ignored)
+            f.write(" ".join(cmd) + "\n" + res.stderr)
     return LIB
 
 

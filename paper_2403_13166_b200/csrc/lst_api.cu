@@ -21,6 +21,7 @@ struct lst_ctx {
   char* zero_base = nullptr; size_t zero_stride = 0;
   char* ones_base = nullptr; size_t ones_stride = 0;
   bool sticky_cuda_error = false;
+  int n_sm = 148;                 // multiprocessors of the context's device (queried by lst_create): sizes every grid
   bool capturing = false;         // run_sequence is being recorded into a graph
   bool use_xs = true;             // a6 with per-surface crossing keys when the geometry carries layers (LST_XS=0: the generic (h, zeta, psi) buckets)
   bool use_pdl = false;           // programmatic dependent launch between the kernels of the chain (LST_PDL=1 enables; measured: no gain under graph replay)
@@ -174,7 +175,9 @@ Layout lay_out(char* base, int M, int nnz, const Caps& k, int n_slots, std::vect
   return L;
 }
 
-// launch with (or without) programmatic stream serialization, see pdl_begin()
+// launch with (or without) programmatic stream serialization, see pdl_begin().  The first launch error of a sequence is kept
+// in t_launch_err (run_sequence clears it on entry and reports it on exit).
+thread_local cudaError_t t_launch_err = cudaSuccess;
 template <typename... KArgs, typename... Args>
 inline void launch(bool pdl, void (*k)(KArgs...), dim3 g, dim3 b, size_t smem, cudaStream_t st, Args... args) {
   cudaLaunchConfig_t cfg = {};
@@ -183,7 +186,8 @@ inline void launch(bool pdl, void (*k)(KArgs...), dim3 g, dim3 b, size_t smem, c
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
-  (void)cudaLaunchKernelEx(&cfg, k, static_cast<KArgs>(args)...);
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, k, static_cast<KArgs>(args)...);
+  if (e != cudaSuccess && t_launch_err == cudaSuccess) t_launch_err = e;
 }
 
 inline bool bad(lst_ctx* c, cudaError_t e) {
@@ -281,6 +285,12 @@ int lst_create(const lst_geometry* geo, const lst_caps* caps, void* dev_workspac
     if (e == cudaSuccess) e = cudaMemset(c->h_slots[i].chain_t5, 0, sizeof(unsigned long long) * (c->caps.max_t3 / TUPLE_TPB + 4));
   }
   if (e == cudaSuccess) e = cudaDeviceSynchronize();       // the memsets above are asynchronous on device memory
+  if (e == cudaSuccess) {
+    int dev = 0;
+    e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess && c->n_sm <= 0) e = cudaErrorInvalidDevice;
+  }
   if (e != cudaSuccess) { delete c; return LST_ECUDA; }
   if (cudaFuncSetAttribute(k_pls_bin, cudaFuncAttributeMaxDynamicSharedMemorySize, PLS_BIN_SMEM) != cudaSuccess) { delete c; return LST_ECUDA; }
   if (const char* g = std::getenv("LST_GRAPHS")) c->use_graphs = !(g[0] == '0');
@@ -346,15 +356,17 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   const Geo g = c->geo;
   const Caps k = c->caps;
   int li = 0;
+  t_launch_err = cudaSuccess;
 #define LST_MARK() do { if (ev && bad(c, cudaEventRecord(ev[li], st))) return LST_ECUDA; ++li; } while (0)
   LST_MARK();
   if (bad(c, cudaMemsetAsync(c->zero_base + first * c->zero_stride, 0, c->zero_stride * n, st))) return LST_ECUDA;
   if (bad(c, cudaMemsetAsync(c->ones_base + first * c->ones_stride, 0xFF, c->ones_stride * n, st))) return LST_ECUDA;
   LST_MARK();
-  // x-extent of the grids: enough blocks to fill 148 SMs several times over across the whole batch
-  int gx = (148 * 8 + n - 1) / n;
+  // x-extent of the grids: enough blocks to fill the SMs (148 on a B200) several times over across the whole batch
+  const int n_sm = c->n_sm;
+  int gx = (n_sm * 8 + n - 1) / n;
   if (gx < 8) gx = 8;
-  if (gx > 592) gx = 592;
+  if (gx > 4 * n_sm) gx = 4 * n_sm;
   const dim3 G(gx, n), G1(1, n), GL(2 * gx, n);   // GL: the 128-thread link kernels
   const dim3 GS(gx < 16 ? gx : 16, n);            // look-back scans: tiles of 2048 entries by ticket
   // the pLS binning depends on the inputs only: under stream capture it becomes a side branch of the graph
@@ -383,7 +395,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
     k_pls_cross<<<GX, XS_TPB, XS_SMEM, c->side>>>(sl, k.max_pls);
     if (bad(c, cudaEventRecord(c->ev_join, c->side))) return LST_ECUDA;
   }
-  launch(pdl, k_ls_sweep, dim3(n < 8 ? 148 * 4 : 148 * LS_GRID_PER_SM, (n + 31) / 32), BP, 0, st, sl, (int)n, g, k); LST_MARK();      // persistent grid: the resident blocks
+  launch(pdl, k_ls_sweep, dim3(n < 8 ? n_sm * 4 : n_sm * LS_GRID_PER_SM, (n + 31) / 32), BP, 0, st, sl, (int)n, g, k); LST_MARK();      // persistent grid: the resident blocks
   launch(pdl, k_scan_lb<SCAN_LSROW>, GS, BS, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_ls_finish, GL, BP, 0, st, sl, g, k); LST_MARK();
   launch(pdl, k_t3_one, GL, BT, 0, st, sl, k); LST_MARK();
@@ -409,6 +421,7 @@ static int run_sequence(lst_ctx* c, int32_t first, int32_t n, cudaStream_t st, c
   launch(pdl, k_tc_clean, GL, dim3(TCC_TPB), 0, st, sl, k); LST_MARK();
 #undef LST_MARK
   if (li != N_LAUNCHES + 2) return LST_EINVAL;
+  if (bad(c, t_launch_err)) { (void)cudaGetLastError(); return LST_ECUDA; }
   return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
 }
 
@@ -584,7 +597,7 @@ int lst_read_tc_hits_batch_host(lst_ctx* c, int32_t first, int32_t n, int32_t* h
 int lst_export_graph(lst_ctx* c, int32_t first, int32_t n, void* cuda_stream) {
   if (!c || first < 0 || n <= 0 || first + n > c->n_slots) return LST_EINVAL;
   if (c->sticky_cuda_error) return LST_ECUDA;
-  int gx = (148 * 4 + n - 1) / n;
+  int gx = (c->n_sm * 4 + n - 1) / n;
   if (gx < 4) gx = 4;
   k_graph_export<<<dim3(gx, n), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(c->d_slots + first);
   return bad(c, cudaGetLastError()) ? LST_ECUDA : LST_OK;
@@ -595,22 +608,29 @@ int lst_measure_fp32(lst_ctx* c, int32_t fused, float* h_tflops, void* cuda_stre
   if (c->sticky_cuda_error) return LST_ECUDA;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   float* scratch = reinterpret_cast<float*>(c->batch_out);
-  cudaEvent_t a, b;
-  if (bad(c, cudaEventCreate(&a)) || bad(c, cudaEventCreate(&b))) return LST_ECUDA;
-  const int blocks = 148 * 8, iters = 8192;
+  // measurement only: a failure here is reported but does not disable the context (no sticky flag)
+  cudaEvent_t a = nullptr, b = nullptr;
+  if (cudaEventCreate(&a) != cudaSuccess) return LST_ECUDA;
+  if (cudaEventCreate(&b) != cudaSuccess) { cudaEventDestroy(a); return LST_ECUDA; }
+  const int blocks = c->n_sm * 8, iters = 8192;
   float best = 0.f;
-  for (int rep = 0; rep < 4; ++rep) {             // first repetition warms up
-    cudaEventRecord(a, st);
+  cudaError_t e = cudaSuccess;
+  for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {             // first repetition warms up
+    e = cudaEventRecord(a, st);
+    if (e != cudaSuccess) break;
     if (fused) k_fp32_probe<true><<<blocks, 256, 0, st>>>(scratch, iters);
     else k_fp32_probe<false><<<blocks, 256, 0, st>>>(scratch, iters);
-    cudaEventRecord(b, st);
-    if (bad(c, cudaEventSynchronize(b))) { cudaEventDestroy(a); cudaEventDestroy(b); return LST_ECUDA; }
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaEventRecord(b, st);
+    if (e == cudaSuccess) e = cudaEventSynchronize(b);
     float ms = 0.f;
-    cudaEventElapsedTime(&ms, a, b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, a, b);
+    if (e != cudaSuccess) break;
     const double flop = 2.0 * 8.0 * iters * 256.0 * blocks;      // one multiply + one add per chain step, fused or not
     if (rep && ms > 0.f) best = fmaxf(best, (float)(flop / (ms * 1e-3) / 1e12));
   }
   cudaEventDestroy(a); cudaEventDestroy(b);
+  if (e != cudaSuccess) return LST_ECUDA;
   *h_tflops = best;
   return LST_OK;
 }

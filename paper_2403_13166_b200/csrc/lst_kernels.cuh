@@ -1229,7 +1229,9 @@ __global__ void __launch_bounds__(TCC_TPB) k_tc_clean(const Slot* __restrict__ s
       if (tile == n_tiles - 1) {       // last kernel of the chain: every counter is final once this tile knows its base
         if (lane == 0) s.cnt[LST_CNT_TCC] = base + btot;
         __syncwarp();
-        if (lane < LST_N_CNT) s.tc_hdr[lane] = s.cnt[lane];      // header copy in front of the TC rows (one D2H copy reads both)
+        // header copy in front of the TC rows (one D2H copy reads both); this kernel's own tile ticket is still being
+        // incremented by other blocks, so the copy carries 0 there (an internal entry, never a result)
+        if (lane < LST_N_CNT) s.tc_hdr[lane] = (lane == LST_CNT_TK_TCC) ? 0 : s.cnt[lane];
       }
     }
     __syncthreads();
