@@ -28,6 +28,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <limits>
 #include <vector>
 #include <algorithm>
 
@@ -268,6 +269,11 @@ inline PLS<R> pls_derive(R px, R py, R pz, R z0, int q) {
   p.z0 = z0;
   return p;
 }
+// SPEC.md 4.6 [R20]: a pair only matches if its finished chi2 is a number below infinity.  On finite inputs every chi2 term is
+// <= 1, so this never bites; a seed with pz = +-inf has dZ = inf, passes |zres| = inf <= dZ and would carry chi2 = NaN, for
+// which argmin over (chi2, index) is undefined.
+template <typename R>
+inline bool chi2_is_a_number(R chi) { return chi < std::numeric_limits<R>::infinity(); }
 // one anchor against one pLS helix; adds its two chi2 terms to *chi2 when it passes
 template <typename R>
 inline bool pls_anchor(const PLS<R>& p, const MD<R>& m, R loosen, R* chi2) {
@@ -494,7 +500,7 @@ Result<R>* run_chain(int32_t M, const uint8_t* subdet, const uint8_t* mtype, con
       R chi = R(0.0f);
       bool ok = true;
       for (int q = 0; q < 5 && ok; ++q) ok = pls_anchor<R>(pls[p], res->md[q5.md[q]], lo.f[CUT_P5], &chi);
-      if (!ok) continue;
+      if (!ok || !chi2_is_a_number<R>(chi)) continue;   // T5 match
       res->n_match5++;
       if (res->best5_pls[t] < 0 || chi < chi5[t]) { res->best5_pls[t] = p; chi5[t] = chi; }
     }
@@ -531,7 +537,7 @@ Result<R>* run_chain(int32_t M, const uint8_t* subdet, const uint8_t* mtype, con
       R chi = R(0.0f);
       bool ok = true;
       for (int q = 0; q < 3 && ok; ++q) ok = pls_anchor<R>(pls[p], res->md[mm[q]], lo.f[CUT_P3], &chi);
-      if (!ok) continue;
+      if (!ok || !chi2_is_a_number<R>(chi)) continue;   // T3 match
       res->n_match3++;
       if (best3[x] < 0 || chi < chi3[x]) { best3[x] = p; chi3[x] = chi; }
     }
@@ -716,6 +722,7 @@ int32_t lst_oracle_pls_match(const float* pls5, int32_t q, const float* anchors,
   float chi = 0.0f;
   for (int i = 0; i < n; ++i)
     if (!pls_anchor<float>(p, mk_md(anchors + 9 * i), 1.0f, &chi)) return 0;
+  if (!chi2_is_a_number<float>(chi)) return 0;
   *chi2_out = chi;
   return 1;
 }

@@ -724,7 +724,8 @@ __device__ __forceinline__ void match_drain2(const Slot& s, unsigned long long* 
 #pragma unroll
     for (int q = 1; q < NA; ++q)
       if (ok) ok = pls_anchor(P, an[q], mt[q], chi);
-    if (ok) atomicMin(&key[o], ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j]);   // chi2 >= 0: bit order = value order
+    // SPEC.md 4.6 [R20]: the finished chi2 must be a number below infinity (only non-finite seeds / anchors can break that)
+    if (ok && chi < __int_as_float(0x7f800000)) atomicMin(&key[o], ((unsigned long long)__float_as_uint(chi) << 32) | (unsigned)s.pls_sidx[j]);   // chi2 >= 0: bit order = value order
   }
 }
 template <int NA, bool IS_T3>

@@ -107,6 +107,8 @@ MUTANTS = [
     ("pT feature clamped at 1e4", "  const float rad = std::fmin(1.0f / ac, 1.0e5f);\n  return std::log10(KAPPA_F * rad);",
      "  const float rad = std::fmin(1.0f / ac, 1.0e4f);\n  return std::log10(KAPPA_F * rad);", [("pin_radius_clamp", None)]),
     ("md_eval: S without the cap at 1", "const R S = std::fmin(R(1.0f), r2 * R(C_HALF_F));", "const R S = r2 * R(C_HALF_F);", [("pin_md_sagitta_cap", None)]),
+    ("a6: T5 match accepts a chi2 that is not a number", "      if (!ok || !chi2_is_a_number<R>(chi)) continue;   // T5 match", "      if (!ok) continue;", [("pin_match_needs_a_chi2_that_is_a_number", "geo")]),
+    ("a6: T3 match accepts a chi2 that is not a number", "      if (!ok || !chi2_is_a_number<R>(chi)) continue;   // T3 match", "      if (!ok) continue;", [("pin_match_needs_a_chi2_that_is_a_number", "geo")]),
     ("f1: upper hits left out of the tuples", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_up];", "hits[10 * i + 2 * k + 1] = ho[res->md[mds[k]].hit_lo];", [("pin_clean_all_pairs", "geo")]),
 ]
 

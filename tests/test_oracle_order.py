@@ -14,6 +14,7 @@ import numpy as np
 
 from lstgen import config_event, xavier_weights
 from oracle import lst_oracle as O
+import test_oracle_terms as T
 
 N_DUP = 3000
 
@@ -114,6 +115,41 @@ def pin_md_sagitta_cap():
     assert ok_in and not ok_between and not ok_out
 
 
+def pin_match_needs_a_chi2_that_is_a_number(geo):
+    """SPEC.md 4.6 [R20]: a pair only matches if its finished chi2 is a number below infinity.
+    Single pair: straight seed along +x (pT = 1000 GeV), anchor at (50, 0, 0.1).  With pz = 0 it matches (|zres| = 0.1 <= 0.2).  With
+    pz = +-inf: cot = sec = inf, dZ = inf, |zres| = |0.1 - inf| = inf <= dZ holds, but b = inf / inf = NaN -> no match.  NaN: no match.
+    (An anchor with delta_r = 0, i.e. a barrel MD, rejects such a seed by itself: 0 * inf = NaN in dZ.  Endcap MDs have delta_r > 0.)
+    Without the clause an infinite seed "matches" all-endcap objects with chi2 = NaN and, if it comes first, keeps them
+    (`chi < NaN` is false for every later seed)."""
+    ok, chi = O.pls_match(T._seed(0.0, 0.0), 1, T.A9(50.0, 0.0, 0.1))
+    assert ok and 0.0 < chi < 2.0
+    for pz in (np.inf, -np.inf, np.nan):
+        assert not O.pls_match([T.PT_STRAIGHT, 0.0, pz, 0.0], 1, T.A9(50.0, 0.0, 0.1))[0]
+    # chain: every seed of a PU50 event preceded by a copy with pz = +-inf.  The copies must match nothing (all of them end as plain
+    # pLS candidates) and the real seeds must get exactly the rows they get without the copies.
+    ev = config_event(geo, 1)
+    r0 = O.run(geo, xavier_weights(2), ev)
+    two = lambda a: np.repeat(a, 2)
+    pz = two(ev.pls_pz).copy()
+    pz[0::2] = np.where(pz[0::2] >= 0, np.inf, -np.inf).astype(np.float32)
+    ev2 = dataclasses.replace(ev, pls_px=two(ev.pls_px), pls_py=two(ev.pls_py), pls_pz=pz, pls_z0=two(ev.pls_z0), pls_q=two(ev.pls_q),
+                              pls_particle=two(ev.pls_particle))
+    r = O.run(geo, xavier_weights(2), ev2)
+    tc = r.tc
+    copies = tc[(tc[:, 1] >= 0) & (tc[:, 1] % 2 == 0)]
+    assert len(copies) == ev.n_pls and (copies[:, 0] == 3).all()
+    real = tc[~((tc[:, 1] >= 0) & (tc[:, 1] % 2 == 0))].copy()
+    real[:, 1] = np.where(real[:, 1] >= 0, real[:, 1] // 2, -1)
+    assert np.array_equal(real, r0.tc)
+    assert np.array_equal(np.where(r.best5_pls >= 0, r.best5_pls // 2, -1), r0.best5_pls) and (r.best5_pls[r.best5_pls >= 0] % 2 == 1).all()
+    assert np.isfinite(r.chi5).all() and np.isfinite(r.chi3).all()
+    # the event has what the clause is about: T5s / T3s whose anchors are all endcap MDs (delta_r * |cot| = inf, not 0 * inf = NaN)
+    sub = np.asarray(geo.subdet)[r.md_mod]
+    assert (sub[r.t5c[r.t5][:, :5]].min(axis=1) == 1).sum() > 20
+
+
 def test_build_order(geo_full): pin_build_order(geo_full)
+def test_match_needs_a_chi2_that_is_a_number(geo_full): pin_match_needs_a_chi2_that_is_a_number(geo_full)
 def test_radius_clamp(): pin_radius_clamp()
 def test_md_sagitta_cap(): pin_md_sagitta_cap()

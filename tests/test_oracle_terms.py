@@ -436,7 +436,7 @@ def _tc_expected(geo, r, ev):
 
 def _muon_with_seeds(geo_barrel, seeds):
     """one noise-free barrel muon (6 layers -> T5s on layers 1-5 and 2-6) and a list of pixel seeds derived from its
-    exact seed: 'exact' = copy, ('pt', f) = momentum scaled by f, ('z0', d) = z0 shifted by d cm"""
+    exact seed: 'exact' = copy, ('pt', f) = momentum scaled by f, ('z0', d) = z0 shifted by d cm, ('pz', v) = pz replaced by v"""
     ev = make_event(geo_barrel, 91, origin_muons=1, smear=False)
     base = (float(ev.pls_px[0]), float(ev.pls_py[0]), float(ev.pls_pz[0]), float(ev.pls_z0[0]), int(ev.pls_q[0]))
     rows = []
@@ -445,6 +445,8 @@ def _muon_with_seeds(geo_barrel, seeds):
             rows.append(base)
         elif s[0] == "pt":
             rows.append((base[0] * s[1], base[1] * s[1], base[2] * s[1], base[3], base[4]))
+        elif s[0] == "pz":
+            rows.append((base[0], base[1], s[1], base[3], base[4]))
         else:
             rows.append((base[0], base[1], base[2], base[3] + s[1], base[4]))
     p = np.array(rows, dtype=np.float64)
