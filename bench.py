@@ -421,6 +421,30 @@ def run_ours(args):
     # fp32 throughput of this GPU, measured with the library's probe kernels
     alu_meas, fma_meas = lst.lst_measure_fp32(False, main), lst.lst_measure_fp32(True, main)
 
+    # ---- configs[3] "per-stage overlap": the same E events split over 1 / 2 / 4 / 8 streams (1, 2, 4, 8 CUDA streams)
+    def sweep_point(n_st):
+        sts = [torch.cuda.Stream(device=dev) for _ in range(n_st)]
+        per_s = E // n_st
+        def stp():
+            ev0 = torch.cuda.Event(); ev0.record(main)
+            for si, st in enumerate(sts):
+                st.wait_event(ev0)
+                lst.lst_run_batch(si * per_s, per_s, st)
+                e = torch.cuda.Event(); e.record(st); main.wait_event(e)
+        for _ in range(3):
+            stp()
+        torch.cuda.synchronize()
+        tt = []
+        for _ in range(max(5, min(args.steps, 20))):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(main); stp(); b.record(main)
+            tt.append((a, b))
+        torch.cuda.synchronize()
+        t_ms = float(np.median([a.elapsed_time(b) for a, b in tt]))
+        return dict(streams=n_st, events_per_launch=per_s, ms_per_step=round(t_ms, 4), events_per_s=round(E / t_ms * 1e3, 1))
+    streams_sweep = [sweep_point(n_st) for n_st in (1, 2, 4, 8) if E % n_st == 0]
+
     def red_max(v):
         if dist is None:
             return v
@@ -438,6 +462,21 @@ def run_ours(args):
     alu_peak = alu_meas if alu_meas > 0 else alu_nominal
     fma_peak = fma_meas if fma_meas > 0 else 2 * alu_nominal
     stage_rows = stage_table(prof, stages, n_prof, pk, alu_peak, fma_peak)
+    roof_stages = {k: dict(us_per_event=v["us_per_event"], bound=v["bound"], frac=v["frac"]) for k, v in stage_rows.items()}
+    # overlap: what one stream's launch sequence takes alone (sum of its kernels, measured with events between them) x S streams,
+    # against the measured step in which the S sequences run concurrently; per stage = the share of the step during which that stage
+    # is busy on some stream (the shares add up to `factor`; > 1 means the streams really overlap)
+    chain_ms = sum(prof.values())
+    stage_busy = {}
+    for k, v in prof.items():
+        sn = "a0" if k == "memset" else stage_of(k)
+        stage_busy[sn] = stage_busy.get(sn, 0.0) + v
+    overlap = dict(streams=S, chain_alone_ms=round(chain_ms, 4), serial_ms=round(S * chain_ms, 4), step_ms=round(ms, 4),
+                   factor=round(S * chain_ms / ms, 3),
+                   busy_share_of_step={k: round(S * v / ms, 3) for k, v in stage_busy.items()},
+                   streams_sweep=streams_sweep,
+                   note="chain_alone_ms: one stream's 16-event sequence timed alone with an event after every kernel (adds launch gaps); "
+                        "factor = S x chain_alone / step; streams_sweep: the same 64 events over 1 / 2 / 4 / 8 streams, median step")
     # dominant kernel
     kname = max((k for k in prof if k != "memset"), key=lambda k: prof[k])
     kst = stage_of(kname)
@@ -461,6 +500,7 @@ def run_ours(args):
                 kernel_share_of_step=round(prof[kname] / sum(prof.values()), 3), algorithmic_per_unit="60 flop per LS pair test (SURVEY.md 8.d)" if kst == "a2" else None,
                 fp32_tflops=dict(unfused_measured=round(alu_meas, 2), fma_measured=round(fma_meas, 2), unfused_nominal=round(alu_nominal, 2),
                                  note="nominal = 148 SM x 128 lanes x sm_max_mhz, one op per lane per clock; the cut kernels may not fuse (north_star)"))
+    roof["stages"] = roof_stages      # every stage of the 16-event launch: us / event, bound, fraction of its own roofline
     single = dict(workload="configs[2] exactly: one HL-LHC PU200 event, seed 3, one stream, one lst_run (CUDA-graph replay)",
                   value=round(1e3 / lat_ms, 1), unit=UNIT, us_per_event=round(lat_ms * 1e3, 1),
                   timing=f"median of {args.single_reps} runs, CUDA events on the launching stream, L2 flushed before every run",
@@ -481,7 +521,8 @@ def run_ours(args):
                         timing="wall clock around K steps incl. pinned H2D of every input and D2H of counters + TC rows with their hit indices",
                         host_link_gbs=round((h2d + d2h) / (e2e_ms * 1e-3) / 1e9, 1)),
                gpu_launches=args.steps * S * lst.launches_per_run(), launch_floor_us=round(launch_floor_us, 2),
-               clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows, single_event=single,
+               step_ms=dict(min=round(float(np.min(step_ms)), 4), median=round(float(np.median(step_ms)), 4), max=round(float(np.max(step_ms)), 4)),
+               clocks=clocks, roofline=roof, cpu_baseline=cpu, stages=stage_rows, overlap=overlap, single_event=single,
                graph_export=dict(us_per_event=round(graph_ms * 1e3 / n_prof, 3), us_per_launch=round(graph_ms * 1e3, 2), events_per_launch=n_prof,
                                  nodes_per_event=round(tot["md"] / n_prof, 1), edges_per_event=round(tot["ls"] / n_prof, 1),
                                  note="lst_export_graph after lst_run: packs node features + CSR columns (SPEC.md 4.8); the paper quotes 1 to 2 ms per event for graph building (PAPER.md:127, other hardware)"),

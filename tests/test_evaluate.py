@@ -36,6 +36,21 @@ def test_clean_muons_are_fully_efficient(geo_barrel):
     s = t.summary()
     assert s["n_particles"] == 30 and s["efficiency"] == 1.0 and s["fake_rate"] == 0.0 and s["duplicate_rate"] == 0.0
     assert sum(b["n"] for b in s["vs"]["pt"]) == 30 and all(b["eff"] in (None, 1.0) for b in s["vs"]["eta"])
+    # every muon is found by a candidate with outer-tracker hits (a pT5), none through a bare seed
+    assert s["efficiency_outer_tracker"] == 1.0 and s["efficiency_by_type"] == {"pT5": 1.0, "T5": 0.0, "pT3": 0.0, "pLS": 0.0}
+
+
+def test_seed_only_candidates_do_not_count_for_the_outer_tracker(geo_barrel):
+    """The pooled efficiency is nearly tautological on this generator (every prompt particle has a seed, a pLS candidate is matched
+    through the seed's label): a candidate list made of bare seeds 'finds' every muon although the outer-tracker chain built
+    nothing.  The outer-tracker headline must read 0 for it."""
+    ev = make_event(geo_barrel, 71, origin_muons=10, smear=False)
+    n = ev.n_pls
+    t = E.Tally()
+    t.add(ev, np.full(n, 3), np.arange(n), -np.ones((n, 10), dtype=np.int64))
+    s = t.summary()
+    assert s["efficiency"] == 1.0 and s["efficiency_outer_tracker"] == 0.0 and s["fake_rate_outer_tracker"] is None
+    assert s["efficiency_by_type"]["pLS"] == 1.0
 
 
 def test_pileup_event_numbers_are_sane(geo_full):
